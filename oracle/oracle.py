@@ -1,0 +1,164 @@
+"""ctypes marshalling for oracle/lqcd_oracle.cpp -- TEST INFRASTRUCTURE ONLY.
+
+No arithmetic of the method happens in this file: it checks shapes/dtypes,
+passes pointers to the C++ oracle and returns numpy arrays in the canonical
+layout (gauge (V,4,3,3), spinor (V,4,3) / (V/2,4,3), complex128).
+"""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "lqcd_oracle.cpp")
+_LIB = os.path.join(_HERE, "liblqcd_oracle.so")
+_lib = None
+
+_c_int_p = ctypes.POINTER(ctypes.c_int)
+_c_dbl_p = ctypes.POINTER(ctypes.c_double)
+_c_long_p = ctypes.POINTER(ctypes.c_long)
+
+
+def build(force=False):
+    """Compile the oracle with g++ (-O2, no FMA contraction, OpenMP over sites)."""
+    if not force and os.path.exists(_LIB) and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC):
+        return _LIB
+    cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
+           "-Wall", "-o", _LIB, _SRC]
+    subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = ctypes.CDLL(_LIB)
+        _lib.orc_cg_mdagm.restype = ctypes.c_int
+        _lib.orc_num_threads.restype = ctypes.c_int
+    return _lib
+
+
+def _dims(dims):
+    d = np.ascontiguousarray(dims, dtype=np.int32)
+    assert d.shape == (4,) and np.all(d >= 2) and np.all(d % 2 == 0), "extents must be even, >= 2"
+    return d
+
+
+def _phases(bc_phase):
+    p = np.ascontiguousarray(np.asarray(bc_phase, dtype=np.complex128))
+    assert p.shape == (4,)
+    return p
+
+
+def _c128(a, shape):
+    a = np.ascontiguousarray(a, dtype=np.complex128)
+    assert a.shape == tuple(shape), (a.shape, shape)
+    return a
+
+
+def _ip(a):
+    return a.ctypes.data_as(_c_int_p)
+
+
+def _dp(a):
+    return a.ctypes.data_as(_c_dbl_p)
+
+
+def gamma(which):
+    """gamma_mu for which in 0..3 (x,y,z,t), gamma5 for which == 4, as a 4x4 array."""
+    out = np.zeros((4, 4), dtype=np.complex128)
+    _load().orc_gamma(ctypes.c_int(which), _dp(out))
+    return out
+
+
+def m_full(dims, bc_phase, U, psi, kappa, mu, dagger=0):
+    d, ph = _dims(dims), _phases(bc_phase)
+    V = int(np.prod(d))
+    U = _c128(U, (V, 4, 3, 3))
+    psi = _c128(psi, (V, 4, 3))
+    out = np.empty_like(psi)
+    _load().orc_m_full(_ip(d), _dp(ph), _dp(U), _dp(psi), _dp(out), ctypes.c_double(kappa),
+                       ctypes.c_double(mu), ctypes.c_int(dagger))
+    return out
+
+
+def dslash_eo(dims, bc_phase, U, half_in, parity, kappa, adjoint=0):
+    d, ph = _dims(dims), _phases(bc_phase)
+    V = int(np.prod(d))
+    U = _c128(U, (V, 4, 3, 3))
+    half_in = _c128(half_in, (V // 2, 4, 3))
+    out = np.empty_like(half_in)
+    _load().orc_dslash_eo(_ip(d), _dp(ph), _dp(U), _dp(half_in), _dp(out), ctypes.c_int(parity),
+                          ctypes.c_double(kappa), ctypes.c_int(adjoint))
+    return out
+
+
+def dslash_eo_sites(dims, bc_phase, U, half_in, sites, parity, kappa, adjoint=0):
+    d, ph = _dims(dims), _phases(bc_phase)
+    V = int(np.prod(d))
+    U = _c128(U, (V, 4, 3, 3))
+    half_in = _c128(half_in, (V // 2, 4, 3))
+    sites = np.ascontiguousarray(sites, dtype=np.int64)
+    out = np.empty((len(sites), 4, 3), dtype=np.complex128)
+    _load().orc_dslash_eo_sites(_ip(d), _dp(ph), _dp(U), _dp(half_in),
+                                sites.ctypes.data_as(_c_long_p), ctypes.c_long(len(sites)),
+                                _dp(out), ctypes.c_int(parity), ctypes.c_double(kappa),
+                                ctypes.c_int(adjoint))
+    return out
+
+
+def mhat(dims, bc_phase, U, half_in, kappa, mu, dagger=0):
+    d, ph = _dims(dims), _phases(bc_phase)
+    V = int(np.prod(d))
+    U = _c128(U, (V, 4, 3, 3))
+    half_in = _c128(half_in, (V // 2, 4, 3))
+    out = np.empty_like(half_in)
+    _load().orc_mhat(_ip(d), _dp(ph), _dp(U), _dp(half_in), _dp(out), ctypes.c_double(kappa),
+                     ctypes.c_double(mu), ctypes.c_int(dagger))
+    return out
+
+
+def mhat_sites(dims, bc_phase, U, half_in, sites, kappa, mu, dagger=0):
+    d, ph = _dims(dims), _phases(bc_phase)
+    V = int(np.prod(d))
+    U = _c128(U, (V, 4, 3, 3))
+    half_in = _c128(half_in, (V // 2, 4, 3))
+    sites = np.ascontiguousarray(sites, dtype=np.int64)
+    out = np.empty((len(sites), 4, 3), dtype=np.complex128)
+    _load().orc_mhat_sites(_ip(d), _dp(ph), _dp(U), _dp(half_in),
+                           sites.ctypes.data_as(_c_long_p), ctypes.c_long(len(sites)), _dp(out),
+                           ctypes.c_double(kappa), ctypes.c_double(mu), ctypes.c_int(dagger))
+    return out
+
+
+def mdagm(dims, bc_phase, U, half_in, kappa, mu):
+    d, ph = _dims(dims), _phases(bc_phase)
+    V = int(np.prod(d))
+    U = _c128(U, (V, 4, 3, 3))
+    half_in = _c128(half_in, (V // 2, 4, 3))
+    out = np.empty_like(half_in)
+    _load().orc_mdagm(_ip(d), _dp(ph), _dp(U), _dp(half_in), _dp(out), ctypes.c_double(kappa),
+                      ctypes.c_double(mu))
+    return out
+
+
+def cg_mdagm(dims, bc_phase, U, b, kappa, mu, tol, maxit):
+    """Returns (status, x, iters, rel_resid_recursive, rel_resid_true)."""
+    d, ph = _dims(dims), _phases(bc_phase)
+    V = int(np.prod(d))
+    U = _c128(U, (V, 4, 3, 3))
+    b = _c128(b, (V // 2, 4, 3))
+    x = np.empty_like(b)
+    it = ctypes.c_int(0)
+    rr = ctypes.c_double(0.0)
+    rt = ctypes.c_double(0.0)
+    st = _load().orc_cg_mdagm(_ip(d), _dp(ph), _dp(U), _dp(b), _dp(x), ctypes.c_double(kappa),
+                              ctypes.c_double(mu), ctypes.c_double(tol), ctypes.c_int(maxit),
+                              ctypes.byref(it), ctypes.byref(rr), ctypes.byref(rt))
+    return st, x, it.value, rr.value, rt.value
+
+
+def num_threads():
+    return int(_load().orc_num_threads())
