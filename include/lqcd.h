@@ -1,0 +1,138 @@
+/* lqcd.h -- C ABI of liblqcd.so: the even-odd preconditioned twisted-mass Wilson
+ * fermion matrix of arxiv 1209.5942 and CG on Mhat^dag Mhat, on one NVIDIA B200.
+ *
+ * What is computed (eq. 6; readings G1-G11 in DESIGN.md):
+ *
+ *   (M psi)(x) = (1 + 2 i kappa mu gamma5) psi(x)
+ *                - kappa sum_{mu=0..3} [ eta+_mu(x) (1 - gamma_mu) U_mu(x)        psi(x + mu)
+ *                                      + eta-_mu(x) (1 + gamma_mu) U_mu(x - mu)^dag psi(x - mu) ]
+ *
+ * with coordinates mod N_mu, eta+_mu(x) = bc_phase_mu on the hop that wraps
+ * (x_mu = N_mu - 1), eta-_mu(x) = conj(bc_phase_mu) at x_mu = 0, else 1.
+ * mu = 0..3 = x,y,z,t.  Sites are split by parity p(x) = (x0+x1+x2+x3) mod 2:
+ *   M = [[M_ee, D_eo], [D_oe, M_oo]],  M_ee = M_oo = 1 + 2 i kappa mu gamma5,
+ *   Mhat = M_ee - D_eo M_oo^{-1} D_oe   on even sites (reading G3).
+ * gamma basis (reading G4; chiral, gamma5 = diag(1,1,-1,-1)), rows top to bottom:
+ *   gamma_x: (0,0,0,-i) (0,0,-i,0) (0,i,0,0) (i,0,0,0)
+ *   gamma_y: (0,0,0,-1) (0,0,1,0)  (0,1,0,0) (-1,0,0,0)
+ *   gamma_z: (0,0,-i,0) (0,0,0,i)  (i,0,0,0) (0,-i,0,0)
+ *   gamma_t: (0,0,1,0)  (0,0,0,1)  (1,0,0,0) (0,1,0,0)
+ *
+ * Canonical (interchange) layout, always complex double, row-major, (re,im):
+ *   gauge        U[lex(x)][mu][a][b]      144 B per link, 576 B per site
+ *   half spinor  psi_p[e][alpha][a]       192 B per site, e = lex(x)/2 over
+ *                                         the sites of parity p, lex(x) = x0 + N0 (x1 + N1 (x2 + N2 x3))
+ * Internal layout: opaque structure-of-arrays on 128-bit elements (the thing
+ * being tuned); sizes from lqcd_gauge_bytes() / lqcd_spinor_bytes(); convert
+ * with lqcd_pack_* / lqcd_unpack_spinor.  In single precision the internal
+ * fields are float (pack rounds to nearest, unpack widens).
+ *
+ * Pointers: every `*_dev` / gauge / in / out / b / x argument is a DEVICE
+ * pointer, 16-byte aligned, allocated and freed by the caller; `*_host`
+ * arguments (only in the lqcd_*_host calls) are HOST pointers.  The library
+ * owns only its context and a lazily allocated CG / staging workspace, released
+ * by lqcd_finalize().  `in` and `out` must not alias.  All device calls are
+ * asynchronous on the stream given to lqcd_set_stream() (default: stream 0)
+ * except lqcd_cg_mdagm, lqcd_cg_finish, lqcd_cg_stats and the *_host calls,
+ * which synchronise that stream before returning.
+ *
+ * Every function returns an int status; no exception crosses the ABI.
+ * The library is not thread safe (one context per process).
+ */
+#ifndef LQCD_H
+#define LQCD_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LQCD_OK               0
+#define LQCD_NOT_CONVERGED    1   /* cg only: maxit reached, x = last iterate        */
+#define LQCD_NOT_INITIALISED (-1)
+#define LQCD_BAD_DIMS        (-2) /* an extent is odd or < 2, or |bc_phase| != 1      */
+#define LQCD_BAD_ARG         (-3) /* null pointer, parity not 0/1, non-finite scalar */
+#define LQCD_CUDA_ERROR      (-4)
+#define LQCD_BREAKDOWN       (-5) /* cg: <p, A p> <= 0 or not finite                  */
+
+#define LQCD_DOUBLE 0
+#define LQCD_SINGLE 1
+
+/* Text of the last error on this process ("" if none). Never NULL. */
+const char* lqcd_last_error(void);
+
+/* Set the lattice extents N_x,N_y,N_z,N_t (all even, >= 2) and the boundary
+ * phases e^{i pi theta_mu} as (re,im) pairs, mu = x,y,z,t (reading G5; the
+ * paper never states its boundary conditions).  Resets format to double/18,
+ * stream to 0.  No device work. */
+int lqcd_init(const int dims[4], const double bc_phase[8]);
+int lqcd_finalize(void);
+
+/* cuda_stream is a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream). */
+int lqcd_set_stream(void* cuda_stream);
+
+/* precision: LQCD_DOUBLE or LQCD_SINGLE; recon: 18 (full link) or 12 (two rows
+ * stored, third = conj(row0 x row1), reading G9).  Fields packed
+ * under one format are only valid under that format. */
+int lqcd_set_format(int precision, int recon);
+
+size_t lqcd_gauge_bytes(void);   /* bytes of one internal gauge field (both parities, 4 mu) */
+size_t lqcd_spinor_bytes(void);  /* bytes of one internal half-spinor field                 */
+
+/* canonical (device) -> internal (device) and back; parity = parity of the sites held. */
+int lqcd_pack_gauge(const void* canon_dev, void* internal_dev);
+int lqcd_pack_spinor(const void* canon_dev, void* internal_dev, int parity);
+int lqcd_unpack_spinor(const void* internal_dev, void* canon_dev, int parity);
+
+/* Hopping block of eq. 6, including the factor -kappa:
+ *   out_p = D_{p,1-p} in_{1-p},   parity = p = parity of the OUTPUT sites
+ * (parity 0: out_e = D_eo in_o).  Internal layouts. */
+int lqcd_dslash_eo(const void* gauge, const void* in, void* out, int parity, double kappa);
+
+/* Even-odd preconditioned operator on even half fields (internal layout):
+ *   dagger = 0: out = Mhat(mu) in;   dagger = 1: out = Mhat(mu)^dag in  (= gamma5 Mhat(-mu) gamma5 in).
+ * Two hopping launches; the diagonal terms are fused into their epilogues.
+ * Uses one half-spinor of library workspace. */
+int lqcd_mtm(const void* gauge, const void* in, void* out, double kappa, double mu, int dagger);
+
+/* Solve Mhat^dag Mhat x = b on even sites by CG (reading G10):
+ * x0 = 0 (input contents of x ignored), stop when |r| <= tol |b| (recursive
+ * residual) or after maxit iterations.  Returns LQCD_OK, LQCD_NOT_CONVERGED or
+ * LQCD_BREAKDOWN.  b, x in internal layout. */
+int lqcd_cg_mdagm(const void* gauge, const void* b, void* x, double kappa, double mu,
+                  double tol, int maxit);
+
+/* The same solve in three steps (what lqcd_cg_mdagm does internally; bench.py
+ * times lqcd_cg_iterate alone):
+ *   lqcd_cg_setup    r = p = b, x = 0, rho = |b|^2                       (async)
+ *   lqcd_cg_iterate  enqueue up to n iterations; iterations after convergence
+ *                    are no-ops on the device                            (async)
+ *   lqcd_cg_finish   synchronise, compute the true residual |b - A x|/|b|;
+ *                    returns the solve status. */
+int lqcd_cg_setup(const void* gauge, const void* b, void* x, double kappa, double mu, double tol);
+int lqcd_cg_iterate(int n);
+int lqcd_cg_finish(void);
+
+/* Results of the last solve: iterations done, recursive and true relative residual.
+ * Any pointer may be NULL. */
+int lqcd_cg_stats(int* iters, double* rel_resid_recursive, double* rel_resid_true);
+
+/* Host-buffer entry points (canonical layout, HOST pointers; pinned memory is
+ * faster but not required).  Each uploads its inputs, packs, computes, unpacks
+ * and downloads the result, synchronously.  Device staging is library workspace. */
+int lqcd_mtm_host(const void* gauge_canon_host, const void* in_canon_host, void* out_canon_host,
+                  double kappa, double mu, int dagger);
+int lqcd_cg_mdagm_host(const void* gauge_canon_host, const void* b_canon_host, void* x_canon_host,
+                       double kappa, double mu, double tol, int maxit);
+
+/* Number of kernels this library has launched since lqcd_init (all streams). */
+long long lqcd_launch_count(void);
+
+/* Hopping-kernel thread-block size (tuning knob; 0 restores the default). */
+int lqcd_set_block_size(int threads);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LQCD_H */

@@ -1,0 +1,222 @@
+"""ctypes binding of liblqcd.so -- same names as include/lqcd.h, marshalling only.
+
+Device buffers are torch CUDA tensors (PyTorch is used for device memory and
+streams only); every ``lqcd_*`` function below passes ``tensor.data_ptr()``
+straight to the C ABI and raises ``LqcdError`` on a negative status.
+"""
+import ctypes
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "liblqcd.so")
+
+LQCD_OK, LQCD_NOT_CONVERGED = 0, 1
+LQCD_NOT_INITIALISED, LQCD_BAD_DIMS, LQCD_BAD_ARG, LQCD_CUDA_ERROR, LQCD_BREAKDOWN = -1, -2, -3, -4, -5
+LQCD_DOUBLE, LQCD_SINGLE = 0, 1
+
+SYMBOLS = [
+    "lqcd_last_error", "lqcd_init", "lqcd_finalize", "lqcd_set_stream", "lqcd_set_format",
+    "lqcd_gauge_bytes", "lqcd_spinor_bytes", "lqcd_pack_gauge", "lqcd_pack_spinor",
+    "lqcd_unpack_spinor", "lqcd_dslash_eo", "lqcd_mtm", "lqcd_cg_mdagm", "lqcd_cg_setup",
+    "lqcd_cg_iterate", "lqcd_cg_finish", "lqcd_cg_stats", "lqcd_mtm_host", "lqcd_cg_mdagm_host",
+    "lqcd_launch_count", "lqcd_set_block_size",
+]
+
+
+class LqcdError(RuntimeError):
+    def __init__(self, status, text):
+        super().__init__(f"liblqcd status {status}: {text}")
+        self.status = status
+
+
+def _load():
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(f"{_LIB_PATH} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                          "(there is no CPU fallback)")
+    lib = ctypes.CDLL(_LIB_PATH)
+    vp, dbl, i32 = ctypes.c_void_p, ctypes.c_double, ctypes.c_int
+    lib.lqcd_last_error.restype = ctypes.c_char_p
+    lib.lqcd_gauge_bytes.restype = ctypes.c_size_t
+    lib.lqcd_spinor_bytes.restype = ctypes.c_size_t
+    lib.lqcd_launch_count.restype = ctypes.c_longlong
+    sig = {
+        "lqcd_init": [ctypes.POINTER(i32), ctypes.POINTER(dbl)],
+        "lqcd_finalize": [],
+        "lqcd_set_stream": [vp],
+        "lqcd_set_format": [i32, i32],
+        "lqcd_pack_gauge": [vp, vp],
+        "lqcd_pack_spinor": [vp, vp, i32],
+        "lqcd_unpack_spinor": [vp, vp, i32],
+        "lqcd_dslash_eo": [vp, vp, vp, i32, dbl],
+        "lqcd_mtm": [vp, vp, vp, dbl, dbl, i32],
+        "lqcd_cg_mdagm": [vp, vp, vp, dbl, dbl, dbl, i32],
+        "lqcd_cg_setup": [vp, vp, vp, dbl, dbl, dbl],
+        "lqcd_cg_iterate": [i32],
+        "lqcd_cg_finish": [],
+        "lqcd_cg_stats": [ctypes.POINTER(i32), ctypes.POINTER(dbl), ctypes.POINTER(dbl)],
+        "lqcd_mtm_host": [vp, vp, vp, dbl, dbl, i32],
+        "lqcd_cg_mdagm_host": [vp, vp, vp, dbl, dbl, dbl, i32],
+        "lqcd_set_block_size": [i32],
+    }
+    for name, args in sig.items():
+        fn = getattr(lib, name)
+        fn.argtypes = args
+        fn.restype = i32
+    return lib
+
+
+_lib = _load()
+_fmt = {"precision": LQCD_DOUBLE}  # mirrors the library's format, for buffer helpers only
+
+
+def _check(status):
+    if status < 0:
+        raise LqcdError(status, _lib.lqcd_last_error().decode())
+    return status
+
+
+def _ptr(t):
+    """Device (torch CUDA tensor) or host (numpy array / CPU tensor) pointer, or a raw int."""
+    if isinstance(t, int):
+        return ctypes.c_void_p(t)
+    if isinstance(t, np.ndarray):
+        assert t.flags["C_CONTIGUOUS"]
+        return ctypes.c_void_p(t.ctypes.data)
+    assert t.is_contiguous()
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def lqcd_last_error():
+    return _lib.lqcd_last_error().decode()
+
+
+def lqcd_init(dims, bc_phase):
+    d = (ctypes.c_int * 4)(*[int(v) for v in dims])
+    ph = np.asarray(bc_phase, dtype=np.complex128)
+    p = (ctypes.c_double * 8)(*[float(v) for z in ph for v in (z.real, z.imag)])
+    rc = _check(_lib.lqcd_init(d, p))
+    _fmt["precision"] = LQCD_DOUBLE
+    return rc
+
+
+def lqcd_finalize():
+    return _check(_lib.lqcd_finalize())
+
+
+def lqcd_set_stream(stream=None):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return _check(_lib.lqcd_set_stream(ctypes.c_void_p(s.cuda_stream)))
+
+
+def lqcd_set_format(precision, recon):
+    rc = _check(_lib.lqcd_set_format(precision, recon))
+    _fmt["precision"] = precision
+    return rc
+
+
+def lqcd_set_block_size(threads):
+    return _check(_lib.lqcd_set_block_size(threads))
+
+
+def lqcd_gauge_bytes():
+    return int(_lib.lqcd_gauge_bytes())
+
+
+def lqcd_spinor_bytes():
+    return int(_lib.lqcd_spinor_bytes())
+
+
+def lqcd_launch_count():
+    return int(_lib.lqcd_launch_count())
+
+
+def lqcd_pack_gauge(canon_dev, internal_dev):
+    return _check(_lib.lqcd_pack_gauge(_ptr(canon_dev), _ptr(internal_dev)))
+
+
+def lqcd_pack_spinor(canon_dev, internal_dev, parity):
+    return _check(_lib.lqcd_pack_spinor(_ptr(canon_dev), _ptr(internal_dev), parity))
+
+
+def lqcd_unpack_spinor(internal_dev, canon_dev, parity):
+    return _check(_lib.lqcd_unpack_spinor(_ptr(internal_dev), _ptr(canon_dev), parity))
+
+
+def lqcd_dslash_eo(gauge, inp, out, parity, kappa):
+    return _check(_lib.lqcd_dslash_eo(_ptr(gauge), _ptr(inp), _ptr(out), parity, kappa))
+
+
+def lqcd_mtm(gauge, inp, out, kappa, mu, dagger):
+    return _check(_lib.lqcd_mtm(_ptr(gauge), _ptr(inp), _ptr(out), kappa, mu, dagger))
+
+
+def lqcd_cg_mdagm(gauge, b, x, kappa, mu, tol, maxit):
+    return _check(_lib.lqcd_cg_mdagm(_ptr(gauge), _ptr(b), _ptr(x), kappa, mu, tol, maxit))
+
+
+def lqcd_cg_setup(gauge, b, x, kappa, mu, tol):
+    return _check(_lib.lqcd_cg_setup(_ptr(gauge), _ptr(b), _ptr(x), kappa, mu, tol))
+
+
+def lqcd_cg_iterate(n):
+    return _check(_lib.lqcd_cg_iterate(n))
+
+
+def lqcd_cg_finish():
+    return _check(_lib.lqcd_cg_finish())
+
+
+def lqcd_cg_stats():
+    it = ctypes.c_int(0)
+    rr = ctypes.c_double(0.0)
+    rt = ctypes.c_double(0.0)
+    _check(_lib.lqcd_cg_stats(ctypes.byref(it), ctypes.byref(rr), ctypes.byref(rt)))
+    return it.value, rr.value, rt.value
+
+
+def lqcd_mtm_host(gauge_canon_host, in_canon_host, out_canon_host, kappa, mu, dagger):
+    return _check(_lib.lqcd_mtm_host(_ptr(gauge_canon_host), _ptr(in_canon_host), _ptr(out_canon_host),
+                                     kappa, mu, dagger))
+
+
+def lqcd_cg_mdagm_host(gauge_canon_host, b_canon_host, x_canon_host, kappa, mu, tol, maxit):
+    return _check(_lib.lqcd_cg_mdagm_host(_ptr(gauge_canon_host), _ptr(b_canon_host), _ptr(x_canon_host),
+                                          kappa, mu, tol, maxit))
+
+
+# ---------------------------------------------------------------------------- buffer helpers
+def alloc_gauge(device="cuda"):
+    """Uninitialised device buffer for one internal gauge field (current format)."""
+    return torch.empty(lqcd_gauge_bytes(), dtype=torch.uint8, device=device)
+
+
+def alloc_spinor(device="cuda"):
+    """Uninitialised device buffer for one internal half-spinor field (current format)."""
+    return torch.empty(lqcd_spinor_bytes(), dtype=torch.uint8, device=device)
+
+
+def upload_gauge(U_canon, device="cuda"):
+    """numpy (V,4,3,3) complex128 -> packed internal device buffer."""
+    canon = torch.from_numpy(np.ascontiguousarray(U_canon)).to(device)
+    g = alloc_gauge(device)
+    lqcd_pack_gauge(canon, g)
+    return g
+
+
+def upload_spinor(psi_canon, parity, device="cuda"):
+    """numpy (V/2,4,3) complex128 -> packed internal device buffer."""
+    canon = torch.from_numpy(np.ascontiguousarray(psi_canon)).to(device)
+    s = alloc_spinor(device)
+    lqcd_pack_spinor(canon, s, parity)
+    return s
+
+
+def download_spinor(s_internal, parity):
+    """packed internal device buffer -> numpy (V/2,4,3) complex128."""
+    n_sites = lqcd_spinor_bytes() // (192 if _fmt["precision"] == LQCD_DOUBLE else 96)
+    canon = torch.empty((n_sites, 4, 3), dtype=torch.complex128, device=s_internal.device)
+    lqcd_unpack_spinor(s_internal, canon, parity)
+    return canon.cpu().numpy()

@@ -1,0 +1,445 @@
+// api.cu -- the C ABI of include/lqcd.h: context, argument checks, the composition of
+// Mhat / Mhat^dag from two hopping launches with fused epilogues, and the CG driver.
+//
+// Mhat(mu)     = M_ee - D_eo M_oo^{-1} D_oe                     (reading G3)
+// Mhat(mu)^dag = M_ee^dag - D_eo^adj (M_oo^{-1})^dag D_oe^adj   (adjoint stencil, c -> -c)
+// with c = 2 kappa mu, M = 1 + i c gamma5, M^{-1} = (1 - i c gamma5)/(1 + c^2), so per
+// chirality chi = +-1 the diagonal terms are the complex numbers (1 + i c chi) and
+// (1 - i c chi)/(1 + c^2); they are folded into the hopping kernel's epilogue:
+//   launch 1: t   = [-kappa (1 - i c chi)/(1 + c^2)] * bracket(in)          (odd sites)
+//   launch 2: out = (1 + i c chi) in + kappa * bracket(t)                  (even sites)
+#include <atomic>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+
+#include "../../include/lqcd.h"
+#include "lqcd_internal.h"
+
+namespace lqcd {
+
+static std::atomic<long long> g_launches{0};
+void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+namespace {
+
+struct Context {
+    bool init = false;
+    int dims[4] = {0, 0, 0, 0};
+    Geometry geo;
+    int precision = LQCD_DOUBLE;
+    int recon = 18;
+    int block = 128;
+    cudaStream_t stream = 0;
+
+    // workspace (owned)
+    size_t ws_spinor_bytes = 0;
+    void* vec[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};  // r, p, q, t1, t2
+    CgScalars* scal = nullptr;
+    CgScalars* scal_host = nullptr;  // pinned, 2 slots
+    cudaEvent_t ev[2] = {nullptr, nullptr};
+    double* partials = nullptr;
+    unsigned int* ticket = nullptr;
+    size_t n_partials = 0;
+
+    // host-call staging (owned)
+    void* st_gauge_canon = nullptr; size_t st_gauge_canon_bytes = 0;
+    void* st_gauge = nullptr;       size_t st_gauge_bytes = 0;
+    void* st_spinor_canon = nullptr; size_t st_spinor_canon_bytes = 0;
+    void* st_in = nullptr;  size_t st_in_bytes = 0;
+    void* st_out = nullptr; size_t st_out_bytes = 0;
+
+    // current solve
+    const void* cg_gauge = nullptr;
+    const void* cg_b = nullptr;
+    void* cg_x = nullptr;
+    double cg_kappa = 0, cg_mu = 0, cg_tol = 0;
+    bool cg_active = false;
+    int st_iters = 0;
+    double st_rr = 0, st_rt = 0;
+};
+
+Context ctx;
+char g_err[512] = "";
+
+int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+int cuda_fail(cudaError_t e, const char* what) {
+    return fail(LQCD_CUDA_ERROR, "%s: %s", what, cudaGetErrorString(e));
+}
+
+#define CU(call)                                                  \
+    do {                                                          \
+        cudaError_t e_ = (call);                                  \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #call);       \
+    } while (0)
+
+size_t spinor_bytes_of(int precision, int Vh) { return (size_t)Vh * 12 * (precision == 0 ? 16 : 8); }
+size_t gauge_bytes_of(int precision, int recon, int Vh) {
+    return (size_t)Vh * 8 * recon * (precision == 0 ? 8 : 4);
+}
+
+void free_workspace() {
+    for (int i = 0; i < 5; ++i) { if (ctx.vec[i]) cudaFree(ctx.vec[i]); ctx.vec[i] = nullptr; }
+    ctx.ws_spinor_bytes = 0;
+}
+
+void free_all() {
+    free_workspace();
+    if (ctx.scal) cudaFree(ctx.scal);
+    if (ctx.scal_host) cudaFreeHost(ctx.scal_host);
+    if (ctx.partials) cudaFree(ctx.partials);
+    if (ctx.ticket) cudaFree(ctx.ticket);
+    for (int i = 0; i < 2; ++i) if (ctx.ev[i]) cudaEventDestroy(ctx.ev[i]);
+    void** st[] = {&ctx.st_gauge_canon, &ctx.st_gauge, &ctx.st_spinor_canon, &ctx.st_in, &ctx.st_out};
+    for (void** p : st) { if (*p) cudaFree(*p); *p = nullptr; }
+    ctx = Context();
+}
+
+int ensure_scalars() {
+    if (!ctx.scal) {
+        CU(cudaMalloc(&ctx.scal, sizeof(CgScalars)));
+        CU(cudaMemset(ctx.scal, 0, sizeof(CgScalars)));
+        CU(cudaMallocHost(&ctx.scal_host, 2 * sizeof(CgScalars)));
+        CU(cudaMalloc(&ctx.ticket, sizeof(unsigned int)));
+        CU(cudaMemset(ctx.ticket, 0, sizeof(unsigned int)));
+        for (int i = 0; i < 2; ++i) CU(cudaEventCreateWithFlags(&ctx.ev[i], cudaEventDisableTiming));
+    }
+    const size_t need = (size_t)ctx.geo.Vh / 32 + 64 + (size_t)vector_grid((size_t)24 * ctx.geo.Vh);
+    if (need > ctx.n_partials) {
+        if (ctx.partials) CU(cudaFree(ctx.partials));
+        ctx.partials = nullptr;
+        CU(cudaMalloc(&ctx.partials, need * sizeof(double)));
+        ctx.n_partials = need;
+    }
+    return LQCD_OK;
+}
+
+int ensure_workspace(int nvec) {
+    int rc = ensure_scalars();
+    if (rc) return rc;
+    const size_t sb = spinor_bytes_of(ctx.precision, ctx.geo.Vh);
+    if (ctx.ws_spinor_bytes != sb) free_workspace();
+    ctx.ws_spinor_bytes = sb;
+    // t1 (index 3) is needed by lqcd_mtm; the rest only by CG
+    const int order[5] = {3, 4, 0, 1, 2};
+    for (int k = 0; k < nvec; ++k) {
+        const int i = order[k];
+        if (!ctx.vec[i]) CU(cudaMalloc(&ctx.vec[i], sb));
+    }
+    return LQCD_OK;
+}
+
+int ensure_buf(void** p, size_t* have, size_t need) {
+    if (*have >= need) return LQCD_OK;
+    if (*p) CU(cudaFree(*p));
+    *p = nullptr; *have = 0;
+    CU(cudaMalloc(p, need));
+    *have = need;
+    return LQCD_OK;
+}
+
+Reduction red() { Reduction r; r.partials = ctx.partials; r.ticket = ctx.ticket; return r; }
+
+int check_scalar(double v, const char* name) {
+    if (!std::isfinite(v)) return fail(LQCD_BAD_ARG, "%s is not finite", name);
+    return LQCD_OK;
+}
+
+// The two hopping launches of Mhat (dagger = 0) or Mhat^dag (dagger = 1) on even half fields.
+// norm_to_pAp: also reduce |out|^2 into scal->pAp (CG's <p, A p> = |Mhat p|^2).
+// scal: device scalars whose `done` flag turns the launches into no-ops (CG), or null.
+int apply_mhat(const void* gauge, const void* in, void* tmp_odd, void* out, double kappa, double mu,
+               int dagger, bool norm_to_pAp, CgScalars* scal) {
+    const double c = (dagger ? -1.0 : 1.0) * 2.0 * kappa * mu;
+    const double d = 1.0 + c * c;
+    Epilogue e1 = {};
+    e1.cu_re = -kappa / d; e1.cu_im = +kappa * c / d;   // -kappa (1 - i c)/(1 + c^2), chi = +1
+    e1.cd_re = -kappa / d; e1.cd_im = -kappa * c / d;   // chi = -1
+    CU(launch_hopping(ctx.precision, ctx.recon, dagger, 0, ctx.geo, e1, gauge, in, tmp_odd, nullptr, 1,
+                      red(), scal, ctx.block, ctx.stream));
+    Epilogue e2 = {};
+    e2.cu_re = kappa; e2.cd_re = kappa;
+    e2.du_re = 1.0; e2.du_im = c;
+    e2.dd_re = 1.0; e2.dd_im = -c;
+    CU(launch_hopping(ctx.precision, ctx.recon, dagger, norm_to_pAp ? 2 : 1, ctx.geo, e2, gauge, tmp_odd,
+                      out, in, 0, red(), scal, ctx.block, ctx.stream));
+    return LQCD_OK;
+}
+
+int enqueue_iteration() {
+    void *r = ctx.vec[0], *p = ctx.vec[1], *q = ctx.vec[2], *t1 = ctx.vec[3], *t2 = ctx.vec[4];
+    const size_t n = (size_t)24 * ctx.geo.Vh;
+    int rc = apply_mhat(ctx.cg_gauge, p, t1, t2, ctx.cg_kappa, ctx.cg_mu, 0, true, ctx.scal);
+    if (rc) return rc;
+    rc = apply_mhat(ctx.cg_gauge, t2, t1, q, ctx.cg_kappa, ctx.cg_mu, 1, false, ctx.scal);
+    if (rc) return rc;
+    CU(launch_cg_update_xr(ctx.precision, n, ctx.cg_x, r, p, q, red(), ctx.scal, ctx.stream));
+    CU(launch_cg_update_p(ctx.precision, n, p, r, ctx.scal, ctx.stream));
+    return LQCD_OK;
+}
+
+}  // namespace
+}  // namespace lqcd
+
+using namespace lqcd;
+
+extern "C" {
+
+const char* lqcd_last_error(void) { return g_err; }
+
+int lqcd_init(const int dims[4], const double bc_phase[8]) {
+    if (!dims || !bc_phase) return fail(LQCD_BAD_ARG, "lqcd_init: null argument");
+    long long V = 1;
+    for (int m = 0; m < 4; ++m) {
+        if (dims[m] < 2 || (dims[m] & 1)) return fail(LQCD_BAD_DIMS, "extent %d = %d must be even and >= 2", m, dims[m]);
+        V *= dims[m];
+        const double a = std::hypot(bc_phase[2 * m], bc_phase[2 * m + 1]);
+        if (!std::isfinite(a) || std::fabs(a - 1.0) > 1e-12)
+            return fail(LQCD_BAD_DIMS, "|bc_phase[%d]| = %g must be 1", m, a);
+    }
+    if (V / 2 > (1LL << 30)) return fail(LQCD_BAD_DIMS, "lattice too large for 32-bit site indices");
+    if (ctx.init) free_all();
+    ctx.init = true;
+    for (int m = 0; m < 4; ++m) {
+        ctx.dims[m] = dims[m];
+        ctx.geo.ph_re[m] = bc_phase[2 * m];
+        ctx.geo.ph_im[m] = bc_phase[2 * m + 1];
+    }
+    ctx.geo.N0h = dims[0] / 2; ctx.geo.N1 = dims[1]; ctx.geo.N2 = dims[2]; ctx.geo.N3 = dims[3];
+    ctx.geo.Vh = (int)(V / 2);
+    ctx.precision = LQCD_DOUBLE; ctx.recon = 18; ctx.block = 128; ctx.stream = 0;
+    g_launches.store(0);
+    g_err[0] = 0;
+    return LQCD_OK;
+}
+
+int lqcd_finalize(void) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "lqcd_finalize: not initialised");
+    cudaDeviceSynchronize();
+    free_all();
+    return LQCD_OK;
+}
+
+int lqcd_set_stream(void* cuda_stream) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    ctx.stream = (cudaStream_t)cuda_stream;
+    return LQCD_OK;
+}
+
+int lqcd_set_format(int precision, int recon) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (precision != LQCD_DOUBLE && precision != LQCD_SINGLE) return fail(LQCD_BAD_ARG, "precision must be 0 or 1");
+    if (recon != 18 && recon != 12) return fail(LQCD_BAD_ARG, "recon must be 18 or 12");
+    ctx.precision = precision; ctx.recon = recon; ctx.cg_active = false;
+    return LQCD_OK;
+}
+
+int lqcd_set_block_size(int threads) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (threads == 0) threads = 128;
+    if (threads < 32 || threads > 128 || (threads % 32)) return fail(LQCD_BAD_ARG, "block size must be 32, 64, 96 or 128");
+    ctx.block = threads;
+    return LQCD_OK;
+}
+
+size_t lqcd_gauge_bytes(void) { return ctx.init ? gauge_bytes_of(ctx.precision, ctx.recon, ctx.geo.Vh) : 0; }
+size_t lqcd_spinor_bytes(void) { return ctx.init ? spinor_bytes_of(ctx.precision, ctx.geo.Vh) : 0; }
+long long lqcd_launch_count(void) { return g_launches.load(); }
+
+int lqcd_pack_gauge(const void* canon_dev, void* internal_dev) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (!canon_dev || !internal_dev) return fail(LQCD_BAD_ARG, "lqcd_pack_gauge: null pointer");
+    CU(launch_pack_gauge(ctx.precision, ctx.recon, ctx.geo, canon_dev, internal_dev, ctx.stream));
+    return LQCD_OK;
+}
+
+int lqcd_pack_spinor(const void* canon_dev, void* internal_dev, int parity) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (!canon_dev || !internal_dev) return fail(LQCD_BAD_ARG, "lqcd_pack_spinor: null pointer");
+    if (parity != 0 && parity != 1) return fail(LQCD_BAD_ARG, "parity must be 0 or 1");
+    CU(launch_pack_spinor(ctx.precision, ctx.geo, canon_dev, internal_dev, parity, ctx.stream));
+    return LQCD_OK;
+}
+
+int lqcd_unpack_spinor(const void* internal_dev, void* canon_dev, int parity) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (!canon_dev || !internal_dev) return fail(LQCD_BAD_ARG, "lqcd_unpack_spinor: null pointer");
+    if (parity != 0 && parity != 1) return fail(LQCD_BAD_ARG, "parity must be 0 or 1");
+    CU(launch_unpack_spinor(ctx.precision, ctx.geo, internal_dev, canon_dev, parity, ctx.stream));
+    return LQCD_OK;
+}
+
+int lqcd_dslash_eo(const void* gauge, const void* in, void* out, int parity, double kappa) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (!gauge || !in || !out) return fail(LQCD_BAD_ARG, "lqcd_dslash_eo: null pointer");
+    if (in == out) return fail(LQCD_BAD_ARG, "lqcd_dslash_eo: in and out alias");
+    if (parity != 0 && parity != 1) return fail(LQCD_BAD_ARG, "parity must be 0 or 1");
+    int rc = check_scalar(kappa, "kappa");
+    if (rc) return rc;
+    Epilogue ep = {};
+    ep.cu_re = -kappa; ep.cd_re = -kappa;
+    Reduction none = {nullptr, nullptr};
+    CU(launch_hopping(ctx.precision, ctx.recon, 0, 0, ctx.geo, ep, gauge, in, out, nullptr, parity, none,
+                      nullptr, ctx.block, ctx.stream));
+    return LQCD_OK;
+}
+
+int lqcd_mtm(const void* gauge, const void* in, void* out, double kappa, double mu, int dagger) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (!gauge || !in || !out) return fail(LQCD_BAD_ARG, "lqcd_mtm: null pointer");
+    if (in == out) return fail(LQCD_BAD_ARG, "lqcd_mtm: in and out alias");
+    if (dagger != 0 && dagger != 1) return fail(LQCD_BAD_ARG, "dagger must be 0 or 1");
+    int rc = check_scalar(kappa, "kappa");
+    if (rc) return rc;
+    rc = check_scalar(mu, "mu");
+    if (rc) return rc;
+    rc = ensure_workspace(1);
+    if (rc) return rc;
+    return apply_mhat(gauge, in, ctx.vec[3], out, kappa, mu, dagger, false, nullptr);
+}
+
+int lqcd_cg_setup(const void* gauge, const void* b, void* x, double kappa, double mu, double tol) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (!gauge || !b || !x) return fail(LQCD_BAD_ARG, "lqcd_cg_setup: null pointer");
+    if (b == x) return fail(LQCD_BAD_ARG, "lqcd_cg_setup: b and x alias");
+    int rc = check_scalar(kappa, "kappa");
+    if (rc) return rc;
+    rc = check_scalar(mu, "mu");
+    if (rc) return rc;
+    if (!std::isfinite(tol) || tol < 0.0) return fail(LQCD_BAD_ARG, "tol must be finite and >= 0");
+    rc = ensure_workspace(5);
+    if (rc) return rc;
+    ctx.cg_gauge = gauge; ctx.cg_b = b; ctx.cg_x = x;
+    ctx.cg_kappa = kappa; ctx.cg_mu = mu; ctx.cg_tol = tol;
+    CU(launch_cg_init(ctx.precision, (size_t)24 * ctx.geo.Vh, b, x, ctx.vec[0], ctx.vec[1], tol, red(),
+                      ctx.scal, ctx.stream));
+    ctx.cg_active = true;
+    return LQCD_OK;
+}
+
+int lqcd_cg_iterate(int n) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (!ctx.cg_active) return fail(LQCD_BAD_ARG, "lqcd_cg_iterate: no solve set up");
+    if (n < 0) return fail(LQCD_BAD_ARG, "n must be >= 0");
+    for (int i = 0; i < n; ++i) {
+        int rc = enqueue_iteration();
+        if (rc) return rc;
+    }
+    return LQCD_OK;
+}
+
+int lqcd_cg_finish(void) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (!ctx.cg_active) return fail(LQCD_BAD_ARG, "lqcd_cg_finish: no solve set up");
+    // true residual |b - A x|: q = A x with the `done` gate off
+    void *q = ctx.vec[2], *t1 = ctx.vec[3], *t2 = ctx.vec[4];
+    int rc = apply_mhat(ctx.cg_gauge, ctx.cg_x, t1, t2, ctx.cg_kappa, ctx.cg_mu, 0, false, nullptr);
+    if (rc) return rc;
+    rc = apply_mhat(ctx.cg_gauge, t2, t1, q, ctx.cg_kappa, ctx.cg_mu, 1, false, nullptr);
+    if (rc) return rc;
+    CU(launch_true_resid(ctx.precision, (size_t)24 * ctx.geo.Vh, ctx.cg_b, q, red(), ctx.scal, ctx.stream));
+    CU(cudaMemcpyAsync(ctx.scal_host, ctx.scal, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx.stream));
+    CU(cudaStreamSynchronize(ctx.stream));
+    const CgScalars& s = ctx.scal_host[0];
+    ctx.st_iters = s.iters;
+    ctx.st_rr = s.bb > 0 ? std::sqrt(s.rho / s.bb) : 0.0;
+    ctx.st_rt = s.bb > 0 ? std::sqrt(s.resid_true / s.bb) : 0.0;
+    ctx.cg_active = false;
+    if (s.status == LQCD_BREAKDOWN) return fail(LQCD_BREAKDOWN, "CG breakdown: <p,Ap> = %g", s.pAp);
+    return s.status;
+}
+
+int lqcd_cg_mdagm(const void* gauge, const void* b, void* x, double kappa, double mu, double tol,
+                  int maxit) {
+    if (maxit < 1) return fail(LQCD_BAD_ARG, "maxit must be >= 1");
+    int rc = lqcd_cg_setup(gauge, b, x, kappa, mu, tol);
+    if (rc) return rc;
+    // Enqueue iterations in chunks; the convergence flag of chunk k is read back while
+    // chunk k+1 is already queued, so the device never idles on the host.
+    const int chunk = 4;
+    int launched = 0, slot = 0;
+    bool pending[2] = {false, false};
+    bool stop = false;
+    while (launched < maxit && !stop) {
+        const int n = (maxit - launched < chunk) ? (maxit - launched) : chunk;
+        rc = lqcd_cg_iterate(n);
+        if (rc) return rc;
+        launched += n;
+        CU(cudaMemcpyAsync(&ctx.scal_host[slot], ctx.scal, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx.stream));
+        CU(cudaEventRecord(ctx.ev[slot], ctx.stream));
+        pending[slot] = true;
+        const int prev = slot ^ 1;
+        if (pending[prev]) {
+            CU(cudaEventSynchronize(ctx.ev[prev]));
+            pending[prev] = false;
+            if (ctx.scal_host[prev].done) stop = true;
+        }
+        slot ^= 1;
+    }
+    return lqcd_cg_finish();
+}
+
+int lqcd_cg_stats(int* iters, double* rel_resid_recursive, double* rel_resid_true) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (iters) *iters = ctx.st_iters;
+    if (rel_resid_recursive) *rel_resid_recursive = ctx.st_rr;
+    if (rel_resid_true) *rel_resid_true = ctx.st_rt;
+    return LQCD_OK;
+}
+
+static int stage_inputs(const void* gauge_host, const void* spinor_host) {
+    const size_t V = 2 * (size_t)ctx.geo.Vh;
+    const size_t gc = V * 576, sc = (size_t)ctx.geo.Vh * 192;
+    int rc;
+    if ((rc = ensure_buf(&ctx.st_gauge_canon, &ctx.st_gauge_canon_bytes, gc))) return rc;
+    if ((rc = ensure_buf(&ctx.st_gauge, &ctx.st_gauge_bytes, lqcd_gauge_bytes()))) return rc;
+    if ((rc = ensure_buf(&ctx.st_spinor_canon, &ctx.st_spinor_canon_bytes, sc))) return rc;
+    if ((rc = ensure_buf(&ctx.st_in, &ctx.st_in_bytes, lqcd_spinor_bytes()))) return rc;
+    if ((rc = ensure_buf(&ctx.st_out, &ctx.st_out_bytes, lqcd_spinor_bytes()))) return rc;
+    CU(cudaMemcpyAsync(ctx.st_gauge_canon, gauge_host, gc, cudaMemcpyHostToDevice, ctx.stream));
+    CU(cudaMemcpyAsync(ctx.st_spinor_canon, spinor_host, sc, cudaMemcpyHostToDevice, ctx.stream));
+    if ((rc = lqcd_pack_gauge(ctx.st_gauge_canon, ctx.st_gauge))) return rc;
+    if ((rc = lqcd_pack_spinor(ctx.st_spinor_canon, ctx.st_in, 0))) return rc;
+    return LQCD_OK;
+}
+
+static int fetch_output(void* out_host) {
+    const size_t sc = (size_t)ctx.geo.Vh * 192;
+    int rc = lqcd_unpack_spinor(ctx.st_out, ctx.st_spinor_canon, 0);
+    if (rc) return rc;
+    CU(cudaMemcpyAsync(out_host, ctx.st_spinor_canon, sc, cudaMemcpyDeviceToHost, ctx.stream));
+    CU(cudaStreamSynchronize(ctx.stream));
+    return LQCD_OK;
+}
+
+int lqcd_mtm_host(const void* gauge_canon_host, const void* in_canon_host, void* out_canon_host,
+                  double kappa, double mu, int dagger) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (!gauge_canon_host || !in_canon_host || !out_canon_host) return fail(LQCD_BAD_ARG, "lqcd_mtm_host: null pointer");
+    int rc = stage_inputs(gauge_canon_host, in_canon_host);
+    if (rc) return rc;
+    if ((rc = lqcd_mtm(ctx.st_gauge, ctx.st_in, ctx.st_out, kappa, mu, dagger))) return rc;
+    return fetch_output(out_canon_host);
+}
+
+int lqcd_cg_mdagm_host(const void* gauge_canon_host, const void* b_canon_host, void* x_canon_host,
+                       double kappa, double mu, double tol, int maxit) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (!gauge_canon_host || !b_canon_host || !x_canon_host) return fail(LQCD_BAD_ARG, "lqcd_cg_mdagm_host: null pointer");
+    int rc = stage_inputs(gauge_canon_host, b_canon_host);
+    if (rc) return rc;
+    const int status = lqcd_cg_mdagm(ctx.st_gauge, ctx.st_in, ctx.st_out, kappa, mu, tol, maxit);
+    if (status < 0) return status;
+    rc = fetch_output(x_canon_host);
+    return rc ? rc : status;
+}
+
+}  // extern "C"

@@ -1,0 +1,364 @@
+// hopping.cu -- the hopping term D_eo / D_oe of eq. 6 with fused
+// diagonal-term epilogues, hand-written for sm_100a.
+//
+// One thread per output site.  Per site:
+//   a1 site -> coordinates -> 8 neighbour indices and wrap flags (integer only)
+//   a2 4 forward links U_mu(x) (own-parity array, own index: coalesced) and
+//      4 backward links U_mu(x-mu) (other-parity array, neighbour's index);
+//      every link of the lattice is read exactly once per application, so the
+//      gauge loads are streamed (ld.global.cs: evict-first, no reuse expected)
+//   a3 neighbour spinor -> spin projection to a half spinor (12 -> 6 complex);
+//      neighbour spinors are reused by 8 output sites, so they go through the
+//      read-only path with default caching (L1 for x/y neighbours, L2 for z/t)
+//   a4 SU(3) x half spinor (U h forward, U^dag h backward)
+//   a5 boundary phase on the hop that wraps, reconstruction to 4 spin rows, accumulate
+//   a6/a7 epilogue: out = c_chi * acc (+ d_chi * aux), c, d complex per chirality:
+//      covers -kappa (dslash_eo), M_oo^{-1} D_oe, and M_ee in - D_eo (.) in one store.
+//
+// Spin projection table (gamma basis of include/lqcd.h; reading G4),
+// (1 + S gamma_mu) psi = (h0, h1, conj(c0) h0 or h1 ...):
+//   h0 = psi_0 + c0 psi_j0,  h1 = psi_1 + c1 psi_j1,  j1 = 5 - j0,
+//   row j0 of the result = conj(c0) h0, row j1 = conj(c1) h1.
+//   S = -1:  mu=x: j0=3 c0=+i c1=+i | y: j0=3 c0=+1 c1=-1 | z: j0=2 c0=+i c1=-i | t: j0=2 c0=-1 c1=-1
+//   S = +1:  all c negated.
+// Forward hops of the operator use S = -1, backward hops S = +1; the adjoint
+// stencil (DAG) swaps them.
+#include "lqcd_internal.h"
+
+#ifndef LQCD_HOP_MIN_BLOCKS
+#define LQCD_HOP_MIN_BLOCKS 3
+#endif
+
+namespace lqcd {
+namespace {
+
+// ----------------------------------------------------------------------------- field access
+__device__ __forceinline__ void load_spinor(const void* base, int Vh, int idx, double (&psi)[24]) {
+    const double2* p = reinterpret_cast<const double2*>(base) + idx;
+#pragma unroll
+    for (int c = 0; c < 12; ++c) {
+        const double2 v = __ldg(p + (size_t)c * Vh);
+        psi[2 * c] = v.x;
+        psi[2 * c + 1] = v.y;
+    }
+}
+__device__ __forceinline__ void load_spinor(const void* base, int Vh, int idx, float (&psi)[24]) {
+    const float4* p = reinterpret_cast<const float4*>(base) + idx;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        const float4 v = __ldg(p + (size_t)k * Vh);
+        psi[4 * k] = v.x;
+        psi[4 * k + 1] = v.y;
+        psi[4 * k + 2] = v.z;
+        psi[4 * k + 3] = v.w;
+    }
+}
+__device__ __forceinline__ void store_spinor(void* base, int Vh, int idx, const double (&o)[24]) {
+    double2* p = reinterpret_cast<double2*>(base) + idx;
+#pragma unroll
+    for (int c = 0; c < 12; ++c) p[(size_t)c * Vh] = make_double2(o[2 * c], o[2 * c + 1]);
+}
+__device__ __forceinline__ void store_spinor(void* base, int Vh, int idx, const float (&o)[24]) {
+    float4* p = reinterpret_cast<float4*>(base) + idx;
+#pragma unroll
+    for (int k = 0; k < 6; ++k)
+        p[(size_t)k * Vh] = make_float4(o[4 * k], o[4 * k + 1], o[4 * k + 2], o[4 * k + 3]);
+}
+
+// third row of an SU(3) matrix from the first two: row2 = conj(row0 x row1)  (G9)
+template <typename T>
+__device__ __forceinline__ void reconstruct_row2(T (&u)[18]) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
+        // (row0 x row1)_c = u0[c1] u1[c2] - u0[c2] u1[c1]
+        const T ar = u[2 * c1], ai = u[2 * c1 + 1], br = u[6 + 2 * c2], bi = u[6 + 2 * c2 + 1];
+        const T cr = u[2 * c2], ci = u[2 * c2 + 1], dr = u[6 + 2 * c1], di = u[6 + 2 * c1 + 1];
+        const T re = (ar * br - ai * bi) - (cr * dr - ci * di);
+        const T im = (ar * bi + ai * br) - (cr * di + ci * dr);
+        u[12 + 2 * c] = re;
+        u[12 + 2 * c + 1] = -im;
+    }
+}
+
+template <int RECON>
+__device__ __forceinline__ void load_link(const void* gauge, int Vh, int par, int mu, int idx,
+                                          double (&u)[18]) {
+    const double2* p =
+        reinterpret_cast<const double2*>(gauge) + (size_t)((par * 4 + mu) * (RECON / 2)) * Vh + idx;
+#pragma unroll
+    for (int j = 0; j < RECON / 2; ++j) {
+        const double2 v = __ldcs(p + (size_t)j * Vh);
+        u[2 * j] = v.x;
+        u[2 * j + 1] = v.y;
+    }
+    if (RECON == 12) reconstruct_row2(u);
+}
+template <int RECON>
+__device__ __forceinline__ void load_link(const void* gauge, int Vh, int par, int mu, int idx,
+                                          float (&u)[18]) {
+    if (RECON == 12) {
+        const float4* p =
+            reinterpret_cast<const float4*>(gauge) + (size_t)((par * 4 + mu) * 3) * Vh + idx;
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            const float4 v = __ldcs(p + (size_t)j * Vh);
+            u[4 * j] = v.x;
+            u[4 * j + 1] = v.y;
+            u[4 * j + 2] = v.z;
+            u[4 * j + 3] = v.w;
+        }
+        reconstruct_row2(u);
+    } else {
+        const float* blk = reinterpret_cast<const float*>(gauge) + (size_t)(par * 4 + mu) * 18 * Vh;
+        const float4* p = reinterpret_cast<const float4*>(blk) + idx;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const float4 v = __ldcs(p + (size_t)j * Vh);
+            u[4 * j] = v.x;
+            u[4 * j + 1] = v.y;
+            u[4 * j + 2] = v.z;
+            u[4 * j + 3] = v.w;
+        }
+        const float2 w = __ldcs(reinterpret_cast<const float2*>(blk + (size_t)16 * Vh) + idx);
+        u[16] = w.x;
+        u[17] = w.y;
+    }
+}
+
+// ----------------------------------------------------------------------------- spin algebra
+// o = a + c b with c = i^C  (C: 0 -> +1, 1 -> +i, 2 -> -1, 3 -> -i)
+template <int C, typename T>
+__device__ __forceinline__ void add_c(T& ore, T& oim, T are, T aim, T bre, T bim) {
+    if (C == 0) { ore = are + bre; oim = aim + bim; }
+    if (C == 1) { ore = are - bim; oim = aim + bre; }
+    if (C == 2) { ore = are - bre; oim = aim - bim; }
+    if (C == 3) { ore = are + bim; oim = aim - bre; }
+}
+
+template <int MU, int S>
+struct Proj {
+    static constexpr int j0 = (MU < 2) ? 3 : 2;
+    static constexpr int j1 = 5 - j0;
+    static constexpr int c0m = (MU == 0) ? 1 : (MU == 1) ? 0 : (MU == 2) ? 1 : 2;  // S = -1 table
+    static constexpr int c1m = (MU == 0) ? 1 : (MU == 1) ? 2 : (MU == 2) ? 3 : 2;
+    static constexpr int c0 = (S < 0) ? c0m : (c0m + 2) % 4;
+    static constexpr int c1 = (S < 0) ? c1m : (c1m + 2) % 4;
+    static constexpr int c0conj = (4 - c0) % 4;
+    static constexpr int c1conj = (4 - c1) % 4;
+};
+
+// h[k][a], k = 0,1: index 2*(3k+a)
+template <int MU, int S, typename T>
+__device__ __forceinline__ void project(const T (&psi)[24], T (&h)[12]) {
+    typedef Proj<MU, S> P;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        add_c<P::c0>(h[2 * a], h[2 * a + 1], psi[2 * a], psi[2 * a + 1], psi[2 * (3 * P::j0 + a)],
+                     psi[2 * (3 * P::j0 + a) + 1]);
+        add_c<P::c1>(h[2 * (3 + a)], h[2 * (3 + a) + 1], psi[2 * (3 + a)], psi[2 * (3 + a) + 1],
+                     psi[2 * (3 * P::j1 + a)], psi[2 * (3 * P::j1 + a) + 1]);
+    }
+}
+
+template <int MU, int S, typename T>
+__device__ __forceinline__ void accumulate(T (&acc)[24], const T (&chi)[12]) {
+    typedef Proj<MU, S> P;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        acc[2 * a] += chi[2 * a];
+        acc[2 * a + 1] += chi[2 * a + 1];
+        acc[2 * (3 + a)] += chi[2 * (3 + a)];
+        acc[2 * (3 + a) + 1] += chi[2 * (3 + a) + 1];
+        add_c<P::c0conj>(acc[2 * (3 * P::j0 + a)], acc[2 * (3 * P::j0 + a) + 1],
+                         acc[2 * (3 * P::j0 + a)], acc[2 * (3 * P::j0 + a) + 1], chi[2 * a],
+                         chi[2 * a + 1]);
+        add_c<P::c1conj>(acc[2 * (3 * P::j1 + a)], acc[2 * (3 * P::j1 + a) + 1],
+                         acc[2 * (3 * P::j1 + a)], acc[2 * (3 * P::j1 + a) + 1], chi[2 * (3 + a)],
+                         chi[2 * (3 + a) + 1]);
+    }
+}
+
+// chi_{k,a} = sum_b U_ab h_{k,b}
+template <typename T>
+__device__ __forceinline__ void su3_mul(const T (&u)[18], const T (&h)[12], T (&chi)[12]) {
+#pragma unroll
+    for (int k = 0; k < 2; ++k)
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            T re = 0, im = 0;
+#pragma unroll
+            for (int b = 0; b < 3; ++b) {
+                const T ur = u[2 * (3 * a + b)], ui = u[2 * (3 * a + b) + 1];
+                const T hr = h[2 * (3 * k + b)], hi = h[2 * (3 * k + b) + 1];
+                re += ur * hr - ui * hi;
+                im += ur * hi + ui * hr;
+            }
+            chi[2 * (3 * k + a)] = re;
+            chi[2 * (3 * k + a) + 1] = im;
+        }
+}
+
+// chi_{k,a} = sum_b conj(U_ba) h_{k,b}
+template <typename T>
+__device__ __forceinline__ void su3_dag_mul(const T (&u)[18], const T (&h)[12], T (&chi)[12]) {
+#pragma unroll
+    for (int k = 0; k < 2; ++k)
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            T re = 0, im = 0;
+#pragma unroll
+            for (int b = 0; b < 3; ++b) {
+                const T ur = u[2 * (3 * b + a)], ui = u[2 * (3 * b + a) + 1];
+                const T hr = h[2 * (3 * k + b)], hi = h[2 * (3 * k + b) + 1];
+                re += ur * hr + ui * hi;
+                im += ur * hi - ui * hr;
+            }
+            chi[2 * (3 * k + a)] = re;
+            chi[2 * (3 * k + a) + 1] = im;
+        }
+}
+
+struct HopArgs {
+    const void* gauge;
+    const void* in;
+    void* out;
+    const void* aux;
+    Geometry g;
+    Epilogue ep;
+    int out_parity;
+    Reduction red;
+    CgScalars* scal;
+};
+
+template <typename T, int RECON, int MU, int FWD, int DAG>
+__device__ __forceinline__ void hop(T (&acc)[24], const HopArgs& a, int e, int e_nb, bool wrap) {
+    constexpr int S = (FWD ? -1 : +1) * (DAG ? -1 : +1);
+    const int Vh = a.g.Vh;
+    T psi[24], u[18], h[12], chi[12];
+    load_spinor(a.in, Vh, e_nb, psi);
+    load_link<RECON>(a.gauge, Vh, FWD ? a.out_parity : 1 - a.out_parity, MU, FWD ? e : e_nb, u);
+    project<MU, S>(psi, h);
+    if (FWD) su3_mul(u, h, chi);
+    else     su3_dag_mul(u, h, chi);
+    if (wrap) {  // boundary phase on the hop that wraps (forward: phase, backward: conj)
+        const T pr = (T)a.g.ph_re[MU], pi = FWD ? (T)a.g.ph_im[MU] : -(T)a.g.ph_im[MU];
+#pragma unroll
+        for (int i = 0; i < 6; ++i) {
+            const T re = chi[2 * i], im = chi[2 * i + 1];
+            chi[2 * i] = pr * re - pi * im;
+            chi[2 * i + 1] = pr * im + pi * re;
+        }
+    }
+    accumulate<MU, S>(acc, chi);
+}
+
+template <typename T, int RECON, int DAG, int MODE>
+__global__ void __launch_bounds__(128, LQCD_HOP_MIN_BLOCKS) hopping_kernel(const HopArgs a) {
+    if (a.scal != nullptr && a.scal->done) return;
+    const int Vh = a.g.Vh;
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    double nrm = 0.0;
+    if (e < Vh) {
+        // a1: e -> (x0h, x1, x2, x3); r = x0 mod 2 follows from the parity
+        const int N0h = a.g.N0h, N1 = a.g.N1, N2 = a.g.N2, N3 = a.g.N3;
+        int t = e;
+        const int x0h = t % N0h; t /= N0h;
+        const int x1 = t % N1;   t /= N1;
+        const int x2 = t % N2;
+        const int x3 = t / N2;
+        const int r = (x1 + x2 + x3 + a.out_parity) & 1;
+        const int s1 = N0h, s2 = N0h * N1, s3 = N0h * N1 * N2;
+
+        T acc[24];
+#pragma unroll
+        for (int i = 0; i < 24; ++i) acc[i] = 0;
+
+        {   // mu = 0: neighbour x0h' = x0h + r (forward), x0h + r - 1 (backward)
+            const bool wf = (r == 1) && (x0h == N0h - 1);
+            const bool wb = (r == 0) && (x0h == 0);
+            hop<T, RECON, 0, 1, DAG>(acc, a, e, wf ? e - (N0h - 1) : e + r, wf);
+            hop<T, RECON, 0, 0, DAG>(acc, a, e, wb ? e + (N0h - 1) : e + r - 1, wb);
+        }
+        {
+            const bool wf = (x1 == N1 - 1), wb = (x1 == 0);
+            hop<T, RECON, 1, 1, DAG>(acc, a, e, wf ? e - (N1 - 1) * s1 : e + s1, wf);
+            hop<T, RECON, 1, 0, DAG>(acc, a, e, wb ? e + (N1 - 1) * s1 : e - s1, wb);
+        }
+        {
+            const bool wf = (x2 == N2 - 1), wb = (x2 == 0);
+            hop<T, RECON, 2, 1, DAG>(acc, a, e, wf ? e - (N2 - 1) * s2 : e + s2, wf);
+            hop<T, RECON, 2, 0, DAG>(acc, a, e, wb ? e + (N2 - 1) * s2 : e - s2, wb);
+        }
+        {
+            const bool wf = (x3 == N3 - 1), wb = (x3 == 0);
+            hop<T, RECON, 3, 1, DAG>(acc, a, e, wf ? e - (N3 - 1) * s3 : e + s3, wf);
+            hop<T, RECON, 3, 0, DAG>(acc, a, e, wb ? e + (N3 - 1) * s3 : e - s3, wb);
+        }
+
+        // a6/a7: epilogue, complex coefficient per chirality
+        T o[24];
+        const T cur = (T)a.ep.cu_re, cui = (T)a.ep.cu_im, cdr = (T)a.ep.cd_re, cdi = (T)a.ep.cd_im;
+#pragma unroll
+        for (int c = 0; c < 12; ++c) {
+            const T cr = (c < 6) ? cur : cdr, ci = (c < 6) ? cui : cdi;
+            o[2 * c] = cr * acc[2 * c] - ci * acc[2 * c + 1];
+            o[2 * c + 1] = cr * acc[2 * c + 1] + ci * acc[2 * c];
+        }
+        if (MODE >= 1) {
+            T x[24];
+            load_spinor(a.aux, Vh, e, x);
+            const T dur = (T)a.ep.du_re, dui = (T)a.ep.du_im, ddr = (T)a.ep.dd_re, ddi = (T)a.ep.dd_im;
+#pragma unroll
+            for (int c = 0; c < 12; ++c) {
+                const T dr = (c < 6) ? dur : ddr, di = (c < 6) ? dui : ddi;
+                o[2 * c] += dr * x[2 * c] - di * x[2 * c + 1];
+                o[2 * c + 1] += dr * x[2 * c + 1] + di * x[2 * c];
+            }
+        }
+        store_spinor(a.out, Vh, e, o);
+        if (MODE == 2) {
+#pragma unroll
+            for (int i = 0; i < 24; ++i) nrm += (double)o[i] * (double)o[i];
+        }
+    }
+    if (MODE == 2) {
+        CgScalars* scal = a.scal;
+        grid_reduce(nrm, a.red, [scal](double s) { scal->pAp = s; });
+    }
+}
+
+template <typename T, int RECON>
+cudaError_t launch_tr(int dagger, int mode, const HopArgs& a, int block, cudaStream_t st) {
+    const int grid = (a.g.Vh + block - 1) / block;
+#define LQCD_HOP_CASE(D, M)                                                        \
+    if (dagger == D && mode == M) {                                                \
+        hopping_kernel<T, RECON, D, M><<<grid, block, 0, st>>>(a);                  \
+        return cudaGetLastError();                                                 \
+    }
+    LQCD_HOP_CASE(0, 0) LQCD_HOP_CASE(0, 1) LQCD_HOP_CASE(0, 2)
+    LQCD_HOP_CASE(1, 0) LQCD_HOP_CASE(1, 1) LQCD_HOP_CASE(1, 2)
+#undef LQCD_HOP_CASE
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace
+
+cudaError_t launch_hopping(int precision, int recon, int dagger, int mode, const Geometry& g,
+                           const Epilogue& ep, const void* gauge, const void* in, void* out,
+                           const void* aux, int out_parity, Reduction red, CgScalars* scal,
+                           int block, cudaStream_t st) {
+    HopArgs a;
+    a.gauge = gauge; a.in = in; a.out = out; a.aux = aux;
+    a.g = g; a.ep = ep; a.out_parity = out_parity; a.red = red; a.scal = scal;
+    if (block <= 0 || block > 128 || (block % 32) != 0) block = 128;
+    count_launch();
+    if (precision == 0) {
+        return recon == 12 ? launch_tr<double, 12>(dagger, mode, a, block, st)
+                           : launch_tr<double, 18>(dagger, mode, a, block, st);
+    }
+    return recon == 12 ? launch_tr<float, 12>(dagger, mode, a, block, st)
+                       : launch_tr<float, 18>(dagger, mode, a, block, st);
+}
+
+}  // namespace lqcd

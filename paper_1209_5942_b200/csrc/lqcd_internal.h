@@ -1,0 +1,127 @@
+// lqcd_internal.h -- shared declarations of the CUDA path (not part of the ABI).
+//
+// Internal field layout (opaque to callers):
+//   Vh = V/2 sites per parity, e = x0/2 + N0h (x1 + N1 (x2 + N2 x3)), N0h = N0/2.
+//   double spinor : double2 s[12][Vh]            component c = 3 alpha + a
+//   float  spinor : float4  s[6][Vh]             element k holds components 2k, 2k+1
+//   double gauge  : double2 g[2][4][9 or 6][Vh]  [parity of origin][mu][row-major entry]
+//   float  gauge 12: float4 g[2][4][3][Vh]
+//   float  gauge 18: per (parity, mu) block of 18 Vh floats: float4 planes 0..3, then one float2 plane
+// The site index is fastest, so a warp touches 512 (double) contiguous bytes per
+// component: 128-bit vectorised, fully coalesced (PAPER.md:221 reached the same
+// conclusion for a 16-byte base type; here it is chosen for LDG.128 / 128 B lines).
+// The gauge field is split by the parity of the link's origin.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stddef.h>
+
+namespace lqcd {
+
+struct Geometry {
+    int N0h, N1, N2, N3;  // N0h = N_x / 2
+    int Vh;               // sites per parity
+    double ph_re[4], ph_im[4];
+};
+
+// Coefficients of the fused epilogue, per chirality (u: alpha = 0,1; d: alpha = 2,3):
+//   out = c_chi * acc  (+ d_chi * aux)        acc = bracket of eq. 6
+struct Epilogue {
+    double cu_re, cu_im, cd_re, cd_im;
+    double du_re, du_im, dd_re, dd_im;
+};
+
+// Device scalars of the CG recurrence.
+struct CgScalars {
+    double rho;        // |r|^2
+    double pAp;        // <p, A p> = |Mhat p|^2
+    double beta;
+    double bb;         // |b|^2
+    double tol2bb;     // tol^2 |b|^2
+    double resid_true; // |b - A x|^2
+    int iters;
+    int done;          // 1 once converged / broken down: later kernels are no-ops
+    int status;        // LQCD_OK / LQCD_NOT_CONVERGED / LQCD_BREAKDOWN
+    int pad;
+};
+
+struct Reduction {
+    double* partials;       // one per block
+    unsigned int* ticket;   // last-block election
+};
+
+enum { FIN_NONE = 0, FIN_PAP = 1, FIN_BB = 2, FIN_RHO = 3, FIN_TRUE = 4 };
+
+// hopping.cu
+// mode 0: out = c * acc;  mode 1: out = d * aux + c * acc;  mode 2: mode 1 + |out|^2 -> scal->pAp
+cudaError_t launch_hopping(int precision, int recon, int dagger, int mode, const Geometry& g,
+                           const Epilogue& ep, const void* gauge, const void* in, void* out,
+                           const void* aux, int out_parity, Reduction red, CgScalars* scal,
+                           int block, cudaStream_t st);
+
+// vector_ops.cu  (n = number of reals in a half-spinor field = 24 Vh)
+cudaError_t launch_cg_init(int precision, size_t n, const void* b, void* x, void* r, void* p,
+                           double tol, Reduction red, CgScalars* scal, cudaStream_t st);
+cudaError_t launch_cg_update_xr(int precision, size_t n, void* x, void* r, const void* p,
+                                const void* q, Reduction red, CgScalars* scal, cudaStream_t st);
+cudaError_t launch_cg_update_p(int precision, size_t n, void* p, const void* r, CgScalars* scal,
+                               cudaStream_t st);
+cudaError_t launch_true_resid(int precision, size_t n, const void* b, const void* ax, Reduction red,
+                              CgScalars* scal, cudaStream_t st);
+int vector_grid(size_t n);
+
+// pack.cu
+cudaError_t launch_pack_gauge(int precision, int recon, const Geometry& g, const void* canon,
+                              void* internal, cudaStream_t st);
+cudaError_t launch_pack_spinor(int precision, const Geometry& g, const void* canon, void* internal,
+                               int parity, cudaStream_t st);
+cudaError_t launch_unpack_spinor(int precision, const Geometry& g, const void* internal, void* canon,
+                                 int parity, cudaStream_t st);
+
+void count_launch(int n = 1);
+
+// Block-wide sum in a fixed order, then election of the last block of the grid,
+// which adds the per-block partials in index order (deterministic for a given
+// grid) and hands the total to `fin`.  All threads of the block must call this.
+template <typename Fin>
+__device__ __forceinline__ void grid_reduce(double v, Reduction red, Fin fin) {
+    __shared__ double sm[32];
+    __shared__ bool last;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if (lane == 0) sm[warp] = v;
+    __syncthreads();
+    if (warp == 0) {
+        v = (lane < nwarp) ? sm[lane] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) {
+            red.partials[blockIdx.x] = v;
+            __threadfence();
+            const unsigned t = atomicAdd(red.ticket, 1u);
+            last = (t == gridDim.x - 1);
+        }
+    }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    double s = 0.0;
+    for (unsigned i = threadIdx.x; i < gridDim.x; i += blockDim.x) s += __ldcg(red.partials + i);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    __syncthreads();
+    if (lane == 0) sm[warp] = s;
+    __syncthreads();
+    if (warp == 0) {
+        s = (lane < nwarp) ? sm[lane] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        if (lane == 0) {
+            *red.ticket = 0u;
+            fin(s);
+        }
+    }
+}
+
+}  // namespace lqcd

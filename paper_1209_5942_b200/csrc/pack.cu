@@ -1,0 +1,139 @@
+// pack.cu -- canonical (array-of-structures, complex double; include/lqcd.h) <-> internal
+// structure-of-arrays layout (lqcd_internal.h).  The paper hides the same conversion
+// behind accessor functions and performs it on host<->device copies;
+// here it is a device kernel so that the interchange format never reaches the hot path.
+#include "lqcd_internal.h"
+
+namespace lqcd {
+namespace {
+
+constexpr int PBLOCK = 128;
+
+__device__ __forceinline__ int site_r(const Geometry& g, int e, int parity) {
+    int t = e / g.N0h;
+    const int x1 = t % g.N1; t /= g.N1;
+    const int x2 = t % g.N2;
+    const int x3 = t / g.N2;
+    return (x1 + x2 + x3 + parity) & 1;
+}
+
+// one thread per (parity, mu, e): reads the 144-byte link U[lex][mu], lex = 2e + r
+template <typename T, int RECON>
+__global__ void __launch_bounds__(PBLOCK) pack_gauge_kernel(Geometry g, const double2* __restrict__ canon,
+                                                            void* __restrict__ internal) {
+    const size_t tid = (size_t)blockIdx.x * PBLOCK + threadIdx.x;
+    const size_t Vh = g.Vh;
+    if (tid >= 8 * Vh) return;
+    const int e = (int)(tid % Vh);
+    const int pm = (int)(tid / Vh);  // parity * 4 + mu
+    const int parity = pm >> 2, mu = pm & 3;
+    const size_t lex = 2 * (size_t)e + site_r(g, e, parity);
+    const double2* src = canon + (lex * 4 + mu) * 9;
+    double2 u[9];
+#pragma unroll
+    for (int j = 0; j < 9; ++j) u[j] = src[j];
+    if (sizeof(T) == 8) {
+        double2* dst = (double2*)internal + (size_t)pm * (RECON / 2) * Vh + e;
+#pragma unroll
+        for (int j = 0; j < RECON / 2; ++j) dst[(size_t)j * Vh] = u[j];
+    } else if (RECON == 12) {
+        float4* dst = (float4*)internal + (size_t)pm * 3 * Vh + e;
+#pragma unroll
+        for (int j = 0; j < 3; ++j)
+            dst[(size_t)j * Vh] = make_float4((float)u[2 * j].x, (float)u[2 * j].y, (float)u[2 * j + 1].x,
+                                              (float)u[2 * j + 1].y);
+    } else {
+        float* blk = (float*)internal + (size_t)pm * 18 * Vh;
+        float4* dst = (float4*)blk + e;
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            dst[(size_t)j * Vh] = make_float4((float)u[2 * j].x, (float)u[2 * j].y, (float)u[2 * j + 1].x,
+                                              (float)u[2 * j + 1].y);
+        ((float2*)(blk + 16 * Vh))[e] = make_float2((float)u[8].x, (float)u[8].y);
+    }
+}
+
+// canonical half spinor psi_p[e][c] -> internal s[c][e]
+template <typename T>
+__global__ void __launch_bounds__(PBLOCK) pack_spinor_kernel(int Vh, const double2* __restrict__ canon,
+                                                             void* __restrict__ internal) {
+    const int e = blockIdx.x * PBLOCK + threadIdx.x;
+    if (e >= Vh) return;
+    const double2* src = canon + (size_t)e * 12;
+    double2 s[12];
+#pragma unroll
+    for (int c = 0; c < 12; ++c) s[c] = src[c];
+    if (sizeof(T) == 8) {
+        double2* dst = (double2*)internal + e;
+#pragma unroll
+        for (int c = 0; c < 12; ++c) dst[(size_t)c * Vh] = s[c];
+    } else {
+        float4* dst = (float4*)internal + e;
+#pragma unroll
+        for (int k = 0; k < 6; ++k)
+            dst[(size_t)k * Vh] = make_float4((float)s[2 * k].x, (float)s[2 * k].y, (float)s[2 * k + 1].x,
+                                              (float)s[2 * k + 1].y);
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(PBLOCK) unpack_spinor_kernel(int Vh, const void* __restrict__ internal,
+                                                               double2* __restrict__ canon) {
+    const int e = blockIdx.x * PBLOCK + threadIdx.x;
+    if (e >= Vh) return;
+    double2 s[12];
+    if (sizeof(T) == 8) {
+        const double2* src = (const double2*)internal + e;
+#pragma unroll
+        for (int c = 0; c < 12; ++c) s[c] = src[(size_t)c * Vh];
+    } else {
+        const float4* src = (const float4*)internal + e;
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            const float4 v = src[(size_t)k * Vh];
+            s[2 * k] = make_double2(v.x, v.y);
+            s[2 * k + 1] = make_double2(v.z, v.w);
+        }
+    }
+    double2* dst = canon + (size_t)e * 12;
+#pragma unroll
+    for (int c = 0; c < 12; ++c) dst[c] = s[c];
+}
+
+}  // namespace
+
+cudaError_t launch_pack_gauge(int precision, int recon, const Geometry& g, const void* canon,
+                              void* internal, cudaStream_t st) {
+    const size_t n = 8 * (size_t)g.Vh;
+    const int grid = (int)((n + PBLOCK - 1) / PBLOCK);
+    count_launch();
+    const double2* c = (const double2*)canon;
+    if (precision == 0) {
+        if (recon == 12) pack_gauge_kernel<double, 12><<<grid, PBLOCK, 0, st>>>(g, c, internal);
+        else             pack_gauge_kernel<double, 18><<<grid, PBLOCK, 0, st>>>(g, c, internal);
+    } else {
+        if (recon == 12) pack_gauge_kernel<float, 12><<<grid, PBLOCK, 0, st>>>(g, c, internal);
+        else             pack_gauge_kernel<float, 18><<<grid, PBLOCK, 0, st>>>(g, c, internal);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_pack_spinor(int precision, const Geometry& g, const void* canon, void* internal,
+                               int /*parity*/, cudaStream_t st) {
+    const int grid = (g.Vh + PBLOCK - 1) / PBLOCK;
+    count_launch();
+    if (precision == 0) pack_spinor_kernel<double><<<grid, PBLOCK, 0, st>>>(g.Vh, (const double2*)canon, internal);
+    else                pack_spinor_kernel<float><<<grid, PBLOCK, 0, st>>>(g.Vh, (const double2*)canon, internal);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_unpack_spinor(int precision, const Geometry& g, const void* internal, void* canon,
+                                 int /*parity*/, cudaStream_t st) {
+    const int grid = (g.Vh + PBLOCK - 1) / PBLOCK;
+    count_launch();
+    if (precision == 0) unpack_spinor_kernel<double><<<grid, PBLOCK, 0, st>>>(g.Vh, internal, (double2*)canon);
+    else                unpack_spinor_kernel<float><<<grid, PBLOCK, 0, st>>>(g.Vh, internal, (double2*)canon);
+    return cudaGetLastError();
+}
+
+}  // namespace lqcd

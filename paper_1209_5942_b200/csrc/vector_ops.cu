@@ -1,0 +1,219 @@
+// vector_ops.cu -- fused CG vector kernels (the paper's
+// "saxpy" and "LAPACK operations", written there
+// "in a straightforward manner").  Here: two passes per iteration instead of five,
+// 128-bit loads, warp-shuffle block sums, last-block finalisation in a fixed
+// order so that alpha, beta and the convergence decision never leave the device.
+//
+//   cg_init      x = 0, r = p = b, rho = bb = |b|^2
+//   cg_update_xr alpha = rho / pAp; x += alpha p; r -= alpha q; rho' = |r|^2;
+//                last block: iters++, done = (rho' <= tol^2 bb), beta = rho'/rho, rho = rho'
+//   cg_update_p  p = r + beta p
+//   true_resid   |b - Ax|^2
+// Reductions accumulate in double whatever the field precision.
+#include "lqcd_internal.h"
+
+namespace lqcd {
+namespace {
+
+constexpr int VBLOCK = 256;
+constexpr int VUNROLL = 4;
+
+template <typename T> struct VecOf;
+template <> struct VecOf<double> { typedef double2 type; static constexpr int width = 2; };
+template <> struct VecOf<float>  { typedef float4 type;  static constexpr int width = 4; };
+
+__device__ __forceinline__ double2 axpy(double a, double2 x, double2 y) {
+    return make_double2(fma(a, x.x, y.x), fma(a, x.y, y.y));
+}
+__device__ __forceinline__ float4 axpy(double a, float4 x, float4 y) {
+    const float f = (float)a;
+    return make_float4(fmaf(f, x.x, y.x), fmaf(f, x.y, y.y), fmaf(f, x.z, y.z), fmaf(f, x.w, y.w));
+}
+__device__ __forceinline__ double2 sub(double2 x, double2 y) { return make_double2(x.x - y.x, x.y - y.y); }
+__device__ __forceinline__ float4 sub(float4 x, float4 y) {
+    return make_float4(x.x - y.x, x.y - y.y, x.z - y.z, x.w - y.w);
+}
+__device__ __forceinline__ double norm2(double2 v) { return v.x * v.x + v.y * v.y; }
+__device__ __forceinline__ double norm2(float4 v) {
+    return (double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z + (double)v.w * v.w;
+}
+__device__ __forceinline__ void zero(double2& v) { v = make_double2(0.0, 0.0); }
+__device__ __forceinline__ void zero(float4& v) { v = make_float4(0.f, 0.f, 0.f, 0.f); }
+
+template <typename T>
+__global__ void __launch_bounds__(VBLOCK) cg_init_kernel(size_t nvec, const void* b_, void* x_, void* r_,
+                                                         void* p_, double tol, Reduction red,
+                                                         CgScalars* scal) {
+    typedef typename VecOf<T>::type V;
+    const V* b = (const V*)b_;
+    V *x = (V*)x_, *r = (V*)r_, *p = (V*)p_;
+    const size_t base = (size_t)blockIdx.x * (VBLOCK * VUNROLL) + threadIdx.x;
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < VUNROLL; ++k) {
+        const size_t i = base + (size_t)k * VBLOCK;
+        if (i < nvec) {
+            const V v = b[i];
+            V z;
+            zero(z);
+            x[i] = z;
+            r[i] = v;
+            p[i] = v;
+            s += norm2(v);
+        }
+    }
+    grid_reduce(s, red, [scal, tol](double bb) {
+        scal->bb = bb;
+        scal->rho = bb;
+        scal->pAp = 0.0;
+        scal->beta = 0.0;
+        scal->tol2bb = tol * tol * bb;
+        scal->resid_true = 0.0;
+        scal->iters = 0;
+        scal->done = (bb == 0.0) ? 1 : 0;
+        scal->status = (bb == 0.0) ? 0 : 1;
+    });
+}
+
+template <typename T>
+__global__ void __launch_bounds__(VBLOCK) cg_update_xr_kernel(size_t nvec, void* x_, void* r_,
+                                                              const void* p_, const void* q_,
+                                                              Reduction red, CgScalars* scal) {
+    typedef typename VecOf<T>::type V;
+    if (scal->done) return;
+    const double rho = scal->rho, pAp = scal->pAp;
+    if (!(pAp > 0.0) || !isfinite(pAp) || !isfinite(rho)) {  // breakdown: leave x, r untouched
+        if (blockIdx.x == 0 && threadIdx.x == 0) {
+            scal->status = -5;
+            scal->done = 1;
+        }
+        return;
+    }
+    const double alpha = rho / pAp;
+    V *x = (V*)x_, *r = (V*)r_;
+    const V *p = (const V*)p_, *q = (const V*)q_;
+    const size_t base = (size_t)blockIdx.x * (VBLOCK * VUNROLL) + threadIdx.x;
+    V xv[VUNROLL], rv[VUNROLL], pv[VUNROLL], qv[VUNROLL];
+#pragma unroll
+    for (int k = 0; k < VUNROLL; ++k) {
+        const size_t i = base + (size_t)k * VBLOCK;
+        if (i < nvec) { xv[k] = x[i]; rv[k] = r[i]; pv[k] = __ldg(p + i); qv[k] = __ldcs(q + i); }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < VUNROLL; ++k) {
+        const size_t i = base + (size_t)k * VBLOCK;
+        if (i < nvec) {
+            x[i] = axpy(alpha, pv[k], xv[k]);
+            const V rn = axpy(-alpha, qv[k], rv[k]);
+            r[i] = rn;
+            s += norm2(rn);
+        }
+    }
+    grid_reduce(s, red, [scal, rho](double rho1) {
+        scal->iters += 1;
+        if (rho1 <= scal->tol2bb) {
+            scal->done = 1;
+            scal->status = 0;
+        }
+        scal->beta = rho1 / rho;
+        scal->rho = rho1;
+    });
+}
+
+template <typename T>
+__global__ void __launch_bounds__(VBLOCK) cg_update_p_kernel(size_t nvec, void* p_, const void* r_,
+                                                             CgScalars* scal) {
+    typedef typename VecOf<T>::type V;
+    if (scal->done) return;
+    const double beta = scal->beta;
+    V* p = (V*)p_;
+    const V* r = (const V*)r_;
+    const size_t base = (size_t)blockIdx.x * (VBLOCK * VUNROLL) + threadIdx.x;
+    V pv[VUNROLL], rv[VUNROLL];
+#pragma unroll
+    for (int k = 0; k < VUNROLL; ++k) {
+        const size_t i = base + (size_t)k * VBLOCK;
+        if (i < nvec) { pv[k] = p[i]; rv[k] = __ldg(r + i); }
+    }
+#pragma unroll
+    for (int k = 0; k < VUNROLL; ++k) {
+        const size_t i = base + (size_t)k * VBLOCK;
+        if (i < nvec) p[i] = axpy(beta, pv[k], rv[k]);
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(VBLOCK) true_resid_kernel(size_t nvec, const void* b_, const void* ax_,
+                                                            Reduction red, CgScalars* scal) {
+    typedef typename VecOf<T>::type V;
+    const V *b = (const V*)b_, *ax = (const V*)ax_;
+    const size_t base = (size_t)blockIdx.x * (VBLOCK * VUNROLL) + threadIdx.x;
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < VUNROLL; ++k) {
+        const size_t i = base + (size_t)k * VBLOCK;
+        if (i < nvec) s += norm2(sub(__ldg(b + i), __ldg(ax + i)));
+    }
+    grid_reduce(s, red, [scal](double t) { scal->resid_true = t; });
+}
+
+inline int grid_for(size_t nvec) { return (int)((nvec + VBLOCK * VUNROLL - 1) / (VBLOCK * VUNROLL)); }
+
+}  // namespace
+
+int vector_grid(size_t n) { return grid_for(n / 2); }  // upper bound over both precisions
+
+cudaError_t launch_cg_init(int precision, size_t n, const void* b, void* x, void* r, void* p,
+                           double tol, Reduction red, CgScalars* scal, cudaStream_t st) {
+    count_launch();
+    if (precision == 0) {
+        const size_t nv = n / 2;
+        cg_init_kernel<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, b, x, r, p, tol, red, scal);
+    } else {
+        const size_t nv = n / 4;
+        cg_init_kernel<float><<<grid_for(nv), VBLOCK, 0, st>>>(nv, b, x, r, p, tol, red, scal);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_cg_update_xr(int precision, size_t n, void* x, void* r, const void* p,
+                                const void* q, Reduction red, CgScalars* scal, cudaStream_t st) {
+    count_launch();
+    if (precision == 0) {
+        const size_t nv = n / 2;
+        cg_update_xr_kernel<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, x, r, p, q, red, scal);
+    } else {
+        const size_t nv = n / 4;
+        cg_update_xr_kernel<float><<<grid_for(nv), VBLOCK, 0, st>>>(nv, x, r, p, q, red, scal);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_cg_update_p(int precision, size_t n, void* p, const void* r, CgScalars* scal,
+                               cudaStream_t st) {
+    count_launch();
+    if (precision == 0) {
+        const size_t nv = n / 2;
+        cg_update_p_kernel<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, p, r, scal);
+    } else {
+        const size_t nv = n / 4;
+        cg_update_p_kernel<float><<<grid_for(nv), VBLOCK, 0, st>>>(nv, p, r, scal);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_true_resid(int precision, size_t n, const void* b, const void* ax, Reduction red,
+                              CgScalars* scal, cudaStream_t st) {
+    count_launch();
+    if (precision == 0) {
+        const size_t nv = n / 2;
+        true_resid_kernel<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, b, ax, red, scal);
+    } else {
+        const size_t nv = n / 4;
+        true_resid_kernel<float><<<grid_for(nv), VBLOCK, 0, st>>>(nv, b, ax, red, scal);
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace lqcd

@@ -1,0 +1,351 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle (-m gpu).
+
+Bar (BASELINE.json north_star): relative L2 error <= 1e-13 in double, <= 1e-5 in
+single (oracle fed the float-rounded inputs), on the same seeded inputs.  CG:
+reading G14 of DESIGN.md (solution unique, iterates not bit-reproducible).
+"""
+import numpy as np
+import pytest
+
+import lattice_util as lu
+import lqcd_inputs as gen
+
+pytestmark = pytest.mark.gpu
+
+TOL_D = 1e-13
+TOL_S = 1e-5
+AP = gen.antiperiodic_t()
+SEED = gen.BASE_SEED
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_1209_5942_b200.binding as b
+    return b
+
+
+class Lat:
+    """One initialised lattice + uploaded gauge field under a given format."""
+
+    def __init__(self, B, dims, phases, U, precision=0, recon=18):
+        self.B, self.dims, self.phases, self.U = B, dims, np.asarray(phases, dtype=complex), U
+        self.precision, self.recon = precision, recon
+        B.lqcd_init(dims, self.phases)
+        B.lqcd_set_format(precision, recon)
+        B.lqcd_set_stream()
+        self.g = B.upload_gauge(U)
+
+    def dslash(self, x, parity, kappa):
+        s = self.B.upload_spinor(x, 1 - parity)
+        o = self.B.alloc_spinor()
+        self.B.lqcd_dslash_eo(self.g, s, o, parity, kappa)
+        return self.B.download_spinor(o, parity)
+
+    def mtm(self, x, kappa, mu, dagger):
+        s = self.B.upload_spinor(x, 0)
+        o = self.B.alloc_spinor()
+        self.B.lqcd_mtm(self.g, s, o, kappa, mu, dagger)
+        return self.B.download_spinor(o, 0)
+
+    def cg(self, b, kappa, mu, tol, maxit):
+        s = self.B.upload_spinor(b, 0)
+        x = self.B.alloc_spinor()
+        st = self.B.lqcd_cg_mdagm(self.g, s, x, kappa, mu, tol, maxit)
+        return st, self.B.download_spinor(x, 0), self.B.lqcd_cg_stats()
+
+
+def _round_inputs(U, x, precision):
+    if precision == 0:
+        return U, x
+    return U.astype(np.complex64).astype(np.complex128), x.astype(np.complex64).astype(np.complex128)
+
+
+GENERIC_PH = np.exp(1j * np.pi * np.array([0.3, 0.0, 1.0, 0.5]))
+
+
+# --------------------------------------------------------------------------- config 1 and friends
+@pytest.mark.parametrize("dims,phases", [
+    ((4, 4, 4, 4), AP),            # BASELINE config 1
+    ((2, 2, 2, 2), AP),            # N_mu = 2: both hops reach the same site (G8)
+    ((2, 2, 2, 2), GENERIC_PH),
+    ((4, 6, 2, 8), GENERIC_PH),    # unequal extents, complex phases on every wrap
+    ((6, 4, 10, 4), AP),           # Vh = 480: ragged tail for 128-thread blocks
+    ((8, 8, 8, 16), AP),           # BASELINE config 2 lattice: several blocks
+])
+def test_dslash_eo_matches_oracle(B, oracle_mod, dims, phases):
+    kappa = 0.15
+    U = gen.gauge_haar(dims, SEED)
+    x = gen.spinor_gaussian(lu.volume(dims) // 2, SEED)
+    L = Lat(B, dims, phases, U)
+    for parity in (0, 1):
+        got = L.dslash(x, parity, kappa)
+        want = oracle_mod.dslash_eo(dims, phases, U, x, parity, kappa)
+        assert lu.rel_err(got, want) <= TOL_D
+        # element by element too: no single site may be off
+        assert np.max(np.abs(got - want)) <= 1e-13 * np.max(np.abs(want))
+
+
+@pytest.mark.parametrize("dims,phases", [((4, 4, 4, 4), AP), ((2, 2, 2, 2), GENERIC_PH),
+                                         ((4, 6, 2, 8), GENERIC_PH), ((8, 8, 8, 16), AP)])
+@pytest.mark.parametrize("dagger", [0, 1])
+def test_mtm_matches_oracle(B, oracle_mod, dims, phases, dagger):
+    kappa, mu = 0.15, 0.1
+    U = gen.gauge_haar(dims, SEED)
+    x = gen.spinor_gaussian(lu.volume(dims) // 2, SEED)
+    L = Lat(B, dims, phases, U)
+    got = L.mtm(x, kappa, mu, dagger)
+    want = oracle_mod.mhat(dims, phases, U, x, kappa, mu, dagger)
+    assert lu.rel_err(got, want) <= TOL_D
+
+
+@pytest.mark.parametrize("block", [32, 64, 96, 128])
+def test_block_sizes(B, oracle_mod, block):
+    dims = (6, 4, 10, 4)
+    U = gen.gauge_haar(dims, SEED)
+    x = gen.spinor_gaussian(lu.volume(dims) // 2, SEED)
+    L = Lat(B, dims, AP, U)
+    B.lqcd_set_block_size(block)
+    got = L.mtm(x, 0.15, 0.1, 0)
+    assert lu.rel_err(got, oracle_mod.mhat(dims, AP, U, x, 0.15, 0.1, 0)) <= TOL_D
+
+
+def test_pack_unpack_roundtrip_is_exact(B):
+    dims = (4, 6, 2, 8)
+    x = gen.spinor_gaussian(lu.volume(dims) // 2, SEED)
+    B.lqcd_init(dims, AP)
+    for parity in (0, 1):
+        s = B.upload_spinor(x, parity)
+        assert np.array_equal(B.download_spinor(s, parity), x)
+    B.lqcd_set_format(B.LQCD_SINGLE, 18)
+    s = B.upload_spinor(x, 0)
+    assert np.array_equal(B.download_spinor(s, 0), x.astype(np.complex64).astype(np.complex128))
+
+
+# --------------------------------------------------------------------------- config 2: invariances on GPU output
+def test_config2_gamma5_hermiticity_and_gauge_covariance_on_gpu(B, oracle_mod):
+    dims = (8, 8, 8, 16)
+    kappa, mu = 0.15, 0.1
+    V = lu.volume(dims)
+    U = gen.gauge_haar(dims, SEED)
+    x = gen.spinor_gaussian(V // 2, SEED)
+    y = gen.spinor_gaussian(V // 2, SEED, gen.STREAM_SOURCE)
+    L = Lat(B, dims, AP, U)
+    Mx, Mdy = L.mtm(x, kappa, mu, 0), L.mtm(y, kappa, mu, 1)
+    for dagger, got in ((0, Mx), (1, Mdy)):
+        want = oracle_mod.mhat(dims, AP, U, x if dagger == 0 else y, kappa, mu, dagger)
+        assert lu.rel_err(got, want) <= TOL_D
+    # <y, M x> = <M^dag y, x>
+    lhs, rhs = np.vdot(y, Mx), np.vdot(Mdy, x)
+    assert abs(lhs - rhs) / abs(lhs) < 1e-13
+    # gamma5 Mhat(mu) gamma5 = Mhat(-mu)^dag
+    g5 = lu.GAMMA5
+    lhs = lu.apply_spin(g5, L.mtm(lu.apply_spin(g5, x), kappa, mu, 0))
+    assert lu.rel_err(lhs, L.mtm(x, kappa, -mu, 1)) < 1e-13
+    # gauge covariance: Mhat[U'] g x = g Mhat[U] x
+    g = gen.su3_haar(V, SEED, gen.STREAM_GTRANS)
+    X = lu.site_coords(dims)
+    Up = np.empty_like(U)
+    for m in range(4):
+        Y = X.copy()
+        Y[:, m] = (Y[:, m] + 1) % dims[m]
+        Up[:, m] = np.einsum("sab,sbc,sdc->sad", g, U[:, m], g[lu.lex_index(dims, Y)].conj())
+    ge = lu.to_half(dims, g, 0)
+    Lp = Lat(B, dims, AP, Up)
+    assert lu.rel_err(Lp.mtm(lu.apply_colour(ge, x), kappa, mu, 0), lu.apply_colour(ge, Mx)) < 1e-13
+
+
+def test_free_field_closed_form_on_gpu(B):
+    dims = (4, 4, 6, 8)
+    kappa, mu = 0.137, 0.21
+    p = lu.momentum(dims, AP, (1, 3, 2, 5))
+    rng = np.random.default_rng(3)
+    u = rng.normal(size=12) + 1j * rng.normal(size=12)
+    psi = lu.plane_wave(dims, p, u)
+    h = lu.free_h(p, kappa)
+    A = np.eye(4) + 2j * kappa * mu * lu.GAMMA5
+    L = Lat(B, dims, AP, gen.gauge_unit(dims))
+    got = L.mtm(lu.to_half(dims, psi, 0), kappa, mu, 0)
+    want = lu.to_half(dims, lu.apply_spin(A - h @ np.linalg.inv(A) @ h, psi), 0)
+    assert lu.rel_err(got, want) < 1e-13
+
+
+# --------------------------------------------------------------------------- storage variants (config 5 formats)
+@pytest.mark.parametrize("precision,recon,tol", [(0, 12, TOL_D), (1, 18, TOL_S), (1, 12, TOL_S)])
+@pytest.mark.parametrize("dims,phases", [((4, 4, 4, 4), AP), ((4, 6, 2, 8), GENERIC_PH), ((8, 8, 8, 16), AP)])
+def test_storage_variants(B, oracle_mod, precision, recon, tol, dims, phases):
+    kappa, mu = 0.15, 0.1
+    U = gen.gauge_haar(dims, SEED)
+    x = gen.spinor_gaussian(lu.volume(dims) // 2, SEED)
+    Ur, xr = _round_inputs(U, x, precision)
+    L = Lat(B, dims, phases, U, precision, recon)
+    for parity in (0, 1):
+        got = L.dslash(x, parity, kappa)
+        assert lu.rel_err(got, oracle_mod.dslash_eo(dims, phases, Ur, xr, parity, kappa)) <= tol
+    for dagger in (0, 1):
+        got = L.mtm(x, kappa, mu, dagger)
+        assert lu.rel_err(got, oracle_mod.mhat(dims, phases, Ur, xr, kappa, mu, dagger)) <= tol
+
+
+def test_near_identity_links_config3_small(B, oracle_mod):
+    dims = (8, 8, 8, 8)
+    kappa, mu = 0.16, 0.05
+    U = gen.gauge_near_identity(dims, SEED, 0.3)
+    x = gen.spinor_gaussian(lu.volume(dims) // 2, SEED)
+    for recon in (18, 12):
+        L = Lat(B, dims, AP, U, 0, recon)
+        assert lu.rel_err(L.mtm(x, kappa, mu, 0), oracle_mod.mhat(dims, AP, U, x, kappa, mu, 0)) <= TOL_D
+
+
+# --------------------------------------------------------------------------- CG
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (8, 8, 8, 16)])
+def test_cg_matches_oracle(B, oracle_mod, dims):
+    kappa, mu, tol = 0.15, 0.1, 1e-10
+    U = gen.gauge_haar(dims, SEED)
+    b = gen.spinor_gaussian(lu.volume(dims) // 2, SEED, gen.STREAM_SOURCE)
+    L = Lat(B, dims, AP, U)
+    st, x, (iters, rr, rt) = L.cg(b, kappa, mu, tol, 2000)
+    st_o, x_o, it_o, rr_o, rt_o = oracle_mod.cg_mdagm(dims, AP, U, b, kappa, mu, tol, 2000)
+    assert st == 0 and st_o == 0
+    assert abs(iters - it_o) <= 2
+    assert rr <= tol
+    # true residual of the GPU's x, evaluated by the ORACLE's operator
+    r = b - oracle_mod.mdagm(dims, AP, U, x, kappa, mu)
+    true_rel = np.linalg.norm(r) / np.linalg.norm(b)
+    assert true_rel <= 1.05 * tol
+    assert abs(rt - true_rel) <= 0.05 * tol          # the library's own true residual agrees
+    assert lu.rel_err(x, x_o) <= 10 * 5.0 * tol       # 10 * sqrt(cond) * tol, cond ~ 10-25 (G14)
+
+
+@pytest.mark.parametrize("k", [1, 3])
+def test_cg_k_iterations_from_identical_state(B, oracle_mod, k):
+    dims = (8, 8, 8, 16)
+    kappa, mu = 0.15, 0.1
+    U = gen.gauge_haar(dims, SEED)
+    b = gen.spinor_gaussian(lu.volume(dims) // 2, SEED, gen.STREAM_SOURCE)
+    L = Lat(B, dims, AP, U)
+    st, x, (iters, rr, rt) = L.cg(b, kappa, mu, 0.0, k)
+    st_o, x_o, it_o, rr_o, rt_o = oracle_mod.cg_mdagm(dims, AP, U, b, kappa, mu, 0.0, k)
+    assert st == 1 and st_o == 1 and iters == k == it_o
+    assert lu.rel_err(x, x_o) <= 1e-13 * (4 if k > 1 else 1)
+    assert abs(rr - rr_o) <= 1e-12 * rr_o
+    assert abs(rt - rt_o) <= 1e-10 * rt_o
+
+
+def test_cg_edge_cases(B):
+    dims = (4, 4, 4, 4)
+    U = gen.gauge_haar(dims, SEED)
+    L = Lat(B, dims, AP, U)
+    zero = np.zeros((lu.volume(dims) // 2, 4, 3), dtype=complex)
+    st, x, (iters, rr, rt) = L.cg(zero, 0.15, 0.1, 1e-10, 50)     # b = 0 -> x = 0 at once
+    assert st == 0 and iters == 0 and np.all(x == 0)
+    b = gen.spinor_gaussian(lu.volume(dims) // 2, SEED, gen.STREAM_SOURCE)
+    st, x, (iters, rr, rt) = L.cg(b, 0.15, 0.1, 1e-10, 5)         # maxit too small
+    assert st == B.LQCD_NOT_CONVERGED and iters == 5 and rr > 1e-10
+    st, x, (iters, rr, rt) = L.cg(b, 0.0, 0.1, 1e-12, 50)         # kappa = 0: A = 1, one step
+    assert st == 0 and iters == 1 and lu.rel_err(x, b) < 1e-14
+
+
+def test_cg_single_precision_converges_loosely(B, oracle_mod):
+    dims = (8, 8, 8, 16)
+    kappa, mu, tol = 0.15, 0.1, 1e-5
+    U = gen.gauge_haar(dims, SEED)
+    b = gen.spinor_gaussian(lu.volume(dims) // 2, SEED, gen.STREAM_SOURCE)
+    for recon in (18, 12):
+        L = Lat(B, dims, AP, U, 1, recon)
+        st, x, (iters, rr, rt) = L.cg(b, kappa, mu, tol, 500)
+        assert st == 0 and rr <= tol
+        r = b - oracle_mod.mdagm(dims, AP, U, x, kappa, mu)
+        assert np.linalg.norm(r) / np.linalg.norm(b) <= 20 * tol
+
+
+# --------------------------------------------------------------------------- ABI behaviour
+def test_error_codes(B):
+    import torch
+    with pytest.raises(B.LqcdError) as e:
+        B.lqcd_init((4, 4, 5, 4), AP)
+    assert e.value.status == B.LQCD_BAD_DIMS
+    with pytest.raises(B.LqcdError) as e:
+        B.lqcd_init((4, 4, 4, 4), [1, 1, 1, 2.0])
+    assert e.value.status == B.LQCD_BAD_DIMS
+    B.lqcd_init((4, 4, 4, 4), AP)
+    g, s, o = B.alloc_gauge(), B.alloc_spinor(), B.alloc_spinor()
+    for call in (lambda: B.lqcd_dslash_eo(g, s, o, 2, 0.1),
+                 lambda: B.lqcd_dslash_eo(g, s, s, 0, 0.1),
+                 lambda: B.lqcd_dslash_eo(g, 0, o, 0, 0.1),
+                 lambda: B.lqcd_dslash_eo(g, s, o, 0, float("nan")),
+                 lambda: B.lqcd_mtm(g, s, o, 0.1, float("inf"), 0),
+                 lambda: B.lqcd_cg_mdagm(g, s, o, 0.1, 0.1, 1e-8, 0),
+                 lambda: B.lqcd_set_format(2, 18),
+                 lambda: B.lqcd_set_format(0, 8)):
+        with pytest.raises(B.LqcdError) as e:
+            call()
+        assert e.value.status == B.LQCD_BAD_ARG
+    assert B.lqcd_gauge_bytes() == 256 * 576 and B.lqcd_spinor_bytes() == 128 * 192
+    B.lqcd_set_format(B.LQCD_SINGLE, 12)
+    assert B.lqcd_gauge_bytes() == 256 * 192 and B.lqcd_spinor_bytes() == 128 * 96
+    torch.cuda.synchronize()
+
+
+def test_host_entry_points(B, oracle_mod):
+    dims = (8, 8, 8, 16)
+    kappa, mu = 0.15, 0.1
+    U = gen.gauge_haar(dims, SEED)
+    x = gen.spinor_gaussian(lu.volume(dims) // 2, SEED)
+    B.lqcd_init(dims, AP)
+    out = np.empty_like(x)
+    n0 = B.lqcd_launch_count()
+    B.lqcd_mtm_host(U, x, out, kappa, mu, 0)
+    assert B.lqcd_launch_count() - n0 == 5      # 2 pack + 2 hopping + 1 unpack
+    assert lu.rel_err(out, oracle_mod.mhat(dims, AP, U, x, kappa, mu, 0)) <= TOL_D
+    sol = np.empty_like(x)
+    st = B.lqcd_cg_mdagm_host(U, x, sol, kappa, mu, 1e-10, 1000)
+    assert st == 0
+    assert lu.rel_err(oracle_mod.mdagm(dims, AP, U, sol, kappa, mu), x) <= 1.05e-10
+
+
+# --------------------------------------------------------------------------- full sizes, sampled
+def _sample_sites(n, count, seed):
+    rng = np.random.default_rng(seed)
+    s = rng.integers(0, n, size=count)
+    s[:4] = [0, 1, n - 1, n // 2]       # corners: wraps in every direction
+    return np.unique(s)
+
+
+@pytest.mark.parametrize("dims,near_id,kappa,mu", [
+    ((16, 16, 16, 32), True, 0.16, 0.05),     # config 3
+    ((24, 24, 24, 48), False, 0.15, 0.1),     # config 4 lattice
+    ((32, 32, 32, 64), False, 0.15, 0.1),     # config 5 (bench workload), bench launch configuration
+])
+def test_full_size_sampled_sites(B, oracle_mod, dims, near_id, kappa, mu):
+    U = gen.gauge_near_identity(dims, SEED, 0.3) if near_id else gen.gauge_haar(dims, SEED)
+    h = lu.volume(dims) // 2
+    x = gen.spinor_gaussian(h, SEED)
+    sites = _sample_sites(h, 300, 17)
+    L = Lat(B, dims, AP, U)
+    for parity in (0, 1):
+        got = L.dslash(x, parity, kappa)[sites]
+        want = oracle_mod.dslash_eo_sites(dims, AP, U, x, sites, parity, kappa)
+        assert lu.rel_err(got, want) <= TOL_D
+    for dagger in (0, 1):
+        got = L.mtm(x, kappa, mu, dagger)
+        want = oracle_mod.mhat_sites(dims, AP, U, x, sites, kappa, mu, dagger)
+        assert lu.rel_err(got[sites], want) <= TOL_D
+        assert np.all(np.isfinite(got))
+    # a property that holds at any size: <x, Mhat^dag Mhat x> = |Mhat x|^2 > 0
+    Mx = L.mtm(x, kappa, mu, 0)
+    MdMx = L.mtm(Mx, kappa, mu, 1)
+    assert abs(np.vdot(x, MdMx) - np.vdot(Mx, Mx)) <= 1e-12 * np.vdot(Mx, Mx).real
+
+
+def test_config4_cg_24c48(B, oracle_mod):
+    dims = (24, 24, 24, 48)
+    kappa, mu, tol = 0.15, 0.1, 1e-10
+    U = gen.gauge_haar(dims, SEED)
+    b = gen.spinor_gaussian(lu.volume(dims) // 2, SEED, gen.STREAM_SOURCE)
+    L = Lat(B, dims, AP, U)
+    st, x, (iters, rr, rt) = L.cg(b, kappa, mu, tol, 2000)
+    assert st == 0 and 20 <= iters <= 80 and rr <= tol
+    r = b - oracle_mod.mdagm(dims, AP, U, x, kappa, mu)     # one oracle application of A
+    assert np.linalg.norm(r) / np.linalg.norm(b) <= 1.05 * tol
