@@ -1,0 +1,359 @@
+#!/usr/bin/env python
+"""bench.py -- D_tm GFLOPS (1320 flop/site) and HBM GB/s of the even-odd twisted-mass hot path.
+
+Workload (BASELINE.json configs[4], the configuration the metric is quoted on):
+32^3 x 64 lattice, complex double, Haar-random SU(3) links, Gaussian source,
+kappa = 0.15, mu = 0.1, antiperiodic in time; synthetic seeded inputs
+(lqcd_inputs).
+
+One step = one CG iteration on Mhat^dag Mhat:
+four hopping launches with fused diagonal-term epilogues (one with the fused
+<p,Ap> reduction) + the two fused vector kernels.  K steps are run as solves of
+SOLVE_LEN iterations each (a real solve at this configuration takes about that
+many), the one-launch solve setup included in the timed region; the recursive
+residual would otherwise underflow after several hundred iterations.
+
+value   = hopping flops (4 x V/2 x 1320 per step; diagonal and vector-kernel
+          flops NOT counted) / time, inputs resident in HBM.
+roofline= the hopping kernel: algorithmic bytes (1536 B/site, +192 B/site for the
+          two launches that also read `aux`) / CUDA-event duration of each launch,
+          recorded live in the timed region by the library (lqcd_profile).
+e2e     = the same per-step work through lqcd_cg_mdagm_host with pinned HOST
+          buffers: every step uploads gauge + source, runs one CG iteration (plus
+          the solve's true-residual check, not counted as flops) and downloads x.
+--impl reference times the CPU oracle (oracle/, test infrastructure) on the host cores.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+FLOP_PER_SITE = 1320          # BASELINE.json metric; SURVEY.md section 8(a) row a5
+BYTES_PER_SITE = 1536         # double, 18-real links: 8 links x 144 + 192 in + 192 out (section 8(d))
+AUX_BYTES_PER_SITE = 192      # launches with the M_ee * aux epilogue read one more half spinor
+DIMS = (32, 32, 32, 64)
+REF_DIMS = (16, 16, 16, 32)   # bounded sample for the oracle legs (same recipe, 1/16 of the sites)
+REF_DIMS_SMALL = (8, 8, 8, 16)  # used by --impl reference when K + W > 100 steps are asked for
+KAPPA, MU = 0.15, 0.1
+SOLVE_LEN = 40
+METRIC = "D_tm GFLOPS (1320 flop/site) & achieved HBM GB/s vs B200 peak, double"
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the plain hopping kernel at this
+# workload, from the committed ncu --set full capture (profiles/); None until captured.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons during the timed region (pynvml, else nvidia-smi)."""
+
+    def __init__(self, index):
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+
+    def _run_nvml(self):
+        import pynvml as nv
+        nv.nvmlInit()
+        h = nv.nvmlDeviceGetHandleByIndex(self.index)
+        self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+        names = {
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake_slowdown",
+        }
+        get_reasons = getattr(nv, "nvmlDeviceGetCurrentClocksEventReasons", None) or \
+            nv.nvmlDeviceGetCurrentClocksThrottleReasons
+        while not self._stop.is_set():
+            self.samples.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+            r = get_reasons(h)
+            for bit, name in names.items():
+                if r & bit:
+                    self.reasons.add(name)
+            time.sleep(0.005)
+
+    def _run_smi(self):
+        import subprocess
+        q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+            "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+        keys = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        while not self._stop.is_set():
+            out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={q}",
+                                  "--format=csv,noheader,nounits"], capture_output=True, text=True).stdout
+            f = [s.strip() for s in out.strip().split(",")]
+            if len(f) >= 6:
+                self.samples.append(float(f[0]))
+                self.max_mhz = float(f[1])
+                for k, v in zip(keys, f[2:6]):
+                    if v.lower().startswith("active"):
+                        self.reasons.add(k)
+
+    def _run(self):
+        try:
+            self._run_nvml()
+        except Exception:
+            try:
+                self._run_smi()
+            except Exception:
+                pass
+
+    def __enter__(self):
+        self._thr = threading.Thread(target=self._run, daemon=True)
+        self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._thr.join(timeout=5)
+
+    def summary(self):
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+def oracle_gflops(dims, steps, warmup):
+    """Oracle as it stands: one application of Mhat^dag Mhat (4 hopping terms = one CG iteration's
+    operator work) per step on the host cores; returns (gflops, ms_per_step, threads)."""
+    import lqcd_inputs as gen
+    import oracle
+    oracle.build()
+    Vh = int(np.prod(dims)) // 2
+    U = gen.gauge_haar(dims)
+    x = gen.spinor_gaussian(Vh, stream=gen.STREAM_SOURCE)
+    ph = gen.antiperiodic_t()
+    for _ in range(warmup):
+        oracle.mdagm(dims, ph, U, x, KAPPA, MU)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        oracle.mdagm(dims, ph, U, x, KAPPA, MU)
+    dt = (time.perf_counter() - t0) / steps
+    return 4 * Vh * FLOP_PER_SITE / dt / 1e9, dt * 1e3, oracle.num_threads()
+
+
+def max_over_ranks(x, world, device):
+    """Max of a per-rank scalar over all ranks (the contract's max-over-ranks timing)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_gflops(world, steps, sites_per_rank, ms_max):
+    """Replicas only: every rank does `steps` steps on its own lattice; whole-job rate."""
+    return world * steps * 4 * sites_per_rank * FLOP_PER_SITE / (ms_max * 1e-3) / 1e9
+
+
+def run_reference(args, rank):
+    if rank != 0:
+        return
+    # bounded sample, sized so that K + W steps end within a few minutes on the host cores
+    dims = REF_DIMS if args.steps + args.warmup <= 100 else REF_DIMS_SMALL
+    gf, ms, threads = oracle_gflops(dims, args.steps, args.warmup)
+    sample = (f"oracle Mhat^dag Mhat (4 hopping terms) per step on a {'x'.join(map(str, dims))} lattice of "
+              f"the same recipe ({np.prod(dims) / np.prod(DIMS):.4f} of the workload's sites), OpenMP over sites")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": gf, "unit": "GFLOPS", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(),
+        "cpu_baseline": {"value": gf, "unit": "GFLOPS", "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": gf, "unit": "GFLOPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_config():
+    return {"workload": "32^3x64 complex double, Haar SU(3) links, Gaussian source, kappa=0.15 mu=0.1, "
+                        "antiperiodic t; one step = one CG iteration on Mhat^dag Mhat (4 hopping + 2 vector launches)",
+            "lattice": list(DIMS), "precision": "double", "recon": 18, "kappa": KAPPA, "mu": MU,
+            "solve_len": SOLVE_LEN,
+            "l2": "inputs larger than L2 (gauge 1.21 GB + 6 half spinors of 201 MB per step vs 126 MB L2)"}
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    import lqcd_inputs as gen
+    import paper_1209_5942_b200.binding as B
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    Vh = int(np.prod(DIMS)) // 2
+    ph = gen.antiperiodic_t()
+    # "replicas only": every rank solves its own seeded system of the same shape
+    seed = gen.BASE_SEED + rank
+    U = gen.gauge_haar(DIMS, seed)
+    b = gen.spinor_gaussian(Vh, seed, gen.STREAM_SOURCE)
+
+    B.lqcd_init(DIMS, ph)
+    stream = torch.cuda.Stream()
+    B.lqcd_set_stream(stream)
+    with torch.cuda.stream(stream):
+        g = B.upload_gauge(U)
+        src = B.upload_spinor(b, 0)
+        x = B.alloc_spinor()
+    stream.synchronize()
+
+    def run_steps(n):
+        done = 0
+        while done < n:
+            k = min(SOLVE_LEN, n - done)
+            B.lqcd_cg_setup(g, src, x, KAPPA, MU, 0.0)
+            B.lqcd_cg_iterate(k)
+            done += k
+
+    # ---- device-resident timing -------------------------------------------------------------
+    run_steps(args.warmup)
+    stream.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    B.lqcd_profile(1)
+    n0 = B.lqcd_launch_count()
+    barrier()
+    with ClockSampler(local_rank) as clk:
+        e0.record(stream)
+        run_steps(args.steps)
+        e1.record(stream)
+        stream.synchronize()
+    barrier()
+    launches = B.lqcd_launch_count() - n0
+    ms_total = e0.elapsed_time(e1)
+    prof = {c: B.lqcd_profile_read(c) for c in range(4)}
+    B.lqcd_profile(0)
+    st = B.lqcd_cg_finish()
+    iters, rr, rt = B.lqcd_cg_stats()
+    last = args.steps % SOLVE_LEN or min(SOLVE_LEN, args.steps)
+    if iters != last or st < 0:
+        raise SystemExit(f"bench: the last solve ran {iters} iterations, expected {last} (status {st})")
+
+    ms_max = max_over_ranks(ms_total, world, "cuda")
+    ms_per_step = ms_max / args.steps
+    value = whole_job_gflops(world, args.steps, Vh, ms_max)
+
+    # ---- roofline of the hopping kernel, from the per-launch events of the timed region -------
+    hop_ms = prof[0][0] + prof[1][0] + prof[2][0]
+    hop_n = prof[0][1] + prof[1][1] + prof[2][1]
+    hop_bytes = Vh * (BYTES_PER_SITE * hop_n + AUX_BYTES_PER_SITE * (prof[1][1] + prof[2][1]))
+    peak, peak_src = measured_peak()
+    achieved = hop_bytes / (hop_ms * 1e-3) / 1e9
+    plain_gbs = Vh * BYTES_PER_SITE * prof[0][1] / (prof[0][0] * 1e-3) / 1e9 if prof[0][1] else None
+    roofline = {
+        "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+        "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH, "peak_source": peak_src,
+        "kernel": "hopping_kernel<double,18,*,*> (all 4 launches of a step)",
+        "launches": hop_n, "avg_launch_us": hop_ms / hop_n * 1e3,
+        "algorithmic_bytes_per_launch": hop_bytes / hop_n,
+        "plain_epilogue_gbs": plain_gbs,
+        "plain_epilogue_gflops": (Vh * FLOP_PER_SITE * prof[0][1] / (prof[0][0] * 1e-3) / 1e9) if prof[0][1] else None,
+        "share_of_step": hop_ms / ms_total,
+        "vector_kernels_share_of_step": prof[3][0] / ms_total,
+    }
+
+    line = {
+        "metric": METRIC, "value": value, "unit": "GFLOPS", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(),
+        "clocks": clk.summary(), "gpu_launches": int(launches), "roofline": roofline,
+        "gbs_effective_step": world * args.steps * Vh * (4 * BYTES_PER_SITE + 2 * AUX_BYTES_PER_SITE + 9 * 192)
+        / (ms_max * 1e-3) / 1e9,
+    }
+
+    # ---- end to end through the host-buffer C-ABI call (pinned host memory) -----------------
+    n_e2e = max(1, min(args.e2e_steps, args.steps))
+    U_pin = torch.from_numpy(U).pin_memory()
+    b_pin = torch.from_numpy(b).pin_memory()
+    x_pin = torch.empty((Vh, 4, 3), dtype=torch.complex128).pin_memory()
+    del U
+    for _ in range(2):
+        B.lqcd_cg_mdagm_host(U_pin, b_pin, x_pin, KAPPA, MU, 0.0, 1)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(n_e2e):
+        B.lqcd_cg_mdagm_host(U_pin, b_pin, x_pin, KAPPA, MU, 0.0, 1)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    barrier()
+    dt = max_over_ranks(dt, world, "cuda")
+    # the amortised figure a user sees: one upload, a whole solve to 1e-10, one download
+    t0 = time.perf_counter()
+    st = B.lqcd_cg_mdagm_host(U_pin, b_pin, x_pin, KAPPA, MU, 1e-10, 2000)
+    dt_solve = time.perf_counter() - t0
+    it_solve, rr, rt = B.lqcd_cg_stats()
+    line["e2e"] = {
+        "value": whole_job_gflops(world, n_e2e, Vh, dt * 1e3), "unit": "GFLOPS",
+        "h2d_bytes_per_step": int(U_pin.numel() * 16 + b_pin.numel() * 16),
+        "d2h_bytes_per_step": int(x_pin.numel() * 16), "steps": n_e2e, "ms_per_step": dt / n_e2e * 1e3,
+        "call": "lqcd_cg_mdagm_host(maxit=1): upload gauge+source, pack, 1 CG iteration (+ true-residual check, "
+                "not counted), unpack, download x",
+        "solve": {"call": "lqcd_cg_mdagm_host(tol=1e-10)", "status": int(st), "iterations": it_solve,
+                  "seconds": dt_solve, "true_rel_resid": rt,
+                  "gflops": world * it_solve * 4 * Vh * FLOP_PER_SITE / dt_solve / 1e9},
+    }
+    del U_pin
+
+    # ---- oracle on the host cores beside it (rank 0, N = 1 only) ------------------------------
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        gf, ms, threads = oracle_gflops(REF_DIMS, 8, 1)
+        line["cpu_baseline"] = {
+            "value": gf, "unit": "GFLOPS", "cores": threads, "kind": "oracle",
+            "sample": f"8 applications of the oracle's Mhat^dag Mhat (4 hopping terms each) on a "
+                      f"{'x'.join(map(str, REF_DIMS))} lattice of the same recipe (1/16 of the workload's sites); "
+                      f"{ms:.0f} ms per application"}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    B.lqcd_finalize()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=400)
+    ap.add_argument("--warmup", type=int, default=40)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

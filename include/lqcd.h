@@ -129,6 +129,14 @@ int lqcd_cg_mdagm_host(const void* gauge_canon_host, const void* b_canon_host, v
 /* Number of kernels this library has launched since lqcd_init (all streams). */
 long long lqcd_launch_count(void);
 
+/* Per-launch device timing.  lqcd_profile(1) starts recording a CUDA-event pair around every
+ * kernel the library launches on its stream (and discards earlier records); lqcd_profile(0)
+ * stops.  lqcd_profile_read synchronises the stream and returns the summed duration and the
+ * launch count of one category: 0 hopping (plain epilogue), 1 hopping + M_ee*aux epilogue,
+ * 2 hopping + M_ee*aux epilogue + fused norm, 3 CG vector kernels, 4 pack/unpack. */
+int lqcd_profile(int enable);
+int lqcd_profile_read(int category, double* total_ms, int* launches);
+
 /* Hopping-kernel thread-block size (tuning knob; 0 restores the default). */
 int lqcd_set_block_size(int threads);
 

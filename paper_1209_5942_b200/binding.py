@@ -22,7 +22,7 @@ SYMBOLS = [
     "lqcd_gauge_bytes", "lqcd_spinor_bytes", "lqcd_pack_gauge", "lqcd_pack_spinor",
     "lqcd_unpack_spinor", "lqcd_dslash_eo", "lqcd_mtm", "lqcd_cg_mdagm", "lqcd_cg_setup",
     "lqcd_cg_iterate", "lqcd_cg_finish", "lqcd_cg_stats", "lqcd_mtm_host", "lqcd_cg_mdagm_host",
-    "lqcd_launch_count", "lqcd_set_block_size",
+    "lqcd_launch_count", "lqcd_set_block_size", "lqcd_profile", "lqcd_profile_read",
 ]
 
 
@@ -60,6 +60,8 @@ def _load():
         "lqcd_mtm_host": [vp, vp, vp, dbl, dbl, i32],
         "lqcd_cg_mdagm_host": [vp, vp, vp, dbl, dbl, dbl, i32],
         "lqcd_set_block_size": [i32],
+        "lqcd_profile": [i32],
+        "lqcd_profile_read": [i32, ctypes.POINTER(dbl), ctypes.POINTER(i32)],
     }
     for name, args in sig.items():
         fn = getattr(lib, name)
@@ -131,6 +133,18 @@ def lqcd_spinor_bytes():
 
 def lqcd_launch_count():
     return int(_lib.lqcd_launch_count())
+
+
+def lqcd_profile(enable):
+    return _check(_lib.lqcd_profile(int(enable)))
+
+
+def lqcd_profile_read(category):
+    """(total_ms, launches) of one kernel category since lqcd_profile(1)."""
+    ms = ctypes.c_double(0.0)
+    n = ctypes.c_int(0)
+    _check(_lib.lqcd_profile_read(category, ctypes.byref(ms), ctypes.byref(n)))
+    return ms.value, n.value
 
 
 def lqcd_pack_gauge(canon_dev, internal_dev):

@@ -13,6 +13,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <vector>
 
 #include "../../include/lqcd.h"
 #include "lqcd_internal.h"
@@ -21,6 +22,32 @@ namespace lqcd {
 
 static std::atomic<long long> g_launches{0};
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+// ---- per-launch event timing (off by default; bench.py turns it on for the roofline figure)
+struct ProfRec { int cat; cudaEvent_t a, b; };
+static bool g_prof_on = false;
+static std::vector<ProfRec> g_prof;
+static std::vector<cudaEvent_t> g_prof_pool;
+static cudaEvent_t prof_event() {
+    cudaEvent_t e = nullptr;
+    if (!g_prof_pool.empty()) { e = g_prof_pool.back(); g_prof_pool.pop_back(); }
+    else cudaEventCreate(&e);
+    return e;
+}
+static void prof_clear() {
+    for (auto& r : g_prof) { g_prof_pool.push_back(r.a); g_prof_pool.push_back(r.b); }
+    g_prof.clear();
+}
+void prof_begin(int category, cudaStream_t st) {
+    if (!g_prof_on) return;
+    ProfRec r; r.cat = category; r.a = prof_event(); r.b = prof_event();
+    cudaEventRecord(r.a, st);
+    g_prof.push_back(r);
+}
+void prof_end(cudaStream_t st) {
+    if (!g_prof_on || g_prof.empty()) return;
+    cudaEventRecord(g_prof.back().b, st);
+}
 
 namespace {
 
@@ -253,6 +280,28 @@ int lqcd_set_block_size(int threads) {
 size_t lqcd_gauge_bytes(void) { return ctx.init ? gauge_bytes_of(ctx.precision, ctx.recon, ctx.geo.Vh) : 0; }
 size_t lqcd_spinor_bytes(void) { return ctx.init ? spinor_bytes_of(ctx.precision, ctx.geo.Vh) : 0; }
 long long lqcd_launch_count(void) { return g_launches.load(); }
+
+int lqcd_profile(int enable) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (enable) { CU(cudaStreamSynchronize(ctx.stream)); prof_clear(); }
+    g_prof_on = enable != 0;
+    return LQCD_OK;
+}
+
+int lqcd_profile_read(int category, double* total_ms, int* launches) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    CU(cudaStreamSynchronize(ctx.stream));
+    double tot = 0.0; int n = 0;
+    for (const auto& r : g_prof) {
+        if (r.cat != category) continue;
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, r.a, r.b));
+        tot += ms; ++n;
+    }
+    if (total_ms) *total_ms = tot;
+    if (launches) *launches = n;
+    return LQCD_OK;
+}
 
 int lqcd_pack_gauge(const void* canon_dev, void* internal_dev) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");

@@ -353,6 +353,7 @@ cudaError_t launch_hopping(int precision, int recon, int dagger, int mode, const
     a.g = g; a.ep = ep; a.out_parity = out_parity; a.red = red; a.scal = scal;
     if (block <= 0 || block > 128 || (block % 32) != 0) block = 128;
     count_launch();
+    ProfScope prof(mode, st);
     if (precision == 0) {
         return recon == 12 ? launch_tr<double, 12>(dagger, mode, a, block, st)
                            : launch_tr<double, 18>(dagger, mode, a, block, st);

@@ -80,6 +80,15 @@ cudaError_t launch_unpack_spinor(int precision, const Geometry& g, const void* i
 
 void count_launch(int n = 1);
 
+// api.cu: optional per-launch event timing (lqcd_profile)
+void prof_begin(int category, cudaStream_t st);
+void prof_end(cudaStream_t st);
+struct ProfScope {
+    cudaStream_t st;
+    ProfScope(int category, cudaStream_t s) : st(s) { prof_begin(category, s); }
+    ~ProfScope() { prof_end(st); }
+};
+
 // Block-wide sum in a fixed order, then election of the last block of the grid,
 // which adds the per-block partials in index order (deterministic for a given
 // grid) and hands the total to `fin`.  All threads of the block must call this.

@@ -107,6 +107,7 @@ cudaError_t launch_pack_gauge(int precision, int recon, const Geometry& g, const
     const size_t n = 8 * (size_t)g.Vh;
     const int grid = (int)((n + PBLOCK - 1) / PBLOCK);
     count_launch();
+    ProfScope prof(4, st);
     const double2* c = (const double2*)canon;
     if (precision == 0) {
         if (recon == 12) pack_gauge_kernel<double, 12><<<grid, PBLOCK, 0, st>>>(g, c, internal);
@@ -122,6 +123,7 @@ cudaError_t launch_pack_spinor(int precision, const Geometry& g, const void* can
                                int /*parity*/, cudaStream_t st) {
     const int grid = (g.Vh + PBLOCK - 1) / PBLOCK;
     count_launch();
+    ProfScope prof(4, st);
     if (precision == 0) pack_spinor_kernel<double><<<grid, PBLOCK, 0, st>>>(g.Vh, (const double2*)canon, internal);
     else                pack_spinor_kernel<float><<<grid, PBLOCK, 0, st>>>(g.Vh, (const double2*)canon, internal);
     return cudaGetLastError();
@@ -131,6 +133,7 @@ cudaError_t launch_unpack_spinor(int precision, const Geometry& g, const void* i
                                  int /*parity*/, cudaStream_t st) {
     const int grid = (g.Vh + PBLOCK - 1) / PBLOCK;
     count_launch();
+    ProfScope prof(4, st);
     if (precision == 0) unpack_spinor_kernel<double><<<grid, PBLOCK, 0, st>>>(g.Vh, internal, (double2*)canon);
     else                unpack_spinor_kernel<float><<<grid, PBLOCK, 0, st>>>(g.Vh, internal, (double2*)canon);
     return cudaGetLastError();

@@ -167,6 +167,7 @@ int vector_grid(size_t n) { return grid_for(n / 2); }  // upper bound over both 
 cudaError_t launch_cg_init(int precision, size_t n, const void* b, void* x, void* r, void* p,
                            double tol, Reduction red, CgScalars* scal, cudaStream_t st) {
     count_launch();
+    ProfScope prof(3, st);
     if (precision == 0) {
         const size_t nv = n / 2;
         cg_init_kernel<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, b, x, r, p, tol, red, scal);
@@ -180,6 +181,7 @@ cudaError_t launch_cg_init(int precision, size_t n, const void* b, void* x, void
 cudaError_t launch_cg_update_xr(int precision, size_t n, void* x, void* r, const void* p,
                                 const void* q, Reduction red, CgScalars* scal, cudaStream_t st) {
     count_launch();
+    ProfScope prof(3, st);
     if (precision == 0) {
         const size_t nv = n / 2;
         cg_update_xr_kernel<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, x, r, p, q, red, scal);
@@ -193,6 +195,7 @@ cudaError_t launch_cg_update_xr(int precision, size_t n, void* x, void* r, const
 cudaError_t launch_cg_update_p(int precision, size_t n, void* p, const void* r, CgScalars* scal,
                                cudaStream_t st) {
     count_launch();
+    ProfScope prof(3, st);
     if (precision == 0) {
         const size_t nv = n / 2;
         cg_update_p_kernel<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, p, r, scal);
@@ -206,6 +209,7 @@ cudaError_t launch_cg_update_p(int precision, size_t n, void* p, const void* r, 
 cudaError_t launch_true_resid(int precision, size_t n, const void* b, const void* ax, Reduction red,
                               CgScalars* scal, cudaStream_t st) {
     count_launch();
+    ProfScope prof(3, st);
     if (precision == 0) {
         const size_t nv = n / 2;
         true_resid_kernel<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, b, ax, red, scal);
