@@ -10,7 +10,7 @@ SOURCES = ["api.cu", "hopping.cu", "vector_ops.cu", "pack.cu"]
 HEADERS = [os.path.join(CSRC, "lqcd_internal.h"), os.path.join(HERE, "..", "include", "lqcd.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-    "--use_fast_math" if False else "-Xptxas=-v", "-Xcompiler", "-fPIC", "-shared",
+    "-Xptxas=-v", "-Xcompiler", "-fPIC", "-shared",
 ]
 
 
@@ -33,7 +33,8 @@ def build(force=False, verbose=False, extra_flags=()):
     """Compile every .cu under csrc/ into paper_1209_5942_b200/liblqcd.so."""
     if not force and not needs_build():
         return LIB
-    cmd = [_nvcc()] + NVCC_FLAGS + list(extra_flags) + ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
+    extra_flags = list(extra_flags) + os.environ.get("LQCD_NVCC_EXTRA", "").split()
+    cmd = [_nvcc()] + NVCC_FLAGS + extra_flags + ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)

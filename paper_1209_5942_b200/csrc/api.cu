@@ -7,7 +7,7 @@
 // chirality chi = +-1 the diagonal terms are the complex numbers (1 + i c chi) and
 // (1 - i c chi)/(1 + c^2); they are folded into the hopping kernel's epilogue:
 //   launch 1: t   = [-kappa (1 - i c chi)/(1 + c^2)] * bracket(in)          (odd sites)
-//   launch 2: out = (1 + i c chi) in + kappa * bracket(t)                  (even sites)
+//   launch 2: out = kappa * (bracket(t) + [(1 + i c chi)/kappa] in)        (even sites)
 #include <atomic>
 #include <cmath>
 #include <cstdarg>
@@ -67,7 +67,6 @@ struct Context {
     CgScalars* scal_host = nullptr;  // pinned, 2 slots
     cudaEvent_t ev[2] = {nullptr, nullptr};
     double* partials = nullptr;
-    unsigned int* ticket = nullptr;
     size_t n_partials = 0;
 
     // host-call staging (owned)
@@ -123,7 +122,6 @@ void free_all() {
     if (ctx.scal) cudaFree(ctx.scal);
     if (ctx.scal_host) cudaFreeHost(ctx.scal_host);
     if (ctx.partials) cudaFree(ctx.partials);
-    if (ctx.ticket) cudaFree(ctx.ticket);
     for (int i = 0; i < 2; ++i) if (ctx.ev[i]) cudaEventDestroy(ctx.ev[i]);
     void** st[] = {&ctx.st_gauge_canon, &ctx.st_gauge, &ctx.st_spinor_canon, &ctx.st_in, &ctx.st_out};
     for (void** p : st) { if (*p) cudaFree(*p); *p = nullptr; }
@@ -135,11 +133,9 @@ int ensure_scalars() {
         CU(cudaMalloc(&ctx.scal, sizeof(CgScalars)));
         CU(cudaMemset(ctx.scal, 0, sizeof(CgScalars)));
         CU(cudaMallocHost(&ctx.scal_host, 2 * sizeof(CgScalars)));
-        CU(cudaMalloc(&ctx.ticket, sizeof(unsigned int)));
-        CU(cudaMemset(ctx.ticket, 0, sizeof(unsigned int)));
         for (int i = 0; i < 2; ++i) CU(cudaEventCreateWithFlags(&ctx.ev[i], cudaEventDisableTiming));
     }
-    const size_t need = (size_t)ctx.geo.Vh / 32 + 64 + (size_t)vector_grid((size_t)24 * ctx.geo.Vh);
+    const size_t need = (size_t)hopping_partials(ctx.geo.Vh, 32) + (size_t)vector_grid((size_t)24 * ctx.geo.Vh) + 64;
     if (need > ctx.n_partials) {
         if (ctx.partials) CU(cudaFree(ctx.partials));
         ctx.partials = nullptr;
@@ -173,7 +169,7 @@ int ensure_buf(void** p, size_t* have, size_t need) {
     return LQCD_OK;
 }
 
-Reduction red() { Reduction r; r.partials = ctx.partials; r.ticket = ctx.ticket; return r; }
+Reduction red() { Reduction r; r.partials = ctx.partials; return r; }
 
 int check_scalar(double v, const char* name) {
     if (!std::isfinite(v)) return fail(LQCD_BAD_ARG, "%s is not finite", name);
@@ -192,12 +188,17 @@ int apply_mhat(const void* gauge, const void* in, void* tmp_odd, void* out, doub
     e1.cd_re = -kappa / d; e1.cd_im = -kappa * c / d;   // chi = -1
     CU(launch_hopping(ctx.precision, ctx.recon, dagger, 0, ctx.geo, e1, gauge, in, tmp_odd, nullptr, 1,
                       red(), scal, ctx.block, ctx.stream));
+    // out = (1 + i c chi) in + kappa * bracket(t) = k2 * (bracket(t) + [(1 + i c chi)/k2] in).
+    // For kappa = 0 launch 1 wrote t = 0 exactly, so bracket(t) = 0 and any k2 != 0 is exact.
+    const double k2 = (kappa != 0.0) ? kappa : 1.0;
     Epilogue e2 = {};
-    e2.cu_re = kappa; e2.cd_re = kappa;
-    e2.du_re = 1.0; e2.du_im = c;
-    e2.dd_re = 1.0; e2.dd_im = -c;
+    e2.cu_re = k2; e2.cd_re = k2;
+    e2.du_re = 1.0 / k2; e2.du_im = c / k2;
+    e2.dd_re = 1.0 / k2; e2.dd_im = -c / k2;
     CU(launch_hopping(ctx.precision, ctx.recon, dagger, norm_to_pAp ? 2 : 1, ctx.geo, e2, gauge, tmp_odd,
                       out, in, 0, red(), scal, ctx.block, ctx.stream));
+    if (norm_to_pAp)
+        CU(launch_finalize(FIN_PAP, red(), hopping_partials(ctx.geo.Vh, ctx.block), 0.0, scal, ctx.stream));
     return LQCD_OK;
 }
 
@@ -335,7 +336,7 @@ int lqcd_dslash_eo(const void* gauge, const void* in, void* out, int parity, dou
     if (rc) return rc;
     Epilogue ep = {};
     ep.cu_re = -kappa; ep.cd_re = -kappa;
-    Reduction none = {nullptr, nullptr};
+    Reduction none = {nullptr};
     CU(launch_hopping(ctx.precision, ctx.recon, 0, 0, ctx.geo, ep, gauge, in, out, nullptr, parity, none,
                       nullptr, ctx.block, ctx.stream));
     return LQCD_OK;

@@ -12,7 +12,7 @@
 //      read-only path with default caching (L1 for x/y neighbours, L2 for z/t)
 //   a4 SU(3) x half spinor (U h forward, U^dag h backward)
 //   a5 boundary phase on the hop that wraps, reconstruction to 4 spin rows, accumulate
-//   a6/a7 epilogue: out = c_chi * acc (+ d_chi * aux), c, d complex per chirality:
+//   a6/a7 epilogue: out = c_chi * (acc + d_chi * aux), c, d complex per chirality:
 //      covers -kappa (dslash_eo), M_oo^{-1} D_oe, and M_ee in - D_eo (.) in one store.
 //
 // Spin projection table (gamma basis of include/lqcd.h; reading G4),
@@ -31,6 +31,9 @@
 
 namespace lqcd {
 namespace {
+
+__device__ __forceinline__ double fma_(double a, double b, double c) { return fma(a, b, c); }
+__device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
 
 // ----------------------------------------------------------------------------- field access
 __device__ __forceinline__ void load_spinor(const void* base, int Vh, int idx, double (&psi)[24]) {
@@ -74,8 +77,8 @@ __device__ __forceinline__ void reconstruct_row2(T (&u)[18]) {
         // (row0 x row1)_c = u0[c1] u1[c2] - u0[c2] u1[c1]
         const T ar = u[2 * c1], ai = u[2 * c1 + 1], br = u[6 + 2 * c2], bi = u[6 + 2 * c2 + 1];
         const T cr = u[2 * c2], ci = u[2 * c2 + 1], dr = u[6 + 2 * c1], di = u[6 + 2 * c1 + 1];
-        const T re = (ar * br - ai * bi) - (cr * dr - ci * di);
-        const T im = (ar * bi + ai * br) - (cr * di + ci * dr);
+        const T re = fma_(ci, di, fma_(-cr, dr, fma_(-ai, bi, ar * br)));
+        const T im = fma_(-ci, dr, fma_(-cr, di, fma_(ai, br, ar * bi)));
         u[12 + 2 * c] = re;
         u[12 + 2 * c + 1] = -im;
     }
@@ -186,13 +189,20 @@ __device__ __forceinline__ void su3_mul(const T (&u)[18], const T (&h)[12], T (&
     for (int k = 0; k < 2; ++k)
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
-            T re = 0, im = 0;
+            // explicit FMA chains: 4 FMA per complex multiply-add (the a*b - c*d form
+            // compiles to MUL + FMA + ADD, 50% more FP64 issue slots and energy)
+            T re = u[2 * (3 * a)] * h[2 * (3 * k)];
+            T im = u[2 * (3 * a)] * h[2 * (3 * k) + 1];
+            re = fma_(-u[2 * (3 * a) + 1], h[2 * (3 * k) + 1], re);
+            im = fma_(u[2 * (3 * a) + 1], h[2 * (3 * k)], im);
 #pragma unroll
-            for (int b = 0; b < 3; ++b) {
+            for (int b = 1; b < 3; ++b) {
                 const T ur = u[2 * (3 * a + b)], ui = u[2 * (3 * a + b) + 1];
                 const T hr = h[2 * (3 * k + b)], hi = h[2 * (3 * k + b) + 1];
-                re += ur * hr - ui * hi;
-                im += ur * hi + ui * hr;
+                re = fma_(ur, hr, re);
+                re = fma_(-ui, hi, re);
+                im = fma_(ur, hi, im);
+                im = fma_(ui, hr, im);
             }
             chi[2 * (3 * k + a)] = re;
             chi[2 * (3 * k + a) + 1] = im;
@@ -206,13 +216,18 @@ __device__ __forceinline__ void su3_dag_mul(const T (&u)[18], const T (&h)[12], 
     for (int k = 0; k < 2; ++k)
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
-            T re = 0, im = 0;
+            T re = u[2 * a] * h[2 * (3 * k)];
+            T im = u[2 * a] * h[2 * (3 * k) + 1];
+            re = fma_(u[2 * a + 1], h[2 * (3 * k) + 1], re);
+            im = fma_(-u[2 * a + 1], h[2 * (3 * k)], im);
 #pragma unroll
-            for (int b = 0; b < 3; ++b) {
+            for (int b = 1; b < 3; ++b) {
                 const T ur = u[2 * (3 * b + a)], ui = u[2 * (3 * b + a) + 1];
                 const T hr = h[2 * (3 * k + b)], hi = h[2 * (3 * k + b) + 1];
-                re += ur * hr + ui * hi;
-                im += ur * hi - ui * hr;
+                re = fma_(ur, hr, re);
+                re = fma_(ui, hi, re);
+                im = fma_(ur, hi, im);
+                im = fma_(-ui, hr, im);
             }
             chi[2 * (3 * k + a)] = re;
             chi[2 * (3 * k + a) + 1] = im;
@@ -246,8 +261,8 @@ __device__ __forceinline__ void hop(T (&acc)[24], const HopArgs& a, int e, int e
 #pragma unroll
         for (int i = 0; i < 6; ++i) {
             const T re = chi[2 * i], im = chi[2 * i + 1];
-            chi[2 * i] = pr * re - pi * im;
-            chi[2 * i + 1] = pr * im + pi * re;
+            chi[2 * i] = fma_(-pi, im, pr * re);
+            chi[2 * i + 1] = fma_(pi, re, pr * im);
         }
     }
     accumulate<MU, S>(acc, chi);
@@ -270,9 +285,24 @@ __global__ void __launch_bounds__(128, LQCD_HOP_MIN_BLOCKS) hopping_kernel(const
         const int r = (x1 + x2 + x3 + a.out_parity) & 1;
         const int s1 = N0h, s2 = N0h * N1, s3 = N0h * N1 * N2;
 
+        // The accumulator starts at d_chi * aux(x) (MODE >= 1), so the M_ee * aux term of the
+        // epilogue costs no registers and its loads are the first in flight instead of a
+        // serialised DRAM round trip after the last hop: out = c_chi * (d_chi aux + bracket).
         T acc[24];
+        if (MODE >= 1) {
+            T x[24];
+            load_spinor(a.aux, Vh, e, x);
+            const T dur = (T)a.ep.du_re, dui = (T)a.ep.du_im, ddr = (T)a.ep.dd_re, ddi = (T)a.ep.dd_im;
 #pragma unroll
-        for (int i = 0; i < 24; ++i) acc[i] = 0;
+            for (int c = 0; c < 12; ++c) {
+                const T dr = (c < 6) ? dur : ddr, di = (c < 6) ? dui : ddi;
+                acc[2 * c] = fma_(-di, x[2 * c + 1], dr * x[2 * c]);
+                acc[2 * c + 1] = fma_(di, x[2 * c], dr * x[2 * c + 1]);
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < 24; ++i) acc[i] = 0;
+        }
 
         {   // mu = 0: neighbour x0h' = x0h + r (forward), x0h + r - 1 (backward)
             const bool wf = (r == 1) && (x0h == N0h - 1);
@@ -302,19 +332,8 @@ __global__ void __launch_bounds__(128, LQCD_HOP_MIN_BLOCKS) hopping_kernel(const
 #pragma unroll
         for (int c = 0; c < 12; ++c) {
             const T cr = (c < 6) ? cur : cdr, ci = (c < 6) ? cui : cdi;
-            o[2 * c] = cr * acc[2 * c] - ci * acc[2 * c + 1];
-            o[2 * c + 1] = cr * acc[2 * c + 1] + ci * acc[2 * c];
-        }
-        if (MODE >= 1) {
-            T x[24];
-            load_spinor(a.aux, Vh, e, x);
-            const T dur = (T)a.ep.du_re, dui = (T)a.ep.du_im, ddr = (T)a.ep.dd_re, ddi = (T)a.ep.dd_im;
-#pragma unroll
-            for (int c = 0; c < 12; ++c) {
-                const T dr = (c < 6) ? dur : ddr, di = (c < 6) ? dui : ddi;
-                o[2 * c] += dr * x[2 * c] - di * x[2 * c + 1];
-                o[2 * c + 1] += dr * x[2 * c + 1] + di * x[2 * c];
-            }
+            o[2 * c] = fma_(-ci, acc[2 * c + 1], cr * acc[2 * c]);
+            o[2 * c + 1] = fma_(ci, acc[2 * c], cr * acc[2 * c + 1]);
         }
         store_spinor(a.out, Vh, e, o);
         if (MODE == 2) {
@@ -322,9 +341,9 @@ __global__ void __launch_bounds__(128, LQCD_HOP_MIN_BLOCKS) hopping_kernel(const
             for (int i = 0; i < 24; ++i) nrm += (double)o[i] * (double)o[i];
         }
     }
-    if (MODE == 2) {
-        CgScalars* scal = a.scal;
-        grid_reduce(nrm, a.red, [scal](double s) { scal->pAp = s; });
+    if (MODE == 2) {  // one partial per warp, plain store; summed by launch_finalize(FIN_PAP)
+        nrm = warp_sum(nrm);
+        if ((threadIdx.x & 31) == 0) a.red.partials[(blockIdx.x * blockDim.x + threadIdx.x) >> 5] = nrm;
     }
 }
 
@@ -343,6 +362,11 @@ cudaError_t launch_tr(int dagger, int mode, const HopArgs& a, int block, cudaStr
 }
 
 }  // namespace
+
+int hopping_partials(int Vh, int block) {
+    if (block <= 0 || block > 128 || (block % 32) != 0) block = 128;
+    return ((Vh + block - 1) / block) * (block / 32);
+}
 
 cudaError_t launch_hopping(int precision, int recon, int dagger, int mode, const Geometry& g,
                            const Epilogue& ep, const void* gauge, const void* in, void* out,

@@ -25,7 +25,8 @@ struct Geometry {
 };
 
 // Coefficients of the fused epilogue, per chirality (u: alpha = 0,1; d: alpha = 2,3):
-//   out = c_chi * acc  (+ d_chi * aux)        acc = bracket of eq. 6
+//   out = c_chi * (bracket + d_chi * aux)     bracket = the sum over 8 hops of eq. 6;
+// the aux term (MODE >= 1) is what the accumulator is initialised with.
 struct Epilogue {
     double cu_re, cu_im, cd_re, cd_im;
     double du_re, du_im, dd_re, dd_im;
@@ -46,14 +47,13 @@ struct CgScalars {
 };
 
 struct Reduction {
-    double* partials;       // one per block
-    unsigned int* ticket;   // last-block election
+    double* partials;       // one per warp (hopping) or per block (vector kernels)
 };
 
 enum { FIN_NONE = 0, FIN_PAP = 1, FIN_BB = 2, FIN_RHO = 3, FIN_TRUE = 4 };
 
 // hopping.cu
-// mode 0: out = c * acc;  mode 1: out = d * aux + c * acc;  mode 2: mode 1 + |out|^2 -> scal->pAp
+// mode 0: out = c * bracket;  mode 1: out = c * (bracket + d * aux);  mode 2: mode 1 + |out|^2 -> scal->pAp
 cudaError_t launch_hopping(int precision, int recon, int dagger, int mode, const Geometry& g,
                            const Epilogue& ep, const void* gauge, const void* in, void* out,
                            const void* aux, int out_parity, Reduction red, CgScalars* scal,
@@ -68,7 +68,11 @@ cudaError_t launch_cg_update_p(int precision, size_t n, void* p, const void* r, 
                                cudaStream_t st);
 cudaError_t launch_true_resid(int precision, size_t n, const void* b, const void* ax, Reduction red,
                               CgScalars* scal, cudaStream_t st);
+// sums red.partials[0..n_partials) in a fixed order and applies the FIN_* action to *scal
+cudaError_t launch_finalize(int fin, Reduction red, int n_partials, double tol, CgScalars* scal,
+                            cudaStream_t st);
 int vector_grid(size_t n);
+int hopping_partials(int Vh, int block);
 
 // pack.cu
 cudaError_t launch_pack_gauge(int precision, int recon, const Geometry& g, const void* canon,
@@ -89,48 +93,16 @@ struct ProfScope {
     ~ProfScope() { prof_end(st); }
 };
 
-// Block-wide sum in a fixed order, then election of the last block of the grid,
-// which adds the per-block partials in index order (deterministic for a given
-// grid) and hands the total to `fin`.  All threads of the block must call this.
-template <typename Fin>
-__device__ __forceinline__ void grid_reduce(double v, Reduction red, Fin fin) {
-    __shared__ double sm[32];
-    __shared__ bool last;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+// Global sums are two-stage and fixed-order (deterministic for a given launch configuration):
+// the producing kernel writes one partial per warp (hopping) or per block (vector kernels)
+// with plain stores -- no fence, no atomic, no last-block election, which cost the hopping
+// kernel 12% when every block had to drain its stores before signalling -- and a one-block
+// finalisation kernel (vector_ops.cu: launch_finalize) adds them in index order and applies
+// the scalar recurrence (FIN_*) on the device.
+__device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    if (lane == 0) sm[warp] = v;
-    __syncthreads();
-    if (warp == 0) {
-        v = (lane < nwarp) ? sm[lane] : 0.0;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-        if (lane == 0) {
-            red.partials[blockIdx.x] = v;
-            __threadfence();
-            const unsigned t = atomicAdd(red.ticket, 1u);
-            last = (t == gridDim.x - 1);
-        }
-    }
-    __syncthreads();
-    if (!last) return;
-    __threadfence();
-    double s = 0.0;
-    for (unsigned i = threadIdx.x; i < gridDim.x; i += blockDim.x) s += __ldcg(red.partials + i);
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-    __syncthreads();
-    if (lane == 0) sm[warp] = s;
-    __syncthreads();
-    if (warp == 0) {
-        s = (lane < nwarp) ? sm[lane] : 0.0;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-        if (lane == 0) {
-            *red.ticket = 0u;
-            fin(s);
-        }
-    }
+    return v;
 }
 
 }  // namespace lqcd

@@ -40,10 +40,65 @@ __device__ __forceinline__ double norm2(float4 v) {
 __device__ __forceinline__ void zero(double2& v) { v = make_double2(0.0, 0.0); }
 __device__ __forceinline__ void zero(float4& v) { v = make_float4(0.f, 0.f, 0.f, 0.f); }
 
+// fixed-order block sum; thread 0 stores the block's partial (no fence, no atomic)
+__device__ __forceinline__ void block_partial(double v, Reduction red) {
+    __shared__ double sm[VBLOCK / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    v = warp_sum(v);
+    if (lane == 0) sm[warp] = v;
+    __syncthreads();
+    if (warp == 0) {
+        v = (lane < VBLOCK / 32) ? sm[lane] : 0.0;
+        v = warp_sum(v);
+        if (lane == 0) red.partials[blockIdx.x] = v;
+    }
+}
+
+// One block: adds the partials in index order (thread-strided, then a fixed tree) and applies
+// the scalar step of the recurrence on the device.
+__global__ void __launch_bounds__(1024) finalize_kernel(int fin, Reduction red, int n, double tol,
+                                                        CgScalars* scal) {
+    __shared__ double sm[32];
+    if (fin != FIN_BB && fin != FIN_TRUE && scal->done) return;
+    double s = 0.0;
+    for (int i = threadIdx.x; i < n; i += 1024) s += red.partials[i];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    s = warp_sum(s);
+    if (lane == 0) sm[warp] = s;
+    __syncthreads();
+    if (warp != 0) return;
+    s = warp_sum(sm[lane]);
+    if (lane != 0) return;
+    if (fin == FIN_PAP) {
+        scal->pAp = s;
+    } else if (fin == FIN_BB) {
+        scal->bb = s;
+        scal->rho = s;
+        scal->pAp = 0.0;
+        scal->beta = 0.0;
+        scal->tol2bb = tol * tol * s;
+        scal->resid_true = 0.0;
+        scal->iters = 0;
+        scal->done = (s == 0.0) ? 1 : 0;
+        scal->status = (s == 0.0) ? 0 : 1;
+    } else if (fin == FIN_RHO) {
+        if (scal->status == -5) return;  // breakdown flagged by cg_update_xr: x, r untouched
+        const double rho = scal->rho;
+        scal->iters += 1;
+        if (s <= scal->tol2bb) {
+            scal->done = 1;
+            scal->status = 0;
+        }
+        scal->beta = s / rho;
+        scal->rho = s;
+    } else if (fin == FIN_TRUE) {
+        scal->resid_true = s;
+    }
+}
+
 template <typename T>
 __global__ void __launch_bounds__(VBLOCK) cg_init_kernel(size_t nvec, const void* b_, void* x_, void* r_,
-                                                         void* p_, double tol, Reduction red,
-                                                         CgScalars* scal) {
+                                                         void* p_, Reduction red) {
     typedef typename VecOf<T>::type V;
     const V* b = (const V*)b_;
     V *x = (V*)x_, *r = (V*)r_, *p = (V*)p_;
@@ -62,17 +117,7 @@ __global__ void __launch_bounds__(VBLOCK) cg_init_kernel(size_t nvec, const void
             s += norm2(v);
         }
     }
-    grid_reduce(s, red, [scal, tol](double bb) {
-        scal->bb = bb;
-        scal->rho = bb;
-        scal->pAp = 0.0;
-        scal->beta = 0.0;
-        scal->tol2bb = tol * tol * bb;
-        scal->resid_true = 0.0;
-        scal->iters = 0;
-        scal->done = (bb == 0.0) ? 1 : 0;
-        scal->status = (bb == 0.0) ? 0 : 1;
-    });
+    block_partial(s, red);
 }
 
 template <typename T>
@@ -83,11 +128,8 @@ __global__ void __launch_bounds__(VBLOCK) cg_update_xr_kernel(size_t nvec, void*
     if (scal->done) return;
     const double rho = scal->rho, pAp = scal->pAp;
     if (!(pAp > 0.0) || !isfinite(pAp) || !isfinite(rho)) {  // breakdown: leave x, r untouched
-        if (blockIdx.x == 0 && threadIdx.x == 0) {
-            scal->status = -5;
-            scal->done = 1;
-        }
-        return;
+        if (blockIdx.x == 0 && threadIdx.x == 0) scal->status = -5;  // done is set by the next
+        return;                                                          // kernel (cg_update_p)
     }
     const double alpha = rho / pAp;
     V *x = (V*)x_, *r = (V*)r_;
@@ -110,15 +152,7 @@ __global__ void __launch_bounds__(VBLOCK) cg_update_xr_kernel(size_t nvec, void*
             s += norm2(rn);
         }
     }
-    grid_reduce(s, red, [scal, rho](double rho1) {
-        scal->iters += 1;
-        if (rho1 <= scal->tol2bb) {
-            scal->done = 1;
-            scal->status = 0;
-        }
-        scal->beta = rho1 / rho;
-        scal->rho = rho1;
-    });
+    block_partial(s, red);
 }
 
 template <typename T>
@@ -126,6 +160,10 @@ __global__ void __launch_bounds__(VBLOCK) cg_update_p_kernel(size_t nvec, void* 
                                                              CgScalars* scal) {
     typedef typename VecOf<T>::type V;
     if (scal->done) return;
+    if (scal->status == -5) {  // breakdown: freeze the solve (all blocks read status before any writes done)
+        if (blockIdx.x == 0 && threadIdx.x == 0) scal->done = 1;
+        return;
+    }
     const double beta = scal->beta;
     V* p = (V*)p_;
     const V* r = (const V*)r_;
@@ -145,7 +183,7 @@ __global__ void __launch_bounds__(VBLOCK) cg_update_p_kernel(size_t nvec, void* 
 
 template <typename T>
 __global__ void __launch_bounds__(VBLOCK) true_resid_kernel(size_t nvec, const void* b_, const void* ax_,
-                                                            Reduction red, CgScalars* scal) {
+                                                            Reduction red) {
     typedef typename VecOf<T>::type V;
     const V *b = (const V*)b_, *ax = (const V*)ax_;
     const size_t base = (size_t)blockIdx.x * (VBLOCK * VUNROLL) + threadIdx.x;
@@ -155,7 +193,7 @@ __global__ void __launch_bounds__(VBLOCK) true_resid_kernel(size_t nvec, const v
         const size_t i = base + (size_t)k * VBLOCK;
         if (i < nvec) s += norm2(sub(__ldg(b + i), __ldg(ax + i)));
     }
-    grid_reduce(s, red, [scal](double t) { scal->resid_true = t; });
+    block_partial(s, red);
 }
 
 inline int grid_for(size_t nvec) { return (int)((nvec + VBLOCK * VUNROLL - 1) / (VBLOCK * VUNROLL)); }
@@ -164,30 +202,42 @@ inline int grid_for(size_t nvec) { return (int)((nvec + VBLOCK * VUNROLL - 1) / 
 
 int vector_grid(size_t n) { return grid_for(n / 2); }  // upper bound over both precisions
 
+cudaError_t launch_finalize(int fin, Reduction red, int n_partials, double tol, CgScalars* scal,
+                            cudaStream_t st) {
+    count_launch();
+    ProfScope prof(3, st);
+    finalize_kernel<<<1, 1024, 0, st>>>(fin, red, n_partials, tol, scal);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_cg_init(int precision, size_t n, const void* b, void* x, void* r, void* p,
                            double tol, Reduction red, CgScalars* scal, cudaStream_t st) {
-    count_launch();
+    count_launch(2);
     ProfScope prof(3, st);
     if (precision == 0) {
         const size_t nv = n / 2;
-        cg_init_kernel<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, b, x, r, p, tol, red, scal);
+        cg_init_kernel<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, b, x, r, p, red);
+        finalize_kernel<<<1, 1024, 0, st>>>(FIN_BB, red, grid_for(nv), tol, scal);
     } else {
         const size_t nv = n / 4;
-        cg_init_kernel<float><<<grid_for(nv), VBLOCK, 0, st>>>(nv, b, x, r, p, tol, red, scal);
+        cg_init_kernel<float><<<grid_for(nv), VBLOCK, 0, st>>>(nv, b, x, r, p, red);
+        finalize_kernel<<<1, 1024, 0, st>>>(FIN_BB, red, grid_for(nv), tol, scal);
     }
     return cudaGetLastError();
 }
 
 cudaError_t launch_cg_update_xr(int precision, size_t n, void* x, void* r, const void* p,
                                 const void* q, Reduction red, CgScalars* scal, cudaStream_t st) {
-    count_launch();
+    count_launch(2);
     ProfScope prof(3, st);
     if (precision == 0) {
         const size_t nv = n / 2;
         cg_update_xr_kernel<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, x, r, p, q, red, scal);
+        finalize_kernel<<<1, 1024, 0, st>>>(FIN_RHO, red, grid_for(nv), 0.0, scal);
     } else {
         const size_t nv = n / 4;
         cg_update_xr_kernel<float><<<grid_for(nv), VBLOCK, 0, st>>>(nv, x, r, p, q, red, scal);
+        finalize_kernel<<<1, 1024, 0, st>>>(FIN_RHO, red, grid_for(nv), 0.0, scal);
     }
     return cudaGetLastError();
 }
@@ -208,14 +258,16 @@ cudaError_t launch_cg_update_p(int precision, size_t n, void* p, const void* r, 
 
 cudaError_t launch_true_resid(int precision, size_t n, const void* b, const void* ax, Reduction red,
                               CgScalars* scal, cudaStream_t st) {
-    count_launch();
+    count_launch(2);
     ProfScope prof(3, st);
     if (precision == 0) {
         const size_t nv = n / 2;
-        true_resid_kernel<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, b, ax, red, scal);
+        true_resid_kernel<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, b, ax, red);
+        finalize_kernel<<<1, 1024, 0, st>>>(FIN_TRUE, red, grid_for(nv), 0.0, scal);
     } else {
         const size_t nv = n / 4;
-        true_resid_kernel<float><<<grid_for(nv), VBLOCK, 0, st>>>(nv, b, ax, red, scal);
+        true_resid_kernel<float><<<grid_for(nv), VBLOCK, 0, st>>>(nv, b, ax, red);
+        finalize_kernel<<<1, 1024, 0, st>>>(FIN_TRUE, red, grid_for(nv), 0.0, scal);
     }
     return cudaGetLastError();
 }
