@@ -8,7 +8,8 @@ kappa = 0.15, mu = 0.1, antiperiodic in time; synthetic seeded inputs
 
 One step = one CG iteration on Mhat^dag Mhat:
 four hopping launches with fused diagonal-term epilogues (one with the fused
-<p,Ap> reduction) + the two fused vector kernels.  K steps are run as solves of
+<p,Ap> partial sums) + the two fused vector kernels + two one-block finalisation
+kernels (8 launches).  K steps are run as solves of
 SOLVE_LEN iterations each (a real solve at this configuration takes about that
 many), the one-launch solve setup included in the timed region; the recursive
 residual would otherwise underflow after several hundred iterations.
@@ -186,7 +187,7 @@ def run_reference(args, rank):
 
 def workload_config():
     return {"workload": "32^3x64 complex double, Haar SU(3) links, Gaussian source, kappa=0.15 mu=0.1, "
-                        "antiperiodic t; one step = one CG iteration on Mhat^dag Mhat (4 hopping + 2 vector launches)",
+                        "antiperiodic t; one step = one CG iteration on Mhat^dag Mhat (4 hopping + 2 vector + 2 one-block finalise launches)",
             "lattice": list(DIMS), "precision": "double", "recon": 18, "kappa": KAPPA, "mu": MU,
             "solve_len": SOLVE_LEN,
             "l2": "inputs larger than L2 (gauge 1.21 GB + 6 half spinors of 201 MB per step vs 126 MB L2)"}
@@ -284,7 +285,8 @@ def run_ours(args, rank, world, local_rank):
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(),
         "clocks": clk.summary(), "gpu_launches": int(launches), "roofline": roofline,
-        "gbs_effective_step": world * args.steps * Vh * (4 * BYTES_PER_SITE + 2 * AUX_BYTES_PER_SITE + 9 * 192)
+        # whole-step algorithmic bytes: 4 hops + 2 aux reads + 8 field transfers of the vector kernels
+        "gbs_effective_step": world * args.steps * Vh * (4 * BYTES_PER_SITE + 2 * AUX_BYTES_PER_SITE + 8 * 192)
         / (ms_max * 1e-3) / 1e9,
     }
 

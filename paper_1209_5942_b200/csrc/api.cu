@@ -187,7 +187,7 @@ int apply_mhat(const void* gauge, const void* in, void* tmp_odd, void* out, doub
     e1.cu_re = -kappa / d; e1.cu_im = +kappa * c / d;   // -kappa (1 - i c)/(1 + c^2), chi = +1
     e1.cd_re = -kappa / d; e1.cd_im = -kappa * c / d;   // chi = -1
     CU(launch_hopping(ctx.precision, ctx.recon, dagger, 0, ctx.geo, e1, gauge, in, tmp_odd, nullptr, 1,
-                      red(), scal, ctx.block, ctx.stream));
+                      0, red(), scal, ctx.block, ctx.stream));
     // out = (1 + i c chi) in + kappa * bracket(t) = k2 * (bracket(t) + [(1 + i c chi)/k2] in).
     // For kappa = 0 launch 1 wrote t = 0 exactly, so bracket(t) = 0 and any k2 != 0 is exact.
     const double k2 = (kappa != 0.0) ? kappa : 1.0;
@@ -196,7 +196,7 @@ int apply_mhat(const void* gauge, const void* in, void* tmp_odd, void* out, doub
     e2.du_re = 1.0 / k2; e2.du_im = c / k2;
     e2.dd_re = 1.0 / k2; e2.dd_im = -c / k2;
     CU(launch_hopping(ctx.precision, ctx.recon, dagger, norm_to_pAp ? 2 : 1, ctx.geo, e2, gauge, tmp_odd,
-                      out, in, 0, red(), scal, ctx.block, ctx.stream));
+                      out, in, 0, 1, red(), scal, ctx.block, ctx.stream));
     if (norm_to_pAp)
         CU(launch_finalize(FIN_PAP, red(), hopping_partials(ctx.geo.Vh, ctx.block), 0.0, scal, ctx.stream));
     return LQCD_OK;
@@ -209,8 +209,8 @@ int enqueue_iteration() {
     if (rc) return rc;
     rc = apply_mhat(ctx.cg_gauge, t2, t1, q, ctx.cg_kappa, ctx.cg_mu, 1, false, ctx.scal);
     if (rc) return rc;
-    CU(launch_cg_update_xr(ctx.precision, n, ctx.cg_x, r, p, q, red(), ctx.scal, ctx.stream));
-    CU(launch_cg_update_p(ctx.precision, n, p, r, ctx.scal, ctx.stream));
+    CU(launch_cg_update_r(ctx.precision, n, r, q, 0, red(), ctx.scal, ctx.stream));
+    CU(launch_cg_update_xp(ctx.precision, n, ctx.cg_x, p, r, 1, ctx.scal, ctx.stream));
     return LQCD_OK;
 }
 
@@ -337,8 +337,8 @@ int lqcd_dslash_eo(const void* gauge, const void* in, void* out, int parity, dou
     Epilogue ep = {};
     ep.cu_re = -kappa; ep.cd_re = -kappa;
     Reduction none = {nullptr};
-    CU(launch_hopping(ctx.precision, ctx.recon, 0, 0, ctx.geo, ep, gauge, in, out, nullptr, parity, none,
-                      nullptr, ctx.block, ctx.stream));
+    CU(launch_hopping(ctx.precision, ctx.recon, 0, 0, ctx.geo, ep, gauge, in, out, nullptr, parity, 0,
+                      none, nullptr, ctx.block, ctx.stream));
     return LQCD_OK;
 }
 

@@ -242,6 +242,7 @@ struct HopArgs {
     Geometry g;
     Epilogue ep;
     int out_parity;
+    int reverse;   // traverse the sites in descending order (see lqcd_internal.h "snake order")
     Reduction red;
     CgScalars* scal;
 };
@@ -272,7 +273,8 @@ template <typename T, int RECON, int DAG, int MODE>
 __global__ void __launch_bounds__(128, LQCD_HOP_MIN_BLOCKS) hopping_kernel(const HopArgs a) {
     if (a.scal != nullptr && a.scal->done) return;
     const int Vh = a.g.Vh;
-    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    const int blk = a.reverse ? (int)(gridDim.x - 1 - blockIdx.x) : (int)blockIdx.x;
+    const int e = blk * blockDim.x + threadIdx.x;
     double nrm = 0.0;
     if (e < Vh) {
         // a1: e -> (x0h, x1, x2, x3); r = x0 mod 2 follows from the parity
@@ -343,7 +345,7 @@ __global__ void __launch_bounds__(128, LQCD_HOP_MIN_BLOCKS) hopping_kernel(const
     }
     if (MODE == 2) {  // one partial per warp, plain store; summed by launch_finalize(FIN_PAP)
         nrm = warp_sum(nrm);
-        if ((threadIdx.x & 31) == 0) a.red.partials[(blockIdx.x * blockDim.x + threadIdx.x) >> 5] = nrm;
+        if ((threadIdx.x & 31) == 0) a.red.partials[(blk * blockDim.x + threadIdx.x) >> 5] = nrm;
     }
 }
 
@@ -370,9 +372,10 @@ int hopping_partials(int Vh, int block) {
 
 cudaError_t launch_hopping(int precision, int recon, int dagger, int mode, const Geometry& g,
                            const Epilogue& ep, const void* gauge, const void* in, void* out,
-                           const void* aux, int out_parity, Reduction red, CgScalars* scal,
-                           int block, cudaStream_t st) {
+                           const void* aux, int out_parity, int reverse, Reduction red,
+                           CgScalars* scal, int block, cudaStream_t st) {
     HopArgs a;
+    a.reverse = reverse;
     a.gauge = gauge; a.in = in; a.out = out; a.aux = aux;
     a.g = g; a.ep = ep; a.out_parity = out_parity; a.red = red; a.scal = scal;
     if (block <= 0 || block > 128 || (block % 32) != 0) block = 128;

@@ -37,13 +37,14 @@ struct CgScalars {
     double rho;        // |r|^2
     double pAp;        // <p, A p> = |Mhat p|^2
     double beta;
+    double alpha;      // rho / pAp of the current iteration (written by cg_update_r)
     double bb;         // |b|^2
     double tol2bb;     // tol^2 |b|^2
     double resid_true; // |b - A x|^2
     int iters;
     int done;          // 1 once converged / broken down: later kernels are no-ops
     int status;        // LQCD_OK / LQCD_NOT_CONVERGED / LQCD_BREAKDOWN
-    int pad;
+    int upd;           // 1 if this iteration updated r, i.e. cg_update_xp has an x-update to apply
 };
 
 struct Reduction {
@@ -52,20 +53,24 @@ struct Reduction {
 
 enum { FIN_NONE = 0, FIN_PAP = 1, FIN_BB = 2, FIN_RHO = 3, FIN_TRUE = 4 };
 
+// "Snake order": consecutive kernels of a chain traverse the sites in opposite directions
+// (reverse = 0, 1, 0, 1, ...).  A field is 201 MB at 32^3 x 64 and L2 holds ~126 MB, so the
+// part of its output a kernel wrote last is still in L2 when the next kernel starts; starting
+// the next kernel at that end turns part of its compulsory DRAM reads into L2 hits.
 // hopping.cu
 // mode 0: out = c * bracket;  mode 1: out = c * (bracket + d * aux);  mode 2: mode 1 + |out|^2 -> scal->pAp
 cudaError_t launch_hopping(int precision, int recon, int dagger, int mode, const Geometry& g,
                            const Epilogue& ep, const void* gauge, const void* in, void* out,
-                           const void* aux, int out_parity, Reduction red, CgScalars* scal,
-                           int block, cudaStream_t st);
+                           const void* aux, int out_parity, int reverse, Reduction red,
+                           CgScalars* scal, int block, cudaStream_t st);
 
 // vector_ops.cu  (n = number of reals in a half-spinor field = 24 Vh)
 cudaError_t launch_cg_init(int precision, size_t n, const void* b, void* x, void* r, void* p,
                            double tol, Reduction red, CgScalars* scal, cudaStream_t st);
-cudaError_t launch_cg_update_xr(int precision, size_t n, void* x, void* r, const void* p,
-                                const void* q, Reduction red, CgScalars* scal, cudaStream_t st);
-cudaError_t launch_cg_update_p(int precision, size_t n, void* p, const void* r, CgScalars* scal,
-                               cudaStream_t st);
+cudaError_t launch_cg_update_r(int precision, size_t n, void* r, const void* q, int reverse,
+                               Reduction red, CgScalars* scal, cudaStream_t st);
+cudaError_t launch_cg_update_xp(int precision, size_t n, void* x, void* p, const void* r, int reverse,
+                                CgScalars* scal, cudaStream_t st);
 cudaError_t launch_true_resid(int precision, size_t n, const void* b, const void* ax, Reduction red,
                               CgScalars* scal, cudaStream_t st);
 // sums red.partials[0..n_partials) in a fixed order and applies the FIN_* action to *scal

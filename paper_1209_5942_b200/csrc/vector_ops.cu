@@ -4,11 +4,12 @@
 // 128-bit loads, warp-shuffle block sums, last-block finalisation in a fixed
 // order so that alpha, beta and the convergence decision never leave the device.
 //
-//   cg_init      x = 0, r = p = b, rho = bb = |b|^2
-//   cg_update_xr alpha = rho / pAp; x += alpha p; r -= alpha q; rho' = |r|^2;
-//                last block: iters++, done = (rho' <= tol^2 bb), beta = rho'/rho, rho = rho'
-//   cg_update_p  p = r + beta p
-//   true_resid   |b - Ax|^2
+//   cg_init      x = 0, r = p = b; finalize(FIN_BB): rho = bb = |b|^2
+//   cg_update_r  alpha = rho / pAp; r -= alpha q; partial |r|^2            (3 fields of traffic)
+//                finalize(FIN_RHO): iters++, done = (rho' <= tol^2 bb), beta = rho'/rho, rho = rho'
+//   cg_update_xp x += alpha p; p = r + beta p (p only while not converged)  (5 fields of traffic)
+//   true_resid   |b - Ax|^2; finalize(FIN_TRUE)
+// i.e. 8 field transfers per iteration instead of the 9 of (x,r | p) or the 12 of unfused BLAS-1.
 // Reductions accumulate in double whatever the field precision.
 #include "lqcd_internal.h"
 
@@ -59,7 +60,10 @@ __device__ __forceinline__ void block_partial(double v, Reduction red) {
 __global__ void __launch_bounds__(1024) finalize_kernel(int fin, Reduction red, int n, double tol,
                                                         CgScalars* scal) {
     __shared__ double sm[32];
-    if (fin != FIN_BB && fin != FIN_TRUE && scal->done) return;
+    if (fin != FIN_BB && fin != FIN_TRUE && scal->done) {
+        if (fin == FIN_RHO && threadIdx.x == 0) scal->upd = 0;  // nothing for cg_update_xp to apply
+        return;
+    }
     double s = 0.0;
     for (int i = threadIdx.x; i < n; i += 1024) s += red.partials[i];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -81,10 +85,16 @@ __global__ void __launch_bounds__(1024) finalize_kernel(int fin, Reduction red, 
         scal->iters = 0;
         scal->done = (s == 0.0) ? 1 : 0;
         scal->status = (s == 0.0) ? 0 : 1;
+        scal->upd = 0;
     } else if (fin == FIN_RHO) {
-        if (scal->status == -5) return;  // breakdown flagged by cg_update_xr: x, r untouched
+        if (scal->status == -5) {  // breakdown flagged by cg_update_r: r untouched, freeze the solve
+            scal->done = 1;
+            scal->upd = 0;
+            return;
+        }
         const double rho = scal->rho;
         scal->iters += 1;
+        scal->upd = 1;
         if (s <= scal->tol2bb) {
             scal->done = 1;
             scal->status = 0;
@@ -121,32 +131,32 @@ __global__ void __launch_bounds__(VBLOCK) cg_init_kernel(size_t nvec, const void
 }
 
 template <typename T>
-__global__ void __launch_bounds__(VBLOCK) cg_update_xr_kernel(size_t nvec, void* x_, void* r_,
-                                                              const void* p_, const void* q_,
-                                                              Reduction red, CgScalars* scal) {
+__global__ void __launch_bounds__(VBLOCK) cg_update_r_kernel(size_t nvec, void* r_, const void* q_,
+                                                             int reverse, Reduction red, CgScalars* scal) {
     typedef typename VecOf<T>::type V;
     if (scal->done) return;
     const double rho = scal->rho, pAp = scal->pAp;
-    if (!(pAp > 0.0) || !isfinite(pAp) || !isfinite(rho)) {  // breakdown: leave x, r untouched
-        if (blockIdx.x == 0 && threadIdx.x == 0) scal->status = -5;  // done is set by the next
-        return;                                                          // kernel (cg_update_p)
+    if (!(pAp > 0.0) || !isfinite(pAp) || !isfinite(rho)) {  // breakdown: leave r untouched
+        if (blockIdx.x == 0 && threadIdx.x == 0) scal->status = -5;
+        return;
     }
     const double alpha = rho / pAp;
-    V *x = (V*)x_, *r = (V*)r_;
-    const V *p = (const V*)p_, *q = (const V*)q_;
-    const size_t base = (size_t)blockIdx.x * (VBLOCK * VUNROLL) + threadIdx.x;
-    V xv[VUNROLL], rv[VUNROLL], pv[VUNROLL], qv[VUNROLL];
+    if (blockIdx.x == 0 && threadIdx.x == 0) scal->alpha = alpha;  // for cg_update_xp
+    V* r = (V*)r_;
+    const V* q = (const V*)q_;
+    const size_t blk = reverse ? (gridDim.x - 1 - blockIdx.x) : blockIdx.x;
+    const size_t base = blk * (VBLOCK * VUNROLL) + threadIdx.x;
+    V rv[VUNROLL], qv[VUNROLL];
 #pragma unroll
     for (int k = 0; k < VUNROLL; ++k) {
         const size_t i = base + (size_t)k * VBLOCK;
-        if (i < nvec) { xv[k] = x[i]; rv[k] = r[i]; pv[k] = __ldg(p + i); qv[k] = __ldcs(q + i); }
+        if (i < nvec) { rv[k] = r[i]; qv[k] = __ldcs(q + i); }
     }
     double s = 0.0;
 #pragma unroll
     for (int k = 0; k < VUNROLL; ++k) {
         const size_t i = base + (size_t)k * VBLOCK;
         if (i < nvec) {
-            x[i] = axpy(alpha, pv[k], xv[k]);
             const V rn = axpy(-alpha, qv[k], rv[k]);
             r[i] = rn;
             s += norm2(rn);
@@ -156,28 +166,30 @@ __global__ void __launch_bounds__(VBLOCK) cg_update_xr_kernel(size_t nvec, void*
 }
 
 template <typename T>
-__global__ void __launch_bounds__(VBLOCK) cg_update_p_kernel(size_t nvec, void* p_, const void* r_,
-                                                             CgScalars* scal) {
+__global__ void __launch_bounds__(VBLOCK) cg_update_xp_kernel(size_t nvec, void* x_, void* p_,
+                                                              const void* r_, int reverse,
+                                                              CgScalars* scal) {
     typedef typename VecOf<T>::type V;
-    if (scal->done) return;
-    if (scal->status == -5) {  // breakdown: freeze the solve (all blocks read status before any writes done)
-        if (blockIdx.x == 0 && threadIdx.x == 0) scal->done = 1;
-        return;
-    }
-    const double beta = scal->beta;
-    V* p = (V*)p_;
+    if (!scal->upd) return;            // no r-update happened in this iteration
+    const bool more = !scal->done;     // converged in this iteration: x gets its last update, p is dead
+    const double alpha = scal->alpha, beta = scal->beta;
+    V *x = (V*)x_, *p = (V*)p_;
     const V* r = (const V*)r_;
-    const size_t base = (size_t)blockIdx.x * (VBLOCK * VUNROLL) + threadIdx.x;
-    V pv[VUNROLL], rv[VUNROLL];
+    const size_t blk = reverse ? (gridDim.x - 1 - blockIdx.x) : blockIdx.x;
+    const size_t base = blk * (VBLOCK * VUNROLL) + threadIdx.x;
+    V xv[VUNROLL], pv[VUNROLL], rv[VUNROLL];
 #pragma unroll
     for (int k = 0; k < VUNROLL; ++k) {
         const size_t i = base + (size_t)k * VBLOCK;
-        if (i < nvec) { pv[k] = p[i]; rv[k] = __ldg(r + i); }
+        if (i < nvec) { xv[k] = x[i]; pv[k] = p[i]; if (more) rv[k] = __ldg(r + i); }
     }
 #pragma unroll
     for (int k = 0; k < VUNROLL; ++k) {
         const size_t i = base + (size_t)k * VBLOCK;
-        if (i < nvec) p[i] = axpy(beta, pv[k], rv[k]);
+        if (i < nvec) {
+            x[i] = axpy(alpha, pv[k], xv[k]);
+            if (more) p[i] = axpy(beta, pv[k], rv[k]);
+        }
     }
 }
 
@@ -226,32 +238,32 @@ cudaError_t launch_cg_init(int precision, size_t n, const void* b, void* x, void
     return cudaGetLastError();
 }
 
-cudaError_t launch_cg_update_xr(int precision, size_t n, void* x, void* r, const void* p,
-                                const void* q, Reduction red, CgScalars* scal, cudaStream_t st) {
+cudaError_t launch_cg_update_r(int precision, size_t n, void* r, const void* q, int reverse,
+                               Reduction red, CgScalars* scal, cudaStream_t st) {
     count_launch(2);
     ProfScope prof(3, st);
     if (precision == 0) {
         const size_t nv = n / 2;
-        cg_update_xr_kernel<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, x, r, p, q, red, scal);
+        cg_update_r_kernel<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, r, q, reverse, red, scal);
         finalize_kernel<<<1, 1024, 0, st>>>(FIN_RHO, red, grid_for(nv), 0.0, scal);
     } else {
         const size_t nv = n / 4;
-        cg_update_xr_kernel<float><<<grid_for(nv), VBLOCK, 0, st>>>(nv, x, r, p, q, red, scal);
+        cg_update_r_kernel<float><<<grid_for(nv), VBLOCK, 0, st>>>(nv, r, q, reverse, red, scal);
         finalize_kernel<<<1, 1024, 0, st>>>(FIN_RHO, red, grid_for(nv), 0.0, scal);
     }
     return cudaGetLastError();
 }
 
-cudaError_t launch_cg_update_p(int precision, size_t n, void* p, const void* r, CgScalars* scal,
-                               cudaStream_t st) {
+cudaError_t launch_cg_update_xp(int precision, size_t n, void* x, void* p, const void* r, int reverse,
+                                CgScalars* scal, cudaStream_t st) {
     count_launch();
     ProfScope prof(3, st);
     if (precision == 0) {
         const size_t nv = n / 2;
-        cg_update_p_kernel<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, p, r, scal);
+        cg_update_xp_kernel<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, x, p, r, reverse, scal);
     } else {
         const size_t nv = n / 4;
-        cg_update_p_kernel<float><<<grid_for(nv), VBLOCK, 0, st>>>(nv, p, r, scal);
+        cg_update_xp_kernel<float><<<grid_for(nv), VBLOCK, 0, st>>>(nv, x, p, r, reverse, scal);
     }
     return cudaGetLastError();
 }
