@@ -46,9 +46,10 @@ REF_DIMS_SMALL = (8, 8, 8, 16)  # used by --impl reference when K + W > 100 step
 KAPPA, MU = 0.15, 0.1
 SOLVE_LEN = 40
 METRIC = "D_tm GFLOPS (1320 flop/site) & achieved HBM GB/s vs B200 peak, double"
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the plain hopping kernel at this
-# workload, from the committed ncu --set full capture (profiles/); None until captured.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+# dram__bytes_read.sum + dram__bytes_write.sum per hopping launch at this workload (mean of the
+# four launches of one step; algorithmic mean 1.7113 GB), from the committed ncu --set full
+# capture profiles/r01_hopping_full.md.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 1694517378
 
 
 def measured_peak():
