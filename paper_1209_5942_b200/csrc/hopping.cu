@@ -25,8 +25,15 @@
 // stencil (DAG) swaps them.
 #include "lqcd_internal.h"
 
+// CTAs of 128 threads per SM the register allocation aims at.  3 (168 registers) is best for
+// double and for single/18 (measured: 2 and 4 are ~20% slower in double; 4, 5, 6 are 4-15% slower
+// for single/18).  Single/12 moves the fewest DRAM bytes per thread and direction (60 B), so at
+// 12 warps/SM it cannot keep enough requests in flight: 7 CTAs (72 registers) is 27% faster.
 #ifndef LQCD_HOP_MIN_BLOCKS
 #define LQCD_HOP_MIN_BLOCKS 3
+#endif
+#ifndef LQCD_HOP_MIN_BLOCKS_F12
+#define LQCD_HOP_MIN_BLOCKS_F12 7
 #endif
 
 namespace lqcd {
@@ -270,7 +277,8 @@ __device__ __forceinline__ void hop(T (&acc)[24], const HopArgs& a, int e, int e
 }
 
 template <typename T, int RECON, int DAG, int MODE>
-__global__ void __launch_bounds__(128, LQCD_HOP_MIN_BLOCKS) hopping_kernel(const HopArgs a) {
+__global__ void __launch_bounds__(128, (sizeof(T) == 4 && RECON == 12) ? LQCD_HOP_MIN_BLOCKS_F12 : LQCD_HOP_MIN_BLOCKS)
+hopping_kernel(const HopArgs a) {
     if (a.scal != nullptr && a.scal->done) return;
     const int Vh = a.g.Vh;
     const int blk = a.reverse ? (int)(gridDim.x - 1 - blockIdx.x) : (int)blockIdx.x;

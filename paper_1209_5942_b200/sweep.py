@@ -1,0 +1,182 @@
+#!/usr/bin/env python
+"""sweep.py -- timings of the BASELINE.json configurations 3, 4, 5 and of the paper's thermal
+lattice shapes (Fig. 7), one JSON line each.  A user-facing companion of bench.py:
+
+    python -m paper_1209_5942_b200.sweep [--configs 3,4,5,thermal] [--out FILE]
+
+config 3: 16^3x32, near-identity links, kappa=.16 mu=.05: 10 warm-up + 100 timed D_eo/D_oe
+          applications, 5 repeats, median (working set fits L2: not a HBM roofline figure)
+config 4: 24^3x48 Haar links: CG on Mhat^dag Mhat to 1e-10; iterations, time to solution,
+          per-iteration split between hopping launches and vector kernels
+config 5: 32^3x64, double/single x 18/12-real links: 20 warm-up + 200 timed D-slash applications
+thermal : N_sigma in {16,24,32,48} x N_tau in {4,8,12,16}, double/18 D-slash
+
+GFLOPS at 1320 flop per output site (BASELINE metric); "gbs_effective" counts the algorithmic
+bytes (each link, each input site and each output once); "gbs_paper_accounting" counts the
+paper's 8 links + 8 spinors + 1 store per site for comparison with its Fig. 7.
+"""
+import argparse
+import json
+import os
+import sys
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import lqcd_inputs as gen  # noqa: E402
+from paper_1209_5942_b200 import binding as B  # noqa: E402
+
+FLOP = 1320
+NOMINAL_GBS = 8000.0
+
+
+def measured_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"])
+    except Exception:
+        return 6650.0
+
+
+def site_bytes(precision, recon):
+    real = 8 if precision == 0 else 4
+    link, spinor = recon * real, 24 * real
+    return 8 * link + 2 * spinor, 8 * link + 9 * spinor
+
+
+def time_dslash(dims, U, precision, recon, kappa, warm, reps, repeats, stream):
+    Vh = int(np.prod(dims)) // 2
+    B.lqcd_init(dims, gen.antiperiodic_t())
+    B.lqcd_set_format(precision, recon)
+    B.lqcd_set_stream(stream)
+    with torch.cuda.stream(stream):
+        g = B.upload_gauge(U)
+        a = B.upload_spinor(gen.spinor_gaussian(Vh), 1)
+        b = B.alloc_spinor()
+        for _ in range(warm // 2):
+            B.lqcd_dslash_eo(g, a, b, 0, kappa)
+            B.lqcd_dslash_eo(g, b, a, 1, kappa)
+        times = []
+        for _ in range(repeats):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            stream.synchronize()
+            e0.record(stream)
+            for _ in range(reps // 2):
+                B.lqcd_dslash_eo(g, a, b, 0, kappa)
+                B.lqcd_dslash_eo(g, b, a, 1, kappa)
+            e1.record(stream)
+            stream.synchronize()
+            times.append(e0.elapsed_time(e1) / (2 * (reps // 2)))
+    B.lqcd_finalize()
+    ms = float(np.median(times))
+    eff, paper = site_bytes(precision, recon)
+    peak = measured_peak()
+    gbs = Vh * eff / ms / 1e6
+    return {"us_per_application": ms * 1e3, "gflops": Vh * FLOP / ms / 1e6, "gbs_effective": gbs,
+            "gbs_paper_accounting": Vh * paper / ms / 1e6, "bytes_per_site": eff,
+            "frac_of_measured_peak": gbs / peak, "frac_of_nominal_peak": gbs / NOMINAL_GBS,
+            "measured_peak_gbs": peak}
+
+
+def config3(stream):
+    dims = (16, 16, 16, 32)
+    U = gen.gauge_near_identity(dims, gen.BASE_SEED, 0.3)
+    r = time_dslash(dims, U, 0, 18, 0.16, 10, 100, 5, stream)
+    r.update({"config": 3, "lattice": list(dims), "precision": "double", "recon": 18,
+              "note": "gauge 75 MB + spinors 25 MB fit the 126 MB L2: DRAM traffic is far below the algorithmic "
+                      "bytes, the fraction of HBM peak is not a roofline result"})
+    return [r]
+
+
+def config4(stream):
+    dims = (24, 24, 24, 48)
+    kappa, mu, tol = 0.15, 0.1, 1e-10
+    Vh = int(np.prod(dims)) // 2
+    U = gen.gauge_haar(dims)
+    src = gen.spinor_gaussian(Vh, stream=gen.STREAM_SOURCE)
+    B.lqcd_init(dims, gen.antiperiodic_t())
+    B.lqcd_set_stream(stream)
+    out = []
+    with torch.cuda.stream(stream):
+        g = B.upload_gauge(U)
+        b = B.upload_spinor(src, 0)
+        x = B.alloc_spinor()
+        B.lqcd_cg_mdagm(g, b, x, kappa, mu, tol, 2000)      # warm-up solve
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        stream.synchronize()
+        e0.record(stream)
+        st = B.lqcd_cg_mdagm(g, b, x, kappa, mu, tol, 2000)
+        e1.record(stream)
+        stream.synchronize()
+        iters, rr, rt = B.lqcd_cg_stats()
+        ms = e0.elapsed_time(e1)
+        # per-iteration split from per-launch events, in a separate profiled solve
+        B.lqcd_profile(1)
+        B.lqcd_cg_setup(g, b, x, kappa, mu, tol)
+        B.lqcd_cg_iterate(iters)
+        hop = sum(B.lqcd_profile_read(c)[0] for c in (0, 1, 2))
+        vec = B.lqcd_profile_read(3)[0]
+        B.lqcd_profile(0)
+        B.lqcd_cg_finish()
+    B.lqcd_finalize()
+    out.append({"config": 4, "lattice": list(dims), "precision": "double", "recon": 18, "status": int(st),
+                "iterations": iters, "time_to_solution_ms": ms, "rel_resid_recursive": rr, "rel_resid_true": rt,
+                "ms_per_iteration": ms / max(iters, 1),
+                "gflops": 4 * iters * Vh * FLOP / ms / 1e6,
+                "per_iteration_us": {"hopping_4_launches": hop / iters * 1e3, "vector_and_finalize_kernels": vec / iters * 1e3},
+                "hopping_share": hop / (hop + vec),
+                "note": "time to solution includes the solve setup and the final true-residual check (one extra "
+                        "application of Mhat^dag Mhat)"})
+    return out
+
+
+def config5(stream):
+    dims = (32, 32, 32, 64)
+    U = gen.gauge_haar(dims)
+    out = []
+    for precision, recon in ((0, 18), (0, 12), (1, 18), (1, 12)):
+        r = time_dslash(dims, U, precision, recon, 0.15, 20, 200, 3, stream)
+        r.update({"config": 5, "lattice": list(dims), "precision": "double" if precision == 0 else "single",
+                  "recon": recon})
+        out.append(r)
+    return out
+
+
+def thermal(stream):
+    out = []
+    for ns in (16, 24, 32, 48):
+        for nt in (4, 8, 12, 16):
+            dims = (ns, ns, ns, nt)
+            U = gen.gauge_haar(dims)
+            r = time_dslash(dims, U, 0, 18, 0.15, 10, 100, 3, stream)
+            r.update({"config": "thermal", "lattice": list(dims), "precision": "double", "recon": 18})
+            out.append(r)
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--configs", default="3,4,5,thermal")
+    ap.add_argument("--out", default=None)
+    args = ap.parse_args()
+    if not torch.cuda.is_available():
+        raise SystemExit("sweep.py needs a CUDA device: there is no CPU fallback")
+    stream = torch.cuda.Stream()
+    table = {"3": config3, "4": config4, "5": config5, "thermal": thermal}
+    lines = []
+    for key in args.configs.split(","):
+        for r in table[key.strip()](stream):
+            line = json.dumps(r)
+            print(line, flush=True)
+            lines.append(line)
+    if args.out:
+        with open(args.out, "w") as f:
+            f.write("\n".join(lines) + "\n")
+
+
+if __name__ == "__main__":
+    main()
