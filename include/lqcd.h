@@ -114,6 +114,21 @@ int lqcd_cg_setup(const void* gauge, const void* b, void* x, double kappa, doubl
 int lqcd_cg_iterate(int n);
 int lqcd_cg_finish(void);
 
+/* Mixed-precision solve of the same system (the paper's planned next step, PAPER.md:352;
+ * SURVEY.md section 8(f) row 1): defect correction with the outer residual in double and the
+ * inner CG in single precision,
+ *   x = 0, r = b;  repeat { solve A e = r/|r| in single to inner_tol;  x += |r| e;  r = b - A x }
+ * until |r| <= tol |b| (a TRUE residual, evaluated in double) or maxit inner iterations in total.
+ * gauge_double / gauge_single: the same field packed under (LQCD_DOUBLE, recon_double) and
+ * (LQCD_SINGLE, recon_single); b, x: double internal layout.  inner_tol in [0,1): 0 (recommended)
+ * asks each inner solve for half the reduction still missing, floored at 1e-6 (what single
+ * precision delivers).  Independent of lqcd_set_format.  Synchronous. */
+int lqcd_cg_mdagm_mixed(const void* gauge_double, int recon_double, const void* gauge_single,
+                        int recon_single, const void* b, void* x, double kappa, double mu, double tol,
+                        int maxit, double inner_tol);
+/* Outer (double-precision) corrections of the last lqcd_cg_mdagm_mixed call; 0 otherwise. */
+int lqcd_cg_outer_iterations(void);
+
 /* Results of the last solve: iterations done, recursive and true relative residual.
  * Any pointer may be NULL. */
 int lqcd_cg_stats(int* iters, double* rel_resid_recursive, double* rel_resid_true);

@@ -60,11 +60,13 @@ struct Context {
     int block = 128;
     cudaStream_t stream = 0;
 
-    // workspace (owned)
-    size_t ws_spinor_bytes = 0;
-    void* vec[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};  // r, p, q, t1, t2
-    CgScalars* scal = nullptr;
-    CgScalars* scal_host = nullptr;  // pinned, 2 slots
+    // workspace (owned), one set of half spinors per precision: r, p, q, t1, t2
+    void* vec[2][5] = {{nullptr, nullptr, nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr, nullptr, nullptr}};
+    void* mx_b = nullptr;            // mixed solver: single-precision right-hand side and correction
+    void* mx_x = nullptr;
+    CgScalars* scal = nullptr;       // scalars of the running CG
+    CgScalars* scal_outer = nullptr; // scalars of the mixed solver's outer (double) loop
+    CgScalars* scal_host = nullptr;  // pinned, 3 slots
     cudaEvent_t ev[2] = {nullptr, nullptr};
     double* partials = nullptr;
     size_t n_partials = 0;
@@ -77,12 +79,13 @@ struct Context {
     void* st_out = nullptr; size_t st_out_bytes = 0;
 
     // current solve
+    int cg_prec = 0, cg_recon = 18;
     const void* cg_gauge = nullptr;
     const void* cg_b = nullptr;
     void* cg_x = nullptr;
     double cg_kappa = 0, cg_mu = 0, cg_tol = 0;
     bool cg_active = false;
-    int st_iters = 0;
+    int st_iters = 0, st_outer = 0;
     double st_rr = 0, st_rt = 0;
 };
 
@@ -113,13 +116,17 @@ size_t gauge_bytes_of(int precision, int recon, int Vh) {
 }
 
 void free_workspace() {
-    for (int i = 0; i < 5; ++i) { if (ctx.vec[i]) cudaFree(ctx.vec[i]); ctx.vec[i] = nullptr; }
-    ctx.ws_spinor_bytes = 0;
+    for (int pr = 0; pr < 2; ++pr)
+        for (int i = 0; i < 5; ++i) { if (ctx.vec[pr][i]) cudaFree(ctx.vec[pr][i]); ctx.vec[pr][i] = nullptr; }
+    if (ctx.mx_b) cudaFree(ctx.mx_b);
+    if (ctx.mx_x) cudaFree(ctx.mx_x);
+    ctx.mx_b = ctx.mx_x = nullptr;
 }
 
 void free_all() {
     free_workspace();
     if (ctx.scal) cudaFree(ctx.scal);
+    if (ctx.scal_outer) cudaFree(ctx.scal_outer);
     if (ctx.scal_host) cudaFreeHost(ctx.scal_host);
     if (ctx.partials) cudaFree(ctx.partials);
     for (int i = 0; i < 2; ++i) if (ctx.ev[i]) cudaEventDestroy(ctx.ev[i]);
@@ -132,7 +139,9 @@ int ensure_scalars() {
     if (!ctx.scal) {
         CU(cudaMalloc(&ctx.scal, sizeof(CgScalars)));
         CU(cudaMemset(ctx.scal, 0, sizeof(CgScalars)));
-        CU(cudaMallocHost(&ctx.scal_host, 2 * sizeof(CgScalars)));
+        CU(cudaMalloc(&ctx.scal_outer, sizeof(CgScalars)));
+        CU(cudaMemset(ctx.scal_outer, 0, sizeof(CgScalars)));
+        CU(cudaMallocHost(&ctx.scal_host, 3 * sizeof(CgScalars)));
         for (int i = 0; i < 2; ++i) CU(cudaEventCreateWithFlags(&ctx.ev[i], cudaEventDisableTiming));
     }
     const size_t need = (size_t)hopping_partials(ctx.geo.Vh, 32) + (size_t)vector_grid((size_t)24 * ctx.geo.Vh) + 64;
@@ -145,17 +154,15 @@ int ensure_scalars() {
     return LQCD_OK;
 }
 
-int ensure_workspace(int nvec) {
+int ensure_workspace(int precision, int nvec) {
     int rc = ensure_scalars();
     if (rc) return rc;
-    const size_t sb = spinor_bytes_of(ctx.precision, ctx.geo.Vh);
-    if (ctx.ws_spinor_bytes != sb) free_workspace();
-    ctx.ws_spinor_bytes = sb;
+    const size_t sb = spinor_bytes_of(precision, ctx.geo.Vh);
     // t1 (index 3) is needed by lqcd_mtm; the rest only by CG
     const int order[5] = {3, 4, 0, 1, 2};
     for (int k = 0; k < nvec; ++k) {
         const int i = order[k];
-        if (!ctx.vec[i]) CU(cudaMalloc(&ctx.vec[i], sb));
+        if (!ctx.vec[precision][i]) CU(cudaMalloc(&ctx.vec[precision][i], sb));
     }
     return LQCD_OK;
 }
@@ -179,14 +186,14 @@ int check_scalar(double v, const char* name) {
 // The two hopping launches of Mhat (dagger = 0) or Mhat^dag (dagger = 1) on even half fields.
 // norm_to_pAp: also reduce |out|^2 into scal->pAp (CG's <p, A p> = |Mhat p|^2).
 // scal: device scalars whose `done` flag turns the launches into no-ops (CG), or null.
-int apply_mhat(const void* gauge, const void* in, void* tmp_odd, void* out, double kappa, double mu,
-               int dagger, bool norm_to_pAp, CgScalars* scal) {
+int apply_mhat(int precision, int recon, const void* gauge, const void* in, void* tmp_odd, void* out,
+               double kappa, double mu, int dagger, bool norm_to_pAp, CgScalars* scal) {
     const double c = (dagger ? -1.0 : 1.0) * 2.0 * kappa * mu;
     const double d = 1.0 + c * c;
     Epilogue e1 = {};
     e1.cu_re = -kappa / d; e1.cu_im = +kappa * c / d;   // -kappa (1 - i c)/(1 + c^2), chi = +1
     e1.cd_re = -kappa / d; e1.cd_im = -kappa * c / d;   // chi = -1
-    CU(launch_hopping(ctx.precision, ctx.recon, dagger, 0, ctx.geo, e1, gauge, in, tmp_odd, nullptr, 1,
+    CU(launch_hopping(precision, recon, dagger, 0, ctx.geo, e1, gauge, in, tmp_odd, nullptr, 1,
                       0, red(), scal, ctx.block, ctx.stream));
     // out = (1 + i c chi) in + kappa * bracket(t) = k2 * (bracket(t) + [(1 + i c chi)/k2] in).
     // For kappa = 0 launch 1 wrote t = 0 exactly, so bracket(t) = 0 and any k2 != 0 is exact.
@@ -195,7 +202,7 @@ int apply_mhat(const void* gauge, const void* in, void* tmp_odd, void* out, doub
     e2.cu_re = k2; e2.cd_re = k2;
     e2.du_re = 1.0 / k2; e2.du_im = c / k2;
     e2.dd_re = 1.0 / k2; e2.dd_im = -c / k2;
-    CU(launch_hopping(ctx.precision, ctx.recon, dagger, norm_to_pAp ? 2 : 1, ctx.geo, e2, gauge, tmp_odd,
+    CU(launch_hopping(precision, recon, dagger, norm_to_pAp ? 2 : 1, ctx.geo, e2, gauge, tmp_odd,
                       out, in, 0, 1, red(), scal, ctx.block, ctx.stream));
     if (norm_to_pAp)
         CU(launch_finalize(FIN_PAP, red(), hopping_partials(ctx.geo.Vh, ctx.block), 0.0, scal, ctx.stream));
@@ -203,15 +210,81 @@ int apply_mhat(const void* gauge, const void* in, void* tmp_odd, void* out, doub
 }
 
 int enqueue_iteration() {
-    void *r = ctx.vec[0], *p = ctx.vec[1], *q = ctx.vec[2], *t1 = ctx.vec[3], *t2 = ctx.vec[4];
+    void** v = ctx.vec[ctx.cg_prec];
+    void *r = v[0], *p = v[1], *q = v[2], *t1 = v[3], *t2 = v[4];
     const size_t n = (size_t)24 * ctx.geo.Vh;
-    int rc = apply_mhat(ctx.cg_gauge, p, t1, t2, ctx.cg_kappa, ctx.cg_mu, 0, true, ctx.scal);
+    int rc = apply_mhat(ctx.cg_prec, ctx.cg_recon, ctx.cg_gauge, p, t1, t2, ctx.cg_kappa, ctx.cg_mu, 0, true, ctx.scal);
     if (rc) return rc;
-    rc = apply_mhat(ctx.cg_gauge, t2, t1, q, ctx.cg_kappa, ctx.cg_mu, 1, false, ctx.scal);
+    rc = apply_mhat(ctx.cg_prec, ctx.cg_recon, ctx.cg_gauge, t2, t1, q, ctx.cg_kappa, ctx.cg_mu, 1, false, ctx.scal);
     if (rc) return rc;
-    CU(launch_cg_update_r(ctx.precision, n, r, q, 0, red(), ctx.scal, ctx.stream));
-    CU(launch_cg_update_xp(ctx.precision, n, ctx.cg_x, p, r, 1, ctx.scal, ctx.stream));
+    CU(launch_cg_update_r(ctx.cg_prec, n, r, q, 0, red(), ctx.scal, ctx.stream));
+    CU(launch_cg_update_xp(ctx.cg_prec, n, ctx.cg_x, p, r, 1, ctx.scal, ctx.stream));
     return LQCD_OK;
+}
+
+int cg_setup_impl(int precision, int recon, const void* gauge, const void* b, void* x, double kappa,
+                  double mu, double tol) {
+    int rc = ensure_workspace(precision, 5);
+    if (rc) return rc;
+    ctx.cg_prec = precision; ctx.cg_recon = recon;
+    ctx.cg_gauge = gauge; ctx.cg_b = b; ctx.cg_x = x;
+    ctx.cg_kappa = kappa; ctx.cg_mu = mu; ctx.cg_tol = tol;
+    CU(launch_cg_init(precision, (size_t)24 * ctx.geo.Vh, b, x, ctx.vec[precision][0], ctx.vec[precision][1],
+                      tol, red(), ctx.scal, ctx.stream));
+    ctx.cg_active = true;
+    return LQCD_OK;
+}
+
+// Enqueue up to maxit iterations in chunks; the convergence flag of chunk k is read back while
+// chunk k+1 is already queued, so the device never idles on the host.
+int cg_run_impl(int maxit) {
+    const int chunk = 4;
+    int launched = 0, slot = 0;
+    bool pending[2] = {false, false};
+    bool stop = false;
+    while (launched < maxit && !stop) {
+        const int n = (maxit - launched < chunk) ? (maxit - launched) : chunk;
+        for (int i = 0; i < n; ++i) {
+            int rc = enqueue_iteration();
+            if (rc) return rc;
+        }
+        launched += n;
+        CU(cudaMemcpyAsync(&ctx.scal_host[slot], ctx.scal, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx.stream));
+        CU(cudaEventRecord(ctx.ev[slot], ctx.stream));
+        pending[slot] = true;
+        const int prev = slot ^ 1;
+        if (pending[prev]) {
+            CU(cudaEventSynchronize(ctx.ev[prev]));
+            pending[prev] = false;
+            if (ctx.scal_host[prev].done) stop = true;
+        }
+        slot ^= 1;
+    }
+    return LQCD_OK;
+}
+
+// Synchronise; optionally compute the true residual |b - A x| (one more application of A with
+// the `done` gate off); fill the statistics; return the solve status.
+int cg_finish_impl(bool true_resid) {
+    void** v = ctx.vec[ctx.cg_prec];
+    if (true_resid) {
+        void *q = v[2], *t1 = v[3], *t2 = v[4];
+        int rc = apply_mhat(ctx.cg_prec, ctx.cg_recon, ctx.cg_gauge, ctx.cg_x, t1, t2, ctx.cg_kappa, ctx.cg_mu, 0, false, nullptr);
+        if (rc) return rc;
+        rc = apply_mhat(ctx.cg_prec, ctx.cg_recon, ctx.cg_gauge, t2, t1, q, ctx.cg_kappa, ctx.cg_mu, 1, false, nullptr);
+        if (rc) return rc;
+        CU(launch_true_resid(ctx.cg_prec, (size_t)24 * ctx.geo.Vh, ctx.cg_b, q, red(), ctx.scal, ctx.stream));
+    }
+    CU(cudaMemcpyAsync(ctx.scal_host, ctx.scal, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx.stream));
+    CU(cudaStreamSynchronize(ctx.stream));
+    const CgScalars& s = ctx.scal_host[0];
+    ctx.st_iters = s.iters;
+    ctx.st_outer = 0;
+    ctx.st_rr = s.bb > 0 ? std::sqrt(s.rho / s.bb) : 0.0;
+    ctx.st_rt = (true_resid && s.bb > 0) ? std::sqrt(s.resid_true / s.bb) : 0.0;
+    ctx.cg_active = false;
+    if (s.status == LQCD_BREAKDOWN) return fail(LQCD_BREAKDOWN, "CG breakdown: <p,Ap> = %g", s.pAp);
+    return s.status;
 }
 
 }  // namespace
@@ -351,9 +424,10 @@ int lqcd_mtm(const void* gauge, const void* in, void* out, double kappa, double 
     if (rc) return rc;
     rc = check_scalar(mu, "mu");
     if (rc) return rc;
-    rc = ensure_workspace(1);
+    rc = ensure_workspace(ctx.precision, 1);
     if (rc) return rc;
-    return apply_mhat(gauge, in, ctx.vec[3], out, kappa, mu, dagger, false, nullptr);
+    return apply_mhat(ctx.precision, ctx.recon, gauge, in, ctx.vec[ctx.precision][3], out, kappa, mu, dagger,
+                      false, nullptr);
 }
 
 int lqcd_cg_setup(const void* gauge, const void* b, void* x, double kappa, double mu, double tol) {
@@ -365,14 +439,7 @@ int lqcd_cg_setup(const void* gauge, const void* b, void* x, double kappa, doubl
     rc = check_scalar(mu, "mu");
     if (rc) return rc;
     if (!std::isfinite(tol) || tol < 0.0) return fail(LQCD_BAD_ARG, "tol must be finite and >= 0");
-    rc = ensure_workspace(5);
-    if (rc) return rc;
-    ctx.cg_gauge = gauge; ctx.cg_b = b; ctx.cg_x = x;
-    ctx.cg_kappa = kappa; ctx.cg_mu = mu; ctx.cg_tol = tol;
-    CU(launch_cg_init(ctx.precision, (size_t)24 * ctx.geo.Vh, b, x, ctx.vec[0], ctx.vec[1], tol, red(),
-                      ctx.scal, ctx.stream));
-    ctx.cg_active = true;
-    return LQCD_OK;
+    return cg_setup_impl(ctx.precision, ctx.recon, gauge, b, x, kappa, mu, tol);
 }
 
 int lqcd_cg_iterate(int n) {
@@ -389,22 +456,7 @@ int lqcd_cg_iterate(int n) {
 int lqcd_cg_finish(void) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
     if (!ctx.cg_active) return fail(LQCD_BAD_ARG, "lqcd_cg_finish: no solve set up");
-    // true residual |b - A x|: q = A x with the `done` gate off
-    void *q = ctx.vec[2], *t1 = ctx.vec[3], *t2 = ctx.vec[4];
-    int rc = apply_mhat(ctx.cg_gauge, ctx.cg_x, t1, t2, ctx.cg_kappa, ctx.cg_mu, 0, false, nullptr);
-    if (rc) return rc;
-    rc = apply_mhat(ctx.cg_gauge, t2, t1, q, ctx.cg_kappa, ctx.cg_mu, 1, false, nullptr);
-    if (rc) return rc;
-    CU(launch_true_resid(ctx.precision, (size_t)24 * ctx.geo.Vh, ctx.cg_b, q, red(), ctx.scal, ctx.stream));
-    CU(cudaMemcpyAsync(ctx.scal_host, ctx.scal, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx.stream));
-    CU(cudaStreamSynchronize(ctx.stream));
-    const CgScalars& s = ctx.scal_host[0];
-    ctx.st_iters = s.iters;
-    ctx.st_rr = s.bb > 0 ? std::sqrt(s.rho / s.bb) : 0.0;
-    ctx.st_rt = s.bb > 0 ? std::sqrt(s.resid_true / s.bb) : 0.0;
-    ctx.cg_active = false;
-    if (s.status == LQCD_BREAKDOWN) return fail(LQCD_BREAKDOWN, "CG breakdown: <p,Ap> = %g", s.pAp);
-    return s.status;
+    return cg_finish_impl(true);
 }
 
 int lqcd_cg_mdagm(const void* gauge, const void* b, void* x, double kappa, double mu, double tol,
@@ -412,30 +464,84 @@ int lqcd_cg_mdagm(const void* gauge, const void* b, void* x, double kappa, doubl
     if (maxit < 1) return fail(LQCD_BAD_ARG, "maxit must be >= 1");
     int rc = lqcd_cg_setup(gauge, b, x, kappa, mu, tol);
     if (rc) return rc;
-    // Enqueue iterations in chunks; the convergence flag of chunk k is read back while
-    // chunk k+1 is already queued, so the device never idles on the host.
-    const int chunk = 4;
-    int launched = 0, slot = 0;
-    bool pending[2] = {false, false};
-    bool stop = false;
-    while (launched < maxit && !stop) {
-        const int n = (maxit - launched < chunk) ? (maxit - launched) : chunk;
-        rc = lqcd_cg_iterate(n);
-        if (rc) return rc;
-        launched += n;
-        CU(cudaMemcpyAsync(&ctx.scal_host[slot], ctx.scal, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx.stream));
-        CU(cudaEventRecord(ctx.ev[slot], ctx.stream));
-        pending[slot] = true;
-        const int prev = slot ^ 1;
-        if (pending[prev]) {
-            CU(cudaEventSynchronize(ctx.ev[prev]));
-            pending[prev] = false;
-            if (ctx.scal_host[prev].done) stop = true;
-        }
-        slot ^= 1;
-    }
-    return lqcd_cg_finish();
+    rc = cg_run_impl(maxit);
+    if (rc) return rc;
+    return cg_finish_impl(true);
 }
+
+// Mixed-precision defect correction:
+//   x = 0, r = b (double); repeat: solve A e = r/|r| in single by CG to inner_tol;
+//   x += |r| e; r = b - A x in double; until |r| <= tol |b|.
+int lqcd_cg_mdagm_mixed(const void* gauge_double, int recon_double, const void* gauge_single,
+                        int recon_single, const void* b, void* x, double kappa, double mu, double tol,
+                        int maxit, double inner_tol) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (!gauge_double || !gauge_single || !b || !x) return fail(LQCD_BAD_ARG, "lqcd_cg_mdagm_mixed: null pointer");
+    if (b == x) return fail(LQCD_BAD_ARG, "lqcd_cg_mdagm_mixed: b and x alias");
+    if ((recon_double != 18 && recon_double != 12) || (recon_single != 18 && recon_single != 12))
+        return fail(LQCD_BAD_ARG, "recon must be 18 or 12");
+    if (maxit < 1) return fail(LQCD_BAD_ARG, "maxit must be >= 1");
+    int rc = check_scalar(kappa, "kappa");
+    if (rc) return rc;
+    if ((rc = check_scalar(mu, "mu"))) return rc;
+    if (!std::isfinite(tol) || tol < 0.0) return fail(LQCD_BAD_ARG, "tol must be finite and >= 0");
+    if (!std::isfinite(inner_tol) || inner_tol < 0.0 || inner_tol >= 1.0)
+        return fail(LQCD_BAD_ARG, "inner_tol must be in [0, 1)");
+    if ((rc = ensure_workspace(LQCD_DOUBLE, 5))) return rc;
+    if ((rc = ensure_workspace(LQCD_SINGLE, 5))) return rc;
+    const size_t sbf = spinor_bytes_of(LQCD_SINGLE, ctx.geo.Vh);
+    if (!ctx.mx_b) CU(cudaMalloc(&ctx.mx_b, sbf));
+    if (!ctx.mx_x) CU(cudaMalloc(&ctx.mx_x, sbf));
+    void** vd = ctx.vec[LQCD_DOUBLE];
+    void *r = vd[0], *q = vd[2], *t1 = vd[3], *t2 = vd[4];
+    const size_t n = (size_t)24 * ctx.geo.Vh;
+    CgScalars* so = ctx.scal_outer;
+    CgScalars* sh = &ctx.scal_host[2];
+    // x = 0, r = b, bb = rho = |b|^2 (p slot vd[1] is scratch here)
+    CU(launch_cg_init(LQCD_DOUBLE, n, b, x, r, vd[1], tol, red(), so, ctx.stream));
+    int total = 0, outer = 0, status = LQCD_NOT_CONVERGED;
+    double rho = 0.0, bb = 0.0;
+    for (;;) {
+        CU(cudaMemcpyAsync(sh, so, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx.stream));
+        CU(cudaStreamSynchronize(ctx.stream));
+        bb = sh->bb;
+        rho = (outer == 0) ? sh->rho : sh->resid_true;
+        if (!(rho > tol * tol * bb) ) { status = LQCD_OK; break; }     // also catches b = 0
+        if (!std::isfinite(rho)) { status = LQCD_BREAKDOWN; break; }
+        if (total >= maxit) break;
+        const double scale = std::sqrt(rho);
+        CU(launch_convert_d2f(n, r, ctx.mx_b, 1.0 / scale, ctx.stream));
+        // inner_tol = 0: ask each inner solve only for the reduction still missing (half of it,
+        // for slack), but never for more than single precision delivers (1e-6)
+        double itol = inner_tol;
+        if (itol == 0.0) {
+            itol = 0.5 * tol * std::sqrt(bb / rho);
+            if (itol < 1e-6) itol = 1e-6;
+            if (itol > 0.1) itol = 0.1;
+        }
+        rc = cg_setup_impl(LQCD_SINGLE, recon_single, gauge_single, ctx.mx_b, ctx.mx_x, kappa, mu, itol);
+        if (rc) return rc;
+        if ((rc = cg_run_impl(maxit - total))) return rc;
+        const int ist = cg_finish_impl(false);
+        if (ist < 0) return ist;
+        total += ctx.st_iters;
+        ++outer;
+        CU(launch_axpy_f2d(n, scale, ctx.mx_x, x, ctx.stream));
+        // r = b - A x in double
+        if ((rc = apply_mhat(LQCD_DOUBLE, recon_double, gauge_double, x, t1, t2, kappa, mu, 0, false, nullptr))) return rc;
+        if ((rc = apply_mhat(LQCD_DOUBLE, recon_double, gauge_double, t2, t1, q, kappa, mu, 1, false, nullptr))) return rc;
+        CU(launch_residual(n, b, q, r, red(), so, ctx.stream));
+        if (ctx.st_iters == 0) { status = LQCD_BREAKDOWN; break; }      // inner solver made no progress
+    }
+    ctx.st_iters = total;
+    ctx.st_outer = outer;
+    ctx.st_rr = ctx.st_rt = bb > 0 ? std::sqrt(rho / bb) : 0.0;   // the outer residual IS a true residual
+    ctx.cg_active = false;
+    if (status == LQCD_BREAKDOWN) return fail(LQCD_BREAKDOWN, "mixed CG: no progress (|r|^2 = %g)", rho);
+    return status;
+}
+
+int lqcd_cg_outer_iterations(void) { return ctx.init ? ctx.st_outer : 0; }
 
 int lqcd_cg_stats(int* iters, double* rel_resid_recursive, double* rel_resid_true) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");

@@ -73,6 +73,11 @@ cudaError_t launch_cg_update_xp(int precision, size_t n, void* x, void* p, const
                                 CgScalars* scal, cudaStream_t st);
 cudaError_t launch_true_resid(int precision, size_t n, const void* b, const void* ax, Reduction red,
                               CgScalars* scal, cudaStream_t st);
+// mixed-precision solver helpers (double layout double2[12][Vh] <-> float layout float4[6][Vh])
+cudaError_t launch_convert_d2f(size_t n, const void* src_d, void* dst_f, double scale, cudaStream_t st);
+cudaError_t launch_axpy_f2d(size_t n, double a, const void* x_f, void* y_d, cudaStream_t st);  // y += a x
+cudaError_t launch_residual(size_t n, const void* b, const void* ax, void* r, Reduction red,
+                            CgScalars* scal, cudaStream_t st);  // r = b - ax (double), |r|^2 -> resid_true
 // sums red.partials[0..n_partials) in a fixed order and applies the FIN_* action to *scal
 cudaError_t launch_finalize(int fin, Reduction red, int n_partials, double tol, CgScalars* scal,
                             cudaStream_t st);

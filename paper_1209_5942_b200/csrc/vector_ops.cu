@@ -208,6 +208,47 @@ __global__ void __launch_bounds__(VBLOCK) true_resid_kernel(size_t nvec, const v
     block_partial(s, red);
 }
 
+// ---- mixed-precision helpers.  Double field: double2 d[12][Vh]; float field: float4 f[6][Vh] with
+// f[k][e] = (d[2k][e], d[2k+1][e]).  One thread per float4 element.
+__global__ void __launch_bounds__(VBLOCK) convert_d2f_kernel(size_t Vh, const double2* __restrict__ d,
+                                                             float4* __restrict__ f, double scale) {
+    const size_t i = (size_t)blockIdx.x * VBLOCK + threadIdx.x;
+    if (i >= 6 * Vh) return;
+    const size_t k = i / Vh, e = i - k * Vh;
+    const double2 a = __ldcs(d + (2 * k) * Vh + e), b = __ldcs(d + (2 * k + 1) * Vh + e);
+    f[i] = make_float4((float)(a.x * scale), (float)(a.y * scale), (float)(b.x * scale), (float)(b.y * scale));
+}
+
+__global__ void __launch_bounds__(VBLOCK) axpy_f2d_kernel(size_t Vh, double a, const float4* __restrict__ x,
+                                                          double2* __restrict__ y) {
+    const size_t i = (size_t)blockIdx.x * VBLOCK + threadIdx.x;
+    if (i >= 6 * Vh) return;
+    const size_t k = i / Vh, e = i - k * Vh;
+    const float4 v = __ldcs(x + i);
+    double2* y0 = y + (2 * k) * Vh + e;
+    double2* y1 = y + (2 * k + 1) * Vh + e;
+    const double2 u0 = *y0, u1 = *y1;
+    *y0 = make_double2(fma(a, (double)v.x, u0.x), fma(a, (double)v.y, u0.y));
+    *y1 = make_double2(fma(a, (double)v.z, u1.x), fma(a, (double)v.w, u1.y));
+}
+
+__global__ void __launch_bounds__(VBLOCK) residual_kernel(size_t nvec, const double2* __restrict__ b,
+                                                          const double2* __restrict__ ax,
+                                                          double2* __restrict__ r, Reduction red) {
+    const size_t base = (size_t)blockIdx.x * (VBLOCK * VUNROLL) + threadIdx.x;
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < VUNROLL; ++k) {
+        const size_t i = base + (size_t)k * VBLOCK;
+        if (i < nvec) {
+            const double2 v = sub(__ldg(b + i), __ldcs(ax + i));
+            r[i] = v;
+            s += norm2(v);
+        }
+    }
+    block_partial(s, red);
+}
+
 inline int grid_for(size_t nvec) { return (int)((nvec + VBLOCK * VUNROLL - 1) / (VBLOCK * VUNROLL)); }
 
 }  // namespace
@@ -219,6 +260,34 @@ cudaError_t launch_finalize(int fin, Reduction red, int n_partials, double tol, 
     count_launch();
     ProfScope prof(3, st);
     finalize_kernel<<<1, 1024, 0, st>>>(fin, red, n_partials, tol, scal);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_convert_d2f(size_t n, const void* src_d, void* dst_f, double scale, cudaStream_t st) {
+    const size_t Vh = n / 24;
+    count_launch();
+    ProfScope prof(3, st);
+    convert_d2f_kernel<<<(int)((6 * Vh + VBLOCK - 1) / VBLOCK), VBLOCK, 0, st>>>(Vh, (const double2*)src_d,
+                                                                                 (float4*)dst_f, scale);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_axpy_f2d(size_t n, double a, const void* x_f, void* y_d, cudaStream_t st) {
+    const size_t Vh = n / 24;
+    count_launch();
+    ProfScope prof(3, st);
+    axpy_f2d_kernel<<<(int)((6 * Vh + VBLOCK - 1) / VBLOCK), VBLOCK, 0, st>>>(Vh, a, (const float4*)x_f,
+                                                                              (double2*)y_d);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_residual(size_t n, const void* b, const void* ax, void* r, Reduction red,
+                            CgScalars* scal, cudaStream_t st) {
+    const size_t nv = n / 2;
+    count_launch(2);
+    ProfScope prof(3, st);
+    residual_kernel<<<grid_for(nv), VBLOCK, 0, st>>>(nv, (const double2*)b, (const double2*)ax, (double2*)r, red);
+    finalize_kernel<<<1, 1024, 0, st>>>(FIN_TRUE, red, grid_for(nv), 0.0, scal);
     return cudaGetLastError();
 }
 

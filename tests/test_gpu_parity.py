@@ -349,3 +349,65 @@ def test_config4_cg_24c48(B, oracle_mod):
     assert st == 0 and 20 <= iters <= 80 and rr <= tol
     r = b - oracle_mod.mdagm(dims, AP, U, x, kappa, mu)     # one oracle application of A
     assert np.linalg.norm(r) / np.linalg.norm(b) <= 1.05 * tol
+
+
+# --------------------------------------------------------------------------- mixed-precision CG
+def _mixed_solve(B, dims, U, b, kappa, mu, tol, maxit, recon_d=18, recon_s=12, inner_tol=0.0):
+    B.lqcd_init(dims, AP)
+    B.lqcd_set_stream()
+    B.lqcd_set_format(B.LQCD_SINGLE, recon_s)
+    gs = B.upload_gauge(U)
+    B.lqcd_set_format(B.LQCD_DOUBLE, recon_d)
+    gd = B.upload_gauge(U)
+    src = B.upload_spinor(b, 0)
+    x = B.alloc_spinor()
+    st = B.lqcd_cg_mdagm_mixed(gd, recon_d, gs, recon_s, src, x, kappa, mu, tol, maxit, inner_tol)
+    return st, B.download_spinor(x, 0), B.lqcd_cg_stats(), B.lqcd_cg_outer_iterations()
+
+
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (8, 8, 8, 16)])
+@pytest.mark.parametrize("recon_d,recon_s", [(18, 12), (18, 18), (12, 12)])
+@pytest.mark.parametrize("tol,inner_tol", [(1e-10, 0.0), (1e-13, 0.0), (1e-10, 1e-4)])
+def test_mixed_precision_cg_reaches_double_accuracy(B, oracle_mod, dims, recon_d, recon_s, tol, inner_tol):
+    kappa, mu = 0.15, 0.1
+    U = gen.gauge_haar(dims, SEED)
+    b = gen.spinor_gaussian(lu.volume(dims) // 2, SEED, gen.STREAM_SOURCE)
+    st, x, (iters, rr, rt), outer = _mixed_solve(B, dims, U, b, kappa, mu, tol, 2000, recon_d, recon_s, inner_tol)
+    assert st == 0 and outer >= 2 and iters > 0
+    assert rr <= tol and rt == rr            # the outer residual is a true residual, evaluated in double
+    # the same solution the double oracle finds: true residual under the ORACLE's operator, and x itself
+    r = b - oracle_mod.mdagm(dims, AP, U, x, kappa, mu)
+    assert np.linalg.norm(r) / np.linalg.norm(b) <= 1.05 * tol + 2e-15
+    st_o, x_o, it_o, rr_o, rt_o = oracle_mod.cg_mdagm(dims, AP, U, b, kappa, mu, min(tol, 1e-12), 2000)
+    assert lu.rel_err(x, x_o) <= 10 * 5.0 * max(tol, 1e-12)
+    # defect correction restarts the Krylov space: a bounded number of extra iterations
+    assert iters <= 2.5 * it_o + 10
+
+
+def test_mixed_precision_cg_edge_cases(B):
+    dims = (4, 4, 4, 4)
+    U = gen.gauge_haar(dims, SEED)
+    h = lu.volume(dims) // 2
+    st, x, (iters, rr, rt), outer = _mixed_solve(B, dims, U, np.zeros((h, 4, 3), dtype=complex), 0.15, 0.1, 1e-10, 100)
+    assert st == 0 and iters == 0 and outer == 0 and np.all(x == 0)
+    b = gen.spinor_gaussian(h, SEED, gen.STREAM_SOURCE)
+    st, x, (iters, rr, rt), outer = _mixed_solve(B, dims, U, b, 0.15, 0.1, 1e-10, 6)
+    assert st == B.LQCD_NOT_CONVERGED and iters == 6 and rr > 1e-10
+    gd, s = B.alloc_gauge(), B.alloc_spinor()
+    for call in (lambda: B.lqcd_cg_mdagm_mixed(gd, 18, gd, 12, s, s, 0.1, 0.1, 1e-8, 10),
+                 lambda: B.lqcd_cg_mdagm_mixed(gd, 17, gd, 12, s, B.alloc_spinor(), 0.1, 0.1, 1e-8, 10),
+                 lambda: B.lqcd_cg_mdagm_mixed(gd, 18, gd, 12, s, B.alloc_spinor(), 0.1, 0.1, 1e-8, 10, 2.0)):
+        with pytest.raises(B.LqcdError) as e:
+            call()
+        assert e.value.status == B.LQCD_BAD_ARG
+
+
+def test_mixed_precision_cg_24c48(B, oracle_mod):
+    dims = (24, 24, 24, 48)
+    kappa, mu, tol = 0.15, 0.1, 1e-10
+    U = gen.gauge_haar(dims, SEED)
+    b = gen.spinor_gaussian(lu.volume(dims) // 2, SEED, gen.STREAM_SOURCE)
+    st, x, (iters, rr, rt), outer = _mixed_solve(B, dims, U, b, kappa, mu, tol, 2000)
+    assert st == 0 and rr <= tol and 20 <= iters <= 120
+    r = b - oracle_mod.mdagm(dims, AP, U, x, kappa, mu)
+    assert np.linalg.norm(r) / np.linalg.norm(b) <= 1.05 * tol
