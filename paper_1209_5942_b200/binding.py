@@ -73,7 +73,7 @@ def _load():
 
 
 _lib = _load()
-_fmt = {"precision": LQCD_DOUBLE}  # mirrors the library's format, for buffer helpers only
+_fmt = {"precision": LQCD_DOUBLE, "vh": 0}  # mirrors format and sites per parity, for buffer helpers only
 
 
 def _check(status):
@@ -103,6 +103,7 @@ def lqcd_init(dims, bc_phase):
     p = (ctypes.c_double * 8)(*[float(v) for z in ph for v in (z.real, z.imag)])
     rc = _check(_lib.lqcd_init(d, p))
     _fmt["precision"] = LQCD_DOUBLE
+    _fmt["vh"] = int(np.prod([int(v) for v in dims])) // 2
     return rc
 
 
@@ -242,7 +243,6 @@ def upload_spinor(psi_canon, parity, device="cuda"):
 
 def download_spinor(s_internal, parity):
     """packed internal device buffer -> numpy (V/2,4,3) complex128."""
-    n_sites = lqcd_spinor_bytes() // (192 if _fmt["precision"] == LQCD_DOUBLE else 96)
-    canon = torch.empty((n_sites, 4, 3), dtype=torch.complex128, device=s_internal.device)
+    canon = torch.empty((_fmt["vh"], 4, 3), dtype=torch.complex128, device=s_internal.device)
     lqcd_unpack_spinor(s_internal, canon, parity)
     return canon.cpu().numpy()

@@ -110,10 +110,12 @@ int cuda_fail(cudaError_t e, const char* what) {
         if (e_ != cudaSuccess) return cuda_fail(e_, #call);       \
     } while (0)
 
-size_t spinor_bytes_of(int precision, int Vh) { return (size_t)Vh * 12 * (precision == 0 ? 16 : 8); }
-size_t gauge_bytes_of(int precision, int recon, int Vh) {
-    return (size_t)Vh * 8 * recon * (precision == 0 ? 8 : 4);
+// sizes of the grouped layout: G groups of 32 sites per parity (pad sites included)
+size_t spinor_bytes_of(int precision, int G) { return (size_t)G * 32 * 12 * (precision == 0 ? 16 : 8); }
+size_t gauge_bytes_of(int precision, int recon, int G) {
+    return (size_t)G * 32 * 8 * recon * (precision == 0 ? 8 : 4);
 }
+size_t n_reals() { return (size_t)24 * 32 * ctx.geo.G; }  // reals in one half-spinor field
 
 void free_workspace() {
     for (int pr = 0; pr < 2; ++pr)
@@ -144,7 +146,7 @@ int ensure_scalars() {
         CU(cudaMallocHost(&ctx.scal_host, 3 * sizeof(CgScalars)));
         for (int i = 0; i < 2; ++i) CU(cudaEventCreateWithFlags(&ctx.ev[i], cudaEventDisableTiming));
     }
-    const size_t need = (size_t)hopping_partials(ctx.geo.Vh, 32) + (size_t)vector_grid((size_t)24 * ctx.geo.Vh) + 64;
+    const size_t need = (size_t)hopping_partials(ctx.geo.Vh, 32) + (size_t)vector_grid(n_reals()) + 64;
     if (need > ctx.n_partials) {
         if (ctx.partials) CU(cudaFree(ctx.partials));
         ctx.partials = nullptr;
@@ -157,7 +159,7 @@ int ensure_scalars() {
 int ensure_workspace(int precision, int nvec) {
     int rc = ensure_scalars();
     if (rc) return rc;
-    const size_t sb = spinor_bytes_of(precision, ctx.geo.Vh);
+    const size_t sb = spinor_bytes_of(precision, ctx.geo.G);
     // t1 (index 3) is needed by lqcd_mtm; the rest only by CG
     const int order[5] = {3, 4, 0, 1, 2};
     for (int k = 0; k < nvec; ++k) {
@@ -212,7 +214,7 @@ int apply_mhat(int precision, int recon, const void* gauge, const void* in, void
 int enqueue_iteration() {
     void** v = ctx.vec[ctx.cg_prec];
     void *r = v[0], *p = v[1], *q = v[2], *t1 = v[3], *t2 = v[4];
-    const size_t n = (size_t)24 * ctx.geo.Vh;
+    const size_t n = n_reals();
     int rc = apply_mhat(ctx.cg_prec, ctx.cg_recon, ctx.cg_gauge, p, t1, t2, ctx.cg_kappa, ctx.cg_mu, 0, true, ctx.scal);
     if (rc) return rc;
     rc = apply_mhat(ctx.cg_prec, ctx.cg_recon, ctx.cg_gauge, t2, t1, q, ctx.cg_kappa, ctx.cg_mu, 1, false, ctx.scal);
@@ -229,7 +231,7 @@ int cg_setup_impl(int precision, int recon, const void* gauge, const void* b, vo
     ctx.cg_prec = precision; ctx.cg_recon = recon;
     ctx.cg_gauge = gauge; ctx.cg_b = b; ctx.cg_x = x;
     ctx.cg_kappa = kappa; ctx.cg_mu = mu; ctx.cg_tol = tol;
-    CU(launch_cg_init(precision, (size_t)24 * ctx.geo.Vh, b, x, ctx.vec[precision][0], ctx.vec[precision][1],
+    CU(launch_cg_init(precision, n_reals(), b, x, ctx.vec[precision][0], ctx.vec[precision][1],
                       tol, red(), ctx.scal, ctx.stream));
     ctx.cg_active = true;
     return LQCD_OK;
@@ -273,7 +275,7 @@ int cg_finish_impl(bool true_resid) {
         if (rc) return rc;
         rc = apply_mhat(ctx.cg_prec, ctx.cg_recon, ctx.cg_gauge, t2, t1, q, ctx.cg_kappa, ctx.cg_mu, 1, false, nullptr);
         if (rc) return rc;
-        CU(launch_true_resid(ctx.cg_prec, (size_t)24 * ctx.geo.Vh, ctx.cg_b, q, red(), ctx.scal, ctx.stream));
+        CU(launch_true_resid(ctx.cg_prec, n_reals(), ctx.cg_b, q, red(), ctx.scal, ctx.stream));
     }
     CU(cudaMemcpyAsync(ctx.scal_host, ctx.scal, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx.stream));
     CU(cudaStreamSynchronize(ctx.stream));
@@ -316,6 +318,7 @@ int lqcd_init(const int dims[4], const double bc_phase[8]) {
     }
     ctx.geo.N0h = dims[0] / 2; ctx.geo.N1 = dims[1]; ctx.geo.N2 = dims[2]; ctx.geo.N3 = dims[3];
     ctx.geo.Vh = (int)(V / 2);
+    ctx.geo.G = (ctx.geo.Vh + 31) / 32;
     ctx.precision = LQCD_DOUBLE; ctx.recon = 18; ctx.block = 128; ctx.stream = 0;
     g_launches.store(0);
     g_err[0] = 0;
@@ -351,8 +354,8 @@ int lqcd_set_block_size(int threads) {
     return LQCD_OK;
 }
 
-size_t lqcd_gauge_bytes(void) { return ctx.init ? gauge_bytes_of(ctx.precision, ctx.recon, ctx.geo.Vh) : 0; }
-size_t lqcd_spinor_bytes(void) { return ctx.init ? spinor_bytes_of(ctx.precision, ctx.geo.Vh) : 0; }
+size_t lqcd_gauge_bytes(void) { return ctx.init ? gauge_bytes_of(ctx.precision, ctx.recon, ctx.geo.G) : 0; }
+size_t lqcd_spinor_bytes(void) { return ctx.init ? spinor_bytes_of(ctx.precision, ctx.geo.G) : 0; }
 long long lqcd_launch_count(void) { return g_launches.load(); }
 
 int lqcd_profile(int enable) {
@@ -489,12 +492,12 @@ int lqcd_cg_mdagm_mixed(const void* gauge_double, int recon_double, const void* 
         return fail(LQCD_BAD_ARG, "inner_tol must be in [0, 1)");
     if ((rc = ensure_workspace(LQCD_DOUBLE, 5))) return rc;
     if ((rc = ensure_workspace(LQCD_SINGLE, 5))) return rc;
-    const size_t sbf = spinor_bytes_of(LQCD_SINGLE, ctx.geo.Vh);
+    const size_t sbf = spinor_bytes_of(LQCD_SINGLE, ctx.geo.G);
     if (!ctx.mx_b) CU(cudaMalloc(&ctx.mx_b, sbf));
     if (!ctx.mx_x) CU(cudaMalloc(&ctx.mx_x, sbf));
     void** vd = ctx.vec[LQCD_DOUBLE];
     void *r = vd[0], *q = vd[2], *t1 = vd[3], *t2 = vd[4];
-    const size_t n = (size_t)24 * ctx.geo.Vh;
+    const size_t n = n_reals();
     CgScalars* so = ctx.scal_outer;
     CgScalars* sh = &ctx.scal_host[2];
     // x = 0, r = b, bb = rho = |b|^2 (p slot vd[1] is scratch here)

@@ -43,36 +43,37 @@ __device__ __forceinline__ double fma_(double a, double b, double c) { return fm
 __device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
 
 // ----------------------------------------------------------------------------- field access
-__device__ __forceinline__ void load_spinor(const void* base, int Vh, int idx, double (&psi)[24]) {
-    const double2* p = reinterpret_cast<const double2*>(base) + idx;
+// Grouped layout (lqcd_internal.h): one address per site, compile-time offsets per component.
+__device__ __forceinline__ void load_spinor(const void* base, int idx, double (&psi)[24]) {
+    const double2* p = reinterpret_cast<const double2*>(base) + (size_t)(idx >> 5) * (12 * 32) + (idx & 31);
 #pragma unroll
     for (int c = 0; c < 12; ++c) {
-        const double2 v = __ldg(p + (size_t)c * Vh);
+        const double2 v = __ldg(p + c * 32);
         psi[2 * c] = v.x;
         psi[2 * c + 1] = v.y;
     }
 }
-__device__ __forceinline__ void load_spinor(const void* base, int Vh, int idx, float (&psi)[24]) {
-    const float4* p = reinterpret_cast<const float4*>(base) + idx;
+__device__ __forceinline__ void load_spinor(const void* base, int idx, float (&psi)[24]) {
+    const float4* p = reinterpret_cast<const float4*>(base) + (size_t)(idx >> 5) * (6 * 32) + (idx & 31);
 #pragma unroll
     for (int k = 0; k < 6; ++k) {
-        const float4 v = __ldg(p + (size_t)k * Vh);
+        const float4 v = __ldg(p + k * 32);
         psi[4 * k] = v.x;
         psi[4 * k + 1] = v.y;
         psi[4 * k + 2] = v.z;
         psi[4 * k + 3] = v.w;
     }
 }
-__device__ __forceinline__ void store_spinor(void* base, int Vh, int idx, const double (&o)[24]) {
-    double2* p = reinterpret_cast<double2*>(base) + idx;
+__device__ __forceinline__ void store_spinor(void* base, int idx, const double (&o)[24]) {
+    double2* p = reinterpret_cast<double2*>(base) + (size_t)(idx >> 5) * (12 * 32) + (idx & 31);
 #pragma unroll
-    for (int c = 0; c < 12; ++c) p[(size_t)c * Vh] = make_double2(o[2 * c], o[2 * c + 1]);
+    for (int c = 0; c < 12; ++c) p[c * 32] = make_double2(o[2 * c], o[2 * c + 1]);
 }
-__device__ __forceinline__ void store_spinor(void* base, int Vh, int idx, const float (&o)[24]) {
-    float4* p = reinterpret_cast<float4*>(base) + idx;
+__device__ __forceinline__ void store_spinor(void* base, int idx, const float (&o)[24]) {
+    float4* p = reinterpret_cast<float4*>(base) + (size_t)(idx >> 5) * (6 * 32) + (idx & 31);
 #pragma unroll
     for (int k = 0; k < 6; ++k)
-        p[(size_t)k * Vh] = make_float4(o[4 * k], o[4 * k + 1], o[4 * k + 2], o[4 * k + 3]);
+        p[k * 32] = make_float4(o[4 * k], o[4 * k + 1], o[4 * k + 2], o[4 * k + 3]);
 }
 
 // third row of an SU(3) matrix from the first two: row2 = conj(row0 x row1)  (G9)
@@ -92,27 +93,27 @@ __device__ __forceinline__ void reconstruct_row2(T (&u)[18]) {
 }
 
 template <int RECON>
-__device__ __forceinline__ void load_link(const void* gauge, int Vh, int par, int mu, int idx,
+__device__ __forceinline__ void load_link(const void* gauge, int G, int par, int mu, int idx,
                                           double (&u)[18]) {
-    const double2* p =
-        reinterpret_cast<const double2*>(gauge) + (size_t)((par * 4 + mu) * (RECON / 2)) * Vh + idx;
+    const double2* p = reinterpret_cast<const double2*>(gauge) +
+                       ((size_t)(par * 4 + mu) * G + (idx >> 5)) * ((RECON / 2) * 32) + (idx & 31);
 #pragma unroll
     for (int j = 0; j < RECON / 2; ++j) {
-        const double2 v = __ldcs(p + (size_t)j * Vh);
+        const double2 v = __ldcs(p + j * 32);
         u[2 * j] = v.x;
         u[2 * j + 1] = v.y;
     }
     if (RECON == 12) reconstruct_row2(u);
 }
 template <int RECON>
-__device__ __forceinline__ void load_link(const void* gauge, int Vh, int par, int mu, int idx,
+__device__ __forceinline__ void load_link(const void* gauge, int G, int par, int mu, int idx,
                                           float (&u)[18]) {
     if (RECON == 12) {
-        const float4* p =
-            reinterpret_cast<const float4*>(gauge) + (size_t)((par * 4 + mu) * 3) * Vh + idx;
+        const float4* p = reinterpret_cast<const float4*>(gauge) +
+                          ((size_t)(par * 4 + mu) * G + (idx >> 5)) * (3 * 32) + (idx & 31);
 #pragma unroll
         for (int j = 0; j < 3; ++j) {
-            const float4 v = __ldcs(p + (size_t)j * Vh);
+            const float4 v = __ldcs(p + j * 32);
             u[4 * j] = v.x;
             u[4 * j + 1] = v.y;
             u[4 * j + 2] = v.z;
@@ -120,17 +121,18 @@ __device__ __forceinline__ void load_link(const void* gauge, int Vh, int par, in
         }
         reconstruct_row2(u);
     } else {
-        const float* blk = reinterpret_cast<const float*>(gauge) + (size_t)(par * 4 + mu) * 18 * Vh;
-        const float4* p = reinterpret_cast<const float4*>(blk) + idx;
+        const float* blk = reinterpret_cast<const float*>(gauge) +
+                           ((size_t)(par * 4 + mu) * G + (idx >> 5)) * (18 * 32);
+        const float4* p = reinterpret_cast<const float4*>(blk) + (idx & 31);
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            const float4 v = __ldcs(p + (size_t)j * Vh);
+            const float4 v = __ldcs(p + j * 32);
             u[4 * j] = v.x;
             u[4 * j + 1] = v.y;
             u[4 * j + 2] = v.z;
             u[4 * j + 3] = v.w;
         }
-        const float2 w = __ldcs(reinterpret_cast<const float2*>(blk + (size_t)16 * Vh) + idx);
+        const float2 w = __ldcs(reinterpret_cast<const float2*>(blk + 16 * 32) + (idx & 31));
         u[16] = w.x;
         u[17] = w.y;
     }
@@ -257,10 +259,9 @@ struct HopArgs {
 template <typename T, int RECON, int MU, int FWD, int DAG>
 __device__ __forceinline__ void hop(T (&acc)[24], const HopArgs& a, int e, int e_nb, bool wrap) {
     constexpr int S = (FWD ? -1 : +1) * (DAG ? -1 : +1);
-    const int Vh = a.g.Vh;
     T psi[24], u[18], h[12], chi[12];
-    load_spinor(a.in, Vh, e_nb, psi);
-    load_link<RECON>(a.gauge, Vh, FWD ? a.out_parity : 1 - a.out_parity, MU, FWD ? e : e_nb, u);
+    load_spinor(a.in, e_nb, psi);
+    load_link<RECON>(a.gauge, a.g.G, FWD ? a.out_parity : 1 - a.out_parity, MU, FWD ? e : e_nb, u);
     project<MU, S>(psi, h);
     if (FWD) su3_mul(u, h, chi);
     else     su3_dag_mul(u, h, chi);
@@ -301,7 +302,7 @@ hopping_kernel(const HopArgs a) {
         T acc[24];
         if (MODE >= 1) {
             T x[24];
-            load_spinor(a.aux, Vh, e, x);
+            load_spinor(a.aux, e, x);
             const T dur = (T)a.ep.du_re, dui = (T)a.ep.du_im, ddr = (T)a.ep.dd_re, ddi = (T)a.ep.dd_im;
 #pragma unroll
             for (int c = 0; c < 12; ++c) {
@@ -345,11 +346,23 @@ hopping_kernel(const HopArgs a) {
             o[2 * c] = fma_(-ci, acc[2 * c + 1], cr * acc[2 * c]);
             o[2 * c + 1] = fma_(ci, acc[2 * c], cr * acc[2 * c + 1]);
         }
-        store_spinor(a.out, Vh, e, o);
-        if (MODE == 2) {
+        store_spinor(a.out, e, o);
+        if (MODE == 2) {  // |out|^2 = |c_u|^2 |acc_upper|^2 + |c_d|^2 |acc_lower|^2
+            double nu = 0.0, nd = 0.0;
 #pragma unroll
-            for (int i = 0; i < 24; ++i) nrm += (double)o[i] * (double)o[i];
+            for (int i = 0; i < 12; ++i) {
+                nu += (double)acc[i] * (double)acc[i];
+                nd += (double)acc[12 + i] * (double)acc[12 + i];
+            }
+            nrm = (a.ep.cu_re * a.ep.cu_re + a.ep.cu_im * a.ep.cu_im) * nu +
+                  (a.ep.cd_re * a.ep.cd_re + a.ep.cd_im * a.ep.cd_im) * nd;
         }
+    }
+    if (e >= Vh && e < a.g.G * 32) {  // pad sites of the last group hold zeros
+        T z[24];
+#pragma unroll
+        for (int i = 0; i < 24; ++i) z[i] = 0;
+        store_spinor(a.out, e, z);
     }
     if (MODE == 2) {  // one partial per warp, plain store; summed by launch_finalize(FIN_PAP)
         nrm = warp_sum(nrm);

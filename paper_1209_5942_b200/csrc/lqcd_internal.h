@@ -2,15 +2,22 @@
 //
 // Internal field layout (opaque to callers):
 //   Vh = V/2 sites per parity, e = x0/2 + N0h (x1 + N1 (x2 + N2 x3)), N0h = N0/2.
-//   double spinor : double2 s[12][Vh]            component c = 3 alpha + a
-//   float  spinor : float4  s[6][Vh]             element k holds components 2k, 2k+1
-//   double gauge  : double2 g[2][4][9 or 6][Vh]  [parity of origin][mu][row-major entry]
-//   float  gauge 12: float4 g[2][4][3][Vh]
-//   float  gauge 18: per (parity, mu) block of 18 Vh floats: float4 planes 0..3, then one float2 plane
-// The site index is fastest, so a warp touches 512 (double) contiguous bytes per
-// component: 128-bit vectorised, fully coalesced (PAPER.md:221 reached the same
-// conclusion for a 16-byte base type; here it is chosen for LDG.128 / 128 B lines).
-// The gauge field is split by the parity of the link's origin.
+//   Sites are grouped in 32s (one warp): G = ceil(Vh/32) groups, site e = (group g = e >> 5,
+//   lane l = e & 31).  Inside a group the component index comes before the lane:
+//   double spinor : double2 s[G][12][32]          component c = 3 alpha + a
+//   float  spinor : float4  s[G][6][32]           element k holds components 2k, 2k+1
+//   double gauge  : double2 g[2][4][G][9 or 6][32]  [parity of origin][mu][group][row-major entry][lane]
+//   float  gauge 12: float4 g[2][4][G][3][32]
+//   float  gauge 18: per (parity, mu, group) 576 floats: float4 planes 0..3 [32], then a float2 plane [32]
+// A warp still touches 512 (double) contiguous, 512-byte aligned bytes per component -- 128-bit
+// vectorised, fully coalesced, the same property the paper found for a 16-byte base type
+// -- but the distance between the components of one site is now a compile-time
+// constant (512 B), so the 12 + 9 loads of a hop take their offsets as instruction immediates
+// from ONE computed address instead of one 64-bit address computation each (a plane-major
+// [component][Vh] layout costs ~3.7 integer instructions per load).
+// Pad sites (e >= Vh in the last group, only when Vh is not a multiple of 32) hold zeros in
+// every spinor field the library writes.  The gauge field is split by the parity of the
+// link's origin.
 #pragma once
 
 #include <cuda_runtime.h>
@@ -21,6 +28,7 @@ namespace lqcd {
 struct Geometry {
     int N0h, N1, N2, N3;  // N0h = N_x / 2
     int Vh;               // sites per parity
+    int G;                // groups of 32 sites per parity = ceil(Vh / 32)
     double ph_re[4], ph_im[4];
 };
 
@@ -64,7 +72,7 @@ cudaError_t launch_hopping(int precision, int recon, int dagger, int mode, const
                            const void* aux, int out_parity, int reverse, Reduction red,
                            CgScalars* scal, int block, cudaStream_t st);
 
-// vector_ops.cu  (n = number of reals in a half-spinor field = 24 Vh)
+// vector_ops.cu  (n = number of reals in a half-spinor field incl. padding = 24 * 32 * G)
 cudaError_t launch_cg_init(int precision, size_t n, const void* b, void* x, void* r, void* p,
                            double tol, Reduction red, CgScalars* scal, cudaStream_t st);
 cudaError_t launch_cg_update_r(int precision, size_t n, void* r, const void* q, int reverse,

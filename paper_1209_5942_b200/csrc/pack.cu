@@ -17,7 +17,8 @@ __device__ __forceinline__ int site_r(const Geometry& g, int e, int parity) {
     return (x1 + x2 + x3 + parity) & 1;
 }
 
-// one thread per (parity, mu, e): reads the 144-byte link U[lex][mu], lex = 2e + r
+// one thread per (parity, mu, e): reads the 144-byte link U[lex][mu], lex = 2e + r, and writes
+// it into group e >> 5, lane e & 31 of the grouped layout (lqcd_internal.h)
 template <typename T, int RECON>
 __global__ void __launch_bounds__(PBLOCK) pack_gauge_kernel(Geometry g, const double2* __restrict__ canon,
                                                             void* __restrict__ internal) {
@@ -32,47 +33,54 @@ __global__ void __launch_bounds__(PBLOCK) pack_gauge_kernel(Geometry g, const do
     double2 u[9];
 #pragma unroll
     for (int j = 0; j < 9; ++j) u[j] = src[j];
+    const size_t grp = (size_t)pm * g.G + (e >> 5);
+    const int lane = e & 31;
     if (sizeof(T) == 8) {
-        double2* dst = (double2*)internal + (size_t)pm * (RECON / 2) * Vh + e;
+        double2* dst = (double2*)internal + grp * ((RECON / 2) * 32) + lane;
 #pragma unroll
-        for (int j = 0; j < RECON / 2; ++j) dst[(size_t)j * Vh] = u[j];
+        for (int j = 0; j < RECON / 2; ++j) dst[j * 32] = u[j];
     } else if (RECON == 12) {
-        float4* dst = (float4*)internal + (size_t)pm * 3 * Vh + e;
+        float4* dst = (float4*)internal + grp * (3 * 32) + lane;
 #pragma unroll
         for (int j = 0; j < 3; ++j)
-            dst[(size_t)j * Vh] = make_float4((float)u[2 * j].x, (float)u[2 * j].y, (float)u[2 * j + 1].x,
-                                              (float)u[2 * j + 1].y);
+            dst[j * 32] = make_float4((float)u[2 * j].x, (float)u[2 * j].y, (float)u[2 * j + 1].x,
+                                      (float)u[2 * j + 1].y);
     } else {
-        float* blk = (float*)internal + (size_t)pm * 18 * Vh;
-        float4* dst = (float4*)blk + e;
+        float* blk = (float*)internal + grp * (18 * 32);
+        float4* dst = (float4*)blk + lane;
 #pragma unroll
         for (int j = 0; j < 4; ++j)
-            dst[(size_t)j * Vh] = make_float4((float)u[2 * j].x, (float)u[2 * j].y, (float)u[2 * j + 1].x,
-                                              (float)u[2 * j + 1].y);
-        ((float2*)(blk + 16 * Vh))[e] = make_float2((float)u[8].x, (float)u[8].y);
+            dst[j * 32] = make_float4((float)u[2 * j].x, (float)u[2 * j].y, (float)u[2 * j + 1].x,
+                                      (float)u[2 * j + 1].y);
+        ((float2*)(blk + 16 * 32))[lane] = make_float2((float)u[8].x, (float)u[8].y);
     }
 }
 
-// canonical half spinor psi_p[e][c] -> internal s[c][e]
+// canonical half spinor psi_p[e][c] -> internal s[e >> 5][c][e & 31]; pad sites get zeros
 template <typename T>
-__global__ void __launch_bounds__(PBLOCK) pack_spinor_kernel(int Vh, const double2* __restrict__ canon,
+__global__ void __launch_bounds__(PBLOCK) pack_spinor_kernel(int Vh, int G, const double2* __restrict__ canon,
                                                              void* __restrict__ internal) {
     const int e = blockIdx.x * PBLOCK + threadIdx.x;
-    if (e >= Vh) return;
-    const double2* src = canon + (size_t)e * 12;
+    if (e >= G * 32) return;
     double2 s[12];
+    if (e < Vh) {
+        const double2* src = canon + (size_t)e * 12;
 #pragma unroll
-    for (int c = 0; c < 12; ++c) s[c] = src[c];
-    if (sizeof(T) == 8) {
-        double2* dst = (double2*)internal + e;
-#pragma unroll
-        for (int c = 0; c < 12; ++c) dst[(size_t)c * Vh] = s[c];
+        for (int c = 0; c < 12; ++c) s[c] = src[c];
     } else {
-        float4* dst = (float4*)internal + e;
+#pragma unroll
+        for (int c = 0; c < 12; ++c) s[c] = make_double2(0.0, 0.0);
+    }
+    if (sizeof(T) == 8) {
+        double2* dst = (double2*)internal + (size_t)(e >> 5) * (12 * 32) + (e & 31);
+#pragma unroll
+        for (int c = 0; c < 12; ++c) dst[c * 32] = s[c];
+    } else {
+        float4* dst = (float4*)internal + (size_t)(e >> 5) * (6 * 32) + (e & 31);
 #pragma unroll
         for (int k = 0; k < 6; ++k)
-            dst[(size_t)k * Vh] = make_float4((float)s[2 * k].x, (float)s[2 * k].y, (float)s[2 * k + 1].x,
-                                              (float)s[2 * k + 1].y);
+            dst[k * 32] = make_float4((float)s[2 * k].x, (float)s[2 * k].y, (float)s[2 * k + 1].x,
+                                      (float)s[2 * k + 1].y);
     }
 }
 
@@ -83,14 +91,14 @@ __global__ void __launch_bounds__(PBLOCK) unpack_spinor_kernel(int Vh, const voi
     if (e >= Vh) return;
     double2 s[12];
     if (sizeof(T) == 8) {
-        const double2* src = (const double2*)internal + e;
+        const double2* src = (const double2*)internal + (size_t)(e >> 5) * (12 * 32) + (e & 31);
 #pragma unroll
-        for (int c = 0; c < 12; ++c) s[c] = src[(size_t)c * Vh];
+        for (int c = 0; c < 12; ++c) s[c] = src[c * 32];
     } else {
-        const float4* src = (const float4*)internal + e;
+        const float4* src = (const float4*)internal + (size_t)(e >> 5) * (6 * 32) + (e & 31);
 #pragma unroll
         for (int k = 0; k < 6; ++k) {
-            const float4 v = src[(size_t)k * Vh];
+            const float4 v = src[k * 32];
             s[2 * k] = make_double2(v.x, v.y);
             s[2 * k + 1] = make_double2(v.z, v.w);
         }
@@ -121,11 +129,11 @@ cudaError_t launch_pack_gauge(int precision, int recon, const Geometry& g, const
 
 cudaError_t launch_pack_spinor(int precision, const Geometry& g, const void* canon, void* internal,
                                int /*parity*/, cudaStream_t st) {
-    const int grid = (g.Vh + PBLOCK - 1) / PBLOCK;
+    const int grid = (g.G * 32 + PBLOCK - 1) / PBLOCK;
     count_launch();
     ProfScope prof(4, st);
-    if (precision == 0) pack_spinor_kernel<double><<<grid, PBLOCK, 0, st>>>(g.Vh, (const double2*)canon, internal);
-    else                pack_spinor_kernel<float><<<grid, PBLOCK, 0, st>>>(g.Vh, (const double2*)canon, internal);
+    if (precision == 0) pack_spinor_kernel<double><<<grid, PBLOCK, 0, st>>>(g.Vh, g.G, (const double2*)canon, internal);
+    else                pack_spinor_kernel<float><<<grid, PBLOCK, 0, st>>>(g.Vh, g.G, (const double2*)canon, internal);
     return cudaGetLastError();
 }
 

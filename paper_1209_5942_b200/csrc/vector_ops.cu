@@ -208,25 +208,26 @@ __global__ void __launch_bounds__(VBLOCK) true_resid_kernel(size_t nvec, const v
     block_partial(s, red);
 }
 
-// ---- mixed-precision helpers.  Double field: double2 d[12][Vh]; float field: float4 f[6][Vh] with
-// f[k][e] = (d[2k][e], d[2k+1][e]).  One thread per float4 element.
-__global__ void __launch_bounds__(VBLOCK) convert_d2f_kernel(size_t Vh, const double2* __restrict__ d,
+// ---- mixed-precision helpers.  Double field: double2 d[G][12][32]; float field: float4 f[G][6][32]
+// with f[g][k][l] = (d[g][2k][l], d[g][2k+1][l]).  One thread per float4 element.
+__global__ void __launch_bounds__(VBLOCK) convert_d2f_kernel(size_t nf4, const double2* __restrict__ d,
                                                              float4* __restrict__ f, double scale) {
     const size_t i = (size_t)blockIdx.x * VBLOCK + threadIdx.x;
-    if (i >= 6 * Vh) return;
-    const size_t k = i / Vh, e = i - k * Vh;
-    const double2 a = __ldcs(d + (2 * k) * Vh + e), b = __ldcs(d + (2 * k + 1) * Vh + e);
+    if (i >= nf4) return;
+    const size_t g = i / 192, r = i - g * 192, k = r >> 5, l = r & 31;
+    const double2* p = d + g * 384 + (2 * k) * 32 + l;
+    const double2 a = __ldcs(p), b = __ldcs(p + 32);
     f[i] = make_float4((float)(a.x * scale), (float)(a.y * scale), (float)(b.x * scale), (float)(b.y * scale));
 }
 
-__global__ void __launch_bounds__(VBLOCK) axpy_f2d_kernel(size_t Vh, double a, const float4* __restrict__ x,
+__global__ void __launch_bounds__(VBLOCK) axpy_f2d_kernel(size_t nf4, double a, const float4* __restrict__ x,
                                                           double2* __restrict__ y) {
     const size_t i = (size_t)blockIdx.x * VBLOCK + threadIdx.x;
-    if (i >= 6 * Vh) return;
-    const size_t k = i / Vh, e = i - k * Vh;
+    if (i >= nf4) return;
+    const size_t g = i / 192, r = i - g * 192, k = r >> 5, l = r & 31;
     const float4 v = __ldcs(x + i);
-    double2* y0 = y + (2 * k) * Vh + e;
-    double2* y1 = y + (2 * k + 1) * Vh + e;
+    double2* y0 = y + g * 384 + (2 * k) * 32 + l;
+    double2* y1 = y0 + 32;
     const double2 u0 = *y0, u1 = *y1;
     *y0 = make_double2(fma(a, (double)v.x, u0.x), fma(a, (double)v.y, u0.y));
     *y1 = make_double2(fma(a, (double)v.z, u1.x), fma(a, (double)v.w, u1.y));
@@ -264,20 +265,20 @@ cudaError_t launch_finalize(int fin, Reduction red, int n_partials, double tol, 
 }
 
 cudaError_t launch_convert_d2f(size_t n, const void* src_d, void* dst_f, double scale, cudaStream_t st) {
-    const size_t Vh = n / 24;
+    const size_t nf4 = n / 4;
     count_launch();
     ProfScope prof(3, st);
-    convert_d2f_kernel<<<(int)((6 * Vh + VBLOCK - 1) / VBLOCK), VBLOCK, 0, st>>>(Vh, (const double2*)src_d,
-                                                                                 (float4*)dst_f, scale);
+    convert_d2f_kernel<<<(int)((nf4 + VBLOCK - 1) / VBLOCK), VBLOCK, 0, st>>>(nf4, (const double2*)src_d,
+                                                                              (float4*)dst_f, scale);
     return cudaGetLastError();
 }
 
 cudaError_t launch_axpy_f2d(size_t n, double a, const void* x_f, void* y_d, cudaStream_t st) {
-    const size_t Vh = n / 24;
+    const size_t nf4 = n / 4;
     count_launch();
     ProfScope prof(3, st);
-    axpy_f2d_kernel<<<(int)((6 * Vh + VBLOCK - 1) / VBLOCK), VBLOCK, 0, st>>>(Vh, a, (const float4*)x_f,
-                                                                              (double2*)y_d);
+    axpy_f2d_kernel<<<(int)((nf4 + VBLOCK - 1) / VBLOCK), VBLOCK, 0, st>>>(nf4, a, (const float4*)x_f,
+                                                                           (double2*)y_d);
     return cudaGetLastError();
 }
 
