@@ -96,6 +96,22 @@ int lqcd_dslash_eo(const void* gauge, const void* in, void* out, int parity, dou
  * Uses one half-spinor of library workspace. */
 int lqcd_mtm(const void* gauge, const void* in, void* out, double kappa, double mu, int dagger);
 
+/* The full operator of eq. 6 on both parities (internal layouts; two hopping launches with the
+ * diagonal term in their epilogues):
+ *   out_e = M_ee in_e + D_eo in_o,   out_o = M_oo in_o + D_oe in_e.   No buffer may alias another. */
+int lqcd_mtm_full(const void* gauge, const void* in_even, const void* in_odd, void* out_even,
+                  void* out_odd, double kappa, double mu);
+
+/* Solve M psi = eta on the WHOLE lattice (eq. 8) through the even-odd system:
+ *   rhs_e = eta_e - D_eo M_oo^{-1} eta_o;   CG on Mhat^dag Mhat psi_e = Mhat^dag rhs_e;
+ *   psi_o = M_oo^{-1} (eta_o - D_oe psi_e).
+ * tol is the CG tolerance on the normal equations (|Mhat^dag (rhs - Mhat psi_e)| <= tol |Mhat^dag rhs|);
+ * the residual of the full system is larger by at most cond(Mhat).  psi_even / psi_odd are used as
+ * scratch before they receive the solution and must not alias eta_*.  Returns the CG status;
+ * lqcd_cg_stats() gives its iterations and residuals.  Synchronous. */
+int lqcd_solve_full(const void* gauge, const void* eta_even, const void* eta_odd, void* psi_even,
+                    void* psi_odd, double kappa, double mu, double tol, int maxit);
+
 /* Solve Mhat^dag Mhat x = b on even sites by CG (reading G10):
  * x0 = 0 (input contents of x ignored), stop when |r| <= tol |b| (recursive
  * residual) or after maxit iterations.  Returns LQCD_OK, LQCD_NOT_CONVERGED or

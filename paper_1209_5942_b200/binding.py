@@ -20,7 +20,7 @@ LQCD_DOUBLE, LQCD_SINGLE = 0, 1
 SYMBOLS = [
     "lqcd_last_error", "lqcd_init", "lqcd_finalize", "lqcd_set_stream", "lqcd_set_format",
     "lqcd_gauge_bytes", "lqcd_spinor_bytes", "lqcd_pack_gauge", "lqcd_pack_spinor",
-    "lqcd_unpack_spinor", "lqcd_dslash_eo", "lqcd_mtm", "lqcd_cg_mdagm", "lqcd_cg_setup",
+    "lqcd_unpack_spinor", "lqcd_dslash_eo", "lqcd_mtm", "lqcd_mtm_full", "lqcd_solve_full", "lqcd_cg_mdagm", "lqcd_cg_setup",
     "lqcd_cg_iterate", "lqcd_cg_finish", "lqcd_cg_stats", "lqcd_cg_mdagm_mixed", "lqcd_cg_outer_iterations", "lqcd_mtm_host", "lqcd_cg_mdagm_host",
     "lqcd_launch_count", "lqcd_set_block_size", "lqcd_profile", "lqcd_profile_read",
 ]
@@ -52,6 +52,8 @@ def _load():
         "lqcd_unpack_spinor": [vp, vp, i32],
         "lqcd_dslash_eo": [vp, vp, vp, i32, dbl],
         "lqcd_mtm": [vp, vp, vp, dbl, dbl, i32],
+        "lqcd_mtm_full": [vp, vp, vp, vp, vp, dbl, dbl],
+        "lqcd_solve_full": [vp, vp, vp, vp, vp, dbl, dbl, dbl, i32],
         "lqcd_cg_mdagm": [vp, vp, vp, dbl, dbl, dbl, i32],
         "lqcd_cg_setup": [vp, vp, vp, dbl, dbl, dbl],
         "lqcd_cg_mdagm_mixed": [vp, i32, vp, i32, vp, vp, dbl, dbl, dbl, i32, dbl],
@@ -168,6 +170,16 @@ def lqcd_dslash_eo(gauge, inp, out, parity, kappa):
 
 def lqcd_mtm(gauge, inp, out, kappa, mu, dagger):
     return _check(_lib.lqcd_mtm(_ptr(gauge), _ptr(inp), _ptr(out), kappa, mu, dagger))
+
+
+def lqcd_mtm_full(gauge, in_even, in_odd, out_even, out_odd, kappa, mu):
+    return _check(_lib.lqcd_mtm_full(_ptr(gauge), _ptr(in_even), _ptr(in_odd), _ptr(out_even), _ptr(out_odd),
+                                     kappa, mu))
+
+
+def lqcd_solve_full(gauge, eta_even, eta_odd, psi_even, psi_odd, kappa, mu, tol, maxit):
+    return _check(_lib.lqcd_solve_full(_ptr(gauge), _ptr(eta_even), _ptr(eta_odd), _ptr(psi_even), _ptr(psi_odd),
+                                       kappa, mu, tol, maxit))
 
 
 def lqcd_cg_mdagm(gauge, b, x, kappa, mu, tol, maxit):

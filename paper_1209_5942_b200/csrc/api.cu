@@ -62,6 +62,7 @@ struct Context {
 
     // workspace (owned), one set of half spinors per precision: r, p, q, t1, t2
     void* vec[2][5] = {{nullptr, nullptr, nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr, nullptr, nullptr}};
+    void* full_b[2] = {nullptr, nullptr};  // lqcd_solve_full: right-hand side of the normal equations
     void* mx_b = nullptr;            // mixed solver: single-precision right-hand side and correction
     void* mx_x = nullptr;
     CgScalars* scal = nullptr;       // scalars of the running CG
@@ -120,6 +121,7 @@ size_t n_reals() { return (size_t)24 * 32 * ctx.geo.G; }  // reals in one half-s
 void free_workspace() {
     for (int pr = 0; pr < 2; ++pr)
         for (int i = 0; i < 5; ++i) { if (ctx.vec[pr][i]) cudaFree(ctx.vec[pr][i]); ctx.vec[pr][i] = nullptr; }
+    for (int pr = 0; pr < 2; ++pr) { if (ctx.full_b[pr]) cudaFree(ctx.full_b[pr]); ctx.full_b[pr] = nullptr; }
     if (ctx.mx_b) cudaFree(ctx.mx_b);
     if (ctx.mx_x) cudaFree(ctx.mx_x);
     ctx.mx_b = ctx.mx_x = nullptr;
@@ -431,6 +433,83 @@ int lqcd_mtm(const void* gauge, const void* in, void* out, double kappa, double 
     if (rc) return rc;
     return apply_mhat(ctx.precision, ctx.recon, gauge, in, ctx.vec[ctx.precision][3], out, kappa, mu, dagger,
                       false, nullptr);
+}
+
+// One hopping launch with the M_diag * aux epilogue: out_p = a_chi * (bracket(in) + d_chi aux).
+static int hop_aux(const void* gauge, const void* in, const void* aux, void* out, int out_parity,
+                   double cur, double cui, double cdr, double cdi, double dur, double dui, double ddr,
+                   double ddi, int reverse) {
+    Epilogue e = {};
+    e.cu_re = cur; e.cu_im = cui; e.cd_re = cdr; e.cd_im = cdi;
+    e.du_re = dur; e.du_im = dui; e.dd_re = ddr; e.dd_im = ddi;
+    CU(launch_hopping(ctx.precision, ctx.recon, 0, 1, ctx.geo, e, gauge, in, out, aux, out_parity, reverse,
+                      red(), nullptr, ctx.block, ctx.stream));
+    return LQCD_OK;
+}
+
+int lqcd_mtm_full(const void* gauge, const void* in_even, const void* in_odd, void* out_even,
+                  void* out_odd, double kappa, double mu) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (!gauge || !in_even || !in_odd || !out_even || !out_odd) return fail(LQCD_BAD_ARG, "lqcd_mtm_full: null pointer");
+    if (out_even == in_even || out_even == in_odd || out_odd == in_even || out_odd == in_odd || out_even == out_odd)
+        return fail(LQCD_BAD_ARG, "lqcd_mtm_full: buffers alias");
+    int rc = check_scalar(kappa, "kappa");
+    if (rc) return rc;
+    if ((rc = check_scalar(mu, "mu"))) return rc;
+    const double c = 2.0 * kappa * mu;
+    if (kappa == 0.0) {  // M = M_diag
+        CU(launch_diag_scale(ctx.precision, n_reals(), in_even, out_even, 1.0, c, 1.0, -c, ctx.stream));
+        CU(launch_diag_scale(ctx.precision, n_reals(), in_odd, out_odd, 1.0, c, 1.0, -c, ctx.stream));
+        return LQCD_OK;
+    }
+    // out_p = (1 + i c chi) in_p - kappa bracket(in_{1-p}) = -kappa (bracket + [(1 + i c chi)/(-kappa)] in_p)
+    if ((rc = hop_aux(gauge, in_odd, in_even, out_even, 0, -kappa, 0, -kappa, 0, -1.0 / kappa, -c / kappa,
+                      -1.0 / kappa, c / kappa, 0))) return rc;
+    return hop_aux(gauge, in_even, in_odd, out_odd, 1, -kappa, 0, -kappa, 0, -1.0 / kappa, -c / kappa,
+                   -1.0 / kappa, c / kappa, 1);
+}
+
+// M psi = eta on the whole lattice through the even-odd system:
+//   rhs_e = eta_e - D_eo M_oo^{-1} eta_o;  Mhat^dag Mhat psi_e = Mhat^dag rhs_e (CG);
+//   psi_o = M_oo^{-1} (eta_o - D_oe psi_e).
+int lqcd_solve_full(const void* gauge, const void* eta_even, const void* eta_odd, void* psi_even,
+                    void* psi_odd, double kappa, double mu, double tol, int maxit) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (!gauge || !eta_even || !eta_odd || !psi_even || !psi_odd) return fail(LQCD_BAD_ARG, "lqcd_solve_full: null pointer");
+    if (psi_even == eta_even || psi_even == eta_odd || psi_odd == eta_even || psi_odd == eta_odd || psi_even == psi_odd)
+        return fail(LQCD_BAD_ARG, "lqcd_solve_full: buffers alias");
+    if (maxit < 1) return fail(LQCD_BAD_ARG, "maxit must be >= 1");
+    int rc = check_scalar(kappa, "kappa");
+    if (rc) return rc;
+    if ((rc = check_scalar(mu, "mu"))) return rc;
+    if (!std::isfinite(tol) || tol < 0.0) return fail(LQCD_BAD_ARG, "tol must be finite and >= 0");
+    const double c = 2.0 * kappa * mu, d = 1.0 + c * c;
+    const size_t n = n_reals();
+    if (kappa == 0.0) {  // M = M_diag: psi = M_diag^{-1} eta
+        CU(launch_diag_scale(ctx.precision, n, eta_even, psi_even, 1.0 / d, -c / d, 1.0 / d, c / d, ctx.stream));
+        CU(launch_diag_scale(ctx.precision, n, eta_odd, psi_odd, 1.0 / d, -c / d, 1.0 / d, c / d, ctx.stream));
+        CU(cudaStreamSynchronize(ctx.stream));
+        ctx.st_iters = 0; ctx.st_outer = 0; ctx.st_rr = ctx.st_rt = 0.0;
+        return LQCD_OK;
+    }
+    if ((rc = ensure_workspace(ctx.precision, 5))) return rc;
+    const int pr = ctx.precision;
+    if (!ctx.full_b[pr]) CU(cudaMalloc(&ctx.full_b[pr], spinor_bytes_of(pr, ctx.geo.G)));
+    // psi_even and psi_odd double as scratch until they receive their results
+    CU(launch_diag_scale(pr, n, eta_odd, psi_even, 1.0 / d, -c / d, 1.0 / d, c / d, ctx.stream));   // u_o = M_oo^-1 eta_o
+    if ((rc = hop_aux(gauge, psi_even, eta_even, psi_odd, 0, kappa, 0, kappa, 0, 1.0 / kappa, 0, 1.0 / kappa, 0, 1)))
+        return rc;                                                                                  // rhs_e = eta_e - D_eo u_o
+    if ((rc = apply_mhat(pr, ctx.recon, gauge, psi_odd, ctx.vec[pr][3], ctx.full_b[pr], kappa, mu, 1, false, nullptr)))
+        return rc;                                                                                  // b = Mhat^dag rhs_e
+    if ((rc = cg_setup_impl(pr, ctx.recon, gauge, ctx.full_b[pr], psi_even, kappa, mu, tol))) return rc;
+    if ((rc = cg_run_impl(maxit))) return rc;
+    const int status = cg_finish_impl(true);
+    if (status < 0) return status;
+    // psi_o = M_oo^{-1} (eta_o - D_oe psi_e) = [kappa (1 - i c chi)/(1 + c^2)] (bracket(psi_e) + eta_o / kappa)
+    if ((rc = hop_aux(gauge, psi_even, eta_odd, psi_odd, 1, kappa / d, -kappa * c / d, kappa / d, kappa * c / d,
+                      1.0 / kappa, 0, 1.0 / kappa, 0, 0))) return rc;
+    CU(cudaStreamSynchronize(ctx.stream));
+    return status;
 }
 
 int lqcd_cg_setup(const void* gauge, const void* b, void* x, double kappa, double mu, double tol) {

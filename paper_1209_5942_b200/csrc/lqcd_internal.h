@@ -81,6 +81,9 @@ cudaError_t launch_cg_update_xp(int precision, size_t n, void* x, void* p, const
                                 CgScalars* scal, cudaStream_t st);
 cudaError_t launch_true_resid(int precision, size_t n, const void* b, const void* ax, Reduction red,
                               CgScalars* scal, cudaStream_t st);
+// out = a_chi * in, a_chi = (ur, ui) on the upper and (dr, di) on the lower chirality
+cudaError_t launch_diag_scale(int precision, size_t n, const void* in, void* out, double ur, double ui,
+                              double dr, double di, cudaStream_t st);
 // mixed-precision solver helpers (double layout double2[12][Vh] <-> float layout float4[6][Vh])
 cudaError_t launch_convert_d2f(size_t n, const void* src_d, void* dst_f, double scale, cudaStream_t st);
 cudaError_t launch_axpy_f2d(size_t n, double a, const void* x_f, void* y_d, cudaStream_t st);  // y += a x

@@ -250,6 +250,30 @@ __global__ void __launch_bounds__(VBLOCK) residual_kernel(size_t nvec, const dou
     block_partial(s, red);
 }
 
+// out = a_chi * in per site, a_chi complex per chirality (upper: components 0..5, lower: 6..11):
+// the diagonal term (1 + i c gamma5) or its inverse on a whole half field.  One thread per
+// double2 / float4 element of the grouped layout (lqcd_internal.h).
+__global__ void __launch_bounds__(VBLOCK) diag_scale_kernel_d(size_t nvec, const double2* __restrict__ in,
+                                                              double2* __restrict__ out, double ur, double ui,
+                                                              double dr, double di) {
+    const size_t i = (size_t)blockIdx.x * VBLOCK + threadIdx.x;
+    if (i >= nvec) return;
+    const bool upper = ((i % 384) >> 5) < 6;
+    const double ar = upper ? ur : dr, ai = upper ? ui : di;
+    const double2 v = in[i];
+    out[i] = make_double2(ar * v.x - ai * v.y, ar * v.y + ai * v.x);
+}
+__global__ void __launch_bounds__(VBLOCK) diag_scale_kernel_f(size_t nvec, const float4* __restrict__ in,
+                                                              float4* __restrict__ out, float ur, float ui,
+                                                              float dr, float di) {
+    const size_t i = (size_t)blockIdx.x * VBLOCK + threadIdx.x;
+    if (i >= nvec) return;
+    const bool upper = ((i % 192) >> 5) < 3;
+    const float ar = upper ? ur : dr, ai = upper ? ui : di;
+    const float4 v = in[i];
+    out[i] = make_float4(ar * v.x - ai * v.y, ar * v.y + ai * v.x, ar * v.z - ai * v.w, ar * v.w + ai * v.z);
+}
+
 inline int grid_for(size_t nvec) { return (int)((nvec + VBLOCK * VUNROLL - 1) / (VBLOCK * VUNROLL)); }
 
 }  // namespace
@@ -261,6 +285,22 @@ cudaError_t launch_finalize(int fin, Reduction red, int n_partials, double tol, 
     count_launch();
     ProfScope prof(3, st);
     finalize_kernel<<<1, 1024, 0, st>>>(fin, red, n_partials, tol, scal);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_diag_scale(int precision, size_t n, const void* in, void* out, double ur, double ui,
+                              double dr, double di, cudaStream_t st) {
+    count_launch();
+    ProfScope prof(3, st);
+    if (precision == 0) {
+        const size_t nv = n / 2;
+        diag_scale_kernel_d<<<(int)((nv + VBLOCK - 1) / VBLOCK), VBLOCK, 0, st>>>(nv, (const double2*)in, (double2*)out,
+                                                                             ur, ui, dr, di);
+    } else {
+        const size_t nv = n / 4;
+        diag_scale_kernel_f<<<(int)((nv + VBLOCK - 1) / VBLOCK), VBLOCK, 0, st>>>(nv, (const float4*)in, (float4*)out,
+                                                                             (float)ur, (float)ui, (float)dr, (float)di);
+    }
     return cudaGetLastError();
 }
 

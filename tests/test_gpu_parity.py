@@ -411,3 +411,75 @@ def test_mixed_precision_cg_24c48(B, oracle_mod):
     assert st == 0 and rr <= tol and 20 <= iters <= 120
     r = b - oracle_mod.mdagm(dims, AP, U, x, kappa, mu)
     assert np.linalg.norm(r) / np.linalg.norm(b) <= 1.05 * tol
+
+
+# --------------------------------------------------------------------------- full-lattice operator and solve
+def _full_apply(B, L, dims, psi, kappa, mu):
+    ie, io = B.upload_spinor(lu.to_half(dims, psi, 0), 0), B.upload_spinor(lu.to_half(dims, psi, 1), 1)
+    oe, oo = B.alloc_spinor(), B.alloc_spinor()
+    B.lqcd_mtm_full(L.g, ie, io, oe, oo, kappa, mu)
+    return lu.from_halves(dims, B.download_spinor(oe, 0), B.download_spinor(oo, 1))
+
+
+@pytest.mark.parametrize("dims,phases", [((4, 4, 4, 4), AP), ((2, 2, 2, 2), GENERIC_PH),
+                                         ((4, 6, 2, 8), GENERIC_PH), ((8, 8, 8, 16), AP)])
+@pytest.mark.parametrize("precision,recon,tol", [(0, 18, TOL_D), (1, 12, TOL_S)])
+def test_mtm_full_matches_oracle_eq6(B, oracle_mod, dims, phases, precision, recon, tol):
+    kappa, mu = 0.15, 0.1
+    V = lu.volume(dims)
+    U = gen.gauge_haar(dims, SEED)
+    psi = gen.spinor_gaussian(V, SEED)
+    Ur, pr = _round_inputs(U, psi, precision)
+    L = Lat(B, dims, phases, U, precision, recon)
+    assert lu.rel_err(_full_apply(B, L, dims, psi, kappa, mu), oracle_mod.m_full(dims, phases, Ur, pr, kappa, mu)) <= tol
+    assert lu.rel_err(_full_apply(B, L, dims, psi, 0.0, 0.3), oracle_mod.m_full(dims, phases, Ur, pr, 0.0, 0.3)) <= tol
+
+
+def test_twisted_mass_identity_on_gpu(B):
+    # PAPER.md:82 in operator form: |M(mu) psi|^2 = |M(0) psi|^2 + 4 kappa^2 mu^2 |psi|^2
+    dims = (8, 8, 8, 16)
+    kappa, mu = 0.15, 0.1
+    U = gen.gauge_haar(dims, SEED)
+    psi = gen.spinor_gaussian(lu.volume(dims), SEED)
+    L = Lat(B, dims, AP, U)
+    n_mu = np.linalg.norm(_full_apply(B, L, dims, psi, kappa, mu)) ** 2
+    n_0 = np.linalg.norm(_full_apply(B, L, dims, psi, kappa, 0.0)) ** 2
+    want = n_0 + 4 * kappa ** 2 * mu ** 2 * np.linalg.norm(psi) ** 2
+    assert abs(n_mu - want) / want < 1e-13
+
+
+def _full_solve(B, L, dims, eta, kappa, mu, tol, maxit):
+    ee, eo_ = B.upload_spinor(lu.to_half(dims, eta, 0), 0), B.upload_spinor(lu.to_half(dims, eta, 1), 1)
+    pe, po = B.alloc_spinor(), B.alloc_spinor()
+    st = B.lqcd_solve_full(L.g, ee, eo_, pe, po, kappa, mu, tol, maxit)
+    return st, lu.from_halves(dims, B.download_spinor(pe, 0), B.download_spinor(po, 1))
+
+
+def test_solve_full_against_dense_solve(B):
+    dims = (2, 2, 2, 4)
+    kappa, mu = 0.15, 0.1
+    V = lu.volume(dims)
+    U = gen.gauge_haar(dims, SEED)
+    eta = gen.spinor_gaussian(V, SEED, gen.STREAM_SOURCE)
+    want = np.linalg.solve(lu.dense_m(dims, AP, U, kappa, mu), eta.ravel()).reshape(V, 4, 3)
+    L = Lat(B, dims, AP, U)
+    st, psi = _full_solve(B, L, dims, eta, kappa, mu, 1e-13, 500)
+    assert st == 0
+    assert lu.rel_err(psi, want) < 1e-11
+
+
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (8, 8, 8, 16)])
+def test_solve_full_residual_under_oracle_operator(B, oracle_mod, dims):
+    kappa, mu, tol = 0.15, 0.1, 1e-10
+    V = lu.volume(dims)
+    U = gen.gauge_haar(dims, SEED)
+    eta = gen.spinor_gaussian(V, SEED, gen.STREAM_SOURCE)
+    L = Lat(B, dims, AP, U)
+    st, psi = _full_solve(B, L, dims, eta, kappa, mu, tol, 2000)
+    iters, rr, rt = B.lqcd_cg_stats()
+    assert st == 0 and rr <= tol and iters > 0
+    r = eta - oracle_mod.m_full(dims, AP, U, psi, kappa, mu)
+    assert np.linalg.norm(r) / np.linalg.norm(eta) <= 10 * tol     # cond(Mhat) ~ 3-5 of slack
+    # kappa = 0: M is site diagonal, no iteration needed
+    st, psi = _full_solve(B, L, dims, eta, 0.0, 0.3, tol, 10)
+    assert st == 0 and lu.rel_err(oracle_mod.m_full(dims, AP, U, psi, 0.0, 0.3), eta) < 1e-14
