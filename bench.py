@@ -7,9 +7,9 @@ kappa = 0.15, mu = 0.1, antiperiodic in time; synthetic seeded inputs
 (lqcd_inputs, DESIGN.md "input recipe").
 
 One step = one CG iteration on Mhat^dag Mhat:
-four hopping launches with fused diagonal-term epilogues (one with the fused
-<p,Ap> partial sums) + the two fused vector kernels + two one-block finalisation
-kernels (8 launches).  K steps are run as solves of
+four hopping launches with fused diagonal-term epilogues (the second with the fused
+<p,Ap> partial sums, the fourth applying r -= alpha q in place with the |r|^2 partial
+sums) + the fused x/p vector kernel + two one-block finalisation kernels (7 launches).  K steps are run as solves of
 SOLVE_LEN iterations each (a real solve at this configuration takes about that
 many), the one-launch solve setup included in the timed region; the recursive
 residual would otherwise underflow after several hundred iterations.
@@ -17,7 +17,7 @@ residual would otherwise underflow after several hundred iterations.
 value   = hopping flops (4 x V/2 x 1320 per step; diagonal and vector-kernel
           flops NOT counted) / time, inputs resident in HBM.
 roofline= the hopping kernel: algorithmic bytes (1536 B/site, +192 B/site for the
-          two launches that also read `aux`) / CUDA-event duration of each launch,
+          launch that also reads `aux`, 1920 B/site for the fused-r launch) / CUDA-event duration of each launch,
           recorded live in the timed region by the library (lqcd_profile).
 e2e     = the same per-step work through lqcd_cg_mdagm_host with pinned HOST
           buffers: every step uploads gauge + source, runs one CG iteration (plus
@@ -40,6 +40,10 @@ if ROOT not in sys.path:
 FLOP_PER_SITE = 1320          # BASELINE.json metric; SURVEY.md section 8(a) row a5
 BYTES_PER_SITE = 1536         # double, 18-real links: 8 links x 144 + 192 in + 192 out (section 8(d))
 AUX_BYTES_PER_SITE = 192      # launches with the M_ee * aux epilogue read one more half spinor
+# the last hopping launch of an iteration (fused r -= alpha q, |r|^2): 8 links + in + aux + r read + r write
+FUSED_R_BYTES_PER_SITE = 8 * 144 + 4 * 192
+# whole CG iteration: 3 x (1536 [+192 aux on one]) + fused-r launch + cg_update_xp (x, p, r read; x, p written)
+STEP_BYTES_PER_SITE = 3 * BYTES_PER_SITE + AUX_BYTES_PER_SITE + FUSED_R_BYTES_PER_SITE + 5 * 192
 DIMS = (32, 32, 32, 64)
 REF_DIMS = (16, 16, 16, 32)   # bounded sample for the oracle legs (same recipe, 1/16 of the sites)
 REF_DIMS_SMALL = (8, 8, 8, 16)  # used by --impl reference when K + W > 100 steps are asked for
@@ -188,7 +192,7 @@ def run_reference(args, rank):
 
 def workload_config():
     return {"workload": "32^3x64 complex double, Haar SU(3) links, Gaussian source, kappa=0.15 mu=0.1, "
-                        "antiperiodic t; one step = one CG iteration on Mhat^dag Mhat (4 hopping + 2 vector + 2 one-block finalise launches)",
+                        "antiperiodic t; one step = one CG iteration on Mhat^dag Mhat (4 hopping launches, the last with the fused r-update, + 1 vector + 2 one-block finalise launches)",
             "lattice": list(DIMS), "precision": "double", "recon": 18, "kappa": KAPPA, "mu": MU,
             "solve_len": SOLVE_LEN,
             "l2": "inputs larger than L2 (gauge 1.21 GB + 6 half spinors of 201 MB per step vs 126 MB L2)"}
@@ -250,7 +254,7 @@ def run_ours(args, rank, world, local_rank):
     barrier()
     launches = B.lqcd_launch_count() - n0
     ms_total = e0.elapsed_time(e1)
-    prof = {c: B.lqcd_profile_read(c) for c in range(4)}
+    prof = {c: B.lqcd_profile_read(c) for c in range(6)}
     B.lqcd_profile(0)
     st = B.lqcd_cg_finish()
     iters, rr, rt = B.lqcd_cg_stats()
@@ -263,9 +267,10 @@ def run_ours(args, rank, world, local_rank):
     value = whole_job_gflops(world, args.steps, Vh, ms_max)
 
     # ---- roofline of the hopping kernel, from the per-launch events of the timed region -------
-    hop_ms = prof[0][0] + prof[1][0] + prof[2][0]
-    hop_n = prof[0][1] + prof[1][1] + prof[2][1]
-    hop_bytes = Vh * (BYTES_PER_SITE * hop_n + AUX_BYTES_PER_SITE * (prof[1][1] + prof[2][1]))
+    hop_ms = prof[0][0] + prof[1][0] + prof[2][0] + prof[5][0]
+    hop_n = prof[0][1] + prof[1][1] + prof[2][1] + prof[5][1]
+    hop_bytes = Vh * (BYTES_PER_SITE * (hop_n - prof[5][1]) + AUX_BYTES_PER_SITE * (prof[1][1] + prof[2][1])
+                      + FUSED_R_BYTES_PER_SITE * prof[5][1])
     peak, peak_src = measured_peak()
     achieved = hop_bytes / (hop_ms * 1e-3) / 1e9
     plain_gbs = Vh * BYTES_PER_SITE * prof[0][1] / (prof[0][0] * 1e-3) / 1e9 if prof[0][1] else None
@@ -286,9 +291,8 @@ def run_ours(args, rank, world, local_rank):
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(),
         "clocks": clk.summary(), "gpu_launches": int(launches), "roofline": roofline,
-        # whole-step algorithmic bytes: 4 hops + 2 aux reads + 8 field transfers of the vector kernels
-        "gbs_effective_step": world * args.steps * Vh * (4 * BYTES_PER_SITE + 2 * AUX_BYTES_PER_SITE + 8 * 192)
-        / (ms_max * 1e-3) / 1e9,
+        # whole-step algorithmic bytes (STEP_BYTES_PER_SITE above)
+        "gbs_effective_step": world * args.steps * Vh * STEP_BYTES_PER_SITE / (ms_max * 1e-3) / 1e9,
     }
 
     # ---- end to end through the host-buffer C-ABI call (pinned host memory) -----------------

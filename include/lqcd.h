@@ -164,7 +164,8 @@ long long lqcd_launch_count(void);
  * kernel the library launches on its stream (and discards earlier records); lqcd_profile(0)
  * stops.  lqcd_profile_read synchronises the stream and returns the summed duration and the
  * launch count of one category: 0 hopping (plain epilogue), 1 hopping + M_ee*aux epilogue,
- * 2 hopping + M_ee*aux epilogue + fused norm, 3 CG vector kernels, 4 pack/unpack. */
+ * 2 hopping + M_ee*aux epilogue + fused norm, 3 CG vector kernels, 4 pack/unpack,
+ * 5 hopping + M_ee*aux epilogue + fused CG residual update (r -= alpha q, |r|^2). */
 int lqcd_profile(int enable);
 int lqcd_profile_read(int category, double* total_ms, int* launches);
 

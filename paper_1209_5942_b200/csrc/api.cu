@@ -59,6 +59,7 @@ struct Context {
     int recon = 18;
     int block = 128;
     cudaStream_t stream = 0;
+    int snake = 1;                   // direction of the last field-sized launch (next_reverse)
 
     // workspace (owned), one set of half spinors per precision: r, p, q, t1, t2
     void* vec[2][5] = {{nullptr, nullptr, nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr, nullptr, nullptr}};
@@ -187,18 +188,25 @@ int check_scalar(double v, const char* name) {
     return LQCD_OK;
 }
 
+// Snake order (lqcd_internal.h): every field-sized launch of a chain traverses the sites in the
+// direction opposite to the launch before it.
+int next_reverse() { return ctx.snake ^= 1; }
+
 // The two hopping launches of Mhat (dagger = 0) or Mhat^dag (dagger = 1) on even half fields.
-// norm_to_pAp: also reduce |out|^2 into scal->pAp (CG's <p, A p> = |Mhat p|^2).
+// fuse = FUSE_PAP: also reduce |out|^2 into scal->pAp (CG's <p, A p> = |Mhat p|^2).
+// fuse = FUSE_R:   `out` is CG's residual r; instead of storing Mhat^(dag) in, the second launch
+//                  applies r -= alpha * (Mhat^(dag) in) in place and reduces |r|^2 (FIN_RHO).
 // scal: device scalars whose `done` flag turns the launches into no-ops (CG), or null.
+enum { FUSE_NONE = 0, FUSE_PAP = 1, FUSE_R = 2 };
 int apply_mhat(int precision, int recon, const void* gauge, const void* in, void* tmp_odd, void* out,
-               double kappa, double mu, int dagger, bool norm_to_pAp, CgScalars* scal) {
+               double kappa, double mu, int dagger, int fuse, CgScalars* scal) {
     const double c = (dagger ? -1.0 : 1.0) * 2.0 * kappa * mu;
     const double d = 1.0 + c * c;
     Epilogue e1 = {};
     e1.cu_re = -kappa / d; e1.cu_im = +kappa * c / d;   // -kappa (1 - i c)/(1 + c^2), chi = +1
     e1.cd_re = -kappa / d; e1.cd_im = -kappa * c / d;   // chi = -1
     CU(launch_hopping(precision, recon, dagger, 0, ctx.geo, e1, gauge, in, tmp_odd, nullptr, 1,
-                      0, red(), scal, ctx.block, ctx.stream));
+                      next_reverse(), red(), scal, ctx.block, ctx.stream));
     // out = (1 + i c chi) in + kappa * bracket(t) = k2 * (bracket(t) + [(1 + i c chi)/k2] in).
     // For kappa = 0 launch 1 wrote t = 0 exactly, so bracket(t) = 0 and any k2 != 0 is exact.
     const double k2 = (kappa != 0.0) ? kappa : 1.0;
@@ -206,23 +214,25 @@ int apply_mhat(int precision, int recon, const void* gauge, const void* in, void
     e2.cu_re = k2; e2.cd_re = k2;
     e2.du_re = 1.0 / k2; e2.du_im = c / k2;
     e2.dd_re = 1.0 / k2; e2.dd_im = -c / k2;
-    CU(launch_hopping(precision, recon, dagger, norm_to_pAp ? 2 : 1, ctx.geo, e2, gauge, tmp_odd,
-                      out, in, 0, 1, red(), scal, ctx.block, ctx.stream));
-    if (norm_to_pAp)
-        CU(launch_finalize(FIN_PAP, red(), hopping_partials(ctx.geo.Vh, ctx.block), 0.0, scal, ctx.stream));
+    const int mode = (fuse == FUSE_PAP) ? 2 : (fuse == FUSE_R) ? 3 : 1;
+    CU(launch_hopping(precision, recon, dagger, mode, ctx.geo, e2, gauge, tmp_odd,
+                      out, in, 0, next_reverse(), red(), scal, ctx.block, ctx.stream));
+    if (fuse != FUSE_NONE)
+        CU(launch_finalize(fuse == FUSE_PAP ? FIN_PAP : FIN_RHO, red(), hopping_partials(ctx.geo.Vh, ctx.block),
+                           0.0, scal, ctx.stream));
     return LQCD_OK;
 }
 
 int enqueue_iteration() {
     void** v = ctx.vec[ctx.cg_prec];
-    void *r = v[0], *p = v[1], *q = v[2], *t1 = v[3], *t2 = v[4];
+    void *r = v[0], *p = v[1], *t1 = v[3], *t2 = v[4];
     const size_t n = n_reals();
-    int rc = apply_mhat(ctx.cg_prec, ctx.cg_recon, ctx.cg_gauge, p, t1, t2, ctx.cg_kappa, ctx.cg_mu, 0, true, ctx.scal);
+    int rc = apply_mhat(ctx.cg_prec, ctx.cg_recon, ctx.cg_gauge, p, t1, t2, ctx.cg_kappa, ctx.cg_mu, 0, FUSE_PAP, ctx.scal);
     if (rc) return rc;
-    rc = apply_mhat(ctx.cg_prec, ctx.cg_recon, ctx.cg_gauge, t2, t1, q, ctx.cg_kappa, ctx.cg_mu, 1, false, ctx.scal);
+    // q = Mhat^dag t2 is never stored: the last hopping launch updates r in place (hopping.cu MODE 3)
+    rc = apply_mhat(ctx.cg_prec, ctx.cg_recon, ctx.cg_gauge, t2, t1, r, ctx.cg_kappa, ctx.cg_mu, 1, FUSE_R, ctx.scal);
     if (rc) return rc;
-    CU(launch_cg_update_r(ctx.cg_prec, n, r, q, 0, red(), ctx.scal, ctx.stream));
-    CU(launch_cg_update_xp(ctx.cg_prec, n, ctx.cg_x, p, r, 1, ctx.scal, ctx.stream));
+    CU(launch_cg_update_xp(ctx.cg_prec, n, ctx.cg_x, p, r, next_reverse(), ctx.scal, ctx.stream));
     return LQCD_OK;
 }
 
@@ -273,9 +283,9 @@ int cg_finish_impl(bool true_resid) {
     void** v = ctx.vec[ctx.cg_prec];
     if (true_resid) {
         void *q = v[2], *t1 = v[3], *t2 = v[4];
-        int rc = apply_mhat(ctx.cg_prec, ctx.cg_recon, ctx.cg_gauge, ctx.cg_x, t1, t2, ctx.cg_kappa, ctx.cg_mu, 0, false, nullptr);
+        int rc = apply_mhat(ctx.cg_prec, ctx.cg_recon, ctx.cg_gauge, ctx.cg_x, t1, t2, ctx.cg_kappa, ctx.cg_mu, 0, FUSE_NONE, nullptr);
         if (rc) return rc;
-        rc = apply_mhat(ctx.cg_prec, ctx.cg_recon, ctx.cg_gauge, t2, t1, q, ctx.cg_kappa, ctx.cg_mu, 1, false, nullptr);
+        rc = apply_mhat(ctx.cg_prec, ctx.cg_recon, ctx.cg_gauge, t2, t1, q, ctx.cg_kappa, ctx.cg_mu, 1, FUSE_NONE, nullptr);
         if (rc) return rc;
         CU(launch_true_resid(ctx.cg_prec, n_reals(), ctx.cg_b, q, red(), ctx.scal, ctx.stream));
     }
@@ -432,7 +442,7 @@ int lqcd_mtm(const void* gauge, const void* in, void* out, double kappa, double 
     rc = ensure_workspace(ctx.precision, 1);
     if (rc) return rc;
     return apply_mhat(ctx.precision, ctx.recon, gauge, in, ctx.vec[ctx.precision][3], out, kappa, mu, dagger,
-                      false, nullptr);
+                      FUSE_NONE, nullptr);
 }
 
 // One hopping launch with the M_diag * aux epilogue: out_p = a_chi * (bracket(in) + d_chi aux).
@@ -499,7 +509,7 @@ int lqcd_solve_full(const void* gauge, const void* eta_even, const void* eta_odd
     CU(launch_diag_scale(pr, n, eta_odd, psi_even, 1.0 / d, -c / d, 1.0 / d, c / d, ctx.stream));   // u_o = M_oo^-1 eta_o
     if ((rc = hop_aux(gauge, psi_even, eta_even, psi_odd, 0, kappa, 0, kappa, 0, 1.0 / kappa, 0, 1.0 / kappa, 0, 1)))
         return rc;                                                                                  // rhs_e = eta_e - D_eo u_o
-    if ((rc = apply_mhat(pr, ctx.recon, gauge, psi_odd, ctx.vec[pr][3], ctx.full_b[pr], kappa, mu, 1, false, nullptr)))
+    if ((rc = apply_mhat(pr, ctx.recon, gauge, psi_odd, ctx.vec[pr][3], ctx.full_b[pr], kappa, mu, 1, FUSE_NONE, nullptr)))
         return rc;                                                                                  // b = Mhat^dag rhs_e
     if ((rc = cg_setup_impl(pr, ctx.recon, gauge, ctx.full_b[pr], psi_even, kappa, mu, tol))) return rc;
     if ((rc = cg_run_impl(maxit))) return rc;
@@ -610,8 +620,8 @@ int lqcd_cg_mdagm_mixed(const void* gauge_double, int recon_double, const void* 
         ++outer;
         CU(launch_axpy_f2d(n, scale, ctx.mx_x, x, ctx.stream));
         // r = b - A x in double
-        if ((rc = apply_mhat(LQCD_DOUBLE, recon_double, gauge_double, x, t1, t2, kappa, mu, 0, false, nullptr))) return rc;
-        if ((rc = apply_mhat(LQCD_DOUBLE, recon_double, gauge_double, t2, t1, q, kappa, mu, 1, false, nullptr))) return rc;
+        if ((rc = apply_mhat(LQCD_DOUBLE, recon_double, gauge_double, x, t1, t2, kappa, mu, 0, FUSE_NONE, nullptr))) return rc;
+        if ((rc = apply_mhat(LQCD_DOUBLE, recon_double, gauge_double, t2, t1, q, kappa, mu, 1, FUSE_NONE, nullptr))) return rc;
         CU(launch_residual(n, b, q, r, red(), so, ctx.stream));
         if (ctx.st_iters == 0) { status = LQCD_BREAKDOWN; break; }      // inner solver made no progress
     }

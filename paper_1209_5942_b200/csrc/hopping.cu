@@ -14,6 +14,9 @@
 //   a5 boundary phase on the hop that wraps, reconstruction to 4 spin rows, accumulate
 //   a6/a7 epilogue: out = c_chi * (acc + d_chi * aux), c, d complex per chirality:
 //      covers -kappa (dslash_eo), M_oo^{-1} D_oe, and M_ee in - D_eo (.) in one store.
+//   a9 (MODE 3) the last hopping launch of a CG iteration never stores q = A p: it
+//      applies r -= alpha q in place and reduces |r|^2 (alpha = rho / pAp read from the
+//      device scalars), which saves one field store, one field load and a launch.
 //
 // Spin projection table (gamma basis of include/lqcd.h; reading G4),
 // (1 + S gamma_mu) psi = (h0, h1, conj(c0) h0 or h1 ...):
@@ -285,6 +288,16 @@ hopping_kernel(const HopArgs a) {
     const int blk = a.reverse ? (int)(gridDim.x - 1 - blockIdx.x) : (int)blockIdx.x;
     const int e = blk * blockDim.x + threadIdx.x;
     double nrm = 0.0;
+    double alpha = 1.0;
+    if (MODE == 3) {  // alpha = rho / <p, A p>; breakdown leaves r untouched and is flagged for FIN_RHO
+        const double rho = a.scal->rho, pAp = a.scal->pAp;
+        if (!(pAp > 0.0) || !isfinite(pAp) || !isfinite(rho)) {
+            if (blockIdx.x == 0 && threadIdx.x == 0) a.scal->status = -5;
+            return;
+        }
+        alpha = rho / pAp;
+        if (blockIdx.x == 0 && threadIdx.x == 0) a.scal->alpha = alpha;  // for cg_update_xp
+    }
     if (e < Vh) {
         // a1: e -> (x0h, x1, x2, x3); r = x0 mod 2 follows from the parity
         const int N0h = a.g.N0h, N1 = a.g.N1, N2 = a.g.N2, N3 = a.g.N3;
@@ -309,6 +322,21 @@ hopping_kernel(const HopArgs a) {
                 const T dr = (c < 6) ? dur : ddr, di = (c < 6) ? dui : ddi;
                 acc[2 * c] = fma_(-di, x[2 * c + 1], dr * x[2 * c]);
                 acc[2 * c + 1] = fma_(di, x[2 * c], dr * x[2 * c + 1]);
+            }
+            if (MODE == 3) {
+                // r - alpha c (bracket + d aux) = (-alpha c) (bracket + d aux - r / (alpha c)):
+                // the old residual joins the accumulator's initial value with s = -1 / (alpha c)
+                load_spinor(a.out, e, x);
+                const double nu = -alpha * (a.ep.cu_re * a.ep.cu_re + a.ep.cu_im * a.ep.cu_im);
+                const double nd = -alpha * (a.ep.cd_re * a.ep.cd_re + a.ep.cd_im * a.ep.cd_im);
+                const T sur = (T)(a.ep.cu_re / nu), sui = (T)(-a.ep.cu_im / nu);
+                const T sdr = (T)(a.ep.cd_re / nd), sdi = (T)(-a.ep.cd_im / nd);
+#pragma unroll
+                for (int c = 0; c < 12; ++c) {
+                    const T sr = (c < 6) ? sur : sdr, si = (c < 6) ? sui : sdi;
+                    acc[2 * c] = fma_(-si, x[2 * c + 1], fma_(sr, x[2 * c], acc[2 * c]));
+                    acc[2 * c + 1] = fma_(si, x[2 * c], fma_(sr, x[2 * c + 1], acc[2 * c + 1]));
+                }
             }
         } else {
 #pragma unroll
@@ -339,7 +367,9 @@ hopping_kernel(const HopArgs a) {
 
         // a6/a7: epilogue, complex coefficient per chirality
         T o[24];
-        const T cur = (T)a.ep.cu_re, cui = (T)a.ep.cu_im, cdr = (T)a.ep.cd_re, cdi = (T)a.ep.cd_im;
+        const double esc = (MODE == 3) ? -alpha : 1.0;
+        const T cur = (T)(esc * a.ep.cu_re), cui = (T)(esc * a.ep.cu_im);
+        const T cdr = (T)(esc * a.ep.cd_re), cdi = (T)(esc * a.ep.cd_im);
 #pragma unroll
         for (int c = 0; c < 12; ++c) {
             const T cr = (c < 6) ? cur : cdr, ci = (c < 6) ? cui : cdi;
@@ -347,15 +377,15 @@ hopping_kernel(const HopArgs a) {
             o[2 * c + 1] = fma_(ci, acc[2 * c], cr * acc[2 * c + 1]);
         }
         store_spinor(a.out, e, o);
-        if (MODE == 2) {  // |out|^2 = |c_u|^2 |acc_upper|^2 + |c_d|^2 |acc_lower|^2
+        if (MODE >= 2) {  // |out|^2 = |c_u|^2 |acc_upper|^2 + |c_d|^2 |acc_lower|^2
             double nu = 0.0, nd = 0.0;
 #pragma unroll
             for (int i = 0; i < 12; ++i) {
                 nu += (double)acc[i] * (double)acc[i];
                 nd += (double)acc[12 + i] * (double)acc[12 + i];
             }
-            nrm = (a.ep.cu_re * a.ep.cu_re + a.ep.cu_im * a.ep.cu_im) * nu +
-                  (a.ep.cd_re * a.ep.cd_re + a.ep.cd_im * a.ep.cd_im) * nd;
+            nrm = (esc * esc) * ((a.ep.cu_re * a.ep.cu_re + a.ep.cu_im * a.ep.cu_im) * nu +
+                                 (a.ep.cd_re * a.ep.cd_re + a.ep.cd_im * a.ep.cd_im) * nd);
         }
     }
     if (e >= Vh && e < a.g.G * 32) {  // pad sites of the last group hold zeros
@@ -364,7 +394,7 @@ hopping_kernel(const HopArgs a) {
         for (int i = 0; i < 24; ++i) z[i] = 0;
         store_spinor(a.out, e, z);
     }
-    if (MODE == 2) {  // one partial per warp, plain store; summed by launch_finalize(FIN_PAP)
+    if (MODE >= 2) {  // one partial per warp, plain store; summed by launch_finalize(FIN_PAP / FIN_RHO)
         nrm = warp_sum(nrm);
         if ((threadIdx.x & 31) == 0) a.red.partials[(blk * blockDim.x + threadIdx.x) >> 5] = nrm;
     }
@@ -379,7 +409,7 @@ cudaError_t launch_tr(int dagger, int mode, const HopArgs& a, int block, cudaStr
         return cudaGetLastError();                                                 \
     }
     LQCD_HOP_CASE(0, 0) LQCD_HOP_CASE(0, 1) LQCD_HOP_CASE(0, 2)
-    LQCD_HOP_CASE(1, 0) LQCD_HOP_CASE(1, 1) LQCD_HOP_CASE(1, 2)
+    LQCD_HOP_CASE(1, 0) LQCD_HOP_CASE(1, 1) LQCD_HOP_CASE(1, 2) LQCD_HOP_CASE(1, 3)
 #undef LQCD_HOP_CASE
     return cudaErrorInvalidValue;
 }
@@ -401,7 +431,7 @@ cudaError_t launch_hopping(int precision, int recon, int dagger, int mode, const
     a.g = g; a.ep = ep; a.out_parity = out_parity; a.red = red; a.scal = scal;
     if (block <= 0 || block > 128 || (block % 32) != 0) block = 128;
     count_launch();
-    ProfScope prof(mode, st);
+    ProfScope prof(mode == 3 ? 5 : mode, st);
     if (precision == 0) {
         return recon == 12 ? launch_tr<double, 12>(dagger, mode, a, block, st)
                            : launch_tr<double, 18>(dagger, mode, a, block, st);

@@ -45,7 +45,7 @@ struct CgScalars {
     double rho;        // |r|^2
     double pAp;        // <p, A p> = |Mhat p|^2
     double beta;
-    double alpha;      // rho / pAp of the current iteration (written by cg_update_r)
+    double alpha;      // rho / pAp of the current iteration (written by the fused r-update, hopping MODE 3)
     double bb;         // |b|^2
     double tol2bb;     // tol^2 |b|^2
     double resid_true; // |b - A x|^2
@@ -66,7 +66,8 @@ enum { FIN_NONE = 0, FIN_PAP = 1, FIN_BB = 2, FIN_RHO = 3, FIN_TRUE = 4 };
 // part of its output a kernel wrote last is still in L2 when the next kernel starts; starting
 // the next kernel at that end turns part of its compulsory DRAM reads into L2 hits.
 // hopping.cu
-// mode 0: out = c * bracket;  mode 1: out = c * (bracket + d * aux);  mode 2: mode 1 + |out|^2 -> scal->pAp
+// mode 0: out = c * bracket;  mode 1: out = c * (bracket + d * aux);  mode 2: mode 1 + |out|^2 partials;
+// mode 3 (dagger = 1 only): out -= alpha * c * (bracket + d * aux) in place, alpha = scal->rho / scal->pAp, + |out|^2 partials
 cudaError_t launch_hopping(int precision, int recon, int dagger, int mode, const Geometry& g,
                            const Epilogue& ep, const void* gauge, const void* in, void* out,
                            const void* aux, int out_parity, int reverse, Reduction red,
@@ -75,8 +76,6 @@ cudaError_t launch_hopping(int precision, int recon, int dagger, int mode, const
 // vector_ops.cu  (n = number of reals in a half-spinor field incl. padding = 24 * 32 * G)
 cudaError_t launch_cg_init(int precision, size_t n, const void* b, void* x, void* r, void* p,
                            double tol, Reduction red, CgScalars* scal, cudaStream_t st);
-cudaError_t launch_cg_update_r(int precision, size_t n, void* r, const void* q, int reverse,
-                               Reduction red, CgScalars* scal, cudaStream_t st);
 cudaError_t launch_cg_update_xp(int precision, size_t n, void* x, void* p, const void* r, int reverse,
                                 CgScalars* scal, cudaStream_t st);
 cudaError_t launch_true_resid(int precision, size_t n, const void* b, const void* ax, Reduction red,

@@ -5,11 +5,13 @@
 // order so that alpha, beta and the convergence decision never leave the device.
 //
 //   cg_init      x = 0, r = p = b; finalize(FIN_BB): rho = bb = |b|^2
-//   cg_update_r  alpha = rho / pAp; r -= alpha q; partial |r|^2            (3 fields of traffic)
+//   (r -= alpha q and |r|^2 live in the epilogue of the iteration's last hopping launch,
+//    hopping.cu MODE 3: q is never stored)
 //                finalize(FIN_RHO): iters++, done = (rho' <= tol^2 bb), beta = rho'/rho, rho = rho'
 //   cg_update_xp x += alpha p; p = r + beta p (p only while not converged)  (5 fields of traffic)
 //   true_resid   |b - Ax|^2; finalize(FIN_TRUE)
-// i.e. 8 field transfers per iteration instead of the 9 of (x,r | p) or the 12 of unfused BLAS-1.
+// i.e. 5 + 2 (r read/written by the hopping launch) field transfers per iteration instead of
+// the 12 of unfused BLAS-1.
 // Reductions accumulate in double whatever the field precision.
 #include "lqcd_internal.h"
 
@@ -87,7 +89,7 @@ __global__ void __launch_bounds__(1024) finalize_kernel(int fin, Reduction red, 
         scal->status = (s == 0.0) ? 0 : 1;
         scal->upd = 0;
     } else if (fin == FIN_RHO) {
-        if (scal->status == -5) {  // breakdown flagged by cg_update_r: r untouched, freeze the solve
+        if (scal->status == -5) {  // breakdown flagged by the fused r-update: r untouched, freeze the solve
             scal->done = 1;
             scal->upd = 0;
             return;
@@ -125,41 +127,6 @@ __global__ void __launch_bounds__(VBLOCK) cg_init_kernel(size_t nvec, const void
             r[i] = v;
             p[i] = v;
             s += norm2(v);
-        }
-    }
-    block_partial(s, red);
-}
-
-template <typename T>
-__global__ void __launch_bounds__(VBLOCK) cg_update_r_kernel(size_t nvec, void* r_, const void* q_,
-                                                             int reverse, Reduction red, CgScalars* scal) {
-    typedef typename VecOf<T>::type V;
-    if (scal->done) return;
-    const double rho = scal->rho, pAp = scal->pAp;
-    if (!(pAp > 0.0) || !isfinite(pAp) || !isfinite(rho)) {  // breakdown: leave r untouched
-        if (blockIdx.x == 0 && threadIdx.x == 0) scal->status = -5;
-        return;
-    }
-    const double alpha = rho / pAp;
-    if (blockIdx.x == 0 && threadIdx.x == 0) scal->alpha = alpha;  // for cg_update_xp
-    V* r = (V*)r_;
-    const V* q = (const V*)q_;
-    const size_t blk = reverse ? (gridDim.x - 1 - blockIdx.x) : blockIdx.x;
-    const size_t base = blk * (VBLOCK * VUNROLL) + threadIdx.x;
-    V rv[VUNROLL], qv[VUNROLL];
-#pragma unroll
-    for (int k = 0; k < VUNROLL; ++k) {
-        const size_t i = base + (size_t)k * VBLOCK;
-        if (i < nvec) { rv[k] = r[i]; qv[k] = __ldcs(q + i); }
-    }
-    double s = 0.0;
-#pragma unroll
-    for (int k = 0; k < VUNROLL; ++k) {
-        const size_t i = base + (size_t)k * VBLOCK;
-        if (i < nvec) {
-            const V rn = axpy(-alpha, qv[k], rv[k]);
-            r[i] = rn;
-            s += norm2(rn);
         }
     }
     block_partial(s, red);
@@ -344,22 +311,6 @@ cudaError_t launch_cg_init(int precision, size_t n, const void* b, void* x, void
         const size_t nv = n / 4;
         cg_init_kernel<float><<<grid_for(nv), VBLOCK, 0, st>>>(nv, b, x, r, p, red);
         finalize_kernel<<<1, 1024, 0, st>>>(FIN_BB, red, grid_for(nv), tol, scal);
-    }
-    return cudaGetLastError();
-}
-
-cudaError_t launch_cg_update_r(int precision, size_t n, void* r, const void* q, int reverse,
-                               Reduction red, CgScalars* scal, cudaStream_t st) {
-    count_launch(2);
-    ProfScope prof(3, st);
-    if (precision == 0) {
-        const size_t nv = n / 2;
-        cg_update_r_kernel<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, r, q, reverse, red, scal);
-        finalize_kernel<<<1, 1024, 0, st>>>(FIN_RHO, red, grid_for(nv), 0.0, scal);
-    } else {
-        const size_t nv = n / 4;
-        cg_update_r_kernel<float><<<grid_for(nv), VBLOCK, 0, st>>>(nv, r, q, reverse, red, scal);
-        finalize_kernel<<<1, 1024, 0, st>>>(FIN_RHO, red, grid_for(nv), 0.0, scal);
     }
     return cudaGetLastError();
 }
