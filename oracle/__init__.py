@@ -18,5 +18,6 @@ from .oracle import (  # noqa: F401
     mhat_sites,
     mdagm,
     cg_mdagm,
+    bicgstab_mhat,
     num_threads,
 )

@@ -22,7 +22,8 @@
 // entry-by-entry comparison with a dense 2^4 build written independently in
 // numpy (P4), the paper's own identity M(mu)^dag M(mu) = M(0)^dag M(0) +
 // 4 kappa^2 mu^2 (P5), Schur identity vs the dense matrix (P6),
-// trivial limits (P7), CG vs a dense Hermitian solve (P8).  The paper prints
+// trivial limits (P7), CG vs a dense Hermitian solve (P8), BiCGStab vs a dense solve
+// of Mhat and the textbook recurrence on the dense matrix (P9).  The paper prints
 // no numeric example for any of these operators, so element values rest on
 // P1-P8.
 //
@@ -406,6 +407,73 @@ int orc_cg_mdagm(const int* dims, const double* bc_phase, const double* U_, cons
         apply_A(L, U, x, q.data(), tmp.data(), kappa, mu);
         for (long i = 0; i < n; ++i) q[i] = b[i] - q[i];
         *rel_resid_true = bb > 0 ? (double)sqrtl(norm2(q.data(), n) / bb) : 0.0;
+    }
+    return status;
+}
+
+// BiCGStab (van der Vorst, SIAM J. Sci. Stat. Comput. 13 (1992) 631) on Mhat x = b, even half
+// fields, x0 = 0 -- the second solver the paper names ("The most common solvers used are CG and
+// BiCGStab").  The paper gives no formulae; reading G15 of DESIGN.md: the
+// textbook recurrence with shadow residual rhat = r0 = b and p0 = r0, complex inner product
+// <a,b> = sum conj(a_i) b_i, one iteration = two applications of Mhat:
+//   rho = <rhat, r>;  loop: v = Mhat p; sigma = <rhat, v>; alpha = rho / sigma; s = r - alpha v;
+//   t = Mhat s; omega = <t,s>/<t,t> (0 if t = 0); x += alpha p + omega s; r = s - omega t;
+//   stop if |r| <= tol |b|; rho' = <rhat, r>; beta = (rho'/rho)(alpha/omega);
+//   p = r + beta (p - omega v); rho = rho'.
+// Returns 0 converged, 1 not converged after maxit iterations (x = last iterate), -5 breakdown
+// (sigma, rho' or omega zero or not finite).
+int orc_bicgstab_mhat(const int* dims, const double* bc_phase, const double* U_, const double* b_,
+                      double* x_, double kappa, double mu, double tol, int maxit, int* iters,
+                      double* rel_resid_recursive, double* rel_resid_true) {
+    Lattice L = make_lattice(dims, bc_phase);
+    const cplx* U = (const cplx*)U_;
+    const cplx* b = (const cplx*)b_;
+    cplx* x = (cplx*)x_;
+    const long n = 12 * (L.V / 2);
+    typedef std::complex<long double> lcplx;
+    auto cdot = [n](const cplx* a, const cplx* c) {  // <a, c> = sum conj(a_i) c_i
+        lcplx s(0.0L, 0.0L);
+        for (long i = 0; i < n; ++i) s += std::conj(lcplx(a[i])) * lcplx(c[i]);
+        return s;
+    };
+    auto bad = [](cplx z) { return z == O_ || !std::isfinite(z.real()) || !std::isfinite(z.imag()); };
+    std::vector<cplx> r(b, b + n), p(b, b + n), v(n), s(n), t(n);
+    const cplx* rhat = b;
+    for (long i = 0; i < n; ++i) x[i] = O_;
+    const long double bb = norm2(b, n);
+    long double rr = bb;
+    int it = 0, status = 1;
+    if (bb == 0.0L) {
+        status = 0;
+    } else {
+        cplx rho = (cplx)cdot(rhat, r.data());
+        while (it < maxit) {
+            mhat(L, U, p.data(), v.data(), kappa, mu, 0);
+            const cplx sigma = (cplx)cdot(rhat, v.data());
+            if (bad(sigma)) { status = -5; break; }
+            const cplx alpha = rho / sigma;
+            for (long i = 0; i < n; ++i) s[i] = r[i] - alpha * v[i];
+            mhat(L, U, s.data(), t.data(), kappa, mu, 0);
+            const long double tt = norm2(t.data(), n);
+            const cplx omega = tt > 0.0L ? (cplx)(cdot(t.data(), s.data()) / tt) : O_;
+            for (long i = 0; i < n; ++i) x[i] += alpha * p[i] + omega * s[i];
+            for (long i = 0; i < n; ++i) r[i] = s[i] - omega * t[i];
+            rr = norm2(r.data(), n);
+            ++it;
+            if (rr <= (long double)tol * tol * bb) { status = 0; break; }
+            const cplx rho1 = (cplx)cdot(rhat, r.data());
+            if (bad(rho1) || bad(omega)) { status = -5; break; }
+            const cplx beta = (rho1 / rho) * (alpha / omega);
+            for (long i = 0; i < n; ++i) p[i] = r[i] + beta * (p[i] - omega * v[i]);
+            rho = rho1;
+        }
+    }
+    if (iters) *iters = it;
+    if (rel_resid_recursive) *rel_resid_recursive = bb > 0 ? (double)sqrtl(rr / bb) : 0.0;
+    if (rel_resid_true) {
+        mhat(L, U, x, t.data(), kappa, mu, 0);
+        for (long i = 0; i < n; ++i) t[i] = b[i] - t[i];
+        *rel_resid_true = bb > 0 ? (double)sqrtl(norm2(t.data(), n) / bb) : 0.0;
     }
     return status;
 }

@@ -36,6 +36,7 @@ def _load():
         build()
         _lib = ctypes.CDLL(_LIB)
         _lib.orc_cg_mdagm.restype = ctypes.c_int
+        _lib.orc_bicgstab_mhat.restype = ctypes.c_int
         _lib.orc_num_threads.restype = ctypes.c_int
     return _lib
 
@@ -157,6 +158,22 @@ def cg_mdagm(dims, bc_phase, U, b, kappa, mu, tol, maxit):
     st = _load().orc_cg_mdagm(_ip(d), _dp(ph), _dp(U), _dp(b), _dp(x), ctypes.c_double(kappa),
                               ctypes.c_double(mu), ctypes.c_double(tol), ctypes.c_int(maxit),
                               ctypes.byref(it), ctypes.byref(rr), ctypes.byref(rt))
+    return st, x, it.value, rr.value, rt.value
+
+
+def bicgstab_mhat(dims, bc_phase, U, b, kappa, mu, tol, maxit):
+    """Returns (status, x, iters, rel_resid_recursive, rel_resid_true)."""
+    d, ph = _dims(dims), _phases(bc_phase)
+    V = int(np.prod(d))
+    U = _c128(U, (V, 4, 3, 3))
+    b = _c128(b, (V // 2, 4, 3))
+    x = np.empty_like(b)
+    it = ctypes.c_int(0)
+    rr = ctypes.c_double(0.0)
+    rt = ctypes.c_double(0.0)
+    st = _load().orc_bicgstab_mhat(_ip(d), _dp(ph), _dp(U), _dp(b), _dp(x), ctypes.c_double(kappa),
+                                   ctypes.c_double(mu), ctypes.c_double(tol), ctypes.c_int(maxit),
+                                   ctypes.byref(it), ctypes.byref(rr), ctypes.byref(rt))
     return st, x, it.value, rr.value, rt.value
 
 

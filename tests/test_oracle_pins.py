@@ -321,3 +321,74 @@ def test_p8_cg_expected_iteration_counts(oracle_mod):
     assert st == 0 and 20 <= iters <= 60
     assert rt < 1.05e-10 * 1.5
     assert lu.rel_err(oracle_mod.mdagm(dims, AP, U, x, 0.15, 0.1), b) < 2e-10
+
+
+# --------------------------------------------------------------------------- P9 BiCGStab
+def test_p9_bicgstab_against_dense_solve(oracle_mod):
+    dims = (2, 2, 2, 4)
+    kappa, mu = 0.15, 0.1
+    U = gen.gauge_haar(dims, SEED)
+    b = gen.spinor_gaussian(lu.volume(dims) // 2, SEED, gen.STREAM_SOURCE)
+    S = lu.dense_mhat(dims, AP, U, kappa, mu)
+    want = np.linalg.solve(S, b.ravel()).reshape(b.shape)
+    st, x, iters, rr, rt = oracle_mod.bicgstab_mhat(dims, AP, U, b, kappa, mu, 1e-12, 500)
+    assert st == 0 and 0 < iters < 200
+    assert rr <= 1e-12 and rt < 5e-12
+    assert lu.rel_err(x, want) < 1e-10
+    # the true residual is the one of Mhat itself (not of the normal equations)
+    assert abs(rt - np.linalg.norm(b.ravel() - S @ x.ravel()) / np.linalg.norm(b)) < 1e-13
+
+
+def test_p9_bicgstab_iterates_follow_textbook_recurrence(oracle_mod):
+    # k steps of the oracle == k steps of van der Vorst's algorithm in its original form
+    # (rho_0 = alpha = omega_0 = 1, v_0 = p_0 = 0) written out in numpy on the dense matrix
+    dims = (2, 2, 2, 2)
+    kappa, mu = 0.15, 0.1
+    U = gen.gauge_haar(dims, SEED)
+    b = gen.spinor_gaussian(lu.volume(dims) // 2, SEED, gen.STREAM_SOURCE)
+    S = lu.dense_mhat(dims, AP, U, kappa, mu)
+    bv = b.ravel()
+    x = np.zeros(bv.size, dtype=complex)
+    r = bv.copy()
+    rhat = bv.copy()
+    rho = alpha = omega = 1.0 + 0j
+    v = np.zeros_like(x)
+    p = np.zeros_like(x)
+    for k in range(1, 7):
+        rho1 = np.vdot(rhat, r)
+        beta = (rho1 / rho) * (alpha / omega)
+        p = r + beta * (p - omega * v)
+        v = S @ p
+        alpha = rho1 / np.vdot(rhat, v)
+        s = r - alpha * v
+        t = S @ s
+        omega = np.vdot(t, s) / np.vdot(t, t)
+        x = x + alpha * p + omega * s
+        r = s - omega * t
+        rho = rho1
+        st, xo, iters, rr, rt = oracle_mod.bicgstab_mhat(dims, AP, U, b, kappa, mu, 0.0, k)
+        assert st == 1 and iters == k
+        assert lu.rel_err(xo.ravel(), x) < 1e-11
+        assert abs(rr - np.linalg.norm(r) / np.linalg.norm(bv)) < 1e-11 * max(rr, 1e-3)
+        # the recursive residual is the true one up to rounding at this size
+        assert abs(rt - np.linalg.norm(bv - S @ x) / np.linalg.norm(bv)) < 1e-12
+
+
+def test_p9_bicgstab_edge_cases_and_cost(oracle_mod):
+    dims = (4, 4, 4, 4)
+    U = gen.gauge_haar(dims, SEED)
+    n = lu.volume(dims) // 2
+    b = gen.spinor_gaussian(n, SEED, gen.STREAM_SOURCE)
+    st, x, iters, rr, rt = oracle_mod.bicgstab_mhat(dims, AP, U, np.zeros_like(b), 0.15, 0.1, 1e-10, 50)
+    assert st == 0 and iters == 0 and np.all(x == 0)
+    st, x, iters, rr, rt = oracle_mod.bicgstab_mhat(dims, AP, U, b, 0.15, 0.1, 1e-10, 3)
+    assert st == 1 and iters == 3 and rr > 1e-10
+    # kappa = 0: Mhat = 1 + 2 i kappa mu gamma5 = 1 -> one iteration
+    st, x, iters, rr, rt = oracle_mod.bicgstab_mhat(dims, AP, U, b, 0.0, 0.1, 1e-12, 50)
+    assert st == 0 and iters == 1 and lu.rel_err(x, b) < 1e-14
+    # two Mhat applications per iteration vs CG's two on the normal equations: BiCGStab needs
+    # fewer iterations than CG for the same reduction of its own residual (PAPER.md:94 names both)
+    st, x, it_b, rr, rt = oracle_mod.bicgstab_mhat(dims, AP, U, b, 0.15, 0.1, 1e-10, 2000)
+    st_c, xc, it_c, rr_c, rt_c = oracle_mod.cg_mdagm(dims, AP, U, b, 0.15, 0.1, 1e-10, 2000)
+    assert st == 0 and st_c == 0 and it_b < it_c
+    assert lu.rel_err(oracle_mod.mhat(dims, AP, U, x, 0.15, 0.1, 0), b) < 2e-10
