@@ -214,6 +214,7 @@ int apply_mhat(int precision, int recon, const void* gauge, const void* in, void
     e2.cu_re = k2; e2.cd_re = k2;
     e2.du_re = 1.0 / k2; e2.du_im = c / k2;
     e2.dd_re = 1.0 / k2; e2.dd_im = -c / k2;
+    e2.su_re = 1.0 / k2; e2.sd_re = 1.0 / k2;
     const int mode = (fuse == FUSE_PAP) ? 2 : (fuse == FUSE_R) ? 3 : 1;
     CU(launch_hopping(precision, recon, dagger, mode, ctx.geo, e2, gauge, tmp_odd,
                       out, in, 0, next_reverse(), red(), scal, ctx.block, ctx.stream));

@@ -67,6 +67,27 @@ __device__ __forceinline__ void load_spinor(const void* base, int idx, float (&p
         psi[4 * k + 3] = v.w;
     }
 }
+// plain (coherent) loads for a field the same kernel also writes (MODE 3 reads r before storing it)
+__device__ __forceinline__ void load_spinor_rw(const void* base, int idx, double (&psi)[24]) {
+    const double2* p = reinterpret_cast<const double2*>(base) + (size_t)(idx >> 5) * (12 * 32) + (idx & 31);
+#pragma unroll
+    for (int c = 0; c < 12; ++c) {
+        const double2 v = p[c * 32];
+        psi[2 * c] = v.x;
+        psi[2 * c + 1] = v.y;
+    }
+}
+__device__ __forceinline__ void load_spinor_rw(const void* base, int idx, float (&psi)[24]) {
+    const float4* p = reinterpret_cast<const float4*>(base) + (size_t)(idx >> 5) * (6 * 32) + (idx & 31);
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        const float4 v = p[k * 32];
+        psi[4 * k] = v.x;
+        psi[4 * k + 1] = v.y;
+        psi[4 * k + 2] = v.z;
+        psi[4 * k + 3] = v.w;
+    }
+}
 __device__ __forceinline__ void store_spinor(void* base, int idx, const double (&o)[24]) {
     double2* p = reinterpret_cast<double2*>(base) + (size_t)(idx >> 5) * (12 * 32) + (idx & 31);
 #pragma unroll
@@ -288,16 +309,9 @@ hopping_kernel(const HopArgs a) {
     const int blk = a.reverse ? (int)(gridDim.x - 1 - blockIdx.x) : (int)blockIdx.x;
     const int e = blk * blockDim.x + threadIdx.x;
     double nrm = 0.0;
-    double alpha = 1.0;
-    if (MODE == 3) {  // alpha = rho / <p, A p>; breakdown leaves r untouched and is flagged for FIN_RHO
-        const double rho = a.scal->rho, pAp = a.scal->pAp;
-        if (!(pAp > 0.0) || !isfinite(pAp) || !isfinite(rho)) {
-            if (blockIdx.x == 0 && threadIdx.x == 0) a.scal->status = -5;
-            return;
-        }
-        alpha = rho / pAp;
-        if (blockIdx.x == 0 && threadIdx.x == 0) a.scal->alpha = alpha;  // for cg_update_xp
-    }
+    // MODE 3: alpha = rho / <p, A p> and its inverse were left in the device scalars by
+    // finalize(FIN_PAP), which also ends the solve (done = 1, caught above) on a breakdown.
+    const double alpha = (MODE == 3) ? a.scal->alpha : 1.0;
     if (e < Vh) {
         // a1: e -> (x0h, x1, x2, x3); r = x0 mod 2 follows from the parity
         const int N0h = a.g.N0h, N1 = a.g.N1, N2 = a.g.N2, N3 = a.g.N3;
@@ -325,12 +339,12 @@ hopping_kernel(const HopArgs a) {
             }
             if (MODE == 3) {
                 // r - alpha c (bracket + d aux) = (-alpha c) (bracket + d aux - r / (alpha c)):
-                // the old residual joins the accumulator's initial value with s = -1 / (alpha c)
-                load_spinor(a.out, e, x);
-                const double nu = -alpha * (a.ep.cu_re * a.ep.cu_re + a.ep.cu_im * a.ep.cu_im);
-                const double nd = -alpha * (a.ep.cd_re * a.ep.cd_re + a.ep.cd_im * a.ep.cd_im);
-                const T sur = (T)(a.ep.cu_re / nu), sui = (T)(-a.ep.cu_im / nu);
-                const T sdr = (T)(a.ep.cd_re / nd), sdi = (T)(-a.ep.cd_im / nd);
+                // the old residual joins the accumulator's initial value with s = -(1/alpha)(1/c),
+                // 1/c = ep.s* prepared on the host
+                load_spinor_rw(a.out, e, x);
+                const double ia = -a.scal->inv_alpha;
+                const T sur = (T)(ia * a.ep.su_re), sui = (T)(ia * a.ep.su_im);
+                const T sdr = (T)(ia * a.ep.sd_re), sdi = (T)(ia * a.ep.sd_im);
 #pragma unroll
                 for (int c = 0; c < 12; ++c) {
                     const T sr = (c < 6) ? sur : sdr, si = (c < 6) ? sui : sdi;

@@ -38,6 +38,7 @@ struct Geometry {
 struct Epilogue {
     double cu_re, cu_im, cd_re, cd_im;
     double du_re, du_im, dd_re, dd_im;
+    double su_re, su_im, sd_re, sd_im;   // 1 / c_chi (used by hopping MODE 3 only)
 };
 
 // Device scalars of the CG recurrence.
@@ -45,7 +46,8 @@ struct CgScalars {
     double rho;        // |r|^2
     double pAp;        // <p, A p> = |Mhat p|^2
     double beta;
-    double alpha;      // rho / pAp of the current iteration (written by the fused r-update, hopping MODE 3)
+    double alpha;      // rho / pAp of the current iteration (written by finalize(FIN_PAP))
+    double inv_alpha;  // pAp / rho
     double bb;         // |b|^2
     double tol2bb;     // tol^2 |b|^2
     double resid_true; // |b - A x|^2

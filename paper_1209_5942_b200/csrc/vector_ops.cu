@@ -76,7 +76,16 @@ __global__ void __launch_bounds__(1024) finalize_kernel(int fin, Reduction red, 
     s = warp_sum(sm[lane]);
     if (lane != 0) return;
     if (fin == FIN_PAP) {
+        const double rho = scal->rho;
         scal->pAp = s;
+        if (!(s > 0.0) || !isfinite(s) || !isfinite(rho)) {  // breakdown: r and x stay untouched
+            scal->status = -5;
+            scal->done = 1;
+            scal->upd = 0;
+        } else {
+            scal->alpha = rho / s;
+            scal->inv_alpha = s / rho;
+        }
     } else if (fin == FIN_BB) {
         scal->bb = s;
         scal->rho = s;
@@ -89,11 +98,6 @@ __global__ void __launch_bounds__(1024) finalize_kernel(int fin, Reduction red, 
         scal->status = (s == 0.0) ? 0 : 1;
         scal->upd = 0;
     } else if (fin == FIN_RHO) {
-        if (scal->status == -5) {  // breakdown flagged by the fused r-update: r untouched, freeze the solve
-            scal->done = 1;
-            scal->upd = 0;
-            return;
-        }
         const double rho = scal->rho;
         scal->iters += 1;
         scal->upd = 1;
