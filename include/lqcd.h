@@ -130,6 +130,15 @@ int lqcd_cg_setup(const void* gauge, const void* b, void* x, double kappa, doubl
 int lqcd_cg_iterate(int n);
 int lqcd_cg_finish(void);
 
+/* Solve Mhat x = b on even sites by BiCGStab, the second solver the paper names (
+ * SURVEY.md section 8(f) row 2; reading G15 of DESIGN.md): shadow residual rhat = b, x0 = 0, one
+ * iteration = two applications of Mhat; stops when |r| <= tol |b| (recursive residual) or after
+ * maxit iterations.  Returns LQCD_OK, LQCD_NOT_CONVERGED or LQCD_BREAKDOWN (<rhat,v>, <rhat,r> or
+ * omega zero or not finite); lqcd_cg_stats() gives iterations and the residuals of Mhat x = b.
+ * b, x in internal layout; b is read throughout the solve.  Synchronous. */
+int lqcd_bicgstab_mhat(const void* gauge, const void* b, void* x, double kappa, double mu, double tol,
+                       int maxit);
+
 /* Mixed-precision solve of the same system (the paper's planned next step, PAPER.md:352;
  * SURVEY.md section 8(f) row 1): defect correction with the outer residual in double and the
  * inner CG in single precision,

@@ -21,7 +21,7 @@ SYMBOLS = [
     "lqcd_last_error", "lqcd_init", "lqcd_finalize", "lqcd_set_stream", "lqcd_set_format",
     "lqcd_gauge_bytes", "lqcd_spinor_bytes", "lqcd_pack_gauge", "lqcd_pack_spinor",
     "lqcd_unpack_spinor", "lqcd_dslash_eo", "lqcd_mtm", "lqcd_mtm_full", "lqcd_solve_full", "lqcd_cg_mdagm", "lqcd_cg_setup",
-    "lqcd_cg_iterate", "lqcd_cg_finish", "lqcd_cg_stats", "lqcd_cg_mdagm_mixed", "lqcd_cg_outer_iterations", "lqcd_mtm_host", "lqcd_cg_mdagm_host",
+    "lqcd_cg_iterate", "lqcd_cg_finish", "lqcd_cg_stats", "lqcd_cg_mdagm_mixed", "lqcd_cg_outer_iterations", "lqcd_bicgstab_mhat", "lqcd_mtm_host", "lqcd_cg_mdagm_host",
     "lqcd_launch_count", "lqcd_set_block_size", "lqcd_profile", "lqcd_profile_read",
 ]
 
@@ -55,6 +55,7 @@ def _load():
         "lqcd_mtm_full": [vp, vp, vp, vp, vp, dbl, dbl],
         "lqcd_solve_full": [vp, vp, vp, vp, vp, dbl, dbl, dbl, i32],
         "lqcd_cg_mdagm": [vp, vp, vp, dbl, dbl, dbl, i32],
+        "lqcd_bicgstab_mhat": [vp, vp, vp, dbl, dbl, dbl, i32],
         "lqcd_cg_setup": [vp, vp, vp, dbl, dbl, dbl],
         "lqcd_cg_mdagm_mixed": [vp, i32, vp, i32, vp, vp, dbl, dbl, dbl, i32, dbl],
         "lqcd_cg_outer_iterations": [],
@@ -184,6 +185,10 @@ def lqcd_solve_full(gauge, eta_even, eta_odd, psi_even, psi_odd, kappa, mu, tol,
 
 def lqcd_cg_mdagm(gauge, b, x, kappa, mu, tol, maxit):
     return _check(_lib.lqcd_cg_mdagm(_ptr(gauge), _ptr(b), _ptr(x), kappa, mu, tol, maxit))
+
+
+def lqcd_bicgstab_mhat(gauge, b, x, kappa, mu, tol, maxit):
+    return _check(_lib.lqcd_bicgstab_mhat(_ptr(gauge), _ptr(b), _ptr(x), kappa, mu, tol, maxit))
 
 
 def lqcd_cg_mdagm_mixed(gauge_double, recon_double, gauge_single, recon_single, b, x, kappa, mu, tol, maxit,

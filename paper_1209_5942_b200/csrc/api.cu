@@ -61,13 +61,15 @@ struct Context {
     cudaStream_t stream = 0;
     int snake = 1;                   // direction of the last field-sized launch (next_reverse)
 
-    // workspace (owned), one set of half spinors per precision: r, p, q, t1, t2
-    void* vec[2][5] = {{nullptr, nullptr, nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr, nullptr, nullptr}};
+    // workspace (owned), one set of half spinors per precision: r, p, q, t1, t2, t3
+    void* vec[2][6] = {{nullptr, nullptr, nullptr, nullptr, nullptr, nullptr},
+                       {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr}};
     void* full_b[2] = {nullptr, nullptr};  // lqcd_solve_full: right-hand side of the normal equations
     void* mx_b = nullptr;            // mixed solver: single-precision right-hand side and correction
     void* mx_x = nullptr;
     CgScalars* scal = nullptr;       // scalars of the running CG
     CgScalars* scal_outer = nullptr; // scalars of the mixed solver's outer (double) loop
+    BiScalars* bscal = nullptr;      // scalars of the running BiCGStab
     CgScalars* scal_host = nullptr;  // pinned, 3 slots
     cudaEvent_t ev[2] = {nullptr, nullptr};
     double* partials = nullptr;
@@ -121,7 +123,7 @@ size_t n_reals() { return (size_t)24 * 32 * ctx.geo.G; }  // reals in one half-s
 
 void free_workspace() {
     for (int pr = 0; pr < 2; ++pr)
-        for (int i = 0; i < 5; ++i) { if (ctx.vec[pr][i]) cudaFree(ctx.vec[pr][i]); ctx.vec[pr][i] = nullptr; }
+        for (int i = 0; i < 6; ++i) { if (ctx.vec[pr][i]) cudaFree(ctx.vec[pr][i]); ctx.vec[pr][i] = nullptr; }
     for (int pr = 0; pr < 2; ++pr) { if (ctx.full_b[pr]) cudaFree(ctx.full_b[pr]); ctx.full_b[pr] = nullptr; }
     if (ctx.mx_b) cudaFree(ctx.mx_b);
     if (ctx.mx_x) cudaFree(ctx.mx_x);
@@ -132,6 +134,7 @@ void free_all() {
     free_workspace();
     if (ctx.scal) cudaFree(ctx.scal);
     if (ctx.scal_outer) cudaFree(ctx.scal_outer);
+    if (ctx.bscal) cudaFree(ctx.bscal);
     if (ctx.scal_host) cudaFreeHost(ctx.scal_host);
     if (ctx.partials) cudaFree(ctx.partials);
     for (int i = 0; i < 2; ++i) if (ctx.ev[i]) cudaEventDestroy(ctx.ev[i]);
@@ -146,10 +149,13 @@ int ensure_scalars() {
         CU(cudaMemset(ctx.scal, 0, sizeof(CgScalars)));
         CU(cudaMalloc(&ctx.scal_outer, sizeof(CgScalars)));
         CU(cudaMemset(ctx.scal_outer, 0, sizeof(CgScalars)));
+        CU(cudaMalloc(&ctx.bscal, sizeof(BiScalars)));
+        CU(cudaMemset(ctx.bscal, 0, sizeof(BiScalars)));
         CU(cudaMallocHost(&ctx.scal_host, 3 * sizeof(CgScalars)));
         for (int i = 0; i < 2; ++i) CU(cudaEventCreateWithFlags(&ctx.ev[i], cudaEventDisableTiming));
     }
-    const size_t need = (size_t)hopping_partials(ctx.geo.Vh, 32) + (size_t)vector_grid(n_reals()) + 64;
+    // one partial per warp of a hopping launch, or up to three per block of a vector kernel (BiCGStab)
+    const size_t need = (size_t)hopping_partials(ctx.geo.Vh, 32) + 3 * (size_t)vector_grid(n_reals()) + 64;
     if (need > ctx.n_partials) {
         if (ctx.partials) CU(cudaFree(ctx.partials));
         ctx.partials = nullptr;
@@ -163,8 +169,8 @@ int ensure_workspace(int precision, int nvec) {
     int rc = ensure_scalars();
     if (rc) return rc;
     const size_t sb = spinor_bytes_of(precision, ctx.geo.G);
-    // t1 (index 3) is needed by lqcd_mtm; the rest only by CG
-    const int order[5] = {3, 4, 0, 1, 2};
+    // t1 (index 3) is needed by lqcd_mtm; the rest only by the solvers (t3 only by BiCGStab)
+    const int order[6] = {3, 4, 0, 1, 2, 5};
     for (int k = 0; k < nvec; ++k) {
         const int i = order[k];
         if (!ctx.vec[precision][i]) CU(cudaMalloc(&ctx.vec[precision][i], sb));
@@ -250,9 +256,29 @@ int cg_setup_impl(int precision, int recon, const void* gauge, const void* b, vo
     return LQCD_OK;
 }
 
+// One BiCGStab iteration on Mhat x = b (vector_ops.cu "BiCGStab"; rhat = b).
+int enqueue_bicg_iteration() {
+    void** w = ctx.vec[ctx.cg_prec];
+    void *r = w[0], *p = w[1], *v = w[2], *t1 = w[3], *s = w[4], *t = w[5];
+    const size_t n = n_reals();
+    const int pr = ctx.cg_prec;
+    CgScalars* gate = &ctx.bscal->cg;
+    int rc = apply_mhat(pr, ctx.cg_recon, ctx.cg_gauge, p, t1, v, ctx.cg_kappa, ctx.cg_mu, 0, FUSE_NONE, gate);
+    if (rc) return rc;
+    CU(launch_bicg_sigma(pr, n, ctx.cg_b, v, next_reverse(), red(), ctx.bscal, ctx.stream));
+    CU(launch_bicg_s(pr, n, r, v, s, next_reverse(), ctx.bscal, ctx.stream));
+    if ((rc = apply_mhat(pr, ctx.cg_recon, ctx.cg_gauge, s, t1, t, ctx.cg_kappa, ctx.cg_mu, 0, FUSE_NONE, gate))) return rc;
+    CU(launch_bicg_omega(pr, n, t, s, next_reverse(), red(), ctx.bscal, ctx.stream));
+    CU(launch_bicg_xr(pr, n, ctx.cg_x, p, s, t, ctx.cg_b, r, next_reverse(), red(), ctx.bscal, ctx.stream));
+    CU(launch_bicg_p(pr, n, p, r, v, next_reverse(), ctx.bscal, ctx.stream));
+    return LQCD_OK;
+}
+
 // Enqueue up to maxit iterations in chunks; the convergence flag of chunk k is read back while
-// chunk k+1 is already queued, so the device never idles on the host.
-int cg_run_impl(int maxit) {
+// chunk k+1 is already queued, so the device never idles on the host.  `scal` is the solver's
+// device scalar block (a CgScalars, or the CgScalars at the head of a BiScalars).
+int cg_run_impl(int maxit, int (*enqueue)() = enqueue_iteration, const CgScalars* scal = nullptr) {
+    if (!scal) scal = ctx.scal;
     const int chunk = 4;
     int launched = 0, slot = 0;
     bool pending[2] = {false, false};
@@ -260,11 +286,11 @@ int cg_run_impl(int maxit) {
     while (launched < maxit && !stop) {
         const int n = (maxit - launched < chunk) ? (maxit - launched) : chunk;
         for (int i = 0; i < n; ++i) {
-            int rc = enqueue_iteration();
+            int rc = enqueue();
             if (rc) return rc;
         }
         launched += n;
-        CU(cudaMemcpyAsync(&ctx.scal_host[slot], ctx.scal, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx.stream));
+        CU(cudaMemcpyAsync(&ctx.scal_host[slot], scal, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx.stream));
         CU(cudaEventRecord(ctx.ev[slot], ctx.stream));
         pending[slot] = true;
         const int prev = slot ^ 1;
@@ -560,6 +586,39 @@ int lqcd_cg_mdagm(const void* gauge, const void* b, void* x, double kappa, doubl
     rc = cg_run_impl(maxit);
     if (rc) return rc;
     return cg_finish_impl(true);
+}
+
+int lqcd_bicgstab_mhat(const void* gauge, const void* b, void* x, double kappa, double mu, double tol,
+                       int maxit) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (!gauge || !b || !x) return fail(LQCD_BAD_ARG, "lqcd_bicgstab_mhat: null pointer");
+    if (b == x) return fail(LQCD_BAD_ARG, "lqcd_bicgstab_mhat: b and x alias");
+    if (maxit < 1) return fail(LQCD_BAD_ARG, "maxit must be >= 1");
+    int rc = check_scalar(kappa, "kappa");
+    if (rc) return rc;
+    if ((rc = check_scalar(mu, "mu"))) return rc;
+    if (!std::isfinite(tol) || tol < 0.0) return fail(LQCD_BAD_ARG, "tol must be finite and >= 0");
+    const int pr = ctx.precision;
+    if ((rc = ensure_workspace(pr, 6))) return rc;
+    ctx.cg_prec = pr; ctx.cg_recon = ctx.recon;
+    ctx.cg_gauge = gauge; ctx.cg_b = b; ctx.cg_x = x;
+    ctx.cg_kappa = kappa; ctx.cg_mu = mu; ctx.cg_tol = tol;
+    ctx.cg_active = false;   // the three-step CG interface is not open on this solve
+    void** w = ctx.vec[pr];
+    CU(launch_bicg_init(pr, n_reals(), b, x, w[0], w[1], tol, red(), ctx.bscal, ctx.stream));
+    if ((rc = cg_run_impl(maxit, enqueue_bicg_iteration, &ctx.bscal->cg))) return rc;
+    // true residual |b - Mhat x| / |b|
+    if ((rc = apply_mhat(pr, ctx.recon, gauge, x, w[3], w[5], kappa, mu, 0, FUSE_NONE, nullptr))) return rc;
+    CU(launch_true_resid(pr, n_reals(), b, w[5], red(), &ctx.bscal->cg, ctx.stream));
+    CU(cudaMemcpyAsync(ctx.scal_host, &ctx.bscal->cg, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx.stream));
+    CU(cudaStreamSynchronize(ctx.stream));
+    const CgScalars& sc = ctx.scal_host[0];
+    ctx.st_iters = sc.iters;
+    ctx.st_outer = 0;
+    ctx.st_rr = sc.bb > 0 ? std::sqrt(sc.rho / sc.bb) : 0.0;
+    ctx.st_rt = sc.bb > 0 ? std::sqrt(sc.resid_true / sc.bb) : 0.0;
+    if (sc.status == LQCD_BREAKDOWN) return fail(LQCD_BREAKDOWN, "BiCGStab breakdown after %d iterations", sc.iters);
+    return sc.status;
 }
 
 // Mixed-precision defect correction:

@@ -57,11 +57,22 @@ struct CgScalars {
     int upd;           // 1 if this iteration updated r, i.e. cg_update_xp has an x-update to apply
 };
 
+// Device scalars of BiCGStab on Mhat: the CG block carries what the shared plumbing reads
+// (done, status, iters, bb, tol2bb, rho = |r|^2, resid_true); the complex recurrence scalars follow.
+struct BiScalars {
+    CgScalars cg;
+    double rho_re, rho_im;      // <rhat, r>
+    double alpha_re, alpha_im;
+    double omega_re, omega_im;
+    double beta_re, beta_im;
+};
+
 struct Reduction {
     double* partials;       // one per warp (hopping) or per block (vector kernels)
 };
 
 enum { FIN_NONE = 0, FIN_PAP = 1, FIN_BB = 2, FIN_RHO = 3, FIN_TRUE = 4 };
+enum { FIN_BI_INIT = 0, FIN_BI_SIGMA = 1, FIN_BI_OMEGA = 2, FIN_BI_R = 3 };
 
 // "Snake order": consecutive kernels of a chain traverse the sites in opposite directions
 // (reverse = 0, 1, 0, 1, ...).  A field is 201 MB at 32^3 x 64 and L2 holds ~126 MB, so the
@@ -93,6 +104,20 @@ cudaError_t launch_residual(size_t n, const void* b, const void* ax, void* r, Re
 // sums red.partials[0..n_partials) in a fixed order and applies the FIN_* action to *scal
 cudaError_t launch_finalize(int fin, Reduction red, int n_partials, double tol, CgScalars* scal,
                             cudaStream_t st);
+// BiCGStab vector kernels (vector_ops.cu); partial sums use up to 3 * vector_grid(n) doubles
+cudaError_t launch_bicg_init(int precision, size_t n, const void* b, void* x, void* r, void* p, double tol,
+                             Reduction red, BiScalars* bs, cudaStream_t st);
+cudaError_t launch_bicg_sigma(int precision, size_t n, const void* rhat, const void* v, int reverse,
+                              Reduction red, BiScalars* bs, cudaStream_t st);
+cudaError_t launch_bicg_s(int precision, size_t n, const void* r, const void* v, void* s, int reverse,
+                          BiScalars* bs, cudaStream_t st);
+cudaError_t launch_bicg_omega(int precision, size_t n, const void* t, const void* s, int reverse,
+                              Reduction red, BiScalars* bs, cudaStream_t st);
+cudaError_t launch_bicg_xr(int precision, size_t n, void* x, const void* p, const void* s, const void* t,
+                           const void* rhat, void* r, int reverse, Reduction red, BiScalars* bs,
+                           cudaStream_t st);
+cudaError_t launch_bicg_p(int precision, size_t n, void* p, const void* r, const void* v, int reverse,
+                          BiScalars* bs, cudaStream_t st);
 int vector_grid(size_t n);
 int hopping_partials(int Vh, int block);
 

@@ -245,6 +245,208 @@ __global__ void __launch_bounds__(VBLOCK) diag_scale_kernel_f(size_t nvec, const
     out[i] = make_float4(ar * v.x - ai * v.y, ar * v.y + ai * v.x, ar * v.z - ai * v.w, ar * v.w + ai * v.z);
 }
 
+// ----------------------------------------------------------------------------- BiCGStab on Mhat
+// (PAPER.md:94 names CG and BiCGStab; reading G15 for the recurrence).  Complex
+// scalars live in BiScalars on the device; one iteration is
+//   v = Mhat p | bicg_sigma: <rhat,v> -> alpha | bicg_s: s = r - alpha v | t = Mhat s |
+//   bicg_omega: <t,s>, |t|^2 -> omega | bicg_xr: x += alpha p + omega s, r = s - omega t,
+//   |r|^2, <rhat,r> -> beta, convergence | bicg_p: p = r + beta (p - omega v)
+// = 18 field transfers besides the four hopping launches.
+struct cd { double re, im; };
+__device__ __forceinline__ cd cmul(cd a, cd b) { return {a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re}; }
+__device__ __forceinline__ cd cdiv(cd a, cd b) {
+    const double d = b.re * b.re + b.im * b.im;
+    return {(a.re * b.re + a.im * b.im) / d, (a.im * b.re - a.re * b.im) / d};
+}
+__device__ __forceinline__ bool cbad(cd a) { return (a.re == 0.0 && a.im == 0.0) || !isfinite(a.re) || !isfinite(a.im); }
+
+// y + a x, a complex, on one (double2) or two (float4) complex numbers
+__device__ __forceinline__ double2 caxpy(cd a, double2 x, double2 y) {
+    return make_double2(fma(-a.im, x.y, fma(a.re, x.x, y.x)), fma(a.im, x.x, fma(a.re, x.y, y.y)));
+}
+__device__ __forceinline__ float4 caxpy(cd a, float4 x, float4 y) {
+    const float ar = (float)a.re, ai = (float)a.im;
+    return make_float4(fmaf(-ai, x.y, fmaf(ar, x.x, y.x)), fmaf(ai, x.x, fmaf(ar, x.y, y.y)),
+                       fmaf(-ai, x.w, fmaf(ar, x.z, y.z)), fmaf(ai, x.z, fmaf(ar, x.w, y.w)));
+}
+// sum conj(a_i) b_i accumulated in double
+__device__ __forceinline__ void cdot_acc(double2 a, double2 b, double& re, double& im) {
+    re += a.x * b.x + a.y * b.y;
+    im += a.x * b.y - a.y * b.x;
+}
+__device__ __forceinline__ void cdot_acc(float4 a, float4 b, double& re, double& im) {
+    re += (double)a.x * b.x + (double)a.y * b.y + (double)a.z * b.z + (double)a.w * b.w;
+    im += (double)a.x * b.y - (double)a.y * b.x + (double)a.z * b.w - (double)a.w * b.z;
+}
+
+// K block sums at once; partial k of block b goes to red.partials[k * gridDim.x + b]
+template <int K>
+__device__ __forceinline__ void block_partials(double (&v)[K], Reduction red) {
+    __shared__ double sm[K][VBLOCK / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        v[k] = warp_sum(v[k]);
+        if (lane == 0) sm[k][warp] = v[k];
+    }
+    __syncthreads();
+    if (warp == 0) {
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            double w = (lane < VBLOCK / 32) ? sm[k][lane] : 0.0;
+            w = warp_sum(w);
+            if (lane == 0) red.partials[(size_t)k * gridDim.x + blockIdx.x] = w;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(1024) bicg_finalize_kernel(int fin, Reduction red, int n, double tol,
+                                                             BiScalars* bs) {
+    __shared__ double sm[3][32];
+    if (fin != FIN_BI_INIT && bs->cg.done) return;
+    double s[3] = {0.0, 0.0, 0.0};
+    const int K = (fin == FIN_BI_INIT) ? 1 : (fin == FIN_BI_SIGMA) ? 2 : 3;
+    for (int k = 0; k < K; ++k)
+        for (int i = threadIdx.x; i < n; i += 1024) s[k] += red.partials[(size_t)k * n + i];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int k = 0; k < K; ++k) {
+        s[k] = warp_sum(s[k]);
+        if (lane == 0) sm[k][warp] = s[k];
+    }
+    __syncthreads();
+    if (warp != 0) return;
+    for (int k = 0; k < K; ++k) s[k] = warp_sum(sm[k][lane]);
+    if (lane != 0) return;
+    if (fin == FIN_BI_INIT) {           // s0 = |b|^2; rhat = r = b so rho = <rhat, r> = |b|^2
+        CgScalars& c = bs->cg;
+        c.bb = s[0]; c.rho = s[0]; c.pAp = 0.0; c.beta = 0.0; c.alpha = 0.0; c.inv_alpha = 0.0;
+        c.tol2bb = tol * tol * s[0]; c.resid_true = 0.0; c.iters = 0;
+        c.done = (s[0] == 0.0) ? 1 : 0;
+        c.status = (s[0] == 0.0) ? 0 : 1;
+        c.upd = 0;
+        bs->rho_re = s[0]; bs->rho_im = 0.0;
+        bs->alpha_re = bs->alpha_im = bs->omega_re = bs->omega_im = bs->beta_re = bs->beta_im = 0.0;
+    } else if (fin == FIN_BI_SIGMA) {   // sigma = <rhat, v>; alpha = rho / sigma
+        const cd sigma = {s[0], s[1]};
+        if (cbad(sigma)) { bs->cg.status = -5; bs->cg.done = 1; return; }
+        const cd a = cdiv({bs->rho_re, bs->rho_im}, sigma);
+        bs->alpha_re = a.re; bs->alpha_im = a.im;
+    } else if (fin == FIN_BI_OMEGA) {   // omega = <t, s> / |t|^2 (0 if t = 0)
+        const double tt = s[2];
+        bs->omega_re = tt > 0.0 ? s[0] / tt : 0.0;
+        bs->omega_im = tt > 0.0 ? s[1] / tt : 0.0;
+    } else if (fin == FIN_BI_R) {       // s0 = |r|^2, (s1, s2) = rho' = <rhat, r>
+        CgScalars& c = bs->cg;
+        c.iters += 1;
+        c.rho = s[0];
+        if (s[0] <= c.tol2bb) { c.done = 1; c.status = 0; return; }
+        const cd rho1 = {s[1], s[2]}, omega = {bs->omega_re, bs->omega_im};
+        if (cbad(rho1) || cbad(omega) || !isfinite(s[0])) { c.status = -5; c.done = 1; return; }
+        const cd beta = cmul(cdiv(rho1, {bs->rho_re, bs->rho_im}), cdiv({bs->alpha_re, bs->alpha_im}, omega));
+        bs->beta_re = beta.re; bs->beta_im = beta.im;
+        bs->rho_re = rho1.re; bs->rho_im = rho1.im;
+    }
+}
+
+#define LQCD_VEC_INDEX                                                              \
+    const size_t blk = reverse ? (gridDim.x - 1 - blockIdx.x) : blockIdx.x;         \
+    const size_t base = blk * (VBLOCK * VUNROLL) + threadIdx.x
+
+template <typename T>
+__global__ void __launch_bounds__(VBLOCK) bicg_sigma_kernel(size_t nvec, const void* rhat_, const void* v_,
+                                                            int reverse, Reduction red, const BiScalars* bs) {
+    typedef typename VecOf<T>::type V;
+    if (bs->cg.done) return;
+    const V *rhat = (const V*)rhat_, *v = (const V*)v_;
+    LQCD_VEC_INDEX;
+    double s[2] = {0.0, 0.0};
+#pragma unroll
+    for (int k = 0; k < VUNROLL; ++k) {
+        const size_t i = base + (size_t)k * VBLOCK;
+        if (i < nvec) cdot_acc(__ldg(rhat + i), __ldg(v + i), s[0], s[1]);
+    }
+    block_partials<2>(s, red);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(VBLOCK) bicg_s_kernel(size_t nvec, const void* r_, const void* v_, void* s_,
+                                                        int reverse, const BiScalars* bs) {
+    typedef typename VecOf<T>::type V;
+    if (bs->cg.done) return;
+    const cd ma = {-bs->alpha_re, -bs->alpha_im};
+    const V *r = (const V*)r_, *v = (const V*)v_;
+    V* s = (V*)s_;
+    LQCD_VEC_INDEX;
+#pragma unroll
+    for (int k = 0; k < VUNROLL; ++k) {
+        const size_t i = base + (size_t)k * VBLOCK;
+        if (i < nvec) s[i] = caxpy(ma, __ldg(v + i), __ldg(r + i));
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(VBLOCK) bicg_omega_kernel(size_t nvec, const void* t_, const void* s_,
+                                                            int reverse, Reduction red, const BiScalars* bs) {
+    typedef typename VecOf<T>::type V;
+    if (bs->cg.done) return;
+    const V *t = (const V*)t_, *s = (const V*)s_;
+    LQCD_VEC_INDEX;
+    double a[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+    for (int k = 0; k < VUNROLL; ++k) {
+        const size_t i = base + (size_t)k * VBLOCK;
+        if (i < nvec) {
+            const V tv = __ldg(t + i);
+            cdot_acc(tv, __ldg(s + i), a[0], a[1]);
+            a[2] += norm2(tv);
+        }
+    }
+    block_partials<3>(a, red);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(VBLOCK) bicg_xr_kernel(size_t nvec, void* x_, const void* p_, const void* s_,
+                                                         const void* t_, const void* rhat_, void* r_,
+                                                         int reverse, Reduction red, const BiScalars* bs) {
+    typedef typename VecOf<T>::type V;
+    if (bs->cg.done) return;
+    const cd alpha = {bs->alpha_re, bs->alpha_im}, omega = {bs->omega_re, bs->omega_im};
+    const cd momega = {-omega.re, -omega.im};
+    V *x = (V*)x_, *r = (V*)r_;
+    const V *p = (const V*)p_, *s = (const V*)s_, *t = (const V*)t_, *rhat = (const V*)rhat_;
+    LQCD_VEC_INDEX;
+    double a[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+    for (int k = 0; k < VUNROLL; ++k) {
+        const size_t i = base + (size_t)k * VBLOCK;
+        if (i < nvec) {
+            const V sv = __ldg(s + i);
+            x[i] = caxpy(omega, sv, caxpy(alpha, __ldg(p + i), x[i]));
+            const V rn = caxpy(momega, __ldcs(t + i), sv);
+            r[i] = rn;
+            a[0] += norm2(rn);
+            cdot_acc(__ldg(rhat + i), rn, a[1], a[2]);
+        }
+    }
+    block_partials<3>(a, red);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(VBLOCK) bicg_p_kernel(size_t nvec, void* p_, const void* r_, const void* v_,
+                                                        int reverse, const BiScalars* bs) {
+    typedef typename VecOf<T>::type V;
+    if (bs->cg.done) return;
+    const cd beta = {bs->beta_re, bs->beta_im}, momega = {-bs->omega_re, -bs->omega_im};
+    V* p = (V*)p_;
+    const V *r = (const V*)r_, *v = (const V*)v_;
+    LQCD_VEC_INDEX;
+#pragma unroll
+    for (int k = 0; k < VUNROLL; ++k) {
+        const size_t i = base + (size_t)k * VBLOCK;
+        if (i < nvec) p[i] = caxpy(beta, caxpy(momega, __ldcs(v + i), p[i]), __ldg(r + i));
+    }
+}
+
 inline int grid_for(size_t nvec) { return (int)((nvec + VBLOCK * VUNROLL - 1) / (VBLOCK * VUNROLL)); }
 
 }  // namespace
@@ -346,6 +548,68 @@ cudaError_t launch_true_resid(int precision, size_t n, const void* b, const void
         true_resid_kernel<float><<<grid_for(nv), VBLOCK, 0, st>>>(nv, b, ax, red);
         finalize_kernel<<<1, 1024, 0, st>>>(FIN_TRUE, red, grid_for(nv), 0.0, scal);
     }
+    return cudaGetLastError();
+}
+
+// ---- BiCGStab launchers (nv = 128-bit elements of one field)
+#define LQCD_BICG_DISPATCH(KERNEL, ...)                                                        \
+    do {                                                                                       \
+        if (precision == 0) { const size_t nv = n / 2; KERNEL<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, __VA_ARGS__); } \
+        else                { const size_t nv = n / 4; KERNEL<float><<<grid_for(nv), VBLOCK, 0, st>>>(nv, __VA_ARGS__); }  \
+    } while (0)
+
+static int bicg_grid(int precision, size_t n) { return grid_for(precision == 0 ? n / 2 : n / 4); }
+
+cudaError_t launch_bicg_init(int precision, size_t n, const void* b, void* x, void* r, void* p, double tol,
+                             Reduction red, BiScalars* bs, cudaStream_t st) {
+    count_launch(2);
+    ProfScope prof(3, st);
+    LQCD_BICG_DISPATCH(cg_init_kernel, b, x, r, p, red);
+    bicg_finalize_kernel<<<1, 1024, 0, st>>>(FIN_BI_INIT, red, bicg_grid(precision, n), tol, bs);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_bicg_sigma(int precision, size_t n, const void* rhat, const void* v, int reverse,
+                              Reduction red, BiScalars* bs, cudaStream_t st) {
+    count_launch(2);
+    ProfScope prof(3, st);
+    LQCD_BICG_DISPATCH(bicg_sigma_kernel, rhat, v, reverse, red, bs);
+    bicg_finalize_kernel<<<1, 1024, 0, st>>>(FIN_BI_SIGMA, red, bicg_grid(precision, n), 0.0, bs);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_bicg_s(int precision, size_t n, const void* r, const void* v, void* s, int reverse,
+                          BiScalars* bs, cudaStream_t st) {
+    count_launch();
+    ProfScope prof(3, st);
+    LQCD_BICG_DISPATCH(bicg_s_kernel, r, v, s, reverse, bs);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_bicg_omega(int precision, size_t n, const void* t, const void* s, int reverse,
+                              Reduction red, BiScalars* bs, cudaStream_t st) {
+    count_launch(2);
+    ProfScope prof(3, st);
+    LQCD_BICG_DISPATCH(bicg_omega_kernel, t, s, reverse, red, bs);
+    bicg_finalize_kernel<<<1, 1024, 0, st>>>(FIN_BI_OMEGA, red, bicg_grid(precision, n), 0.0, bs);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_bicg_xr(int precision, size_t n, void* x, const void* p, const void* s, const void* t,
+                           const void* rhat, void* r, int reverse, Reduction red, BiScalars* bs,
+                           cudaStream_t st) {
+    count_launch(2);
+    ProfScope prof(3, st);
+    LQCD_BICG_DISPATCH(bicg_xr_kernel, x, p, s, t, rhat, r, reverse, red, bs);
+    bicg_finalize_kernel<<<1, 1024, 0, st>>>(FIN_BI_R, red, bicg_grid(precision, n), 0.0, bs);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_bicg_p(int precision, size_t n, void* p, const void* r, const void* v, int reverse,
+                          BiScalars* bs, cudaStream_t st) {
+    count_launch();
+    ProfScope prof(3, st);
+    LQCD_BICG_DISPATCH(bicg_p_kernel, p, r, v, reverse, bs);
     return cudaGetLastError();
 }
 

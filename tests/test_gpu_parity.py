@@ -55,6 +55,12 @@ class Lat:
         st = self.B.lqcd_cg_mdagm(self.g, s, x, kappa, mu, tol, maxit)
         return st, self.B.download_spinor(x, 0), self.B.lqcd_cg_stats()
 
+    def bicgstab(self, b, kappa, mu, tol, maxit):
+        s = self.B.upload_spinor(b, 0)
+        x = self.B.alloc_spinor()
+        st = self.B.lqcd_bicgstab_mhat(self.g, s, x, kappa, mu, tol, maxit)
+        return st, self.B.download_spinor(x, 0), self.B.lqcd_cg_stats()
+
 
 def _round_inputs(U, x, precision):
     if precision == 0:
@@ -258,6 +264,68 @@ def test_cg_single_precision_converges_loosely(B, oracle_mod):
         assert st == 0 and rr <= tol
         r = b - oracle_mod.mdagm(dims, AP, U, x, kappa, mu)
         assert np.linalg.norm(r) / np.linalg.norm(b) <= 20 * tol
+
+
+# --------------------------------------------------------------------------- BiCGStab on Mhat
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (6, 4, 10, 4), (8, 8, 8, 16)])
+def test_bicgstab_matches_oracle(B, oracle_mod, dims):
+    kappa, mu, tol = 0.15, 0.1, 1e-10
+    U = gen.gauge_haar(dims, SEED)
+    b = gen.spinor_gaussian(lu.volume(dims) // 2, SEED, gen.STREAM_SOURCE)
+    L = Lat(B, dims, AP, U)
+    st, x, (iters, rr, rt) = L.bicgstab(b, kappa, mu, tol, 2000)
+    st_o, x_o, it_o, rr_o, rt_o = oracle_mod.bicgstab_mhat(dims, AP, U, b, kappa, mu, tol, 2000)
+    assert st == 0 and st_o == 0
+    assert abs(iters - it_o) <= 2          # BiCGStab's iterates are sensitive to rounding (G14)
+    assert rr <= tol
+    # true residual of the GPU's x under the ORACLE's Mhat
+    true_rel = np.linalg.norm(b - oracle_mod.mhat(dims, AP, U, x, kappa, mu, 0)) / np.linalg.norm(b)
+    assert true_rel <= 1.05 * tol
+    assert abs(rt - true_rel) <= 0.05 * tol
+    assert lu.rel_err(x, x_o) <= 10 * 5.0 * tol
+
+
+@pytest.mark.parametrize("k", [1, 3])
+def test_bicgstab_k_iterations_from_identical_state(B, oracle_mod, k):
+    dims = (8, 8, 8, 16)
+    kappa, mu = 0.15, 0.1
+    U = gen.gauge_haar(dims, SEED)
+    b = gen.spinor_gaussian(lu.volume(dims) // 2, SEED, gen.STREAM_SOURCE)
+    L = Lat(B, dims, AP, U)
+    st, x, (iters, rr, rt) = L.bicgstab(b, kappa, mu, 0.0, k)
+    st_o, x_o, it_o, rr_o, rt_o = oracle_mod.bicgstab_mhat(dims, AP, U, b, kappa, mu, 0.0, k)
+    assert st == 1 and st_o == 1 and iters == k == it_o
+    assert lu.rel_err(x, x_o) <= 1e-13 * (10 if k > 1 else 1)
+    assert abs(rr - rr_o) <= 1e-11 * rr_o
+    assert abs(rt - rt_o) <= 1e-10 * rt_o
+
+
+def test_bicgstab_edge_cases_and_formats(B, oracle_mod):
+    dims = (4, 4, 4, 4)
+    U = gen.gauge_haar(dims, SEED)
+    L = Lat(B, dims, AP, U)
+    n = lu.volume(dims) // 2
+    zero = np.zeros((n, 4, 3), dtype=complex)
+    st, x, (iters, rr, rt) = L.bicgstab(zero, 0.15, 0.1, 1e-10, 50)
+    assert st == 0 and iters == 0 and np.all(x == 0)
+    b = gen.spinor_gaussian(n, SEED, gen.STREAM_SOURCE)
+    st, x, (iters, rr, rt) = L.bicgstab(b, 0.15, 0.1, 1e-10, 3)
+    assert st == B.LQCD_NOT_CONVERGED and iters == 3 and rr > 1e-10
+    st, x, (iters, rr, rt) = L.bicgstab(b, 0.0, 0.1, 1e-12, 50)      # kappa = 0: Mhat = 1
+    assert st == 0 and iters == 1 and lu.rel_err(x, b) < 1e-14
+    with pytest.raises(B.LqcdError) as e:
+        B.lqcd_bicgstab_mhat(L.g, 0, L.g, 0.1, 0.1, 1e-8, 10)
+    assert e.value.status == B.LQCD_BAD_ARG
+    # single precision and 12-real links converge to what single precision allows
+    dims = (8, 8, 8, 16)
+    U = gen.gauge_haar(dims, SEED)
+    b = gen.spinor_gaussian(lu.volume(dims) // 2, SEED, gen.STREAM_SOURCE)
+    for precision, recon, tol in ((1, 18, 1e-5), (1, 12, 1e-5), (0, 12, 1e-10)):
+        L = Lat(B, dims, AP, U, precision, recon)
+        st, x, (iters, rr, rt) = L.bicgstab(b, 0.15, 0.1, tol, 500)
+        assert st == 0 and rr <= tol
+        true_rel = np.linalg.norm(b - oracle_mod.mhat(dims, AP, U, x, 0.15, 0.1, 0)) / np.linalg.norm(b)
+        assert true_rel <= (20 if precision else 1.05) * tol
 
 
 # --------------------------------------------------------------------------- ABI behaviour
