@@ -19,5 +19,9 @@ from .oracle import (  # noqa: F401
     mdagm,
     cg_mdagm,
     bicgstab_mhat,
+    fermion_force,
+    fermion_force_links,
+    force_fields,
+    force_tm,
     num_threads,
 )

@@ -23,7 +23,8 @@
 // numpy (P4), the paper's own identity M(mu)^dag M(mu) = M(0)^dag M(0) +
 // 4 kappa^2 mu^2 (P5), Schur identity vs the dense matrix (P6),
 // trivial limits (P7), CG vs a dense Hermitian solve (P8), BiCGStab vs a dense solve
-// of Mhat and the textbook recurrence on the dense matrix (P9).  The paper prints
+// of Mhat and the textbook recurrence on the dense matrix (P9), the fermion force vs central
+// differences of the action computed from dense matrices (P10).  The paper prints
 // no numeric example for any of these operators, so element values rest on
 // P1-P8.
 //
@@ -484,6 +485,136 @@ void orc_mdagm(const int* dims, const double* bc_phase, const double* U, const d
     Lattice L = make_lattice(dims, bc_phase);
     std::vector<cplx> tmp(12 * (L.V / 2));
     apply_A(L, (const cplx*)U, (const cplx*)in, (cplx*)out, tmp.data(), kappa, mu);
+}
+
+// ---------------------------------------------------------------------------
+// Fermion force (eq. 9-10; Table 2 row F_fermion, PAPER.md:236;
+// Table 3 "P, F: (N_C^2 - 1) x N_D" reals per site).
+//
+// The paper states F = -dS/dU (eq. 9), that F_mu(x) is a real (N_C^2 - 1)-vector, that it
+// follows from d(D^-1) = -D^-1 (dD) D^-1 and that only the hopping part of the matrix
+// contributes; it prints no formula.  Reading G16 of DESIGN.md:
+//   * components are taken along T^a = lambda^a / 2 (Gell-Mann matrices, standard order),
+//     with the link varied from the left:  U_mu(x) -> exp(i w T^a) U_mu(x),
+//     F^a_mu(x) = - dS/dw at w = 0;
+//   * for two spinor fields X, Y on the whole lattice the "outer product" force is
+//     F^a_mu(x) = 2 Re d/dw [ Y^dag D(w) X ]
+//               = 2 kappa Im [ Y(x)^dag T^a a(x) - b(x)^dag T^a X(x) ],
+//     a(x) = eta+_mu(x) (1 - gamma_mu) U_mu(x) X(x+mu),  b(x) = eta+_mu(x) (1 + gamma_mu) U_mu(x) Y(x+mu),
+//     which is what dS = -2 Re (Y^dag dD X) gives for S = phi^dag (M^dag M)^-1 phi with
+//     X = (M^dag M)^-1 phi, Y = M X (the minus of F = -dS/dU cancels the minus of d(A^-1));
+//   * for the even-odd action S = phi_e^dag (Mhat^dag Mhat)^-1 phi_e the same formula holds
+//     with X_e = (Mhat^dag Mhat)^-1 phi, Y_e = Mhat X_e, X_o = -M_oo^-1 D_oe X_e,
+//     Y_o = -(M_oo^-1)^dag (D_eo)^dag Y_e, since d Mhat = -dD_eo M_oo^-1 D_oe - D_eo M_oo^-1 dD_oe.
+// Pinned in tests/test_oracle_pins.py (P10) by central differences of S computed from
+// dense matrices in numpy, and by gauge covariance.
+// ---------------------------------------------------------------------------
+
+namespace {
+
+// Gell-Mann matrices lambda^1..lambda^8, row-major.
+void gell_mann(int a, cplx* l) {
+    for (int i = 0; i < 9; ++i) l[i] = O_;
+    const double s3 = 1.0 / std::sqrt(3.0);
+    switch (a) {
+        case 0: l[1] = E_; l[3] = E_; break;
+        case 1: l[1] = -I_; l[3] = I_; break;
+        case 2: l[0] = E_; l[4] = -E_; break;
+        case 3: l[2] = E_; l[6] = E_; break;
+        case 4: l[2] = -I_; l[6] = I_; break;
+        case 5: l[5] = E_; l[7] = E_; break;
+        case 6: l[5] = -I_; l[7] = I_; break;
+        case 7: l[0] = s3; l[4] = s3; l[8] = -2.0 * s3; break;
+    }
+}
+
+// u^dag T^a v for two spinors (sum over Dirac and colour), T^a = lambda^a / 2
+cplx sandwich(const cplx* u, int a, const cplx* v) {
+    cplx lam[9];
+    gell_mann(a, lam);
+    cplx s = O_;
+    for (int al = 0; al < 4; ++al)
+        for (int c = 0; c < 3; ++c)
+            for (int d = 0; d < 3; ++d) s += std::conj(u[3 * al + c]) * (0.5 * lam[3 * c + d]) * v[3 * al + d];
+    return s;
+}
+
+// F^a_mu(x), a = 0..7, for the link U_mu(x): the formula of reading G16 written out.
+void force_link(const Lattice& L, const cplx* U, const cplx* X, const cplx* Y, const int* x, int mu,
+                double kappa, double* F8) {
+    const long sx = lex(L, x);
+    int y[4] = {x[0], x[1], x[2], x[3]};
+    y[mu] = (x[mu] + 1) % L.N[mu];
+    const long sy = lex(L, y);
+    const cplx eta = (x[mu] == L.N[mu] - 1) ? L.phase[mu] : E_;
+    cplx t[12], a[12], b[12];
+    su3_mul(U + (sx * 4 + mu) * 9, X + 12 * sy, t);
+    one_plus_sgamma(mu, -1.0, t, a);
+    su3_mul(U + (sx * 4 + mu) * 9, Y + 12 * sy, t);
+    one_plus_sgamma(mu, +1.0, t, b);
+    for (int i = 0; i < 12; ++i) { a[i] *= eta; b[i] *= eta; }
+    for (int g = 0; g < 8; ++g)
+        F8[g] = 2.0 * kappa * (sandwich(Y + 12 * sx, g, a) - sandwich(b, g, X + 12 * sx)).imag();
+}
+
+}  // namespace
+
+// Outer-product force for two full-lattice spinor fields (canonical layouts):
+// F[lex(x)][mu][a], a = 0..7 real.
+void orc_fermion_force(const int* dims, const double* bc_phase, const double* U_, const double* X_,
+                       const double* Y_, double kappa, double* F) {
+    Lattice L = make_lattice(dims, bc_phase);
+#pragma omp parallel for schedule(static)
+    for (long sx = 0; sx < L.V; ++sx) {
+        int x[4];
+        coords(L, sx, x);
+        for (int mu = 0; mu < 4; ++mu)
+            force_link(L, (const cplx*)U_, (const cplx*)X_, (const cplx*)Y_, x, mu, kappa, F + (sx * 4 + mu) * 8);
+    }
+}
+
+// The same at the listed links only: link k is (lex site sites[k], direction mus[k]).
+void orc_fermion_force_links(const int* dims, const double* bc_phase, const double* U_, const double* X_,
+                             const double* Y_, const long* sites, const int* mus, long n_links, double kappa,
+                             double* F) {
+    Lattice L = make_lattice(dims, bc_phase);
+    for (long k = 0; k < n_links; ++k) {
+        int x[4];
+        coords(L, sites[k], x);
+        force_link(L, (const cplx*)U_, (const cplx*)X_, (const cplx*)Y_, x, mus[k], kappa, F + 8 * k);
+    }
+}
+
+// Fields of the even-odd force from a solution X_e:  Y_e = Mhat X_e, X_o = -M_oo^-1 D_oe X_e,
+// Y_o = -(M_oo^-1)^dag (D_eo)^dag Y_e, returned as full-lattice fields X, Y (canonical).
+void orc_force_fields(const int* dims, const double* bc_phase, const double* U_, const double* Xe_,
+                      double kappa, double mu, double* X_, double* Y_) {
+    Lattice L = make_lattice(dims, bc_phase);
+    const cplx* U = (const cplx*)U_;
+    const cplx* Xe = (const cplx*)Xe_;
+    cplx* X = (cplx*)X_;
+    cplx* Y = (cplx*)Y_;
+    const long half = L.V / 2;
+    const double c = 2.0 * kappa * mu;
+    std::vector<cplx> Ye(12 * half), t(12 * half), Xo(12 * half), Yo(12 * half);
+    mhat(L, U, Xe, Ye.data(), kappa, mu, 0);
+    dslash_half(L, U, Xe, t.data(), 1, kappa, +1.0);            // D_oe X_e
+    for (long e = 0; e < half; ++e) {
+        mdiag_inv_site(c, &t[12 * e], &Xo[12 * e]);
+        for (int i = 0; i < 12; ++i) Xo[12 * e + i] = -Xo[12 * e + i];
+    }
+    dslash_half(L, U, Ye.data(), t.data(), 1, kappa, -1.0);     // (D_eo)^dag Y_e: adjoint stencil, odd sites
+    for (long e = 0; e < half; ++e) {
+        mdiag_inv_site(-c, &t[12 * e], &Yo[12 * e]);            // (M_oo^-1)^dag
+        for (int i = 0; i < 12; ++i) Yo[12 * e + i] = -Yo[12 * e + i];
+    }
+    for (long e = 0; e < half; ++e) {
+        const long se = lex_of_eo(L, e, 0), so = lex_of_eo(L, e, 1);
+        for (int i = 0; i < 12; ++i) {
+            X[12 * se + i] = Xe[12 * e + i]; Y[12 * se + i] = Ye[12 * e + i];
+            X[12 * so + i] = Xo[12 * e + i]; Y[12 * so + i] = Yo[12 * e + i];
+        }
+    }
 }
 
 int orc_num_threads(void) {

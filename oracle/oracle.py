@@ -177,5 +177,54 @@ def bicgstab_mhat(dims, bc_phase, U, b, kappa, mu, tol, maxit):
     return st, x, it.value, rr.value, rt.value
 
 
+def fermion_force(dims, bc_phase, U, X, Y, kappa):
+    """Outer-product force of two full-lattice spinor fields: F (V,4,8) float64."""
+    d, ph = _dims(dims), _phases(bc_phase)
+    V = int(np.prod(d))
+    U = _c128(U, (V, 4, 3, 3))
+    X = _c128(X, (V, 4, 3))
+    Y = _c128(Y, (V, 4, 3))
+    F = np.empty((V, 4, 8), dtype=np.float64)
+    _load().orc_fermion_force(_ip(d), _dp(ph), _dp(U), _dp(X), _dp(Y), ctypes.c_double(kappa), _dp(F))
+    return F
+
+
+def fermion_force_links(dims, bc_phase, U, X, Y, sites, mus, kappa):
+    """The same at the listed links (lex site, direction) only: (n,8) float64."""
+    d, ph = _dims(dims), _phases(bc_phase)
+    V = int(np.prod(d))
+    U = _c128(U, (V, 4, 3, 3))
+    X = _c128(X, (V, 4, 3))
+    Y = _c128(Y, (V, 4, 3))
+    sites = np.ascontiguousarray(sites, dtype=np.int64)
+    mus = np.ascontiguousarray(mus, dtype=np.int32)
+    assert sites.shape == mus.shape
+    F = np.empty((len(sites), 8), dtype=np.float64)
+    _load().orc_fermion_force_links(_ip(d), _dp(ph), _dp(U), _dp(X), _dp(Y), sites.ctypes.data_as(_c_long_p),
+                                    _ip(mus), ctypes.c_long(len(sites)), ctypes.c_double(kappa), _dp(F))
+    return F
+
+
+def force_fields(dims, bc_phase, U, X_even, kappa, mu):
+    """Full-lattice (X, Y) of the even-odd force from X_e (see lqcd_oracle.cpp)."""
+    d, ph = _dims(dims), _phases(bc_phase)
+    V = int(np.prod(d))
+    U = _c128(U, (V, 4, 3, 3))
+    X_even = _c128(X_even, (V // 2, 4, 3))
+    X = np.empty((V, 4, 3), dtype=np.complex128)
+    Y = np.empty_like(X)
+    _load().orc_force_fields(_ip(d), _dp(ph), _dp(U), _dp(X_even), ctypes.c_double(kappa), ctypes.c_double(mu),
+                             _dp(X), _dp(Y))
+    return X, Y
+
+
+def force_tm(dims, bc_phase, U, phi_even, kappa, mu, tol, maxit):
+    """Force of S = phi^dag (Mhat^dag Mhat)^-1 phi: CG solve, force fields, outer product.
+    Returns (status, F, iters)."""
+    st, Xe, iters, rr, rt = cg_mdagm(dims, bc_phase, U, phi_even, kappa, mu, tol, maxit)
+    X, Y = force_fields(dims, bc_phase, U, Xe, kappa, mu)
+    return st, fermion_force(dims, bc_phase, U, X, Y, kappa), iters
+
+
 def num_threads():
     return int(_load().orc_num_threads())

@@ -118,10 +118,23 @@ def config4(stream):
         B.lqcd_profile(1)
         B.lqcd_cg_setup(g, b, x, kappa, mu, tol)
         B.lqcd_cg_iterate(iters)
-        hop = sum(B.lqcd_profile_read(c)[0] for c in (0, 1, 2))
+        hop = sum(B.lqcd_profile_read(c)[0] for c in (0, 1, 2, 5))
         vec = B.lqcd_profile_read(3)[0]
         B.lqcd_profile(0)
         B.lqcd_cg_finish()
+        # BiCGStab on Mhat x = b (the other solver the paper names): same operator, the system
+        # itself instead of the normal equations, two Mhat applications per iteration
+        B.lqcd_bicgstab_mhat(g, b, x, kappa, mu, tol, 2000)
+        b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        stream.synchronize()
+        b0.record(stream)
+        bst = B.lqcd_bicgstab_mhat(g, b, x, kappa, mu, tol, 2000)
+        b1.record(stream)
+        stream.synchronize()
+        bit, brr, brt = B.lqcd_cg_stats()
+        bicg = {"status": int(bst), "iterations": bit, "time_to_solution_ms": b0.elapsed_time(b1),
+                "ms_per_iteration": b0.elapsed_time(b1) / max(bit, 1), "rel_resid_recursive": brr,
+                "rel_resid_true": brt, "gflops": 4 * bit * Vh * FLOP / b0.elapsed_time(b1) / 1e6}
         # the same solve by mixed-precision defect correction (single/12 inner CG)
         B.lqcd_set_format(B.LQCD_SINGLE, 12)
         gs = B.upload_gauge(U)
@@ -145,6 +158,7 @@ def config4(stream):
                 "per_iteration_us": {"hopping_4_launches": hop / iters * 1e3, "vector_and_finalize_kernels": vec / iters * 1e3},
                 "hopping_share": hop / (hop + vec),
                 "mixed_precision_single12_inner": mixed,
+                "bicgstab_on_mhat": bicg,
                 "note": "time to solution includes the solve setup and the final true-residual check (one extra "
                         "application of Mhat^dag Mhat)"})
     return out

@@ -142,3 +142,29 @@ def apply_colour(g, psi):
 
 def rel_err(a, b):
     return float(np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300))
+
+
+# Gell-Mann matrices lambda^1..lambda^8 (standard order), retyped here independently of the
+# oracle; the force components are taken along T^a = lambda^a / 2 (reading G16).
+_s3 = 1.0 / np.sqrt(3.0)
+GELL_MANN = np.array([
+    [[0, 1, 0], [1, 0, 0], [0, 0, 0]],
+    [[0, -_i, 0], [_i, 0, 0], [0, 0, 0]],
+    [[1, 0, 0], [0, -1, 0], [0, 0, 0]],
+    [[0, 0, 1], [0, 0, 0], [1, 0, 0]],
+    [[0, 0, -_i], [0, 0, 0], [_i, 0, 0]],
+    [[0, 0, 0], [0, 0, 1], [0, 1, 0]],
+    [[0, 0, 0], [0, 0, -_i], [0, _i, 0]],
+    [[_s3, 0, 0], [0, _s3, 0], [0, 0, -2 * _s3]],
+], dtype=np.complex128)
+
+
+def exp_i_w_T(a, w):
+    """exp(i w T^a), T^a = lambda^a / 2, by eigendecomposition of the Hermitian generator."""
+    ev, V = np.linalg.eigh(0.5 * GELL_MANN[a])
+    return (V * np.exp(1j * w * ev)) @ V.conj().T
+
+
+def algebra_matrix(F8):
+    """sum_a F^a T^a for F8[..., 8] -> [..., 3, 3] (Hermitian, traceless)."""
+    return 0.5 * np.einsum("...a,aij->...ij", F8, GELL_MANN)

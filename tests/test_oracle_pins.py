@@ -12,6 +12,9 @@ is not the oracle itself:
   P6 Schur identity against the dense matrix       (G3)
   P7 trivial limits
   P8 CG against a dense Hermitian solve, orthogonality of residuals
+  P9 BiCGStab against a dense solve of Mhat and van der Vorst's recurrence on the dense matrix
+  P10 fermion force = -dS/dU by central differences of the action built from dense matrices,
+      force fields closing the even-odd system, gauge covariance (reading G16)
 """
 import numpy as np
 import pytest
@@ -392,3 +395,90 @@ def test_p9_bicgstab_edge_cases_and_cost(oracle_mod):
     st_c, xc, it_c, rr_c, rt_c = oracle_mod.cg_mdagm(dims, AP, U, b, 0.15, 0.1, 1e-10, 2000)
     assert st == 0 and st_c == 0 and it_b < it_c
     assert lu.rel_err(oracle_mod.mhat(dims, AP, U, x, 0.15, 0.1, 0), b) < 2e-10
+
+
+# --------------------------------------------------------------------------- P10 fermion force
+def _vary_link(U, s, m, a, w):
+    U2 = U.copy()
+    U2[s, m] = lu.exp_i_w_T(a, w) @ U[s, m]
+    return U2
+
+
+@pytest.mark.parametrize("dims,phases", [((2, 2, 2, 2), AP), ((4, 2, 2, 2), np.exp(1j * np.pi * np.array([0.3, 0.0, 1.0, 0.5])))])
+def test_p10_outer_product_force_is_the_derivative_of_the_bilinear(oracle_mod, dims, phases):
+    # F^a_mu(x) = d/dw 2 Re [Y^dag M(U_mu(x) -> exp(i w T^a) U_mu(x)) X] for ARBITRARY X, Y,
+    # the matrix built densely in numpy (eq. 6); central differences, error O(h^2)
+    kappa, h = 0.15, 1e-4
+    V = lu.volume(dims)
+    U = gen.gauge_haar(dims, SEED)
+    X, Y = _rand_spinor(V, 7), _rand_spinor(V, 8)
+    F = oracle_mod.fermion_force(dims, phases, U, X, Y, kappa)
+    assert F.shape == (V, 4, 8)
+    rng = np.random.default_rng(5)
+    links = [(0, 0), (V - 1, 3), (1, 1)] + [(int(rng.integers(V)), int(rng.integers(4))) for _ in range(5)]
+    # every wrapping hop of the 2-extent directions is among them (x_mu = N_mu - 1 carries the phase)
+    f = lambda Uv: 2.0 * np.real(np.vdot(Y.ravel(), lu.dense_m(dims, phases, Uv, kappa, 0.0) @ X.ravel()))
+    for s, m in links:
+        for a in range(8):
+            fd = (f(_vary_link(U, s, m, a, h)) - f(_vary_link(U, s, m, a, -h))) / (2 * h)
+            assert abs(F[s, m, a] - fd) < 1e-6 * max(1.0, abs(fd)), (s, m, a, F[s, m, a], fd)
+    # the listed-links evaluator agrees with the whole-field one
+    ss = np.array([l[0] for l in links]); mm = np.array([l[1] for l in links])
+    assert np.array_equal(oracle_mod.fermion_force_links(dims, phases, U, X, Y, ss, mm, kappa), F[ss, mm])
+
+
+def test_p10_force_is_minus_the_derivative_of_the_action(oracle_mod):
+    # S[U] = phi^dag (Mhat^dag Mhat)^-1 phi from the dense Schur complement (numpy only);
+    # F^a_mu(x) = -dS/dw (eq. 9) by central differences
+    dims = (2, 2, 2, 2)
+    kappa, mu, h = 0.15, 0.1, 1e-4
+    V = lu.volume(dims)
+    U = gen.gauge_haar(dims, SEED)
+    phi = gen.spinor_gaussian(V // 2, SEED, gen.STREAM_SOURCE)
+
+    def action(Uv):
+        S = lu.dense_mhat(dims, AP, Uv, kappa, mu)
+        return np.real(np.vdot(phi.ravel(), np.linalg.solve(S.conj().T @ S, phi.ravel())))
+
+    st, F, iters = oracle_mod.force_tm(dims, AP, U, phi, kappa, mu, 1e-13, 500)
+    assert st == 0
+    rng = np.random.default_rng(6)
+    links = [(0, 3), (V - 1, 3), (5, 0)] + [(int(rng.integers(V)), int(rng.integers(4))) for _ in range(5)]
+    for s, m in links:
+        for a in range(8):
+            fd = -(action(_vary_link(U, s, m, a, h)) - action(_vary_link(U, s, m, a, -h))) / (2 * h)
+            assert abs(F[s, m, a] - fd) < 1e-6 * max(1.0, abs(fd)), (s, m, a, F[s, m, a], fd)
+    assert np.max(np.abs(F)) > 1e-3      # not trivially zero
+
+
+def test_p10_force_fields_close_the_even_odd_system(oracle_mod):
+    # X_o, Y_o are defined so that (M X)_odd = 0, (M X)_even = Y_e = Mhat X_e, (M^dag Y)_odd = 0
+    dims = (4, 2, 2, 4)
+    kappa, mu = 0.15, 0.1
+    V = lu.volume(dims)
+    U = gen.gauge_haar(dims, SEED)
+    Xe = _rand_spinor(V // 2, 9)
+    X, Y = oracle_mod.force_fields(dims, AP, U, Xe, kappa, mu)
+    M = lu.dense_m(dims, AP, U, kappa, mu)
+    MX = (M @ X.ravel()).reshape(V, 4, 3)
+    MdY = (M.conj().T @ Y.ravel()).reshape(V, 4, 3)
+    assert np.array_equal(lu.to_half(dims, X, 0), Xe)
+    assert np.linalg.norm(lu.to_half(dims, MX, 1)) < 1e-14 * np.linalg.norm(X)
+    assert lu.rel_err(lu.to_half(dims, MX, 0), lu.to_half(dims, Y, 0)) < 1e-14
+    assert lu.rel_err(lu.to_half(dims, Y, 0).ravel(), lu.dense_mhat(dims, AP, U, kappa, mu) @ Xe.ravel()) < 1e-14
+    assert np.linalg.norm(lu.to_half(dims, MdY, 1)) < 1e-14 * np.linalg.norm(Y)
+
+
+def test_p10_force_gauge_covariance(oracle_mod):
+    # U' = g U g^dag(x+mu), X' = g X, Y' = g Y  =>  F'^a T^a = g(x) (F^a T^a) g(x)^dag
+    dims = (4, 2, 2, 4)
+    kappa = 0.15
+    V = lu.volume(dims)
+    U = gen.gauge_haar(dims, SEED)
+    g = gen.su3_haar(V, SEED, gen.STREAM_GTRANS)
+    X, Y = _rand_spinor(V, 7), _rand_spinor(V, 8)
+    F = oracle_mod.fermion_force(dims, AP, U, X, Y, kappa)
+    Up = _gauge_transform(dims, U, g)
+    Fp = oracle_mod.fermion_force(dims, AP, Up, lu.apply_colour(g, X), lu.apply_colour(g, Y), kappa)
+    want = np.einsum("sab,smbc,sdc->smad", g, lu.algebra_matrix(F), g.conj())
+    assert lu.rel_err(lu.algebra_matrix(Fp), want) < 1e-14
