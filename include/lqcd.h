@@ -139,6 +139,29 @@ int lqcd_cg_finish(void);
 int lqcd_bicgstab_mhat(const void* gauge, const void* b, void* x, double kappa, double mu, double tol,
                        int maxit);
 
+/* Fermion force of the HMC (eq. 9-10: F = -dS/dU, a real 8-vector per link,
+ * PAPER.md:106, :255; reading G16 of DESIGN.md).  Components are
+ * taken along T^a = lambda^a / 2 (Gell-Mann matrices in the standard order) with the link varied
+ * from the left, U_mu(x) -> exp(i w T^a) U_mu(x), F^a_mu(x) = -dS/dw at w = 0.
+ *
+ * lqcd_fermion_force: the outer-product kernel for two spinor fields X, Y on the WHOLE lattice,
+ * given as even and odd half fields (internal layout, current format):
+ *   F^a_mu(x) = 2 Re d/dw [Y^dag M(w) X] = 2 kappa Im [ Y(x)^dag T^a a(x) - b(x)^dag T^a X(x) ],
+ *   a(x) = eta+_mu(x) (1 - gamma_mu) U_mu(x) X(x+mu),  b(x) = eta+_mu(x) (1 + gamma_mu) U_mu(x) Y(x+mu).
+ * force: lqcd_force_bytes() bytes, internal layout, always double; lqcd_unpack_force converts to
+ * the canonical double F[lex(x)][mu][8] (64 B per link, 256 B per site: Table 3).  Asynchronous.
+ *
+ * lqcd_force_tm: the whole force of S = phi^dag (Mhat^dag Mhat)^-1 phi, phi on even sites:
+ * X_e = (Mhat^dag Mhat)^-1 phi by CG (tol, maxit as in lqcd_cg_mdagm), Y_e = Mhat X_e,
+ * X_o = -M_oo^-1 D_oe X_e, Y_o = -(M_oo^-1)^dag (D_eo)^dag Y_e, then the kernel above.
+ * Returns the CG status; synchronous; uses six half spinors of library workspace. */
+size_t lqcd_force_bytes(void);
+int lqcd_unpack_force(const void* force_internal_dev, void* canon_dev);
+int lqcd_fermion_force(const void* gauge, const void* x_even, const void* x_odd, const void* y_even,
+                       const void* y_odd, void* force, double kappa);
+int lqcd_force_tm(const void* gauge, const void* phi, void* force, double kappa, double mu, double tol,
+                  int maxit);
+
 /* Mixed-precision solve of the same system (the paper's planned next step, PAPER.md:352;
  * SURVEY.md section 8(f) row 1): defect correction with the outer residual in double and the
  * inner CG in single precision,
@@ -174,7 +197,8 @@ long long lqcd_launch_count(void);
  * stops.  lqcd_profile_read synchronises the stream and returns the summed duration and the
  * launch count of one category: 0 hopping (plain epilogue), 1 hopping + M_ee*aux epilogue,
  * 2 hopping + M_ee*aux epilogue + fused norm, 3 CG vector kernels, 4 pack/unpack,
- * 5 hopping + M_ee*aux epilogue + fused CG residual update (r -= alpha q, |r|^2). */
+ * 5 hopping + M_ee*aux epilogue + fused CG residual update (r -= alpha q, |r|^2),
+ * 6 fermion-force kernel. */
 int lqcd_profile(int enable);
 int lqcd_profile_read(int category, double* total_ms, int* launches);
 

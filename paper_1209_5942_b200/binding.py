@@ -21,7 +21,7 @@ SYMBOLS = [
     "lqcd_last_error", "lqcd_init", "lqcd_finalize", "lqcd_set_stream", "lqcd_set_format",
     "lqcd_gauge_bytes", "lqcd_spinor_bytes", "lqcd_pack_gauge", "lqcd_pack_spinor",
     "lqcd_unpack_spinor", "lqcd_dslash_eo", "lqcd_mtm", "lqcd_mtm_full", "lqcd_solve_full", "lqcd_cg_mdagm", "lqcd_cg_setup",
-    "lqcd_cg_iterate", "lqcd_cg_finish", "lqcd_cg_stats", "lqcd_cg_mdagm_mixed", "lqcd_cg_outer_iterations", "lqcd_bicgstab_mhat", "lqcd_mtm_host", "lqcd_cg_mdagm_host",
+    "lqcd_cg_iterate", "lqcd_cg_finish", "lqcd_cg_stats", "lqcd_cg_mdagm_mixed", "lqcd_cg_outer_iterations", "lqcd_bicgstab_mhat", "lqcd_force_bytes", "lqcd_unpack_force", "lqcd_fermion_force", "lqcd_force_tm", "lqcd_mtm_host", "lqcd_cg_mdagm_host",
     "lqcd_launch_count", "lqcd_set_block_size", "lqcd_profile", "lqcd_profile_read",
 ]
 
@@ -41,6 +41,7 @@ def _load():
     lib.lqcd_last_error.restype = ctypes.c_char_p
     lib.lqcd_gauge_bytes.restype = ctypes.c_size_t
     lib.lqcd_spinor_bytes.restype = ctypes.c_size_t
+    lib.lqcd_force_bytes.restype = ctypes.c_size_t
     lib.lqcd_launch_count.restype = ctypes.c_longlong
     sig = {
         "lqcd_init": [ctypes.POINTER(i32), ctypes.POINTER(dbl)],
@@ -56,6 +57,9 @@ def _load():
         "lqcd_solve_full": [vp, vp, vp, vp, vp, dbl, dbl, dbl, i32],
         "lqcd_cg_mdagm": [vp, vp, vp, dbl, dbl, dbl, i32],
         "lqcd_bicgstab_mhat": [vp, vp, vp, dbl, dbl, dbl, i32],
+        "lqcd_unpack_force": [vp, vp],
+        "lqcd_fermion_force": [vp, vp, vp, vp, vp, vp, dbl],
+        "lqcd_force_tm": [vp, vp, vp, dbl, dbl, dbl, i32],
         "lqcd_cg_setup": [vp, vp, vp, dbl, dbl, dbl],
         "lqcd_cg_mdagm_mixed": [vp, i32, vp, i32, vp, vp, dbl, dbl, dbl, i32, dbl],
         "lqcd_cg_outer_iterations": [],
@@ -191,6 +195,23 @@ def lqcd_bicgstab_mhat(gauge, b, x, kappa, mu, tol, maxit):
     return _check(_lib.lqcd_bicgstab_mhat(_ptr(gauge), _ptr(b), _ptr(x), kappa, mu, tol, maxit))
 
 
+def lqcd_force_bytes():
+    return int(_lib.lqcd_force_bytes())
+
+
+def lqcd_unpack_force(force_internal_dev, canon_dev):
+    return _check(_lib.lqcd_unpack_force(_ptr(force_internal_dev), _ptr(canon_dev)))
+
+
+def lqcd_fermion_force(gauge, x_even, x_odd, y_even, y_odd, force, kappa):
+    return _check(_lib.lqcd_fermion_force(_ptr(gauge), _ptr(x_even), _ptr(x_odd), _ptr(y_even), _ptr(y_odd),
+                                          _ptr(force), kappa))
+
+
+def lqcd_force_tm(gauge, phi, force, kappa, mu, tol, maxit):
+    return _check(_lib.lqcd_force_tm(_ptr(gauge), _ptr(phi), _ptr(force), kappa, mu, tol, maxit))
+
+
 def lqcd_cg_mdagm_mixed(gauge_double, recon_double, gauge_single, recon_single, b, x, kappa, mu, tol, maxit,
                         inner_tol=0.0):
     return _check(_lib.lqcd_cg_mdagm_mixed(_ptr(gauge_double), recon_double, _ptr(gauge_single), recon_single,
@@ -240,6 +261,18 @@ def alloc_gauge(device="cuda"):
 def alloc_spinor(device="cuda"):
     """Uninitialised device buffer for one internal half-spinor field (current format)."""
     return torch.empty(lqcd_spinor_bytes(), dtype=torch.uint8, device=device)
+
+
+def alloc_force(device="cuda"):
+    """Uninitialised device buffer for one internal force field (8 reals per link, double)."""
+    return torch.empty(lqcd_force_bytes(), dtype=torch.uint8, device=device)
+
+
+def download_force(f_internal):
+    """internal force field -> numpy (V,4,8) float64."""
+    canon = torch.empty((2 * _fmt["vh"], 4, 8), dtype=torch.float64, device=f_internal.device)
+    lqcd_unpack_force(f_internal, canon)
+    return canon.cpu().numpy()
 
 
 def upload_gauge(U_canon, device="cuda"):

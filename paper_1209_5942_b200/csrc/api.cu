@@ -198,6 +198,21 @@ int check_scalar(double v, const char* name) {
 // direction opposite to the launch before it.
 int next_reverse() { return ctx.snake ^= 1; }
 
+// The first hopping launch of Mhat (dagger = 0) or Mhat^dag (dagger = 1): even -> odd,
+//   out_odd = M_oo^-1 D_oe in           (dagger = 0)
+//   out_odd = (M_oo^-1)^dag (D_eo)^dag in   (dagger = 1; adjoint stencil, c -> -c)
+int hop_minv(int precision, int recon, const void* gauge, const void* in, void* out_odd, double kappa,
+             double mu, int dagger, CgScalars* scal) {
+    const double c = (dagger ? -1.0 : 1.0) * 2.0 * kappa * mu;
+    const double d = 1.0 + c * c;
+    Epilogue e1 = {};
+    e1.cu_re = -kappa / d; e1.cu_im = +kappa * c / d;   // -kappa (1 - i c)/(1 + c^2), chi = +1
+    e1.cd_re = -kappa / d; e1.cd_im = -kappa * c / d;   // chi = -1
+    CU(launch_hopping(precision, recon, dagger, 0, ctx.geo, e1, gauge, in, out_odd, nullptr, 1,
+                      next_reverse(), red(), scal, ctx.block, ctx.stream));
+    return LQCD_OK;
+}
+
 // The two hopping launches of Mhat (dagger = 0) or Mhat^dag (dagger = 1) on even half fields.
 // fuse = FUSE_PAP: also reduce |out|^2 into scal->pAp (CG's <p, A p> = |Mhat p|^2).
 // fuse = FUSE_R:   `out` is CG's residual r; instead of storing Mhat^(dag) in, the second launch
@@ -207,12 +222,8 @@ enum { FUSE_NONE = 0, FUSE_PAP = 1, FUSE_R = 2 };
 int apply_mhat(int precision, int recon, const void* gauge, const void* in, void* tmp_odd, void* out,
                double kappa, double mu, int dagger, int fuse, CgScalars* scal) {
     const double c = (dagger ? -1.0 : 1.0) * 2.0 * kappa * mu;
-    const double d = 1.0 + c * c;
-    Epilogue e1 = {};
-    e1.cu_re = -kappa / d; e1.cu_im = +kappa * c / d;   // -kappa (1 - i c)/(1 + c^2), chi = +1
-    e1.cd_re = -kappa / d; e1.cd_im = -kappa * c / d;   // chi = -1
-    CU(launch_hopping(precision, recon, dagger, 0, ctx.geo, e1, gauge, in, tmp_odd, nullptr, 1,
-                      next_reverse(), red(), scal, ctx.block, ctx.stream));
+    int rc = hop_minv(precision, recon, gauge, in, tmp_odd, kappa, mu, dagger, scal);
+    if (rc) return rc;
     // out = (1 + i c chi) in + kappa * bracket(t) = k2 * (bracket(t) + [(1 + i c chi)/k2] in).
     // For kappa = 0 launch 1 wrote t = 0 exactly, so bracket(t) = 0 and any k2 != 0 is exact.
     const double k2 = (kappa != 0.0) ? kappa : 1.0;
@@ -619,6 +630,54 @@ int lqcd_bicgstab_mhat(const void* gauge, const void* b, void* x, double kappa, 
     ctx.st_rt = sc.bb > 0 ? std::sqrt(sc.resid_true / sc.bb) : 0.0;
     if (sc.status == LQCD_BREAKDOWN) return fail(LQCD_BREAKDOWN, "BiCGStab breakdown after %d iterations", sc.iters);
     return sc.status;
+}
+
+size_t lqcd_force_bytes(void) { return ctx.init ? (size_t)ctx.geo.G * 32 * 2 * 4 * 8 * sizeof(double) : 0; }
+
+int lqcd_unpack_force(const void* force_internal_dev, void* canon_dev) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (!force_internal_dev || !canon_dev) return fail(LQCD_BAD_ARG, "lqcd_unpack_force: null pointer");
+    CU(launch_unpack_force(ctx.geo, force_internal_dev, canon_dev, ctx.stream));
+    return LQCD_OK;
+}
+
+int lqcd_fermion_force(const void* gauge, const void* x_even, const void* x_odd, const void* y_even,
+                       const void* y_odd, void* force, double kappa) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (!gauge || !x_even || !x_odd || !y_even || !y_odd || !force) return fail(LQCD_BAD_ARG, "lqcd_fermion_force: null pointer");
+    int rc = check_scalar(kappa, "kappa");
+    if (rc) return rc;
+    CU(launch_fermion_force(ctx.precision, ctx.recon, ctx.geo, gauge, x_even, x_odd, y_even, y_odd, force, kappa,
+                            1.0, 1.0, ctx.stream));
+    return LQCD_OK;
+}
+
+// Force of S = phi^dag (Mhat^dag Mhat)^-1 phi (reading G16):
+//   X_e = (Mhat^dag Mhat)^-1 phi (CG);  Y_e = Mhat X_e, whose first hopping launch leaves
+//   t1 = M_oo^-1 D_oe X_e = -X_o;  t2 = (M_oo^-1)^dag (D_eo)^dag Y_e = -Y_o (the first launch of
+//   Mhat^dag on Y_e);  the force kernel takes the two signs as arguments.
+int lqcd_force_tm(const void* gauge, const void* phi, void* force, double kappa, double mu, double tol,
+                  int maxit) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (!gauge || !phi || !force) return fail(LQCD_BAD_ARG, "lqcd_force_tm: null pointer");
+    if (maxit < 1) return fail(LQCD_BAD_ARG, "maxit must be >= 1");
+    int rc = check_scalar(kappa, "kappa");
+    if (rc) return rc;
+    if ((rc = check_scalar(mu, "mu"))) return rc;
+    if (!std::isfinite(tol) || tol < 0.0) return fail(LQCD_BAD_ARG, "tol must be finite and >= 0");
+    const int pr = ctx.precision;
+    if ((rc = ensure_workspace(pr, 6))) return rc;
+    void** w = ctx.vec[pr];
+    void *ye = w[2], *t1 = w[3], *t2 = w[4], *xe = w[5];
+    if ((rc = cg_setup_impl(pr, ctx.recon, gauge, phi, xe, kappa, mu, tol))) return rc;
+    if ((rc = cg_run_impl(maxit))) return rc;
+    const int status = cg_finish_impl(true);
+    if (status < 0) return status;
+    if ((rc = apply_mhat(pr, ctx.recon, gauge, xe, t1, ye, kappa, mu, 0, FUSE_NONE, nullptr))) return rc;
+    if ((rc = hop_minv(pr, ctx.recon, gauge, ye, t2, kappa, mu, 1, nullptr))) return rc;
+    CU(launch_fermion_force(pr, ctx.recon, ctx.geo, gauge, xe, t1, ye, t2, force, kappa, -1.0, -1.0, ctx.stream));
+    CU(cudaStreamSynchronize(ctx.stream));
+    return status;
 }
 
 // Mixed-precision defect correction:

@@ -129,6 +129,15 @@ cudaError_t launch_pack_spinor(int precision, const Geometry& g, const void* can
 cudaError_t launch_unpack_spinor(int precision, const Geometry& g, const void* internal, void* canon,
                                  int parity, cudaStream_t st);
 
+// force.cu: F^a_mu(x) for every link from full-lattice X, Y given as half fields; the odd halves
+// handed in are sx_odd * X_o and sy_odd * Y_o (signs +-1).  force: double2 f[2][4][G][4][32],
+// element j of a link = (F^{2j+1}, F^{2j+2}); always double.
+cudaError_t launch_fermion_force(int precision, int recon, const Geometry& g, const void* gauge,
+                                 const void* x_even, const void* x_odd, const void* y_even,
+                                 const void* y_odd, void* force, double kappa, double sx_odd, double sy_odd,
+                                 cudaStream_t st);
+cudaError_t launch_unpack_force(const Geometry& g, const void* force, void* canon, cudaStream_t st);
+
 void count_launch(int n = 1);
 
 // api.cu: optional per-launch event timing (lqcd_profile)

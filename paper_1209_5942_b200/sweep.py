@@ -2,7 +2,7 @@
 """sweep.py -- timings of the BASELINE.json configurations 3, 4, 5 and of the paper's thermal
 lattice shapes (Fig. 7), one JSON line each.  A user-facing companion of bench.py:
 
-    python -m paper_1209_5942_b200.sweep [--configs 3,4,5,thermal] [--out FILE]
+    python -m paper_1209_5942_b200.sweep [--configs 3,4,5,thermal,force] [--out FILE]
 
 config 3: 16^3x32, near-identity links, kappa=.16 mu=.05: 10 warm-up + 100 timed D_eo/D_oe
           applications, 5 repeats, median (working set fits L2: not a HBM roofline figure)
@@ -10,6 +10,7 @@ config 4: 24^3x48 Haar links: CG on Mhat^dag Mhat to 1e-10; iterations, time to 
           per-iteration split between hopping launches and vector kernels
 config 5: 32^3x64, double/single x 18/12-real links: 20 warm-up + 200 timed D-slash applications
 thermal : N_sigma in {16,24,32,48} x N_tau in {4,8,12,16}, double/18 D-slash
+force   : the fermion-force kernel at 32^3x64 in the four storage variants
 
 GFLOPS at 1320 flop per output site (BASELINE metric); "gbs_effective" counts the algorithmic
 bytes (each link, each input site and each output once); "gbs_paper_accounting" counts the
@@ -176,6 +177,48 @@ def config5(stream):
     return out
 
 
+def force(stream):
+    """Fermion-force kernel at 32^3x64: one launch computes all 4 V links.
+    Algorithmic bytes per site of V: 4 links + X + Y (each site once) + 4 x 8 force reals."""
+    dims = (32, 32, 32, 64)
+    V = int(np.prod(dims))
+    U = gen.gauge_haar(dims)
+    out = []
+    for precision, recon in ((0, 18), (0, 12), (1, 18), (1, 12)):
+        B.lqcd_init(dims, gen.antiperiodic_t())
+        B.lqcd_set_format(precision, recon)
+        B.lqcd_set_stream(stream)
+        with torch.cuda.stream(stream):
+            g = B.upload_gauge(U)
+            f = B.alloc_force()
+            h = [B.upload_spinor(gen.spinor_gaussian(V // 2, stream=10 + i), i % 2) for i in range(4)]
+            for _ in range(10):
+                B.lqcd_fermion_force(g, h[0], h[1], h[2], h[3], f, 0.15)
+            times = []
+            for _ in range(3):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                stream.synchronize()
+                e0.record(stream)
+                for _ in range(100):
+                    B.lqcd_fermion_force(g, h[0], h[1], h[2], h[3], f, 0.15)
+                e1.record(stream)
+                stream.synchronize()
+                times.append(e0.elapsed_time(e1) / 100)
+        B.lqcd_finalize()
+        ms = float(np.median(times))
+        real = 8 if precision == 0 else 4
+        bytes_site = 4 * recon * real + 2 * 24 * real + 4 * 8 * 8
+        paper_bytes = 4 * (2 * recon * real + 4 * 24 * real + 2 * 8 * 8)   # PAPER.md:236 accounting (4736 in double/18)
+        peak = measured_peak()
+        gbs = V * bytes_site / ms / 1e6
+        out.append({"config": "force", "kernel": "fermion_force", "lattice": list(dims),
+                    "precision": "double" if precision == 0 else "single", "recon": recon,
+                    "us_per_launch": ms * 1e3, "links_per_s": 4 * V / ms * 1e3, "bytes_per_site": bytes_site,
+                    "gbs_effective": gbs, "gbs_paper_accounting": V * paper_bytes / ms / 1e6,
+                    "frac_of_measured_peak": gbs / peak, "measured_peak_gbs": peak})
+    return out
+
+
 def thermal(stream):
     out = []
     for ns in (16, 24, 32, 48):
@@ -196,7 +239,7 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("sweep.py needs a CUDA device: there is no CPU fallback")
     stream = torch.cuda.Stream()
-    table = {"3": config3, "4": config4, "5": config5, "thermal": thermal}
+    table = {"3": config3, "4": config4, "5": config5, "thermal": thermal, "force": force}
     lines = []
     for key in args.configs.split(","):
         for r in table[key.strip()](stream):

@@ -551,3 +551,134 @@ def test_solve_full_residual_under_oracle_operator(B, oracle_mod, dims):
     # kappa = 0: M is site diagonal, no iteration needed
     st, psi = _full_solve(B, L, dims, eta, 0.0, 0.3, tol, 10)
     assert st == 0 and lu.rel_err(oracle_mod.m_full(dims, AP, U, psi, 0.0, 0.3), eta) < 1e-14
+
+
+# --------------------------------------------------------------------------- fermion force
+def _gpu_force(B, dims, phases, U, X, Y, kappa, precision=0, recon=18):
+    L = Lat(B, dims, phases, U, precision, recon)
+    xe, xo = B.upload_spinor(lu.to_half(dims, X, 0), 0), B.upload_spinor(lu.to_half(dims, X, 1), 1)
+    ye, yo = B.upload_spinor(lu.to_half(dims, Y, 0), 0), B.upload_spinor(lu.to_half(dims, Y, 1), 1)
+    f = B.alloc_force()
+    B.lqcd_fermion_force(L.g, xe, xo, ye, yo, f, kappa)
+    return B.download_force(f)
+
+
+@pytest.mark.parametrize("dims,phases", [
+    ((4, 4, 4, 4), AP),
+    ((2, 2, 2, 2), GENERIC_PH),    # every forward hop in a 2-extent direction from x_mu = 1 wraps
+    ((4, 6, 2, 8), GENERIC_PH),
+    ((6, 4, 10, 4), AP),           # Vh = 480: a ragged last group of 32 sites
+    ((8, 8, 8, 16), AP),
+])
+@pytest.mark.parametrize("precision,recon,tol", [(0, 18, TOL_D), (0, 12, TOL_D), (1, 18, TOL_S), (1, 12, TOL_S)])
+def test_fermion_force_matches_oracle(B, oracle_mod, dims, phases, precision, recon, tol):
+    kappa = 0.15
+    V = lu.volume(dims)
+    U = gen.gauge_haar(dims, SEED)
+    X = gen.spinor_gaussian(V, SEED, 7)
+    Y = gen.spinor_gaussian(V, SEED, 8)
+    Ur, Xr = _round_inputs(U, X, precision)
+    _, Yr = _round_inputs(U, Y, precision)
+    want = oracle_mod.fermion_force(dims, phases, Ur, Xr, Yr, kappa)
+    got = _gpu_force(B, dims, phases, U, X, Y, kappa, precision, recon)
+    assert got.shape == want.shape == (V, 4, 8)
+    assert lu.rel_err(got, want) <= tol
+    assert np.max(np.abs(got - want)) <= 10 * tol * np.max(np.abs(want))
+
+
+def test_fermion_force_gauge_covariance_on_gpu(B):
+    # F'^a T^a = g(x) (F^a T^a) g(x)^dag under U' = g U g^dag(x+mu), X' = g X, Y' = g Y -- no oracle involved
+    dims = (8, 8, 8, 16)
+    kappa = 0.15
+    V = lu.volume(dims)
+    U = gen.gauge_haar(dims, SEED)
+    g = gen.su3_haar(V, SEED, gen.STREAM_GTRANS)
+    X, Y = gen.spinor_gaussian(V, SEED, 7), gen.spinor_gaussian(V, SEED, 8)
+    F = _gpu_force(B, dims, AP, U, X, Y, kappa)
+    Xc = lu.site_coords(dims)
+    Up = np.empty_like(U)
+    for m in range(4):
+        Yc = Xc.copy()
+        Yc[:, m] = (Yc[:, m] + 1) % dims[m]
+        Up[:, m] = np.einsum("sab,sbc,sdc->sad", g, U[:, m], g[lu.lex_index(dims, Yc)].conj())
+    Fp = _gpu_force(B, dims, AP, Up, lu.apply_colour(g, X), lu.apply_colour(g, Y), kappa)
+    want = np.einsum("sab,smbc,sdc->smad", g, lu.algebra_matrix(F), g.conj())
+    assert lu.rel_err(lu.algebra_matrix(Fp), want) < 1e-13
+
+
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (8, 8, 8, 16)])
+def test_force_tm_matches_oracle(B, oracle_mod, dims):
+    # the whole force of S = phi^dag (Mhat^dag Mhat)^-1 phi: CG + odd-site fields + outer product
+    kappa, mu, tol = 0.15, 0.1, 1e-12
+    U = gen.gauge_haar(dims, SEED)
+    phi = gen.spinor_gaussian(lu.volume(dims) // 2, SEED, gen.STREAM_SOURCE)
+    st_o, want, it_o = oracle_mod.force_tm(dims, AP, U, phi, kappa, mu, tol, 2000)
+    L = Lat(B, dims, AP, U)
+    src = B.upload_spinor(phi, 0)
+    f = B.alloc_force()
+    st = B.lqcd_force_tm(L.g, src, f, kappa, mu, tol, 2000)
+    iters, rr, rt = B.lqcd_cg_stats()
+    got = B.download_force(f)
+    assert st == 0 and st_o == 0 and abs(iters - it_o) <= 2
+    # both solves stop at |r| <= tol |phi|; the force is bilinear in the solution: 2 sqrt(cond) tol of slack
+    assert lu.rel_err(got, want) <= 100 * tol
+    assert np.max(np.abs(want)) > 1e-3
+
+
+def test_force_tm_is_minus_the_action_derivative_on_gpu(B):
+    # independent of the oracle: central differences of S from the dense Schur complement (numpy)
+    dims = (2, 2, 2, 2)
+    kappa, mu, h = 0.15, 0.1, 1e-4
+    V = lu.volume(dims)
+    U = gen.gauge_haar(dims, SEED)
+    phi = gen.spinor_gaussian(V // 2, SEED, gen.STREAM_SOURCE)
+    L = Lat(B, dims, AP, U)
+    f = B.alloc_force()
+    assert B.lqcd_force_tm(L.g, B.upload_spinor(phi, 0), f, kappa, mu, 1e-13, 500) == 0
+    F = B.download_force(f)
+
+    def action(Uv):
+        S = lu.dense_mhat(dims, AP, Uv, kappa, mu)
+        return np.real(np.vdot(phi.ravel(), np.linalg.solve(S.conj().T @ S, phi.ravel())))
+
+    for s, m in [(0, 3), (V - 1, 3), (5, 0), (10, 1), (7, 2)]:
+        for a in range(8):
+            Up, Um = U.copy(), U.copy()
+            Up[s, m] = lu.exp_i_w_T(a, h) @ U[s, m]
+            Um[s, m] = lu.exp_i_w_T(a, -h) @ U[s, m]
+            fd = -(action(Up) - action(Um)) / (2 * h)
+            assert abs(F[s, m, a] - fd) < 1e-6 * max(1.0, abs(fd))
+
+
+def test_force_edge_cases(B):
+    dims = (4, 4, 4, 4)
+    U = gen.gauge_haar(dims, SEED)
+    L = Lat(B, dims, AP, U)
+    V = lu.volume(dims)
+    assert B.lqcd_force_bytes() == V * 4 * 8 * 8         # 256 B per site
+    zero = np.zeros((V // 2, 4, 3), dtype=complex)
+    f = B.alloc_force()
+    assert B.lqcd_force_tm(L.g, B.upload_spinor(zero, 0), f, 0.15, 0.1, 1e-10, 50) == 0
+    assert np.all(B.download_force(f) == 0)                # phi = 0 -> X = Y = 0 -> F = 0
+    phi = gen.spinor_gaussian(V // 2, SEED, gen.STREAM_SOURCE)
+    assert B.lqcd_force_tm(L.g, B.upload_spinor(phi, 0), f, 0.0, 0.1, 1e-10, 50) == 0
+    assert np.all(B.download_force(f) == 0)                # kappa = 0 -> no hopping term -> F = 0
+    with pytest.raises(B.LqcdError) as e:
+        B.lqcd_fermion_force(L.g, 0, f, f, f, f, 0.1)
+    assert e.value.status == B.LQCD_BAD_ARG
+
+
+def test_fermion_force_full_size_sampled_links(B, oracle_mod):
+    # BASELINE config 5 lattice: 300 sampled links through the oracle's link-wise evaluator
+    dims = (32, 32, 32, 64)
+    kappa = 0.15
+    V = lu.volume(dims)
+    U = gen.gauge_haar(dims, SEED)
+    X, Y = gen.spinor_gaussian(V, SEED, 7), gen.spinor_gaussian(V, SEED, 8)
+    got = _gpu_force(B, dims, AP, U, X, Y, kappa)
+    rng = np.random.default_rng(11)
+    sites = np.concatenate([rng.integers(0, V, 290), [0, 1, V - 1, V - 2, V // 2, 31, 32, 1023, 32767, V - 32 * 32 * 32]])
+    mus = np.concatenate([rng.integers(0, 4, 290), [0, 1, 2, 3, 0, 0, 1, 2, 3, 3]])
+    want = oracle_mod.fermion_force_links(dims, AP, U, X, Y, sites, mus, kappa)
+    assert lu.rel_err(got[sites, mus], want) <= TOL_D
+    assert np.all(np.isfinite(got))
