@@ -367,6 +367,9 @@ int lqcd_init(const int dims[4], const double bc_phase[8]) {
         ctx.geo.ph_im[m] = bc_phase[2 * m + 1];
     }
     ctx.geo.N0h = dims[0] / 2; ctx.geo.N1 = dims[1]; ctx.geo.N2 = dims[2]; ctx.geo.N3 = dims[3];
+    ctx.geo.d0h = make_fastdiv((unsigned)ctx.geo.N0h);
+    ctx.geo.d1 = make_fastdiv((unsigned)ctx.geo.N1);
+    ctx.geo.d2 = make_fastdiv((unsigned)ctx.geo.N2);
     ctx.geo.Vh = (int)(V / 2);
     ctx.geo.G = (ctx.geo.Vh + 31) / 32;
     ctx.precision = LQCD_DOUBLE; ctx.recon = 18; ctx.block = 128; ctx.stream = 0;
@@ -648,14 +651,14 @@ int lqcd_fermion_force(const void* gauge, const void* x_even, const void* x_odd,
     int rc = check_scalar(kappa, "kappa");
     if (rc) return rc;
     CU(launch_fermion_force(ctx.precision, ctx.recon, ctx.geo, gauge, x_even, x_odd, y_even, y_odd, force, kappa,
-                            1.0, 1.0, ctx.stream));
+                            ctx.stream));
     return LQCD_OK;
 }
 
 // Force of S = phi^dag (Mhat^dag Mhat)^-1 phi (reading G16):
 //   X_e = (Mhat^dag Mhat)^-1 phi (CG);  Y_e = Mhat X_e, whose first hopping launch leaves
 //   t1 = M_oo^-1 D_oe X_e = -X_o;  t2 = (M_oo^-1)^dag (D_eo)^dag Y_e = -Y_o (the first launch of
-//   Mhat^dag on Y_e);  the force kernel takes the two signs as arguments.
+//   Mhat^dag on Y_e);  the common sign is handed to the force kernel as the sign of kappa.
 int lqcd_force_tm(const void* gauge, const void* phi, void* force, double kappa, double mu, double tol,
                   int maxit) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
@@ -675,7 +678,9 @@ int lqcd_force_tm(const void* gauge, const void* phi, void* force, double kappa,
     if (status < 0) return status;
     if ((rc = apply_mhat(pr, ctx.recon, gauge, xe, t1, ye, kappa, mu, 0, FUSE_NONE, nullptr))) return rc;
     if ((rc = hop_minv(pr, ctx.recon, gauge, ye, t2, kappa, mu, 1, nullptr))) return rc;
-    CU(launch_fermion_force(pr, ctx.recon, ctx.geo, gauge, xe, t1, ye, t2, force, kappa, -1.0, -1.0, ctx.stream));
+    // every term of the force holds exactly one odd-site field (X(x+mu) Y(x) or X(x) Y(x+mu) with x, x+mu of
+    // opposite parity), so handing in t1 = -X_o and t2 = -Y_o flips the sign of the whole force: kappa -> -kappa
+    CU(launch_fermion_force(pr, ctx.recon, ctx.geo, gauge, xe, t1, ye, t2, force, -kappa, ctx.stream));
     CU(cudaStreamSynchronize(ctx.stream));
     return status;
 }

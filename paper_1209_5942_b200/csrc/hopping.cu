@@ -90,11 +90,8 @@ hopping_kernel(const HopArgs a) {
     if (e < Vh) {
         // a1: e -> (x0h, x1, x2, x3); r = x0 mod 2 follows from the parity
         const int N0h = a.g.N0h, N1 = a.g.N1, N2 = a.g.N2, N3 = a.g.N3;
-        int t = e;
-        const int x0h = t % N0h; t /= N0h;
-        const int x1 = t % N1;   t /= N1;
-        const int x2 = t % N2;
-        const int x3 = t / N2;
+        int x0h, x1, x2, x3;
+        site_coords(a.g, e, x0h, x1, x2, x3);
         const int r = (x1 + x2 + x3 + a.out_parity) & 1;
         const int s1 = N0h, s2 = N0h * N1, s3 = N0h * N1 * N2;
 

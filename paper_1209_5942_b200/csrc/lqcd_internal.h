@@ -25,12 +25,50 @@
 
 namespace lqcd {
 
+// Division of a site index by a lattice extent without the ~20-instruction
+// runtime integer division: for 2 <= d < 2^31, l = ceil(log2 d), mul = ceil(2^(31+l) / d) (< 2^32),
+//   n / d = umulhi(n, mul) >> (l - 1)   exactly for every 0 <= n < 2^31
+// (the rounding error n e / (d 2^(31+l)), e < d, is below 2^-l <= 1/d).  d = 1 is passed through.
+struct FastDiv {
+    unsigned d, mul, sh;
+};
+inline FastDiv make_fastdiv(unsigned d) {
+    FastDiv f;
+    f.d = d; f.mul = 0; f.sh = 0;
+    if (d < 2) return f;
+    unsigned l = 0;
+    while ((1ull << l) < d) ++l;
+    f.mul = (unsigned)(((1ull << (31 + l)) + d - 1) / d);
+    f.sh = l - 1;
+    return f;
+}
+#ifdef __CUDACC__
+__device__ __forceinline__ int fd_div(int n, const FastDiv& f) {
+    return f.d == 1 ? n : (int)(__umulhi((unsigned)n, f.mul) >> f.sh);
+}
+#endif
+
 struct Geometry {
     int N0h, N1, N2, N3;  // N0h = N_x / 2
     int Vh;               // sites per parity
     int G;                // groups of 32 sites per parity = ceil(Vh / 32)
+    FastDiv d0h, d1, d2;  // division by N0h, N1, N2
     double ph_re[4], ph_im[4];
 };
+
+#ifdef __CUDACC__
+// a1: eo index e -> (x0h, x1, x2, x3), e = x0h + N0h (x1 + N1 (x2 + N2 x3))
+__device__ __forceinline__ void site_coords(const Geometry& g, int e, int& x0h, int& x1, int& x2, int& x3) {
+    int q = fd_div(e, g.d0h);
+    x0h = e - q * g.N0h;
+    int t = q;
+    q = fd_div(t, g.d1);
+    x1 = t - q * g.N1;
+    t = q;
+    x3 = fd_div(t, g.d2);
+    x2 = t - x3 * g.N2;
+}
+#endif
 
 // Coefficients of the fused epilogue, per chirality (u: alpha = 0,1; d: alpha = 2,3):
 //   out = c_chi * (bracket + d_chi * aux)     bracket = the sum over 8 hops of eq. 6;
@@ -129,13 +167,12 @@ cudaError_t launch_pack_spinor(int precision, const Geometry& g, const void* can
 cudaError_t launch_unpack_spinor(int precision, const Geometry& g, const void* internal, void* canon,
                                  int parity, cudaStream_t st);
 
-// force.cu: F^a_mu(x) for every link from full-lattice X, Y given as half fields; the odd halves
-// handed in are sx_odd * X_o and sy_odd * Y_o (signs +-1).  force: double2 f[2][4][G][4][32],
-// element j of a link = (F^{2j+1}, F^{2j+2}); always double.
+// force.cu: F^a_mu(x) for every link from full-lattice X, Y given as half fields (the force is
+// linear in kappa, so a common sign of the odd halves is passed as the sign of kappa).
+// force: double2 f[2][4][G][4][32], element j of a link = (F^{2j+1}, F^{2j+2}); always double.
 cudaError_t launch_fermion_force(int precision, int recon, const Geometry& g, const void* gauge,
                                  const void* x_even, const void* x_odd, const void* y_even,
-                                 const void* y_odd, void* force, double kappa, double sx_odd, double sy_odd,
-                                 cudaStream_t st);
+                                 const void* y_odd, void* force, double kappa, cudaStream_t st);
 cudaError_t launch_unpack_force(const Geometry& g, const void* force, void* canon, cudaStream_t st);
 
 void count_launch(int n = 1);
