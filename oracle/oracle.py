@@ -12,6 +12,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "lqcd_oracle.cpp")
+_SRC_GAUGE = os.path.join(_HERE, "gauge_oracle.cpp")
 _LIB = os.path.join(_HERE, "liblqcd_oracle.so")
 _lib = None
 
@@ -22,10 +23,11 @@ _c_long_p = ctypes.POINTER(ctypes.c_long)
 
 def build(force=False):
     """Compile the oracle with g++ (-O2, no FMA contraction, OpenMP over sites)."""
-    if not force and os.path.exists(_LIB) and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC):
+    if not force and os.path.exists(_LIB) and os.path.getmtime(_LIB) >= max(os.path.getmtime(_SRC),
+                                                                            os.path.getmtime(_SRC_GAUGE)):
         return _LIB
     cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
-           "-Wall", "-o", _LIB, _SRC]
+           "-Wall", "-o", _LIB, _SRC, _SRC_GAUGE]
     subprocess.run(cmd, check=True)
     return _LIB
 
@@ -38,6 +40,7 @@ def _load():
         _lib.orc_cg_mdagm.restype = ctypes.c_int
         _lib.orc_bicgstab_mhat.restype = ctypes.c_int
         _lib.orc_num_threads.restype = ctypes.c_int
+        _lib.orc_plaquette.restype = ctypes.c_double
     return _lib
 
 
@@ -224,6 +227,69 @@ def force_tm(dims, bc_phase, U, phi_even, kappa, mu, tol, maxit):
     st, Xe, iters, rr, rt = cg_mdagm(dims, bc_phase, U, phi_even, kappa, mu, tol, maxit)
     X, Y = force_fields(dims, bc_phase, U, Xe, kappa, mu)
     return st, fermion_force(dims, bc_phase, U, X, Y, kappa), iters
+
+
+# ----------------------------------------------------------------------------- gauge_oracle.cpp
+def plaquette(dims, U):
+    """Average plaquette (1/3) Re tr P over the 6 V plaquettes."""
+    d = _dims(dims)
+    V = int(np.prod(d))
+    U = _c128(U, (V, 4, 3, 3))
+    return float(_load().orc_plaquette(_ip(d), _dp(U)))
+
+
+def staple(dims, U, site, mu):
+    """Staple sum A (3,3) of the link (lex site, mu): Re tr(U A) = sum over its 6 plaquettes."""
+    d = _dims(dims)
+    V = int(np.prod(d))
+    U = _c128(U, (V, 4, 3, 3))
+    A = np.empty((3, 3), dtype=np.complex128)
+    _load().orc_staple(_ip(d), _dp(U), ctypes.c_long(int(site)), ctypes.c_int(int(mu)), _dp(A))
+    return A
+
+
+def update_links(dims, U, sites, mus, mode, beta, seed, tag, subgroups=7):
+    """Fig. 2 for the listed links, each computed from the same input field: (n,3,3)."""
+    d = _dims(dims)
+    V = int(np.prod(d))
+    U = _c128(U, (V, 4, 3, 3))
+    sites = np.ascontiguousarray(sites, dtype=np.int64)
+    mus = np.ascontiguousarray(mus, dtype=np.int32)
+    assert sites.shape == mus.shape
+    out = np.empty((len(sites), 3, 3), dtype=np.complex128)
+    _load().orc_update_links(_ip(d), _dp(U), sites.ctypes.data_as(_c_long_p), _ip(mus), ctypes.c_long(len(sites)),
+                             ctypes.c_int(mode), ctypes.c_int(subgroups), ctypes.c_double(beta),
+                             ctypes.c_ulonglong(seed), ctypes.c_ulonglong(tag), _dp(out))
+    return out
+
+
+def gauge_subsweep(dims, U, mu, parity, mode, beta, seed, tag):
+    """Update every link U_mu(x), parity(x) = parity; returns the new field (input untouched)."""
+    d = _dims(dims)
+    V = int(np.prod(d))
+    U = _c128(U, (V, 4, 3, 3)).copy()
+    _load().orc_gauge_subsweep(_ip(d), _dp(U), ctypes.c_int(mu), ctypes.c_int(parity), ctypes.c_int(mode),
+                               ctypes.c_double(beta), ctypes.c_ulonglong(seed), ctypes.c_ulonglong(tag))
+    return U
+
+
+def gauge_sweep(dims, U, mode, beta, seed, tag):
+    """One sweep (mu = 0..3, parity 0 then 1); mode 0 heatbath, 1 overrelax; returns the new field."""
+    d = _dims(dims)
+    V = int(np.prod(d))
+    U = _c128(U, (V, 4, 3, 3)).copy()
+    _load().orc_gauge_sweep(_ip(d), _dp(U), ctypes.c_int(mode), ctypes.c_double(beta), ctypes.c_ulonglong(seed),
+                            ctypes.c_ulonglong(tag))
+    return U
+
+
+def kp_samples(lam, seed, tag, n):
+    """n Kennedy-Pendleton samples: (g (n,4), attempts (n,)); attempts 0 = all rejected."""
+    g = np.empty((n, 4), dtype=np.float64)
+    att = np.empty(n, dtype=np.int32)
+    _load().orc_kp_samples(ctypes.c_double(lam), ctypes.c_ulonglong(seed), ctypes.c_ulonglong(tag), ctypes.c_long(n),
+                           _dp(g), _ip(att))
+    return g, att
 
 
 def num_threads():
