@@ -162,6 +162,31 @@ int lqcd_fermion_force(const void* gauge, const void* x_even, const void* x_odd,
 int lqcd_force_tm(const void* gauge, const void* phi, void* force, double kappa, double mu, double tol,
                   int maxit);
 
+/* Pure-gauge heatbath and overrelaxation, the paper's second workload (Fig. 2;
+ * Table 2; readings G17-G21 of DESIGN.md), for the
+ * Wilson plaquette action S = beta sum_{x, mu<nu} (1 - Re tr P_mu_nu(x) / 3) (eq. 5 with c_1 = 0) on a
+ * periodic gauge field.  Per link, with A the sum of its 6 staples and for the SU(2)
+ * subgroups (0,1), (1,2), (0,2) in turn:  W = L A;  w = project(W);  v = update(w);  L = extend(v) L,
+ *   LQCD_HEATBATH : v w = g drawn with density sqrt(1 - g0^2) exp((2 beta k / 3) g0) (Kennedy-Pendleton,
+ *                   at most 32 attempts, else the subgroup is left unchanged), k^2 = det-like norm of w;
+ *   LQCD_OVERRELAX: v w = w^dag (the action is unchanged; beta, seed, tag are ignored).
+ * Random numbers: the counter-based generator of the input recipe, uniform(seed, stream = tag, counter),
+ * counter = (((4 lex(x) + mu) 3 + subgroup) 33 + attempt) 4 + j; tag < 2^24 must differ from sweep to sweep.
+ *
+ * lqcd_gauge_update: one sub-sweep, in place: every link U_mu(x) with parity(x) = parity (these links
+ *   are mutually independent).  gauge: internal layout of the current format.  Asynchronous.
+ * lqcd_gauge_sweep : the 8 sub-sweeps mu = 0..3, parity 0 then 1.  Asynchronous.
+ * lqcd_plaquette   : average of Re tr P / 3 over the 6 V plaquettes, written to a HOST double; synchronous.
+ * lqcd_unpack_gauge: internal -> canonical U[lex(x)][mu][a][b] (complex double; 12-real storage
+ *   rebuilds the third row).  Asynchronous. */
+#define LQCD_HEATBATH  0
+#define LQCD_OVERRELAX 1
+int lqcd_gauge_update(void* gauge, int mu, int parity, int mode, double beta, unsigned long long seed,
+                      unsigned long long tag);
+int lqcd_gauge_sweep(void* gauge, int mode, double beta, unsigned long long seed, unsigned long long tag);
+int lqcd_plaquette(const void* gauge, double* plaquette_host);
+int lqcd_unpack_gauge(const void* internal_dev, void* canon_dev);
+
 /* Mixed-precision solve of the same system (the paper's planned next step, PAPER.md:352;
  * SURVEY.md section 8(f) row 1): defect correction with the outer residual in double and the
  * inner CG in single precision,
@@ -198,7 +223,7 @@ long long lqcd_launch_count(void);
  * launch count of one category: 0 hopping (plain epilogue), 1 hopping + M_ee*aux epilogue,
  * 2 hopping + M_ee*aux epilogue + fused norm, 3 CG vector kernels, 4 pack/unpack,
  * 5 hopping + M_ee*aux epilogue + fused CG residual update (r -= alpha q, |r|^2),
- * 6 fermion-force kernel. */
+ * 6 fermion-force kernel, 7 gauge update (heatbath / overrelaxation sub-sweep), 8 plaquette. */
 int lqcd_profile(int enable);
 int lqcd_profile_read(int category, double* total_ms, int* launches);
 

@@ -16,6 +16,7 @@ _LIB_PATH = os.path.join(_HERE, "liblqcd.so")
 LQCD_OK, LQCD_NOT_CONVERGED = 0, 1
 LQCD_NOT_INITIALISED, LQCD_BAD_DIMS, LQCD_BAD_ARG, LQCD_CUDA_ERROR, LQCD_BREAKDOWN = -1, -2, -3, -4, -5
 LQCD_DOUBLE, LQCD_SINGLE = 0, 1
+LQCD_HEATBATH, LQCD_OVERRELAX = 0, 1
 
 SYMBOLS = [
     "lqcd_last_error", "lqcd_init", "lqcd_finalize", "lqcd_set_stream", "lqcd_set_format",
@@ -23,6 +24,7 @@ SYMBOLS = [
     "lqcd_unpack_spinor", "lqcd_dslash_eo", "lqcd_mtm", "lqcd_mtm_full", "lqcd_solve_full", "lqcd_cg_mdagm", "lqcd_cg_setup",
     "lqcd_cg_iterate", "lqcd_cg_finish", "lqcd_cg_stats", "lqcd_cg_mdagm_mixed", "lqcd_cg_outer_iterations", "lqcd_bicgstab_mhat", "lqcd_force_bytes", "lqcd_unpack_force", "lqcd_fermion_force", "lqcd_force_tm", "lqcd_mtm_host", "lqcd_cg_mdagm_host",
     "lqcd_launch_count", "lqcd_set_block_size", "lqcd_profile", "lqcd_profile_read",
+    "lqcd_gauge_update", "lqcd_gauge_sweep", "lqcd_plaquette", "lqcd_unpack_gauge",
 ]
 
 
@@ -37,7 +39,7 @@ def _load():
         raise ImportError(f"{_LIB_PATH} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
                           "(there is no CPU fallback)")
     lib = ctypes.CDLL(_LIB_PATH)
-    vp, dbl, i32 = ctypes.c_void_p, ctypes.c_double, ctypes.c_int
+    vp, dbl, i32, u64 = ctypes.c_void_p, ctypes.c_double, ctypes.c_int, ctypes.c_ulonglong
     lib.lqcd_last_error.restype = ctypes.c_char_p
     lib.lqcd_gauge_bytes.restype = ctypes.c_size_t
     lib.lqcd_spinor_bytes.restype = ctypes.c_size_t
@@ -69,6 +71,10 @@ def _load():
         "lqcd_mtm_host": [vp, vp, vp, dbl, dbl, i32],
         "lqcd_cg_mdagm_host": [vp, vp, vp, dbl, dbl, dbl, i32],
         "lqcd_set_block_size": [i32],
+        "lqcd_gauge_update": [vp, i32, i32, i32, dbl, u64, u64],
+        "lqcd_gauge_sweep": [vp, i32, dbl, u64, u64],
+        "lqcd_plaquette": [vp, ctypes.POINTER(dbl)],
+        "lqcd_unpack_gauge": [vp, vp],
         "lqcd_profile": [i32],
         "lqcd_profile_read": [i32, ctypes.POINTER(dbl), ctypes.POINTER(i32)],
     }
@@ -252,6 +258,24 @@ def lqcd_cg_mdagm_host(gauge_canon_host, b_canon_host, x_canon_host, kappa, mu, 
                                           kappa, mu, tol, maxit))
 
 
+def lqcd_gauge_update(gauge, mu, parity, mode, beta, seed, tag):
+    return _check(_lib.lqcd_gauge_update(_ptr(gauge), mu, parity, mode, beta, seed, tag))
+
+
+def lqcd_gauge_sweep(gauge, mode, beta, seed, tag):
+    return _check(_lib.lqcd_gauge_sweep(_ptr(gauge), mode, beta, seed, tag))
+
+
+def lqcd_plaquette(gauge):
+    p = ctypes.c_double(0.0)
+    _check(_lib.lqcd_plaquette(_ptr(gauge), ctypes.byref(p)))
+    return p.value
+
+
+def lqcd_unpack_gauge(internal_dev, canon_dev):
+    return _check(_lib.lqcd_unpack_gauge(_ptr(internal_dev), _ptr(canon_dev)))
+
+
 # ---------------------------------------------------------------------------- buffer helpers
 def alloc_gauge(device="cuda"):
     """Uninitialised device buffer for one internal gauge field (current format)."""
@@ -281,6 +305,13 @@ def upload_gauge(U_canon, device="cuda"):
     g = alloc_gauge(device)
     lqcd_pack_gauge(canon, g)
     return g
+
+
+def download_gauge(g_internal):
+    """packed internal gauge buffer -> numpy (V,4,3,3) complex128."""
+    canon = torch.empty((2 * _fmt["vh"], 4, 3, 3), dtype=torch.complex128, device=g_internal.device)
+    lqcd_unpack_gauge(g_internal, canon)
+    return canon.cpu().numpy()
 
 
 def upload_spinor(psi_canon, parity, device="cuda"):

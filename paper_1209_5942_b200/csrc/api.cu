@@ -155,7 +155,8 @@ int ensure_scalars() {
         for (int i = 0; i < 2; ++i) CU(cudaEventCreateWithFlags(&ctx.ev[i], cudaEventDisableTiming));
     }
     // one partial per warp of a hopping launch, or up to three per block of a vector kernel (BiCGStab)
-    const size_t need = (size_t)hopping_partials(ctx.geo.Vh, 32) + 3 * (size_t)vector_grid(n_reals()) + 64;
+    size_t need = (size_t)hopping_partials(ctx.geo.Vh, 32) + 3 * (size_t)vector_grid(n_reals()) + 64;
+    if (need < (size_t)plaquette_partials(ctx.geo.Vh)) need = (size_t)plaquette_partials(ctx.geo.Vh);
     if (need > ctx.n_partials) {
         if (ctx.partials) CU(cudaFree(ctx.partials));
         ctx.partials = nullptr;
@@ -437,6 +438,52 @@ int lqcd_pack_gauge(const void* canon_dev, void* internal_dev) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
     if (!canon_dev || !internal_dev) return fail(LQCD_BAD_ARG, "lqcd_pack_gauge: null pointer");
     CU(launch_pack_gauge(ctx.precision, ctx.recon, ctx.geo, canon_dev, internal_dev, ctx.stream));
+    return LQCD_OK;
+}
+
+int lqcd_unpack_gauge(const void* internal_dev, void* canon_dev) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (!canon_dev || !internal_dev) return fail(LQCD_BAD_ARG, "lqcd_unpack_gauge: null pointer");
+    CU(launch_unpack_gauge(ctx.precision, ctx.recon, ctx.geo, internal_dev, canon_dev, ctx.stream));
+    return LQCD_OK;
+}
+
+// ---- pure-gauge sector (gauge_update.cu): one launch per sub-sweep, 8 sub-sweeps per sweep
+int lqcd_gauge_update(void* gauge, int mu, int parity, int mode, double beta, unsigned long long seed,
+                      unsigned long long tag) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (!gauge) return fail(LQCD_BAD_ARG, "lqcd_gauge_update: null pointer");
+    if (mu < 0 || mu > 3) return fail(LQCD_BAD_ARG, "mu must be 0..3");
+    if (parity != 0 && parity != 1) return fail(LQCD_BAD_ARG, "parity must be 0 or 1");
+    if (mode != LQCD_HEATBATH && mode != LQCD_OVERRELAX) return fail(LQCD_BAD_ARG, "mode must be LQCD_HEATBATH or LQCD_OVERRELAX");
+    int rc = check_scalar(beta, "beta");
+    if (rc) return rc;
+    if (mode == LQCD_HEATBATH && !(beta > 0.0)) return fail(LQCD_BAD_ARG, "heatbath needs beta > 0");
+    if (tag >= (1ull << 24)) return fail(LQCD_BAD_ARG, "tag must be below 2^24");
+    CU(launch_gauge_update(ctx.precision, ctx.recon, mode, ctx.geo, gauge, mu, parity, beta, seed, tag, ctx.stream));
+    return LQCD_OK;
+}
+
+int lqcd_gauge_sweep(void* gauge, int mode, double beta, unsigned long long seed, unsigned long long tag) {
+    for (int mu = 0; mu < 4; ++mu)
+        for (int parity = 0; parity < 2; ++parity) {
+            int rc = lqcd_gauge_update(gauge, mu, parity, mode, beta, seed, tag);
+            if (rc) return rc;
+        }
+    return LQCD_OK;
+}
+
+int lqcd_plaquette(const void* gauge, double* plaquette_host) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (!gauge || !plaquette_host) return fail(LQCD_BAD_ARG, "lqcd_plaquette: null pointer");
+    int rc = ensure_scalars();
+    if (rc) return rc;
+    CU(launch_plaquette(ctx.precision, ctx.recon, ctx.geo, gauge, red(), ctx.stream));
+    CU(launch_finalize(FIN_TRUE, red(), plaquette_partials(ctx.geo.Vh), 0.0, ctx.scal_outer, ctx.stream));
+    CU(cudaMemcpyAsync(&ctx.scal_host[2], ctx.scal_outer, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx.stream));
+    CU(cudaStreamSynchronize(ctx.stream));
+    // sum of Re tr over the 6 V plaquettes -> average of Re tr / 3
+    *plaquette_host = ctx.scal_host[2].resid_true / (3.0 * 6.0 * 2.0 * (double)ctx.geo.Vh);
     return LQCD_OK;
 }
 

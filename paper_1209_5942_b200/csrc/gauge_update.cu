@@ -1,0 +1,389 @@
+// gauge_update.cu -- the paper's second workload: pure-gauge heatbath and overrelaxation
+// (Fig. 2; Table 2 rows "heatbath" / "overrelax", PAPER.md:237-238;
+// SURVEY.md section 8(f) row 4; readings G17-G21), plus the average plaquette.
+//
+// One launch = one sub-sweep: every link U_mu(x) with parity(x) = p, one thread per link.  Those
+// links are independent: the 6 staples of U_mu(x) hold links of the other directions, and
+// direction-mu links only at x +- nu, which have the other parity.  Per link (Fig. 2):
+//   A = sum_{nu != mu} [ U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag + U_nu(x+mu-nu)^dag U_mu(x-nu)^dag U_nu(x-nu) ]
+//   for the subgroups (0,1), (1,2), (0,2):  W = L A;  w = project(W);  v = update(w);  L = extend(v) L
+// with update = Kennedy-Pendleton heatbath (v w = g, g ~ sqrt(1 - g0^2) exp(lambda g0), lambda =
+// 2 beta k / 3) or overrelaxation (v w = w^dag).  The 3x3 products run in the storage precision
+// T; the SU(2) step (projection, k, the random draws, the accept/reject decision, v) always runs
+// in double, so that single-precision fields take the same decisions as a double evaluation of
+// the same W.  Random numbers: the counter-based generator of the input
+// recipe (reading G21), re-implemented here.
+//
+// Traffic: the paper's kernel moved 2880 B per link (19 links read, 1 written, no reuse).  A
+// sub-sweep needs every link of the lattice once (4 V links) and writes V/2: algorithmic
+// 9 x 144 = 1296 B per updated link in double/18; the 2.1-fold reuse of the 18 loads is left to
+// L1/L2, as for the neighbour spinors of the hopping kernel.
+#include "site_ops.cuh"
+
+#ifndef LQCD_GAUGE_MIN_BLOCKS_D
+#define LQCD_GAUGE_MIN_BLOCKS_D 2
+#endif
+#ifndef LQCD_GAUGE_MIN_BLOCKS_F
+#define LQCD_GAUGE_MIN_BLOCKS_F 4
+#endif
+
+namespace lqcd {
+namespace {
+
+struct GaugeArgs {
+    void* gauge;
+    Geometry g;
+    int mu, parity;
+    double beta;
+    unsigned long long seed, tag;
+    Reduction red;          // plaquette only
+};
+
+// ------------------------------------------------------------------------------- indexing
+struct SiteIdx {
+    int e, x0h, x1, x2, x3, r;   // r = x0 mod 2
+};
+
+__device__ __forceinline__ SiteIdx site_of(const Geometry& g, int e, int parity) {
+    SiteIdx s;
+    s.e = e;
+    site_coords(g, e, s.x0h, s.x1, s.x2, s.x3);
+    s.r = (s.x1 + s.x2 + s.x3 + parity) & 1;
+    return s;
+}
+
+// neighbour in direction dir, sgn = +1 / -1 (periodic; the neighbour has the other parity)
+__device__ __forceinline__ SiteIdx step(const Geometry& g, SiteIdx s, int dir, int sgn) {
+    if (dir == 0) {
+        if (sgn > 0) {
+            if (s.r) {
+                if (s.x0h == g.N0h - 1) { s.e -= g.N0h - 1; s.x0h = 0; }
+                else { s.e += 1; s.x0h += 1; }
+            }
+        } else {
+            if (!s.r) {
+                if (s.x0h == 0) { s.e += g.N0h - 1; s.x0h = g.N0h - 1; }
+                else { s.e -= 1; s.x0h -= 1; }
+            }
+        }
+        s.r ^= 1;
+        return s;
+    }
+    const int stride = (dir == 1) ? g.N0h : (dir == 2) ? g.N0h * g.N1 : g.N0h * g.N1 * g.N2;
+    const int n = (dir == 1) ? g.N1 : (dir == 2) ? g.N2 : g.N3;
+    int& c = (dir == 1) ? s.x1 : (dir == 2) ? s.x2 : s.x3;
+    if (sgn > 0) {
+        if (c == n - 1) { s.e -= (n - 1) * stride; c = 0; }
+        else { s.e += stride; c += 1; }
+    } else {
+        if (c == 0) { s.e += (n - 1) * stride; c = n - 1; }
+        else { s.e -= stride; c -= 1; }
+    }
+    return s;
+}
+
+// ------------------------------------------------------------------------------- link access
+// Links are reused by several threads here (unlike in the hopping kernel), so they are read
+// with default caching, not evict-first.  COHERENT = the link this thread rewrites.
+template <int RECON, bool COHERENT>
+__device__ __forceinline__ void gload(const void* gauge, int G, int par, int mu, int idx, double (&u)[18]) {
+    const double2* p = reinterpret_cast<const double2*>(gauge) +
+                       ((size_t)(par * 4 + mu) * G + (idx >> 5)) * ((RECON / 2) * 32) + (idx & 31);
+#pragma unroll
+    for (int j = 0; j < RECON / 2; ++j) {
+        const double2 v = COHERENT ? p[j * 32] : __ldg(p + j * 32);
+        u[2 * j] = v.x;
+        u[2 * j + 1] = v.y;
+    }
+    if (RECON == 12) reconstruct_row2(u);
+}
+template <int RECON, bool COHERENT>
+__device__ __forceinline__ void gload(const void* gauge, int G, int par, int mu, int idx, float (&u)[18]) {
+    if (RECON == 12) {
+        const float4* p = reinterpret_cast<const float4*>(gauge) +
+                          ((size_t)(par * 4 + mu) * G + (idx >> 5)) * (3 * 32) + (idx & 31);
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            const float4 v = COHERENT ? p[j * 32] : __ldg(p + j * 32);
+            u[4 * j] = v.x; u[4 * j + 1] = v.y; u[4 * j + 2] = v.z; u[4 * j + 3] = v.w;
+        }
+        reconstruct_row2(u);
+    } else {
+        const float* blk = reinterpret_cast<const float*>(gauge) + ((size_t)(par * 4 + mu) * G + (idx >> 5)) * (18 * 32);
+        const float4* p = reinterpret_cast<const float4*>(blk) + (idx & 31);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const float4 v = COHERENT ? p[j * 32] : __ldg(p + j * 32);
+            u[4 * j] = v.x; u[4 * j + 1] = v.y; u[4 * j + 2] = v.z; u[4 * j + 3] = v.w;
+        }
+        const float2* q = reinterpret_cast<const float2*>(blk + 16 * 32) + (idx & 31);
+        const float2 w = COHERENT ? *q : __ldg(q);
+        u[16] = w.x;
+        u[17] = w.y;
+    }
+}
+template <int RECON>
+__device__ __forceinline__ void gstore(void* gauge, int G, int par, int mu, int idx, const double (&u)[18]) {
+    double2* p = reinterpret_cast<double2*>(gauge) + ((size_t)(par * 4 + mu) * G + (idx >> 5)) * ((RECON / 2) * 32) + (idx & 31);
+#pragma unroll
+    for (int j = 0; j < RECON / 2; ++j) p[j * 32] = make_double2(u[2 * j], u[2 * j + 1]);
+}
+template <int RECON>
+__device__ __forceinline__ void gstore(void* gauge, int G, int par, int mu, int idx, const float (&u)[18]) {
+    if (RECON == 12) {
+        float4* p = reinterpret_cast<float4*>(gauge) + ((size_t)(par * 4 + mu) * G + (idx >> 5)) * (3 * 32) + (idx & 31);
+#pragma unroll
+        for (int j = 0; j < 3; ++j) p[j * 32] = make_float4(u[4 * j], u[4 * j + 1], u[4 * j + 2], u[4 * j + 3]);
+    } else {
+        float* blk = reinterpret_cast<float*>(gauge) + ((size_t)(par * 4 + mu) * G + (idx >> 5)) * (18 * 32);
+        float4* p = reinterpret_cast<float4*>(blk) + (idx & 31);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) p[j * 32] = make_float4(u[4 * j], u[4 * j + 1], u[4 * j + 2], u[4 * j + 3]);
+        reinterpret_cast<float2*>(blk + 16 * 32)[idx & 31] = make_float2(u[16], u[17]);
+    }
+}
+
+// c (+)= op(a) op(b), op = identity or dagger; 3x3 complex, row-major, explicit FMA chains
+template <bool DA, bool DB, bool ACC, typename T>
+__device__ __forceinline__ void mm3(const T (&a)[18], const T (&b)[18], T (&c)[18]) {
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            T re = ACC ? c[2 * (3 * i + j)] : (T)0, im = ACC ? c[2 * (3 * i + j) + 1] : (T)0;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const T ar = DA ? a[2 * (3 * k + i)] : a[2 * (3 * i + k)];
+                const T ai = DA ? -a[2 * (3 * k + i) + 1] : a[2 * (3 * i + k) + 1];
+                const T br = DB ? b[2 * (3 * j + k)] : b[2 * (3 * k + j)];
+                const T bi = DB ? -b[2 * (3 * j + k) + 1] : b[2 * (3 * k + j) + 1];
+                re = fma_(ar, br, re);
+                re = fma_(-ai, bi, re);
+                im = fma_(ar, bi, im);
+                im = fma_(ai, br, im);
+            }
+            c[2 * (3 * i + j)] = re;
+            c[2 * (3 * i + j) + 1] = im;
+        }
+}
+
+// ------------------------------------------------------------------------------- random numbers
+// uniform in (0,1]: bits = splitmix64_mix(seed * GOLD + (stream << 40) + counter), top 53 bits
+__device__ __forceinline__ double uniform01(unsigned long long seed, unsigned long long stream,
+                                            unsigned long long counter) {
+    unsigned long long z = seed * 0x9E3779B97F4A7C15ULL + (stream << 40) + counter;
+    z += 0x9E3779B97F4A7C15ULL;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+    z ^= z >> 31;
+    return ((double)(z >> 11) + 1.0) * (1.0 / 9007199254740992.0);
+}
+
+constexpr int MAXTRY = 32;   // reading G20
+
+// Kennedy-Pendleton: g0 with density sqrt(1 - g0^2) exp(lambda g0), direction uniform.
+// Counters: attempt t uses base + 4 t + (0..3), the direction base + 4 MAXTRY + (0, 1).
+__device__ __forceinline__ bool kp_sample(double lambda, unsigned long long seed, unsigned long long tag,
+                                          unsigned long long base, double (&g)[4]) {
+    const double two_pi = 6.283185307179586476925286766559;
+    for (int t = 0; t < MAXTRY; ++t) {
+        const unsigned long long c = base + 4ull * t;
+        const double r1 = uniform01(seed, tag, c), r2 = uniform01(seed, tag, c + 1);
+        const double r3 = uniform01(seed, tag, c + 2), r4 = uniform01(seed, tag, c + 3);
+        const double cs = cos(two_pi * r2);
+        const double delta = -(log(r1) + cs * cs * log(r3)) / lambda;
+        if (r4 * r4 <= 1.0 - 0.5 * delta) {
+            const unsigned long long cd = base + 4ull * MAXTRY;
+            const double r5 = uniform01(seed, tag, cd), r6 = uniform01(seed, tag, cd + 1);
+            const double g0 = 1.0 - delta;
+            const double rad = sqrt(1.0 - g0 * g0);
+            const double ct = 2.0 * r5 - 1.0;
+            const double st = sqrt(1.0 - ct * ct);
+            double sp, cp;
+            sincos(two_pi * r6, &sp, &cp);
+            g[0] = g0;
+            g[1] = rad * st * cp;
+            g[2] = rad * st * sp;
+            g[3] = rad * ct;
+            return true;
+        }
+    }
+    return false;
+}
+
+// One subgroup step of Fig. 2 on the link L with staple sum A: subgroup (P, Q), I = its index.
+// SU(2) elements are quaternions (a0, a1, a2, a3) = a0 + i a.sigma
+//   = [[a0 + i a3, a2 + i a1], [-a2 + i a1, a0 - i a3]]   (reading G19);
+// (a0, a)(b0, b) = (a0 b0 - a.b, a0 b + b0 a - a x b).
+template <int MODE, int I, int P, int Q, typename T>
+__device__ __forceinline__ void subgroup_step(T (&L)[18], const T (&A)[18], double beta, unsigned long long seed,
+                                              unsigned long long tag, unsigned long long link_id) {
+    // the four entries (P,P), (P,Q), (Q,P), (Q,Q) of W = L A
+    T wr[4], wi[4];
+#pragma unroll
+    for (int n = 0; n < 4; ++n) {
+        const int i = (n < 2) ? P : Q, j = (n & 1) ? Q : P;
+        T re = 0, im = 0;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const T ar = L[2 * (3 * i + k)], ai = L[2 * (3 * i + k) + 1];
+            const T br = A[2 * (3 * k + j)], bi = A[2 * (3 * k + j) + 1];
+            re = fma_(ar, br, re);
+            re = fma_(-ai, bi, re);
+            im = fma_(ar, bi, im);
+            im = fma_(ai, br, im);
+        }
+        wr[n] = re;
+        wi[n] = im;
+    }
+    double w0 = 0.5 * ((double)wr[0] + (double)wr[3]);
+    double w1 = 0.5 * ((double)wi[1] + (double)wi[2]);
+    double w2 = 0.5 * ((double)wr[1] - (double)wr[2]);
+    double w3 = 0.5 * ((double)wi[0] - (double)wi[3]);
+    const double k = sqrt(w0 * w0 + w1 * w1 + w2 * w2 + w3 * w3);
+    if (!(k > 0.0)) return;
+    w0 /= k; w1 /= k; w2 /= k; w3 /= k;
+    double v0, v1, v2, v3;
+    if (MODE == 0) {   // heatbath: v = g w^dag
+        double g[4];
+        const unsigned long long base = ((link_id * 3ull + (unsigned long long)I) * (unsigned long long)(MAXTRY + 1)) * 4ull;
+        if (!kp_sample(2.0 * beta * k / 3.0, seed, tag, base, g)) return;
+        v0 = g[0] * w0 + (g[1] * w1 + g[2] * w2 + g[3] * w3);
+        v1 = w0 * g[1] - g[0] * w1 + (g[2] * w3 - g[3] * w2);
+        v2 = w0 * g[2] - g[0] * w2 + (g[3] * w1 - g[1] * w3);
+        v3 = w0 * g[3] - g[0] * w3 + (g[1] * w2 - g[2] * w1);
+    } else {           // overrelaxation: v = (w^dag)^2
+        v0 = w0 * w0 - (w1 * w1 + w2 * w2 + w3 * w3);
+        v1 = -2.0 * w0 * w1;
+        v2 = -2.0 * w0 * w2;
+        v3 = -2.0 * w0 * w3;
+    }
+    // L <- extend(v) L: rows P, Q become v00 L_P + v01 L_Q and v10 L_P + v11 L_Q
+    const T ar = (T)v0, ai = (T)v3, br = (T)v2, bi = (T)v1;   // v00 = a, v01 = b, v10 = -conj(b), v11 = conj(a)
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const T pr = L[2 * (3 * P + c)], pi = L[2 * (3 * P + c) + 1];
+        const T qr = L[2 * (3 * Q + c)], qi = L[2 * (3 * Q + c) + 1];
+        L[2 * (3 * P + c)]     = fma_(-bi, qi, fma_(br, qr, fma_(-ai, pi, ar * pr)));
+        L[2 * (3 * P + c) + 1] = fma_(bi, qr, fma_(br, qi, fma_(ai, pr, ar * pi)));
+        L[2 * (3 * Q + c)]     = fma_(ai, qi, fma_(ar, qr, fma_(-bi, pi, -br * pr)));
+        L[2 * (3 * Q + c) + 1] = fma_(-ai, qr, fma_(ar, qi, fma_(bi, pr, -br * pi)));
+    }
+}
+
+template <typename T, int RECON, int MODE>
+__global__ void __launch_bounds__(128, sizeof(T) == 8 ? LQCD_GAUGE_MIN_BLOCKS_D : LQCD_GAUGE_MIN_BLOCKS_F)
+gauge_update_kernel(const GaugeArgs a) {
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= a.g.Vh) return;
+    const int G = a.g.G, mu = a.mu, p = a.parity;
+    const SiteIdx x = site_of(a.g, e, p);
+    const SiteIdx xpm = step(a.g, x, mu, +1);
+    T A[18];
+#pragma unroll
+    for (int i = 0; i < 18; ++i) A[i] = 0;
+#pragma unroll 1
+    for (int nu = 0; nu < 4; ++nu) {
+        if (nu == mu) continue;
+        const SiteIdx xpn = step(a.g, x, nu, +1), xmn = step(a.g, x, nu, -1), xpmmn = step(a.g, xpm, nu, -1);
+        T u[18], w[18], t[18];
+        gload<RECON, false>(a.gauge, G, 1 - p, nu, xpm.e, u);     // U_nu(x+mu)
+        gload<RECON, false>(a.gauge, G, 1 - p, mu, xpn.e, w);     // U_mu(x+nu)
+        mm3<false, true, false>(u, w, t);
+        gload<RECON, false>(a.gauge, G, p, nu, x.e, u);           // U_nu(x)
+        mm3<false, true, true>(t, u, A);
+        gload<RECON, false>(a.gauge, G, p, nu, xpmmn.e, u);       // U_nu(x+mu-nu)
+        gload<RECON, false>(a.gauge, G, 1 - p, mu, xmn.e, w);     // U_mu(x-nu)
+        mm3<true, true, false>(u, w, t);
+        gload<RECON, false>(a.gauge, G, 1 - p, nu, xmn.e, u);     // U_nu(x-nu)
+        mm3<false, false, true>(t, u, A);
+    }
+    T L[18];
+    gload<RECON, true>(a.gauge, G, p, mu, e, L);
+    // link id of reading G21: 4 lex(x) + mu, lex(x) = 2 e + r
+    const unsigned long long link_id = 4ull * (2ull * (unsigned long long)e + (unsigned long long)x.r) + (unsigned long long)mu;
+    subgroup_step<MODE, 0, 0, 1>(L, A, a.beta, a.seed, a.tag, link_id);
+    subgroup_step<MODE, 1, 1, 2>(L, A, a.beta, a.seed, a.tag, link_id);
+    subgroup_step<MODE, 2, 0, 2>(L, A, a.beta, a.seed, a.tag, link_id);
+    gstore<RECON>(a.gauge, G, p, mu, e, L);
+}
+
+// Average plaquette: one thread per site of parity blockIdx.y, 6 plaquettes
+//   P_mu_nu(x) = U_mu(x) U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag,  mu < nu;
+// one partial sum of Re tr per warp (fixed-order two-stage sum, lqcd_internal.h).
+template <typename T, int RECON>
+__global__ void __launch_bounds__(128, 3) plaquette_kernel(const GaugeArgs a) {
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    const int p = blockIdx.y;
+    const int G = a.g.G;
+    double sum = 0.0;
+    if (e < a.g.Vh) {
+        const SiteIdx x = site_of(a.g, e, p);
+#pragma unroll 1
+        for (int mu = 0; mu < 3; ++mu) {
+            const SiteIdx xpm = step(a.g, x, mu, +1);
+            T um[18];
+            gload<RECON, false>(a.gauge, G, p, mu, e, um);
+#pragma unroll 1
+            for (int nu = mu + 1; nu < 4; ++nu) {
+                const SiteIdx xpn = step(a.g, x, nu, +1);
+                T u[18], t[18], s[18];
+                gload<RECON, false>(a.gauge, G, 1 - p, nu, xpm.e, u);
+                mm3<false, false, false>(um, u, t);                    // U_mu(x) U_nu(x+mu)
+                gload<RECON, false>(a.gauge, G, 1 - p, mu, xpn.e, u);
+                mm3<false, true, false>(t, u, s);                      // ... U_mu(x+nu)^dag
+                gload<RECON, false>(a.gauge, G, p, nu, e, u);
+                // Re tr(s U_nu(x)^dag) = sum_ij Re(s_ij conj(u_ij))
+#pragma unroll
+                for (int i = 0; i < 18; ++i) sum += (double)s[i] * (double)u[i];
+            }
+        }
+    }
+    sum = warp_sum(sum);
+    if ((threadIdx.x & 31) == 0)
+        a.red.partials[(size_t)p * (gridDim.x * (blockDim.x >> 5)) + ((blockIdx.x * blockDim.x + threadIdx.x) >> 5)] = sum;
+}
+
+}  // namespace
+
+cudaError_t launch_gauge_update(int precision, int recon, int mode, const Geometry& g, void* gauge, int mu,
+                                int parity, double beta, unsigned long long seed, unsigned long long tag,
+                                cudaStream_t st) {
+    GaugeArgs a;
+    a.gauge = gauge; a.g = g; a.mu = mu; a.parity = parity; a.beta = beta; a.seed = seed; a.tag = tag;
+    a.red.partials = nullptr;
+    const int grid = (g.Vh + 127) / 128;
+    count_launch();
+    ProfScope prof(7, st);
+#define LQCD_GU(TT, RR)                                                                   \
+    do {                                                                                  \
+        if (mode == 0) gauge_update_kernel<TT, RR, 0><<<grid, 128, 0, st>>>(a);           \
+        else           gauge_update_kernel<TT, RR, 1><<<grid, 128, 0, st>>>(a);           \
+    } while (0)
+    if (precision == 0) { if (recon == 12) LQCD_GU(double, 12); else LQCD_GU(double, 18); }
+    else                { if (recon == 12) LQCD_GU(float, 12);  else LQCD_GU(float, 18); }
+#undef LQCD_GU
+    return cudaGetLastError();
+}
+
+int plaquette_partials(int Vh) { return 2 * ((Vh + 127) / 128) * 4; }
+
+cudaError_t launch_plaquette(int precision, int recon, const Geometry& g, const void* gauge, Reduction red,
+                             cudaStream_t st) {
+    GaugeArgs a;
+    a.gauge = const_cast<void*>(gauge); a.g = g; a.mu = 0; a.parity = 0; a.beta = 0; a.seed = 0; a.tag = 0;
+    a.red = red;
+    const dim3 grid((g.Vh + 127) / 128, 2);
+    count_launch();
+    ProfScope prof(8, st);
+    if (precision == 0) {
+        if (recon == 12) plaquette_kernel<double, 12><<<grid, 128, 0, st>>>(a);
+        else             plaquette_kernel<double, 18><<<grid, 128, 0, st>>>(a);
+    } else {
+        if (recon == 12) plaquette_kernel<float, 12><<<grid, 128, 0, st>>>(a);
+        else             plaquette_kernel<float, 18><<<grid, 128, 0, st>>>(a);
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace lqcd

@@ -167,6 +167,19 @@ cudaError_t launch_pack_spinor(int precision, const Geometry& g, const void* can
 cudaError_t launch_unpack_spinor(int precision, const Geometry& g, const void* internal, void* canon,
                                  int parity, cudaStream_t st);
 
+cudaError_t launch_unpack_gauge(int precision, int recon, const Geometry& g, const void* internal, void* canon,
+                                cudaStream_t st);
+
+// gauge_update.cu: one sub-sweep (all links U_mu(x), parity(x) = parity) of the heatbath (mode 0)
+// or overrelaxation (mode 1) update, in place; the average plaquette as per-warp partial sums of
+// Re tr P over the 6 V plaquettes (plaquette_partials(Vh) of them).
+cudaError_t launch_gauge_update(int precision, int recon, int mode, const Geometry& g, void* gauge, int mu,
+                                int parity, double beta, unsigned long long seed, unsigned long long tag,
+                                cudaStream_t st);
+cudaError_t launch_plaquette(int precision, int recon, const Geometry& g, const void* gauge, Reduction red,
+                             cudaStream_t st);
+int plaquette_partials(int Vh);
+
 // force.cu: F^a_mu(x) for every link from full-lattice X, Y given as half fields (the force is
 // linear in kappa, so a common sign of the odd halves is passed as the sign of kappa).
 // force: double2 f[2][4][G][4][32], element j of a link = (F^{2j+1}, F^{2j+2}); always double.

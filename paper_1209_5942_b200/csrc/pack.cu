@@ -56,6 +56,59 @@ __global__ void __launch_bounds__(PBLOCK) pack_gauge_kernel(Geometry g, const do
     }
 }
 
+// internal -> canonical U[lex][mu] (row 2 rebuilt as conj(row0 x row1) for 12-real storage)
+template <typename T, int RECON>
+__global__ void __launch_bounds__(PBLOCK) unpack_gauge_kernel(Geometry g, const void* __restrict__ internal,
+                                                              double2* __restrict__ canon) {
+    const size_t tid = (size_t)blockIdx.x * PBLOCK + threadIdx.x;
+    const size_t Vh = g.Vh;
+    if (tid >= 8 * Vh) return;
+    const int e = (int)(tid % Vh);
+    const int pm = (int)(tid / Vh);
+    const int parity = pm >> 2, mu = pm & 3;
+    const size_t lex = 2 * (size_t)e + site_r(g, e, parity);
+    const size_t grp = (size_t)pm * g.G + (e >> 5);
+    const int lane = e & 31;
+    double2 u[9];
+    if (sizeof(T) == 8) {
+        const double2* src = (const double2*)internal + grp * ((RECON / 2) * 32) + lane;
+#pragma unroll
+        for (int j = 0; j < RECON / 2; ++j) u[j] = src[j * 32];
+    } else if (RECON == 12) {
+        const float4* src = (const float4*)internal + grp * (3 * 32) + lane;
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            const float4 v = src[j * 32];
+            u[2 * j] = make_double2(v.x, v.y);
+            u[2 * j + 1] = make_double2(v.z, v.w);
+        }
+    } else {
+        const float* blk = (const float*)internal + grp * (18 * 32);
+        const float4* src = (const float4*)blk + lane;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const float4 v = src[j * 32];
+            u[2 * j] = make_double2(v.x, v.y);
+            u[2 * j + 1] = make_double2(v.z, v.w);
+        }
+        const float2 w = ((const float2*)(blk + 16 * 32))[lane];
+        u[8] = make_double2(w.x, w.y);
+    }
+    if (RECON == 12) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {   // conj(row0 x row1)_c, in the storage precision's values widened to double
+            const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
+            const double2 a = u[c1], b = u[3 + c2], cc = u[c2], d = u[3 + c1];
+            const double re = (a.x * b.x - a.y * b.y) - (cc.x * d.x - cc.y * d.y);
+            const double im = (a.x * b.y + a.y * b.x) - (cc.x * d.y + cc.y * d.x);
+            u[6 + c] = make_double2(re, -im);
+        }
+    }
+    double2* dst = canon + (lex * 4 + mu) * 9;
+#pragma unroll
+    for (int j = 0; j < 9; ++j) dst[j] = u[j];
+}
+
 // canonical half spinor psi_p[e][c] -> internal s[e >> 5][c][e & 31]; pad sites get zeros
 template <typename T>
 __global__ void __launch_bounds__(PBLOCK) pack_spinor_kernel(int Vh, int G, const double2* __restrict__ canon,
@@ -123,6 +176,23 @@ cudaError_t launch_pack_gauge(int precision, int recon, const Geometry& g, const
     } else {
         if (recon == 12) pack_gauge_kernel<float, 12><<<grid, PBLOCK, 0, st>>>(g, c, internal);
         else             pack_gauge_kernel<float, 18><<<grid, PBLOCK, 0, st>>>(g, c, internal);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_unpack_gauge(int precision, int recon, const Geometry& g, const void* internal, void* canon,
+                                cudaStream_t st) {
+    const size_t n = 8 * (size_t)g.Vh;
+    const int grid = (int)((n + PBLOCK - 1) / PBLOCK);
+    count_launch();
+    ProfScope prof(4, st);
+    double2* c = (double2*)canon;
+    if (precision == 0) {
+        if (recon == 12) unpack_gauge_kernel<double, 12><<<grid, PBLOCK, 0, st>>>(g, internal, c);
+        else             unpack_gauge_kernel<double, 18><<<grid, PBLOCK, 0, st>>>(g, internal, c);
+    } else {
+        if (recon == 12) unpack_gauge_kernel<float, 12><<<grid, PBLOCK, 0, st>>>(g, internal, c);
+        else             unpack_gauge_kernel<float, 18><<<grid, PBLOCK, 0, st>>>(g, internal, c);
     }
     return cudaGetLastError();
 }
