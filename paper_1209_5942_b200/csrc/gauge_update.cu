@@ -20,8 +20,15 @@
 // L1/L2, as for the neighbour spinors of the hopping kernel.
 #include "site_ops.cuh"
 
+// Measured at 32^3 x 64 (us per sub-sweep, heatbath / overrelaxation): double with 2 CTAs per SM
+// (246 registers) 460 / 289, with 3 (168 registers, 8 B of spills) 415 / 291, with the staple loop
+// unrolled as well 403 / 267; single with 3, 4, 5, 6 CTAs 331 / 172, 310 / 164, 306 / 178, 307 / 169,
+// unrolled at 4 CTAs 310 / 149.
 #ifndef LQCD_GAUGE_MIN_BLOCKS_D
-#define LQCD_GAUGE_MIN_BLOCKS_D 2
+#define LQCD_GAUGE_MIN_BLOCKS_D 3
+#endif
+#ifndef LQCD_GAUGE_UNROLL
+#define LQCD_GAUGE_UNROLL 3
 #endif
 #ifndef LQCD_GAUGE_MIN_BLOCKS_F
 #define LQCD_GAUGE_MIN_BLOCKS_F 4
@@ -122,6 +129,39 @@ __device__ __forceinline__ void gload(const void* gauge, int G, int par, int mu,
         u[17] = w.y;
     }
 }
+// 12-real storage keeps rows 0, 1 and rebuilds row 2 = conj(row0 x row1) on every load.  A rounding
+// defect eps of the stored rows comes back as 2 eps in the rebuilt row and is mixed into rows 0, 1
+// by the (1,2) and (0,2) subgroup steps: measured growth x1.35 per overrelaxation sweep in single
+// precision (unitarity defect 1e-5 -> 0.1 in 30 sweeps) where 18-real storage only random-walks
+// (2e-6).  So the two rows are re-orthonormalised (Gram-Schmidt) before they are stored.
+template <typename T>
+__device__ __forceinline__ void orthonormalise_rows01(T (&u)[18]) {
+    T n0 = 0;
+#pragma unroll
+    for (int i = 0; i < 6; ++i) n0 = fma_(u[i], u[i], n0);
+    const T i0 = (T)1 / sqrt(n0);
+#pragma unroll
+    for (int i = 0; i < 6; ++i) u[i] *= i0;
+    T dr = 0, di = 0;   // <row0, row1> = sum conj(row0_c) row1_c
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        dr = fma_(u[2 * c], u[6 + 2 * c], fma_(u[2 * c + 1], u[6 + 2 * c + 1], dr));
+        di = fma_(u[2 * c], u[6 + 2 * c + 1], fma_(-u[2 * c + 1], u[6 + 2 * c], di));
+    }
+    T n1 = 0;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const T re = u[6 + 2 * c] - (dr * u[2 * c] - di * u[2 * c + 1]);
+        const T im = u[6 + 2 * c + 1] - (dr * u[2 * c + 1] + di * u[2 * c]);
+        u[6 + 2 * c] = re;
+        u[6 + 2 * c + 1] = im;
+        n1 = fma_(re, re, fma_(im, im, n1));
+    }
+    const T i1 = (T)1 / sqrt(n1);
+#pragma unroll
+    for (int i = 6; i < 12; ++i) u[i] *= i1;
+}
+
 template <int RECON>
 __device__ __forceinline__ void gstore(void* gauge, int G, int par, int mu, int idx, const double (&u)[18]) {
     double2* p = reinterpret_cast<double2*>(gauge) + ((size_t)(par * 4 + mu) * G + (idx >> 5)) * ((RECON / 2) * 32) + (idx & 31);
@@ -180,17 +220,17 @@ __device__ __forceinline__ double uniform01(unsigned long long seed, unsigned lo
 }
 
 constexpr int MAXTRY = 32;   // reading G20
+constexpr int kStapleUnroll = LQCD_GAUGE_UNROLL;
 
 // Kennedy-Pendleton: g0 with density sqrt(1 - g0^2) exp(lambda g0), direction uniform.
 // Counters: attempt t uses base + 4 t + (0..3), the direction base + 4 MAXTRY + (0, 1).
 __device__ __forceinline__ bool kp_sample(double lambda, unsigned long long seed, unsigned long long tag,
                                           unsigned long long base, double (&g)[4]) {
-    const double two_pi = 6.283185307179586476925286766559;
     for (int t = 0; t < MAXTRY; ++t) {
         const unsigned long long c = base + 4ull * t;
         const double r1 = uniform01(seed, tag, c), r2 = uniform01(seed, tag, c + 1);
         const double r3 = uniform01(seed, tag, c + 2), r4 = uniform01(seed, tag, c + 3);
-        const double cs = cos(two_pi * r2);
+        const double cs = cospi(2.0 * r2);
         const double delta = -(log(r1) + cs * cs * log(r3)) / lambda;
         if (r4 * r4 <= 1.0 - 0.5 * delta) {
             const unsigned long long cd = base + 4ull * MAXTRY;
@@ -200,7 +240,7 @@ __device__ __forceinline__ bool kp_sample(double lambda, unsigned long long seed
             const double ct = 2.0 * r5 - 1.0;
             const double st = sqrt(1.0 - ct * ct);
             double sp, cp;
-            sincos(two_pi * r6, &sp, &cp);
+            sincospi(2.0 * r6, &sp, &cp);
             g[0] = g0;
             g[1] = rad * st * cp;
             g[2] = rad * st * sp;
@@ -282,9 +322,9 @@ gauge_update_kernel(const GaugeArgs a) {
     T A[18];
 #pragma unroll
     for (int i = 0; i < 18; ++i) A[i] = 0;
-#pragma unroll 1
-    for (int nu = 0; nu < 4; ++nu) {
-        if (nu == mu) continue;
+#pragma unroll kStapleUnroll
+    for (int j = 1; j < 4; ++j) {
+        const int nu = (mu + j) & 3;   // the three directions nu != mu
         const SiteIdx xpn = step(a.g, x, nu, +1), xmn = step(a.g, x, nu, -1), xpmmn = step(a.g, xpm, nu, -1);
         T u[18], w[18], t[18];
         gload<RECON, false>(a.gauge, G, 1 - p, nu, xpm.e, u);     // U_nu(x+mu)
@@ -305,6 +345,7 @@ gauge_update_kernel(const GaugeArgs a) {
     subgroup_step<MODE, 0, 0, 1>(L, A, a.beta, a.seed, a.tag, link_id);
     subgroup_step<MODE, 1, 1, 2>(L, A, a.beta, a.seed, a.tag, link_id);
     subgroup_step<MODE, 2, 0, 2>(L, A, a.beta, a.seed, a.tag, link_id);
+    if (RECON == 12) orthonormalise_rows01(L);
     gstore<RECON>(a.gauge, G, p, mu, e, L);
 }
 

@@ -2,7 +2,7 @@
 """sweep.py -- timings of the BASELINE.json configurations 3, 4, 5 and of the paper's thermal
 lattice shapes (Fig. 7), one JSON line each.  A user-facing companion of bench.py:
 
-    python -m paper_1209_5942_b200.sweep [--configs 3,4,5,thermal,force] [--out FILE]
+    python -m paper_1209_5942_b200.sweep [--configs 3,4,5,thermal,force,gauge] [--out FILE]
 
 config 3: 16^3x32, near-identity links, kappa=.16 mu=.05: 10 warm-up + 100 timed D_eo/D_oe
           applications, 5 repeats, median (working set fits L2: not a HBM roofline figure)
@@ -11,6 +11,7 @@ config 4: 24^3x48 Haar links: CG on Mhat^dag Mhat to 1e-10; iterations, time to 
 config 5: 32^3x64, double/single x 18/12-real links: 20 warm-up + 200 timed D-slash applications
 thermal : N_sigma in {16,24,32,48} x N_tau in {4,8,12,16}, double/18 D-slash
 force   : the fermion-force kernel at 32^3x64 in the four storage variants
+gauge   : heatbath and overrelaxation sweeps at 32^3x64 in the four storage variants
 
 GFLOPS at 1320 flop per output site (BASELINE metric); "gbs_effective" counts the algorithmic
 bytes (each link, each input site and each output once); "gbs_paper_accounting" counts the
@@ -226,6 +227,50 @@ def force(stream):
     return out
 
 
+def gauge(stream):
+    """Heatbath / overrelaxation sweeps at 32^3x64, thermalised-like links,
+    beta = 5.7: one sweep = 8 sub-sweep launches = 4 V link updates.  GFLOPS with the paper's counts
+    (3912 / 3846 flop per link); algorithmic bytes per updated link = 9 links (a sub-sweep
+    reads every link of the lattice once and writes V/2), paper accounting = 20 links."""
+    dims = (32, 32, 32, 64)
+    V = int(np.prod(dims))
+    U = gen.gauge_near_identity(dims, gen.BASE_SEED, 0.3)
+    out = []
+    for precision, recon in ((0, 18), (1, 18), (0, 12), (1, 12)):
+        B.lqcd_init(dims, gen.antiperiodic_t())
+        B.lqcd_set_format(precision, recon)
+        B.lqcd_set_stream(stream)
+        with torch.cuda.stream(stream):
+            g = B.upload_gauge(U)
+            for mode, name, flop in ((B.LQCD_HEATBATH, "heatbath", 3912), (B.LQCD_OVERRELAX, "overrelax", 3846)):
+                for k in range(3):
+                    B.lqcd_gauge_sweep(g, mode, 5.7, gen.BASE_SEED, 100 + k)
+                times = []
+                for rep in range(3):
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    stream.synchronize()
+                    e0.record(stream)
+                    for k in range(10):
+                        B.lqcd_gauge_sweep(g, mode, 5.7, gen.BASE_SEED, 200 + 10 * rep + k)
+                    e1.record(stream)
+                    stream.synchronize()
+                    times.append(e0.elapsed_time(e1) / 10)
+                ms = float(np.median(times))
+                real = 8 if precision == 0 else 4
+                link = recon * real
+                peak = measured_peak()
+                gbs = 4 * V * 9 * link / ms / 1e6
+                out.append({"config": "gauge", "kernel": name, "lattice": list(dims),
+                            "precision": "double" if precision == 0 else "single", "recon": recon,
+                            "ms_per_sweep": ms, "us_per_subsweep": ms * 1e3 / 8, "links_per_s": 4 * V / ms * 1e3,
+                            "gflops_paper_count": 4 * V * flop / ms / 1e6, "bytes_per_link": 9 * link,
+                            "gbs_effective": gbs, "gbs_paper_accounting": 4 * V * 20 * link / ms / 1e6,
+                            "frac_of_measured_peak": gbs / peak, "measured_peak_gbs": peak,
+                            "plaquette_after": B.lqcd_plaquette(g)})
+        B.lqcd_finalize()
+    return out
+
+
 def thermal(stream):
     out = []
     for ns in (16, 24, 32, 48):
@@ -246,7 +291,7 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("sweep.py needs a CUDA device: there is no CPU fallback")
     stream = torch.cuda.Stream()
-    table = {"3": config3, "4": config4, "5": config5, "thermal": thermal, "force": force}
+    table = {"3": config3, "4": config4, "5": config5, "thermal": thermal, "force": force, "gauge": gauge}
     lines = []
     for key in args.configs.split(","):
         for r in table[key.strip()](stream):

@@ -229,3 +229,17 @@ def test_full_size_subsweep_sampled_links(B, oracle_mod):
         assert np.array_equal(got[other], U[other])
         assert np.array_equal(got[sites][:, [m for m in range(4) if m != mu]], U[sites][:, [m for m in range(4) if m != mu]])
         del g, got
+
+
+def test_recon12_rows_stay_orthonormal_over_many_sweeps(B):
+    """12-real storage: without the re-orthonormalisation before the store the unitarity defect grows
+    x1.35 per overrelaxation sweep in single precision (1e-5 -> 0.1 in 30 sweeps, measured)."""
+    dims = (8, 8, 8, 16)
+    g = _setup(B, dims, gen.gauge_near_identity(dims, SEED, 0.3), 1, 12)
+    for k in range(6):
+        B.lqcd_gauge_sweep(g, B.LQCD_HEATBATH, 5.7, SEED, 100 + k)
+    p0 = B.lqcd_plaquette(g)
+    for k in range(40):
+        B.lqcd_gauge_sweep(g, B.LQCD_OVERRELAX, 0.0, 0, 0)
+    assert _su3_defect(B.download_gauge(g)) < 5e-6
+    assert abs(B.lqcd_plaquette(g) - p0) < 2e-6
