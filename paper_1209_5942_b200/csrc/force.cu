@@ -15,8 +15,11 @@
 // (X, Y once each) + 256 (force written) = 1216 in double/18.
 #include "site_ops.cuh"
 
+// CTAs of 128 threads per SM.  The kernel is latency bound (ncu: DRAM traffic = algorithmic bytes,
+// DRAM throughput 62%, 12 warps/SM): in double 4 CTAs (128 registers, no spills) run 460 us at
+// 32^3 x 64 against 497 us with 3 (168 registers) and 497 us with 5 (96 registers, 140 B of spills).
 #ifndef LQCD_FORCE_MIN_BLOCKS
-#define LQCD_FORCE_MIN_BLOCKS 3
+#define LQCD_FORCE_MIN_BLOCKS 4
 #endif
 
 namespace lqcd {
