@@ -373,7 +373,7 @@ int lqcd_init(const int dims[4], const double bc_phase[8]) {
     ctx.geo.d2 = make_fastdiv((unsigned)ctx.geo.N2);
     ctx.geo.Vh = (int)(V / 2);
     ctx.geo.G = (ctx.geo.Vh + 31) / 32;
-    ctx.precision = LQCD_DOUBLE; ctx.recon = 18; ctx.block = 128; ctx.stream = 0;
+    ctx.precision = LQCD_DOUBLE; ctx.recon = 18; ctx.block = LQCD_DEFAULT_BLOCK; ctx.stream = 0;
     g_launches.store(0);
     g_err[0] = 0;
     return LQCD_OK;
@@ -402,8 +402,8 @@ int lqcd_set_format(int precision, int recon) {
 
 int lqcd_set_block_size(int threads) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
-    if (threads == 0) threads = 128;
-    if (threads < 32 || threads > 128 || (threads % 32)) return fail(LQCD_BAD_ARG, "block size must be 32, 64, 96 or 128");
+    if (threads == 0) threads = LQCD_DEFAULT_BLOCK;
+    if (threads < 32 || threads > LQCD_HOP_MAX_THREADS || (threads % 32)) return fail(LQCD_BAD_ARG, "block size must be 32, 64, 96 or 128");
     ctx.block = threads;
     return LQCD_OK;
 }

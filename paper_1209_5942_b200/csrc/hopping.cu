@@ -77,7 +77,7 @@ __device__ __forceinline__ void hop(T (&acc)[24], const HopArgs& a, int e, int e
 }
 
 template <typename T, int RECON, int DAG, int MODE>
-__global__ void __launch_bounds__(128, (sizeof(T) == 4 && RECON == 12) ? LQCD_HOP_MIN_BLOCKS_F12 : LQCD_HOP_MIN_BLOCKS)
+__global__ void __launch_bounds__(LQCD_HOP_MAX_THREADS, (sizeof(T) == 4 && RECON == 12) ? LQCD_HOP_MIN_BLOCKS_F12 : LQCD_HOP_MIN_BLOCKS)
 hopping_kernel(const HopArgs a) {
     if (a.scal != nullptr && a.scal->done) return;
     const int Vh = a.g.Vh;
@@ -203,7 +203,7 @@ cudaError_t launch_tr(int dagger, int mode, const HopArgs& a, int block, cudaStr
 }  // namespace
 
 int hopping_partials(int Vh, int block) {
-    if (block <= 0 || block > 128 || (block % 32) != 0) block = 128;
+    if (block <= 0 || block > LQCD_HOP_MAX_THREADS || (block % 32) != 0) block = LQCD_HOP_MAX_THREADS;
     return ((Vh + block - 1) / block) * (block / 32);
 }
 
@@ -215,7 +215,7 @@ cudaError_t launch_hopping(int precision, int recon, int dagger, int mode, const
     a.reverse = reverse;
     a.gauge = gauge; a.in = in; a.out = out; a.aux = aux;
     a.g = g; a.ep = ep; a.out_parity = out_parity; a.red = red; a.scal = scal;
-    if (block <= 0 || block > 128 || (block % 32) != 0) block = 128;
+    if (block <= 0 || block > LQCD_HOP_MAX_THREADS || (block % 32) != 0) block = LQCD_HOP_MAX_THREADS;
     count_launch();
     ProfScope prof(mode == 3 ? 5 : mode, st);
     if (precision == 0) {

@@ -112,6 +112,14 @@ struct Reduction {
 enum { FIN_NONE = 0, FIN_PAP = 1, FIN_BB = 2, FIN_RHO = 3, FIN_TRUE = 4 };
 enum { FIN_BI_INIT = 0, FIN_BI_SIGMA = 1, FIN_BI_OMEGA = 2, FIN_BI_R = 3 };
 
+// Thread-block size of the hopping kernel: LQCD_HOP_MAX_THREADS is its __launch_bounds__ limit,
+// LQCD_DEFAULT_BLOCK what lqcd_init selects (lqcd_set_block_size overrides, up to the limit).
+#ifndef LQCD_HOP_MAX_THREADS
+#define LQCD_HOP_MAX_THREADS 128
+#endif
+#ifndef LQCD_DEFAULT_BLOCK
+#define LQCD_DEFAULT_BLOCK LQCD_HOP_MAX_THREADS
+#endif
 // "Snake order": consecutive kernels of a chain traverse the sites in opposite directions
 // (reverse = 0, 1, 0, 1, ...).  A field is 201 MB at 32^3 x 64 and L2 holds ~126 MB, so the
 // part of its output a kernel wrote last is still in L2 when the next kernel starts; starting
