@@ -32,8 +32,15 @@
 // double and for single/18 (measured: 2 and 4 are ~20% slower in double; 4, 5, 6 are 4-15% slower
 // for single/18).  Single/12 moves the fewest DRAM bytes per thread and direction (60 B), so at
 // 12 warps/SM it cannot keep enough requests in flight: 7 CTAs (72 registers) is 27% faster.
+// Re-measured with the grouped layout (32^3 x 64, us per launch at 3 / 4 CTAs of 128, 8 CTAs of 64):
+// double/18 252 / 288 / 287, double/12 213.5 / 207.5 / 208, single/18 123.7 / 122.2 / 120.5; at
+// 16^3 x 32 (1.15 waves at 3 CTAs) the 128-register builds are 6% faster (17.5 vs 18.6 us), not
+// enough to carry a second set of instantiations.  Only double/12 moves to 4 CTAs.
 #ifndef LQCD_HOP_MIN_BLOCKS
 #define LQCD_HOP_MIN_BLOCKS 3
+#endif
+#ifndef LQCD_HOP_MIN_BLOCKS_D12
+#define LQCD_HOP_MIN_BLOCKS_D12 4
 #endif
 #ifndef LQCD_HOP_MIN_BLOCKS_F12
 #define LQCD_HOP_MIN_BLOCKS_F12 7
@@ -77,7 +84,8 @@ __device__ __forceinline__ void hop(T (&acc)[24], const HopArgs& a, int e, int e
 }
 
 template <typename T, int RECON, int DAG, int MODE>
-__global__ void __launch_bounds__(LQCD_HOP_MAX_THREADS, (sizeof(T) == 4 && RECON == 12) ? LQCD_HOP_MIN_BLOCKS_F12 : LQCD_HOP_MIN_BLOCKS)
+__global__ void __launch_bounds__(LQCD_HOP_MAX_THREADS, (RECON == 12) ? (sizeof(T) == 4 ? LQCD_HOP_MIN_BLOCKS_F12 : LQCD_HOP_MIN_BLOCKS_D12)
+                                                                      : LQCD_HOP_MIN_BLOCKS)
 hopping_kernel(const HopArgs a) {
     if (a.scal != nullptr && a.scal->done) return;
     const int Vh = a.g.Vh;
