@@ -15,13 +15,14 @@
 // (X, Y once each) + 256 (force written) = 1216 in double/18.
 #include "site_ops.cuh"
 
-// CTAs of 256 threads per SM.  The kernel is latency bound (ncu: DRAM traffic = algorithmic bytes):
-// what counts is how many independent loads are in flight per SM.
-#ifndef LQCD_FORCE_MIN_BLOCKS_D
-#define LQCD_FORCE_MIN_BLOCKS_D 3
-#endif
-#ifndef LQCD_FORCE_MIN_BLOCKS_F
-#define LQCD_FORCE_MIN_BLOCKS_F 4
+// CTAs of 128 threads per SM.  The kernel is latency bound (ncu: DRAM traffic = algorithmic bytes,
+// DRAM throughput 62%, 12 warps/SM): in double 4 CTAs (128 registers, no spills) run 460 us at
+// 32^3 x 64 against 497 us with 3 (168 registers) and 497 us with 5 (96 registers, 140 B of spills).
+// Tried and dropped: two threads per link (one per term of W, CTAs of 256, partial sums combined through
+// shared memory; 80 registers, 24 warps/SM): 581 us -- the link is fetched twice and the local spinors
+// lose their L1 sharing, which costs more than the extra warps hide.
+#ifndef LQCD_FORCE_MIN_BLOCKS
+#define LQCD_FORCE_MIN_BLOCKS 4
 #endif
 
 namespace lqcd {
@@ -81,95 +82,78 @@ __device__ __forceinline__ void phase_mul(T (&chi)[12], T pr, T pi) {
 
 // The second term of W is -h+[X(x)] (x) (eta U h+[Y(x+mu)])^dag; its anti-Hermitian part equals
 // that of +(eta U h+[Y(x+mu)]) (x) h+[X(x)]^dag, so both terms go through the same accumulation
-// with the transported half spinor first:  TERM 0 transports X(x+mu) and pairs it with Y(x)
-// (projection sign -1), TERM 1 transports Y(x+mu) and pairs it with X(x) (sign +1).
-template <typename T, int RECON, int MU, int TERM>
-__device__ __forceinline__ void force_term(const ForceArgs& a, int p, int e, int e_nb, bool wrap, AntiHerm<T>& w) {
-    constexpr int S = TERM ? +1 : -1;
-    T u[18], psi[24], h[12], uh[12], v[12];
-    load_link<RECON>(a.gauge, a.g.G, p, MU, e, u);
-    load_spinor(TERM ? a.y[1 - p] : a.x[1 - p], e_nb, psi);
-    project<MU, S>(psi, h);
-    su3_mul(u, h, uh);
-    if (wrap) phase_mul(uh, (T)a.g.ph_re[MU], (T)a.g.ph_im[MU]);   // boundary phase on the wrapping hop only
-    load_spinor(TERM ? a.x[p] : a.y[p], e, psi);
-    project<MU, S>(psi, v);
-    outer_acc(w, uh, v);
-}
-
+// with the transported half spinor first.
 template <typename T, int RECON, int MU>
-__device__ __forceinline__ void force_term_mu(const ForceArgs& a, int term, int p, int e, int e_nb, bool wrap,
-                                              AntiHerm<T>& w) {
-    if (term == 0) force_term<T, RECON, MU, 0>(a, p, e, e_nb, wrap, w);
-    else           force_term<T, RECON, MU, 1>(a, p, e, e_nb, wrap, w);
-}
-
-// grid = 2 G blocks of 256 threads: block b works on the 32 sites of group b / 2 of parity b mod 2;
-// warp w takes direction mu = w mod 4 and term w / 4 of W (one link, one transported and one local
-// spinor: 33 LDG.128 per thread in double, all independent, against 57 in two dependent halves
-// when one thread did both terms).  The TERM 1 warps hand their nine partial sums to the TERM 0
-// warps through shared memory; those project on the Gell-Mann basis and store.
-// The two parities are interleaved because every spinor site is read twice, as X(x) by its own
-// block and as X(x+mu) by blocks of the other parity: sweeping one parity after the other put a
-// whole field (805 MB of X, Y) between the two reads and cost a second DRAM pass (ncu: 3.35 GB of
-// traffic against 2.55 GB algorithmic).
-template <typename T, int RECON>
-__global__ void __launch_bounds__(256, sizeof(T) == 8 ? LQCD_FORCE_MIN_BLOCKS_D : LQCD_FORCE_MIN_BLOCKS_F) force_kernel(const ForceArgs a) {
-    __shared__ T part[4][9][32];
-    const int G = a.g.G;
-    const int p = (int)blockIdx.x & 1;
-    const int lane = threadIdx.x & 31;
-    const int e = ((int)blockIdx.x >> 1) * 32 + lane;
-    const int mu = (threadIdx.x >> 5) & 3;
-    const int term = threadIdx.x >> 7;
-    const bool live = e < a.g.Vh;   // pad sites of the last group: zero force
+__device__ __forceinline__ void force_link(const ForceArgs& a, int p, int e, int e_nb, bool wrap) {
+    T u[18], psi[24], h[12], uh[12], v[12];
     AntiHerm<T> w;
 #pragma unroll
     for (int i = 0; i < 3; ++i) w.s[i] = w.r[i] = w.d[i] = 0;
-    if (live) {
-        const int N0h = a.g.N0h, N1 = a.g.N1, N2 = a.g.N2, N3 = a.g.N3;
-        int x0h, x1, x2, x3;
-        site_coords(a.g, e, x0h, x1, x2, x3);
-        const int r = (x1 + x2 + x3 + p) & 1;
-        const int s1 = N0h, s2 = N0h * N1, s3 = N0h * N1 * N2;
-        if (mu == 0) {
-            const bool wf = (r == 1) && (x0h == N0h - 1);
-            force_term_mu<T, RECON, 0>(a, term, p, e, wf ? e - (N0h - 1) : e + r, wf, w);
-        } else if (mu == 1) {
-            const bool wf = (x1 == N1 - 1);
-            force_term_mu<T, RECON, 1>(a, term, p, e, wf ? e - (N1 - 1) * s1 : e + s1, wf, w);
-        } else if (mu == 2) {
-            const bool wf = (x2 == N2 - 1);
-            force_term_mu<T, RECON, 2>(a, term, p, e, wf ? e - (N2 - 1) * s2 : e + s2, wf, w);
-        } else {
-            const bool wf = (x3 == N3 - 1);
-            force_term_mu<T, RECON, 3>(a, term, p, e, wf ? e - (N3 - 1) * s3 : e + s3, wf, w);
-        }
-    }
-    if (term == 1) {
-#pragma unroll
-        for (int i = 0; i < 3; ++i) {
-            part[mu][i][lane] = w.s[i];
-            part[mu][3 + i][lane] = w.r[i];
-            part[mu][6 + i][lane] = w.d[i];
-        }
-    }
-    __syncthreads();
-    if (term == 1) return;
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-        w.s[i] += part[mu][i][lane];
-        w.r[i] += part[mu][3 + i][lane];
-        w.d[i] += part[mu][6 + i][lane];
-    }
+    load_link<RECON>(a.gauge, a.g.G, p, MU, e, u);
+    const T er = (T)a.g.ph_re[MU], ei = (T)a.g.ph_im[MU];   // boundary phase, used on the wrapping hop only
+
+    load_spinor(a.x[1 - p], e_nb, psi);
+    project<MU, -1>(psi, h);
+    su3_mul(u, h, uh);
+    if (wrap) phase_mul(uh, er, ei);
+    load_spinor(a.y[p], e, psi);
+    project<MU, -1>(psi, v);
+    outer_acc(w, uh, v);
+
+    load_spinor(a.y[1 - p], e_nb, psi);
+    project<MU, +1>(psi, h);
+    su3_mul(u, h, uh);
+    if (wrap) phase_mul(uh, er, ei);
+    load_spinor(a.x[p], e, psi);
+    project<MU, +1>(psi, v);
+    outer_acc(w, uh, v);
+
     // F^a = 2 kappa Im tr(T^a W) = kappa Im tr(lambda^a W)
     const double k = a.kappa;
-    double2* out = reinterpret_cast<double2*>(a.force) + ((size_t)(p * 4 + mu) * G + (e >> 5)) * (4 * 32) + (e & 31);
+    double2* out = reinterpret_cast<double2*>(a.force) +
+                   ((size_t)(p * 4 + MU) * a.g.G + (e >> 5)) * (4 * 32) + (e & 31);
     out[0] = make_double2(k * (double)w.s[0], k * (double)w.r[0]);                          // lambda 1, 2
     out[32] = make_double2(k * ((double)w.d[0] - (double)w.d[1]), k * (double)w.s[1]);      // lambda 3, 4
     out[64] = make_double2(k * (double)w.r[1], k * (double)w.s[2]);                         // lambda 5, 6
     out[96] = make_double2(k * (double)w.r[2],                                              // lambda 7, 8
                            k * 0.57735026918962576451 * ((double)w.d[0] + (double)w.d[1] - 2.0 * (double)w.d[2]));
+}
+
+// grid = 2 G blocks of 128 threads: block b works on the 32 sites of group b / 2 of parity
+// b mod 2; warp w takes direction mu = w.  The two parities are interleaved because every spinor
+// site is read twice, as X(x) by its own block and as X(x+mu) by blocks of the other parity:
+// sweeping one parity after the other put a whole field (805 MB of X, Y) between the two reads
+// and cost a second DRAM pass (ncu: 3.35 GB of traffic against 2.55 GB algorithmic).
+template <typename T, int RECON>
+__global__ void __launch_bounds__(128, LQCD_FORCE_MIN_BLOCKS) force_kernel(const ForceArgs a) {
+    const int G = a.g.G;
+    const int p = (int)blockIdx.x & 1;
+    const int e = ((int)blockIdx.x >> 1) * 32 + (threadIdx.x & 31);
+    const int mu = threadIdx.x >> 5;
+    if (e >= a.g.Vh) {   // pad sites of the last group: zero force
+        double2* out = reinterpret_cast<double2*>(a.force) + ((size_t)(p * 4 + mu) * G + (e >> 5)) * (4 * 32) + (e & 31);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) out[32 * j] = make_double2(0.0, 0.0);
+        return;
+    }
+    const int N0h = a.g.N0h, N1 = a.g.N1, N2 = a.g.N2, N3 = a.g.N3;
+    int x0h, x1, x2, x3;
+    site_coords(a.g, e, x0h, x1, x2, x3);
+    const int r = (x1 + x2 + x3 + p) & 1;
+    const int s1 = N0h, s2 = N0h * N1, s3 = N0h * N1 * N2;
+    if (mu == 0) {
+        const bool wf = (r == 1) && (x0h == N0h - 1);
+        force_link<T, RECON, 0>(a, p, e, wf ? e - (N0h - 1) : e + r, wf);
+    } else if (mu == 1) {
+        const bool wf = (x1 == N1 - 1);
+        force_link<T, RECON, 1>(a, p, e, wf ? e - (N1 - 1) * s1 : e + s1, wf);
+    } else if (mu == 2) {
+        const bool wf = (x2 == N2 - 1);
+        force_link<T, RECON, 2>(a, p, e, wf ? e - (N2 - 1) * s2 : e + s2, wf);
+    } else {
+        const bool wf = (x3 == N3 - 1);
+        force_link<T, RECON, 3>(a, p, e, wf ? e - (N3 - 1) * s3 : e + s3, wf);
+    }
 }
 
 // internal double2 f[2][4][G][4][32] -> canonical double F[lex(x)][mu][8]
@@ -208,11 +192,11 @@ cudaError_t launch_fermion_force(int precision, int recon, const Geometry& g, co
     ProfScope prof(6, st);
     const int grid = 2 * g.G;
     if (precision == 0) {
-        if (recon == 12) force_kernel<double, 12><<<grid, 256, 0, st>>>(a);
-        else             force_kernel<double, 18><<<grid, 256, 0, st>>>(a);
+        if (recon == 12) force_kernel<double, 12><<<grid, 128, 0, st>>>(a);
+        else             force_kernel<double, 18><<<grid, 128, 0, st>>>(a);
     } else {
-        if (recon == 12) force_kernel<float, 12><<<grid, 256, 0, st>>>(a);
-        else             force_kernel<float, 18><<<grid, 256, 0, st>>>(a);
+        if (recon == 12) force_kernel<float, 12><<<grid, 128, 0, st>>>(a);
+        else             force_kernel<float, 18><<<grid, 128, 0, st>>>(a);
     }
     return cudaGetLastError();
 }
