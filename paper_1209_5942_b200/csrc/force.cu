@@ -20,7 +20,10 @@
 // 32^3 x 64 against 497 us with 3 (168 registers) and 497 us with 5 (96 registers, 140 B of spills).
 // Tried and dropped: two threads per link (one per term of W, CTAs of 256, partial sums combined through
 // shared memory; 80 registers, 24 warps/SM): 581 us -- the link is fetched twice and the local spinors
-// lose their L1 sharing, which costs more than the extra warps hide.
+// lose their L1 sharing, which costs more than the extra warps hide.  X(x), Y(x) of the CTA's 32 sites staged
+// once in shared memory instead of read through L1 by each direction-warp: 480 us (no change: the
+// L2 -> L1 traffic it removes is not the limiter).  One thread per site looping over the four directions
+// with the staged X(x), Y(x) (64-thread CTAs, 168 registers): 513 us; at 128 registers 707 us.
 #ifndef LQCD_FORCE_MIN_BLOCKS
 #define LQCD_FORCE_MIN_BLOCKS 4
 #endif
