@@ -23,7 +23,9 @@
 // Measured at 32^3 x 64 (us per sub-sweep, heatbath / overrelaxation): double with 2 CTAs per SM
 // (246 registers) 460 / 289, with 3 (168 registers, 8 B of spills) 415 / 291, with the staple loop
 // unrolled as well 403 / 267; single with 3, 4, 5, 6 CTAs 331 / 172, 310 / 164, 306 / 178, 307 / 169,
-// unrolled at 4 CTAs 310 / 149.
+// unrolled at 4 CTAs 310 / 149.  Re-measured: double at 4 CTAs (128 registers, 60-80 B of spills) 406 / 279.
+// Kennedy-Pendleton draws of the first two attempts precomputed ahead of the staple loads
+// (kp_precompute): heatbath 401 -> 395 (double), 310 -> 279 (single/18), 331 -> 308 (single/12).
 #ifndef LQCD_GAUGE_MIN_BLOCKS_D
 #define LQCD_GAUGE_MIN_BLOCKS_D 3
 #endif
@@ -224,31 +226,76 @@ constexpr int kStapleUnroll = LQCD_GAUGE_UNROLL;
 
 // Kennedy-Pendleton: g0 with density sqrt(1 - g0^2) exp(lambda g0), direction uniform.
 // Counters: attempt t uses base + 4 t + (0..3), the direction base + 4 MAXTRY + (0, 1).
+//
+// Everything but the division by lambda depends on the random numbers alone, i.e. on the link id,
+// not on the fields: X_t = -(ln r1 + cos^2(2 pi r2) ln r3), q_t = r4^2, and the direction.  So the
+// first KP_PRE attempts and the direction of all three subgroups are worked out at the start of the
+// kernel -- straight-line code with three-fold instruction-level parallelism that overlaps the
+// staple loads -- and parked in shared memory; the serial, divergent accept loop that used to
+// follow the staple sum only remains for the lanes that reject KP_PRE times (0.5% at beta = 5.7).
+// A divergent attempt costs a warp as much as a full one, so computing attempt 1 for every lane
+// costs nothing extra.  Values and decisions are bit-identical to the one-loop form.
+constexpr int KP_PRE = 2;
+constexpr int KP_SLOTS = 2 * KP_PRE + 4;   // X_t, q_t for t < KP_PRE; sin(theta), cos(theta), sin(phi), cos(phi)
+
+__device__ __forceinline__ void kp_attempt(unsigned long long seed, unsigned long long tag, unsigned long long c,
+                                           double& X, double& q) {
+    const double r1 = uniform01(seed, tag, c), r2 = uniform01(seed, tag, c + 1);
+    const double r3 = uniform01(seed, tag, c + 2), r4 = uniform01(seed, tag, c + 3);
+    const double cs = cospi(2.0 * r2);
+    X = -(log(r1) + cs * cs * log(r3));
+    q = r4 * r4;
+}
+
+// pre[slot * stride]: the thread's KP_SLOTS values of one subgroup
+__device__ __forceinline__ void kp_precompute(unsigned long long seed, unsigned long long tag, unsigned long long base,
+                                              double* pre, int stride) {
+#pragma unroll
+    for (int t = 0; t < KP_PRE; ++t) {
+        double X, q;
+        kp_attempt(seed, tag, base + 4ull * t, X, q);
+        pre[(2 * t) * stride] = X;
+        pre[(2 * t + 1) * stride] = q;
+    }
+    const unsigned long long cd = base + 4ull * MAXTRY;
+    const double r5 = uniform01(seed, tag, cd), r6 = uniform01(seed, tag, cd + 1);
+    const double ct = 2.0 * r5 - 1.0;
+    const double st = sqrt(1.0 - ct * ct);
+    double sp, cp;
+    sincospi(2.0 * r6, &sp, &cp);
+    pre[(2 * KP_PRE) * stride] = st;
+    pre[(2 * KP_PRE + 1) * stride] = ct;
+    pre[(2 * KP_PRE + 2) * stride] = sp;
+    pre[(2 * KP_PRE + 3) * stride] = cp;
+}
+
 __device__ __forceinline__ bool kp_sample(double lambda, unsigned long long seed, unsigned long long tag,
-                                          unsigned long long base, double (&g)[4]) {
-    for (int t = 0; t < MAXTRY; ++t) {
-        const unsigned long long c = base + 4ull * t;
-        const double r1 = uniform01(seed, tag, c), r2 = uniform01(seed, tag, c + 1);
-        const double r3 = uniform01(seed, tag, c + 2), r4 = uniform01(seed, tag, c + 3);
-        const double cs = cospi(2.0 * r2);
-        const double delta = -(log(r1) + cs * cs * log(r3)) / lambda;
-        if (r4 * r4 <= 1.0 - 0.5 * delta) {
-            const unsigned long long cd = base + 4ull * MAXTRY;
-            const double r5 = uniform01(seed, tag, cd), r6 = uniform01(seed, tag, cd + 1);
-            const double g0 = 1.0 - delta;
-            const double rad = sqrt(1.0 - g0 * g0);
-            const double ct = 2.0 * r5 - 1.0;
-            const double st = sqrt(1.0 - ct * ct);
-            double sp, cp;
-            sincospi(2.0 * r6, &sp, &cp);
-            g[0] = g0;
-            g[1] = rad * st * cp;
-            g[2] = rad * st * sp;
-            g[3] = rad * ct;
-            return true;
+                                          unsigned long long base, const double* pre, int stride, double (&g)[4]) {
+    bool ok = false;
+    double delta = 0.0;
+#pragma unroll
+    for (int t = 0; t < KP_PRE; ++t) {
+        if (!ok) {
+            delta = pre[(2 * t) * stride] / lambda;
+            ok = pre[(2 * t + 1) * stride] <= 1.0 - 0.5 * delta;
         }
     }
-    return false;
+    for (int t = KP_PRE; t < MAXTRY && !ok; ++t) {
+        double X, q;
+        kp_attempt(seed, tag, base + 4ull * t, X, q);
+        delta = X / lambda;
+        ok = q <= 1.0 - 0.5 * delta;
+    }
+    if (!ok) return false;
+    const double st = pre[(2 * KP_PRE) * stride], ct = pre[(2 * KP_PRE + 1) * stride];
+    const double sp = pre[(2 * KP_PRE + 2) * stride], cp = pre[(2 * KP_PRE + 3) * stride];
+    const double g0 = 1.0 - delta;
+    const double rad = sqrt(1.0 - g0 * g0);
+    g[0] = g0;
+    g[1] = rad * st * cp;
+    g[2] = rad * st * sp;
+    g[3] = rad * ct;
+    return true;
 }
 
 // One subgroup step of Fig. 2 on the link L with staple sum A: subgroup (P, Q), I = its index.
@@ -257,7 +304,8 @@ __device__ __forceinline__ bool kp_sample(double lambda, unsigned long long seed
 // (a0, a)(b0, b) = (a0 b0 - a.b, a0 b + b0 a - a x b).
 template <int MODE, int I, int P, int Q, typename T>
 __device__ __forceinline__ void subgroup_step(T (&L)[18], const T (&A)[18], double beta, unsigned long long seed,
-                                              unsigned long long tag, unsigned long long link_id) {
+                                              unsigned long long tag, unsigned long long link_id, const double* pre,
+                                              int stride) {
     // the four entries (P,P), (P,Q), (Q,P), (Q,Q) of W = L A
     T wr[4], wi[4];
 #pragma unroll
@@ -287,7 +335,7 @@ __device__ __forceinline__ void subgroup_step(T (&L)[18], const T (&A)[18], doub
     if (MODE == 0) {   // heatbath: v = g w^dag
         double g[4];
         const unsigned long long base = ((link_id * 3ull + (unsigned long long)I) * (unsigned long long)(MAXTRY + 1)) * 4ull;
-        if (!kp_sample(2.0 * beta * k / 3.0, seed, tag, base, g)) return;
+        if (!kp_sample(2.0 * beta * k / 3.0, seed, tag, base, pre + (size_t)I * KP_SLOTS * stride, stride, g)) return;
         v0 = g[0] * w0 + (g[1] * w1 + g[2] * w2 + g[3] * w3);
         v1 = w0 * g[1] - g[0] * w1 + (g[2] * w3 - g[3] * w2);
         v2 = w0 * g[2] - g[0] * w2 + (g[3] * w1 - g[1] * w3);
@@ -319,6 +367,17 @@ gauge_update_kernel(const GaugeArgs a) {
     const int G = a.g.G, mu = a.mu, p = a.parity;
     const SiteIdx x = site_of(a.g, e, p);
     const SiteIdx xpm = step(a.g, x, mu, +1);
+    // link id of reading G21: 4 lex(x) + mu, lex(x) = 2 e + r
+    const unsigned long long link_id = 4ull * (2ull * (unsigned long long)e + (unsigned long long)x.r) + (unsigned long long)mu;
+    // heatbath: the random-number part of the three Kennedy-Pendleton steps (see kp_precompute)
+    __shared__ double pre_s[MODE == 0 ? 3 * KP_SLOTS * 128 : 1];
+    double* pre = pre_s + threadIdx.x;
+    if (MODE == 0) {
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+            kp_precompute(a.seed, a.tag, ((link_id * 3ull + (unsigned long long)i) * (unsigned long long)(MAXTRY + 1)) * 4ull,
+                          pre + (size_t)i * KP_SLOTS * 128, 128);
+    }
     T A[18];
 #pragma unroll
     for (int i = 0; i < 18; ++i) A[i] = 0;
@@ -340,11 +399,9 @@ gauge_update_kernel(const GaugeArgs a) {
     }
     T L[18];
     gload<RECON, true>(a.gauge, G, p, mu, e, L);
-    // link id of reading G21: 4 lex(x) + mu, lex(x) = 2 e + r
-    const unsigned long long link_id = 4ull * (2ull * (unsigned long long)e + (unsigned long long)x.r) + (unsigned long long)mu;
-    subgroup_step<MODE, 0, 0, 1>(L, A, a.beta, a.seed, a.tag, link_id);
-    subgroup_step<MODE, 1, 1, 2>(L, A, a.beta, a.seed, a.tag, link_id);
-    subgroup_step<MODE, 2, 0, 2>(L, A, a.beta, a.seed, a.tag, link_id);
+    subgroup_step<MODE, 0, 0, 1>(L, A, a.beta, a.seed, a.tag, link_id, pre, 128);
+    subgroup_step<MODE, 1, 1, 2>(L, A, a.beta, a.seed, a.tag, link_id, pre, 128);
+    subgroup_step<MODE, 2, 0, 2>(L, A, a.beta, a.seed, a.tag, link_id, pre, 128);
     if (RECON == 12) orthonormalise_rows01(L);
     gstore<RECON>(a.gauge, G, p, mu, e, L);
 }
