@@ -214,6 +214,63 @@ int lqcd_mtm_host(const void* gauge_canon_host, const void* in_canon_host, void*
 int lqcd_cg_mdagm_host(const void* gauge_canon_host, const void* b_canon_host, void* x_canon_host,
                        double kappa, double mu, double tol, int maxit);
 
+/* ---------------------------------------------------------------------------------------------
+ * Slab decomposition of the time direction over several ranks, one GPU each (the paper lists
+ * multi-GPU as future work).
+ * Rank r of R owns the time slices [r N_t/R, (r+1) N_t/R) (N_t/R even, N_x N_y N_z / 2 a multiple
+ * of 32) as a local lattice in the usual layouts.  Behind the sites of every half-spinor field sit
+ * two ghost time slices: slice t = N_t/R of rank r+1 and slice t = -1 of rank r-1 (cyclically);
+ * behind the time-like links the links U_t(x - t) of slice t = -1.  All are contiguous blocks of
+ * the internal layout at the byte offsets the *_halo calls return, so a halo exchange is two
+ * plain block copies per field (NCCL send/recv, peer-to-peer copies, or stores into peer memory).
+ * The boundary phase of the time direction is applied on the ranks that own the global boundary.
+ * The library computes and never communicates: the caller fills the ghosts of the field a call
+ * reads (stated per call) and all-reduces the two scalars of a CG iteration in place on the
+ * device.  Every hopping launch can be split (part = 1: interior time slices, which read no ghost
+ * and can overlap the exchange; part = 2: the two boundary slices; part = 0: all sites).
+ *
+ * lqcd_select_context: up to 8 independent contexts per process (lattice, format, stream,
+ * workspace, solver state); every call acts on the selected one.  Lets one process hold several
+ * slabs (how the single-GPU tests check the decomposition); the default is context 0.
+ * After lqcd_slab_init, lqcd_gauge_bytes / lqcd_spinor_bytes include the ghosts; lqcd_pack_* /
+ * lqcd_unpack_* take the rank's LOCAL canonical fields; lqcd_dslash_eo covers all local sites
+ * (ghosts of `in` must be current); the single-GPU solvers, force and gauge-update calls return
+ * LQCD_BAD_ARG. */
+int lqcd_select_context(int id);
+int lqcd_slab_init(const int dims_global[4], const double bc_phase[8], int rank, int nranks);
+/* Byte offsets inside an internal half-spinor field: send_lo / send_hi = this rank's first / last
+ * time slice (go to the forward ghost of rank-1 / the backward ghost of rank+1), ghost_fwd /
+ * ghost_bwd = where slice N_t/R of rank+1 / slice -1 of rank-1 are received; bytes per block. */
+int lqcd_slab_spinor_halo(size_t* send_lo, size_t* send_hi, size_t* ghost_fwd, size_t* ghost_bwd, size_t* bytes);
+/* The same for the time-like links of one origin parity (exchanged once, after lqcd_pack_gauge):
+ * send_hi = this rank's last slice (goes to rank+1), ghost_bwd = where rank-1's is received. */
+int lqcd_slab_gauge_halo(int parity, size_t* send_hi, size_t* ghost_bwd, size_t* bytes);
+/* out_p = D_{p,1-p} in on the sites of `part` (reads the ghosts of `in` unless part = 1). */
+int lqcd_slab_dslash(const void* gauge, const void* in, void* out, int parity, double kappa, int part);
+/* Mhat / Mhat^dag in its two hopping launches:
+ *   stage 1: tmp_odd = M_oo^-1 D_oe in         (ghosts of `in`)
+ *   stage 2: out     = M_ee in - D_eo tmp_odd  (ghosts of `tmp_odd`)      even half fields in, out. */
+int lqcd_slab_mhat_stage(const void* gauge, const void* in, void* tmp_odd, void* out, double kappa, double mu,
+                         int dagger, int stage, int part);
+/* CG on Mhat^dag Mhat across the ranks (reading G10), one stage at a time, all asynchronous:
+ *   0  r = p = b, x = 0, own |b|^2 -> sum        [all-reduce sum]     1  rho = |b|^2
+ *   2  t1 = M_oo^-1 D_oe p        (ghosts of p)   3  t2 = Mhat p, partial |t2|^2 (ghosts of t1)
+ *   4  own <p, A p> -> sum        [all-reduce]    5  alpha
+ *   6  t1 = (M_oo^-1)^dag (D_eo)^dag t2 (ghosts of t2)   7  r -= alpha Mhat^dag t2, partial |r|^2 (ghosts of t1)
+ *   8  own |r|^2 -> sum           [all-reduce]    9  beta, convergence flag, x += alpha p, p = r + beta p
+ *   11-14 the four launches of Mhat^dag Mhat x (ghosts of x, t1, t2, t1), 15 own |b - A x|^2 -> sum
+ *   [all-reduce], 16 true residual.
+ * Stages 2, 3, 6, 7, 11-14 take `part`.  lqcd_slab_cg_halo_field(stage) is the field whose ghosts
+ * that stage reads (NULL: none); lqcd_slab_sum_ptr() the device double to all-reduce.  After
+ * convergence the stages are no-ops on the device; lqcd_slab_cg_poll synchronises and reports the
+ * flag; lqcd_slab_cg_end returns the status and fills lqcd_cg_stats. */
+int lqcd_slab_cg_begin(const void* gauge, const void* b, void* x, double kappa, double mu, double tol);
+int lqcd_slab_cg_stage(int stage, int part);
+void* lqcd_slab_cg_halo_field(int stage);
+void* lqcd_slab_sum_ptr(void);
+int lqcd_slab_cg_poll(int* done, int* iters);
+int lqcd_slab_cg_end(int with_true_resid);
+
 /* Number of kernels this library has launched since lqcd_init (all streams). */
 long long lqcd_launch_count(void);
 

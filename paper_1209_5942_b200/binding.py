@@ -25,6 +25,9 @@ SYMBOLS = [
     "lqcd_cg_iterate", "lqcd_cg_finish", "lqcd_cg_stats", "lqcd_cg_mdagm_mixed", "lqcd_cg_outer_iterations", "lqcd_bicgstab_mhat", "lqcd_force_bytes", "lqcd_unpack_force", "lqcd_fermion_force", "lqcd_force_tm", "lqcd_mtm_host", "lqcd_cg_mdagm_host",
     "lqcd_launch_count", "lqcd_set_block_size", "lqcd_profile", "lqcd_profile_read",
     "lqcd_gauge_update", "lqcd_gauge_sweep", "lqcd_plaquette", "lqcd_unpack_gauge",
+    "lqcd_select_context", "lqcd_slab_init", "lqcd_slab_spinor_halo", "lqcd_slab_gauge_halo", "lqcd_slab_dslash",
+    "lqcd_slab_mhat_stage", "lqcd_slab_cg_begin", "lqcd_slab_cg_stage", "lqcd_slab_cg_halo_field",
+    "lqcd_slab_sum_ptr", "lqcd_slab_cg_poll", "lqcd_slab_cg_end",
 ]
 
 
@@ -75,6 +78,16 @@ def _load():
         "lqcd_gauge_sweep": [vp, i32, dbl, u64, u64],
         "lqcd_plaquette": [vp, ctypes.POINTER(dbl)],
         "lqcd_unpack_gauge": [vp, vp],
+        "lqcd_select_context": [i32],
+        "lqcd_slab_init": [ctypes.POINTER(i32), ctypes.POINTER(dbl), i32, i32],
+        "lqcd_slab_spinor_halo": [ctypes.POINTER(ctypes.c_size_t)] * 5,
+        "lqcd_slab_gauge_halo": [i32] + [ctypes.POINTER(ctypes.c_size_t)] * 3,
+        "lqcd_slab_dslash": [vp, vp, vp, i32, dbl, i32],
+        "lqcd_slab_mhat_stage": [vp, vp, vp, vp, dbl, dbl, i32, i32, i32],
+        "lqcd_slab_cg_begin": [vp, vp, vp, dbl, dbl, dbl],
+        "lqcd_slab_cg_stage": [i32, i32],
+        "lqcd_slab_cg_poll": [ctypes.POINTER(i32), ctypes.POINTER(i32)],
+        "lqcd_slab_cg_end": [i32],
         "lqcd_profile": [i32],
         "lqcd_profile_read": [i32, ctypes.POINTER(dbl), ctypes.POINTER(i32)],
     }
@@ -82,11 +95,17 @@ def _load():
         fn = getattr(lib, name)
         fn.argtypes = args
         fn.restype = i32
+    lib.lqcd_slab_cg_halo_field.argtypes = [i32]
+    lib.lqcd_slab_cg_halo_field.restype = vp
+    lib.lqcd_slab_sum_ptr.argtypes = []
+    lib.lqcd_slab_sum_ptr.restype = vp
     return lib
 
 
 _lib = _load()
-_fmt = {"precision": LQCD_DOUBLE, "vh": 0}  # mirrors format and sites per parity, for buffer helpers only
+# mirrors format and sites per parity of each context (lqcd_select_context), for buffer helpers only
+_fmts = [{"precision": LQCD_DOUBLE, "vh": 0} for _ in range(8)]
+_fmt = _fmts[0]
 
 
 def _check(status):
@@ -327,3 +346,173 @@ def download_spinor(s_internal, parity):
     canon = torch.empty((_fmt["vh"], 4, 3), dtype=torch.complex128, device=s_internal.device)
     lqcd_unpack_spinor(s_internal, canon, parity)
     return canon.cpu().numpy()
+
+
+# ---------------------------------------------------------------------------- slab decomposition
+# Several ranks, one GPU each, each owning a slab of time slices (include/lqcd.h "Slab
+# decomposition").  The library computes; what follows only moves halos and sums scalars with
+# torch.distributed (NCCL between GPUs; the same code runs on CPU tensors over gloo in the tests).
+def lqcd_select_context(ctx_id):
+    global _fmt
+    rc = _check(_lib.lqcd_select_context(int(ctx_id)))
+    _fmt = _fmts[int(ctx_id)]
+    return rc
+
+
+def lqcd_slab_init(dims_global, bc_phase, rank, nranks):
+    d = (ctypes.c_int * 4)(*[int(v) for v in dims_global])
+    ph = np.asarray(bc_phase, dtype=np.complex128)
+    p = (ctypes.c_double * 8)(*[float(v) for z in ph for v in (z.real, z.imag)])
+    rc = _check(_lib.lqcd_slab_init(d, p, int(rank), int(nranks)))
+    _fmt["precision"] = LQCD_DOUBLE
+    _fmt["vh"] = int(np.prod([int(v) for v in dims_global])) // (2 * int(nranks))
+    return rc
+
+
+def lqcd_slab_spinor_halo():
+    v = [ctypes.c_size_t() for _ in range(5)]
+    _check(_lib.lqcd_slab_spinor_halo(*[ctypes.byref(x) for x in v]))
+    return dict(zip(("send_lo", "send_hi", "ghost_fwd", "ghost_bwd", "bytes"), (int(x.value) for x in v)))
+
+
+def lqcd_slab_gauge_halo(parity):
+    v = [ctypes.c_size_t() for _ in range(3)]
+    _check(_lib.lqcd_slab_gauge_halo(int(parity), *[ctypes.byref(x) for x in v]))
+    return dict(zip(("send_hi", "ghost_bwd", "bytes"), (int(x.value) for x in v)))
+
+
+def lqcd_slab_dslash(gauge, inp, out, parity, kappa, part=0):
+    return _check(_lib.lqcd_slab_dslash(_ptr(gauge), _ptr(inp), _ptr(out), parity, kappa, part))
+
+
+def lqcd_slab_mhat_stage(gauge, inp, tmp_odd, out, kappa, mu, dagger, stage, part=0):
+    return _check(_lib.lqcd_slab_mhat_stage(_ptr(gauge), _ptr(inp), _ptr(tmp_odd), _ptr(out), kappa, mu, dagger,
+                                            stage, part))
+
+
+def lqcd_slab_cg_begin(gauge, b, x, kappa, mu, tol):
+    return _check(_lib.lqcd_slab_cg_begin(_ptr(gauge), _ptr(b), _ptr(x), kappa, mu, tol))
+
+
+def lqcd_slab_cg_stage(stage, part=0):
+    return _check(_lib.lqcd_slab_cg_stage(stage, part))
+
+
+def lqcd_slab_cg_halo_field(stage):
+    """Raw device pointer (int) of the field whose ghosts `stage` reads, or None."""
+    return _lib.lqcd_slab_cg_halo_field(stage)
+
+
+def lqcd_slab_sum_ptr():
+    return _lib.lqcd_slab_sum_ptr()
+
+
+def lqcd_slab_cg_poll():
+    done, iters = ctypes.c_int(0), ctypes.c_int(0)
+    _check(_lib.lqcd_slab_cg_poll(ctypes.byref(done), ctypes.byref(iters)))
+    return bool(done.value), iters.value
+
+
+def lqcd_slab_cg_end(with_true_resid=True):
+    return _check(_lib.lqcd_slab_cg_end(1 if with_true_resid else 0))
+
+
+class _DevMem:
+    """A raw device allocation as a CUDA-array-interface object (uint8), for torch.as_tensor."""
+
+    def __init__(self, ptr, nbytes):
+        self.__cuda_array_interface__ = {"shape": (int(nbytes),), "typestr": "|u1", "data": (int(ptr), False),
+                                         "version": 2}
+
+
+def device_bytes(ptr, nbytes, device="cuda"):
+    """uint8 tensor view of `nbytes` of device memory at raw pointer `ptr` (no copy)."""
+    return torch.as_tensor(_DevMem(ptr, nbytes), device=device)
+
+
+def slab_exchange_blocks(buf, sends, recvs, rank, world, group=None):
+    """The halo exchange of one field: `buf` is the field as a flat uint8 tensor (device or CPU);
+    sends = [(offset, nbytes, 'prev'|'next'), ...], recvs likewise, posted in order as ONE batch of
+    point-to-point operations (rank r: prev = r-1, next = r+1, cyclically).  Returns the requests;
+    the caller waits on them (or lets later work on the same stream wait, NCCL) before the ghosts
+    are read.  world = 1: the rank is its own neighbour, plain copies."""
+    import torch.distributed as dist
+    if world == 1:
+        for (so, n, _), (ro, _, _) in zip(sends, recvs):
+            buf[ro:ro + n].copy_(buf[so:so + n])
+        return []
+    peer = {"prev": (rank - 1) % world, "next": (rank + 1) % world}
+    ops = []
+    for tag, (off, n, to) in enumerate(sends):
+        ops.append(dist.P2POp(dist.isend, buf[off:off + n], peer[to], group=group, tag=tag))
+    for tag, (off, n, frm) in enumerate(recvs):
+        ops.append(dist.P2POp(dist.irecv, buf[off:off + n], peer[frm], group=group, tag=tag))
+    return dist.batch_isend_irecv(ops)
+
+
+def slab_exchange_spinor(field, rank, world, group=None, wait=True):
+    """Fill the two ghost time slices of an internal half-spinor field (tensor or raw pointer)."""
+    h = lqcd_slab_spinor_halo()
+    if not torch.is_tensor(field):
+        field = device_bytes(field, lqcd_spinor_bytes())
+    n = h["bytes"]
+    # first slice -> forward ghost of the previous rank; last slice -> backward ghost of the next
+    reqs = slab_exchange_blocks(field, [(h["send_lo"], n, "prev"), (h["send_hi"], n, "next")],
+                                [(h["ghost_fwd"], n, "next"), (h["ghost_bwd"], n, "prev")], rank, world, group)
+    if wait:
+        for r in reqs:
+            r.wait()
+        return []
+    return reqs
+
+
+def slab_exchange_gauge(gauge, rank, world, group=None):
+    """Once, after lqcd_pack_gauge: receive the time-like links of the previous rank's last slice."""
+    for parity in (0, 1):
+        h = lqcd_slab_gauge_halo(parity)
+        for r in slab_exchange_blocks(gauge, [(h["send_hi"], h["bytes"], "next")],
+                                      [(h["ghost_bwd"], h["bytes"], "prev")], rank, world, group):
+            r.wait()
+
+
+def slab_cg(gauge, b, x, kappa, mu, tol, maxit, rank, world, group=None, overlap=True, check_every=4):
+    """CG on Mhat^dag Mhat across `world` ranks (one process per GPU, torch.distributed initialised):
+    the stages of lqcd_slab_cg_stage with the halo exchanges and the three all-reduces between
+    them.  overlap: a hopping stage runs its interior sites while its halos are in flight.  Returns
+    the solve status; lqcd_cg_stats() gives iterations and residuals."""
+    import torch.distributed as dist
+    lqcd_slab_cg_begin(gauge, b, x, kappa, mu, tol)
+    total = device_bytes(lqcd_slab_sum_ptr(), 8).view(torch.float64)
+
+    def allreduce():
+        if world > 1:
+            dist.all_reduce(total, group=group)
+
+    def hop(stage):
+        f = lqcd_slab_cg_halo_field(stage)
+        if overlap:
+            reqs = slab_exchange_spinor(f, rank, world, group, wait=False)
+            lqcd_slab_cg_stage(stage, 1)
+            for r in reqs:
+                r.wait()
+            lqcd_slab_cg_stage(stage, 2)
+        else:
+            slab_exchange_spinor(f, rank, world, group)
+            lqcd_slab_cg_stage(stage, 0)
+
+    lqcd_slab_cg_stage(0); allreduce(); lqcd_slab_cg_stage(1)
+    it = 0
+    while it < maxit:
+        hop(2); hop(3)
+        lqcd_slab_cg_stage(4); allreduce(); lqcd_slab_cg_stage(5)
+        hop(6); hop(7)
+        lqcd_slab_cg_stage(8); allreduce(); lqcd_slab_cg_stage(9)
+        it += 1
+        if it % check_every == 0 or it == maxit:
+            done, _ = lqcd_slab_cg_poll()
+            if done:
+                break
+    for stage in (11, 12, 13, 14):
+        hop(stage)
+    lqcd_slab_cg_stage(15); allreduce(); lqcd_slab_cg_stage(16)
+    return lqcd_slab_cg_end(True)

@@ -91,9 +91,20 @@ struct Context {
     bool cg_active = false;
     int st_iters = 0, st_outer = 0;
     double st_rr = 0, st_rt = 0;
+
+    // slab decomposition (lqcd_slab_init): this rank's slab of the time direction
+    bool slab = false;
+    int rank = 0, nranks = 1;
+    int s3 = 0;                      // sites per time slice and parity
+    double* slab_sum = nullptr;      // the rank's partial sum awaiting the caller's all-reduce
 };
 
-Context ctx;
+// lqcd_select_context switches between independent contexts (lattice, format, stream, workspace,
+// solver state): one per slab when several ranks of a slab decomposition share a process (tests).
+constexpr int MAX_CONTEXTS = 8;
+Context g_ctx[MAX_CONTEXTS];
+int g_cur = 0;
+#define ctx (g_ctx[g_cur])
 char g_err[512] = "";
 
 int fail(int code, const char* fmt, ...) {
@@ -137,6 +148,7 @@ void free_all() {
     if (ctx.bscal) cudaFree(ctx.bscal);
     if (ctx.scal_host) cudaFreeHost(ctx.scal_host);
     if (ctx.partials) cudaFree(ctx.partials);
+    if (ctx.slab_sum) cudaFree(ctx.slab_sum);
     for (int i = 0; i < 2; ++i) if (ctx.ev[i]) cudaEventDestroy(ctx.ev[i]);
     void** st[] = {&ctx.st_gauge_canon, &ctx.st_gauge, &ctx.st_spinor_canon, &ctx.st_in, &ctx.st_out};
     for (void** p : st) { if (*p) cudaFree(*p); *p = nullptr; }
@@ -169,7 +181,7 @@ int ensure_scalars() {
 int ensure_workspace(int precision, int nvec) {
     int rc = ensure_scalars();
     if (rc) return rc;
-    const size_t sb = spinor_bytes_of(precision, ctx.geo.G);
+    const size_t sb = spinor_bytes_of(precision, ctx.geo.Gg);
     // t1 (index 3) is needed by lqcd_mtm; the rest only by the solvers (t3 only by BiCGStab)
     const int order[6] = {3, 4, 0, 1, 2, 5};
     for (int k = 0; k < nvec; ++k) {
@@ -318,6 +330,7 @@ int cg_run_impl(int maxit, int (*enqueue)() = enqueue_iteration, const CgScalars
 
 // Synchronise; optionally compute the true residual |b - A x| (one more application of A with
 // the `done` gate off); fill the statistics; return the solve status.
+int cg_finish_stats(bool true_resid);
 int cg_finish_impl(bool true_resid) {
     void** v = ctx.vec[ctx.cg_prec];
     if (true_resid) {
@@ -328,6 +341,11 @@ int cg_finish_impl(bool true_resid) {
         if (rc) return rc;
         CU(launch_true_resid(ctx.cg_prec, n_reals(), ctx.cg_b, q, red(), ctx.scal, ctx.stream));
     }
+    return cg_finish_stats(true_resid);
+}
+
+// Synchronise, fill the statistics of lqcd_cg_stats from the device scalars, return the solve status.
+int cg_finish_stats(bool true_resid) {
     CU(cudaMemcpyAsync(ctx.scal_host, ctx.scal, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx.stream));
     CU(cudaStreamSynchronize(ctx.stream));
     const CgScalars& s = ctx.scal_host[0];
@@ -373,6 +391,13 @@ int lqcd_init(const int dims[4], const double bc_phase[8]) {
     ctx.geo.d2 = make_fastdiv((unsigned)ctx.geo.N2);
     ctx.geo.Vh = (int)(V / 2);
     ctx.geo.G = (ctx.geo.Vh + 31) / 32;
+    ctx.geo.Gg = ctx.geo.G;
+    ctx.s3 = ctx.geo.N0h * ctx.geo.N1 * ctx.geo.N2;
+    ctx.geo.goff_f = -(ctx.geo.N3 - 1) * ctx.s3;   // periodic wrap of the time direction
+    ctx.geo.goff_b = +(ctx.geo.N3 - 1) * ctx.s3;
+    ctx.geo.tph_f = ctx.geo.tph_b = 1;
+    ctx.geo.slab = 0;
+    ctx.slab = false; ctx.rank = 0; ctx.nranks = 1;
     ctx.precision = LQCD_DOUBLE; ctx.recon = 18; ctx.block = LQCD_DEFAULT_BLOCK; ctx.stream = 0;
     g_launches.store(0);
     g_err[0] = 0;
@@ -408,8 +433,8 @@ int lqcd_set_block_size(int threads) {
     return LQCD_OK;
 }
 
-size_t lqcd_gauge_bytes(void) { return ctx.init ? gauge_bytes_of(ctx.precision, ctx.recon, ctx.geo.G) : 0; }
-size_t lqcd_spinor_bytes(void) { return ctx.init ? spinor_bytes_of(ctx.precision, ctx.geo.G) : 0; }
+size_t lqcd_gauge_bytes(void) { return ctx.init ? gauge_bytes_of(ctx.precision, ctx.recon, ctx.geo.Gg) : 0; }
+size_t lqcd_spinor_bytes(void) { return ctx.init ? spinor_bytes_of(ctx.precision, ctx.geo.Gg) : 0; }
 long long lqcd_launch_count(void) { return g_launches.load(); }
 
 int lqcd_profile(int enable) {
@@ -452,6 +477,7 @@ int lqcd_unpack_gauge(const void* internal_dev, void* canon_dev) {
 int lqcd_gauge_update(void* gauge, int mu, int parity, int mode, double beta, unsigned long long seed,
                       unsigned long long tag) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (ctx.slab) return fail(LQCD_BAD_ARG, "lqcd_gauge_update: not available after lqcd_slab_init (use the lqcd_slab_* calls)");
     if (!gauge) return fail(LQCD_BAD_ARG, "lqcd_gauge_update: null pointer");
     if (mu < 0 || mu > 3) return fail(LQCD_BAD_ARG, "mu must be 0..3");
     if (parity != 0 && parity != 1) return fail(LQCD_BAD_ARG, "parity must be 0 or 1");
@@ -475,6 +501,8 @@ int lqcd_gauge_sweep(void* gauge, int mode, double beta, unsigned long long seed
 
 int lqcd_plaquette(const void* gauge, double* plaquette_host) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (ctx.slab) return fail(LQCD_BAD_ARG, "lqcd_plaquette: not available after lqcd_slab_init (use the lqcd_slab_* calls)");
+    if (ctx.slab) return fail(LQCD_BAD_ARG, "lqcd_gauge_sweep: not available after lqcd_slab_init (use the lqcd_slab_* calls)");
     if (!gauge || !plaquette_host) return fail(LQCD_BAD_ARG, "lqcd_plaquette: null pointer");
     int rc = ensure_scalars();
     if (rc) return rc;
@@ -520,6 +548,7 @@ int lqcd_dslash_eo(const void* gauge, const void* in, void* out, int parity, dou
 
 int lqcd_mtm(const void* gauge, const void* in, void* out, double kappa, double mu, int dagger) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (ctx.slab) return fail(LQCD_BAD_ARG, "lqcd_mtm: not available after lqcd_slab_init (use the lqcd_slab_* calls)");
     if (!gauge || !in || !out) return fail(LQCD_BAD_ARG, "lqcd_mtm: null pointer");
     if (in == out) return fail(LQCD_BAD_ARG, "lqcd_mtm: in and out alias");
     if (dagger != 0 && dagger != 1) return fail(LQCD_BAD_ARG, "dagger must be 0 or 1");
@@ -548,6 +577,7 @@ static int hop_aux(const void* gauge, const void* in, const void* aux, void* out
 int lqcd_mtm_full(const void* gauge, const void* in_even, const void* in_odd, void* out_even,
                   void* out_odd, double kappa, double mu) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (ctx.slab) return fail(LQCD_BAD_ARG, "lqcd_mtm_full: not available after lqcd_slab_init (use the lqcd_slab_* calls)");
     if (!gauge || !in_even || !in_odd || !out_even || !out_odd) return fail(LQCD_BAD_ARG, "lqcd_mtm_full: null pointer");
     if (out_even == in_even || out_even == in_odd || out_odd == in_even || out_odd == in_odd || out_even == out_odd)
         return fail(LQCD_BAD_ARG, "lqcd_mtm_full: buffers alias");
@@ -573,6 +603,7 @@ int lqcd_mtm_full(const void* gauge, const void* in_even, const void* in_odd, vo
 int lqcd_solve_full(const void* gauge, const void* eta_even, const void* eta_odd, void* psi_even,
                     void* psi_odd, double kappa, double mu, double tol, int maxit) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (ctx.slab) return fail(LQCD_BAD_ARG, "lqcd_solve_full: not available after lqcd_slab_init (use the lqcd_slab_* calls)");
     if (!gauge || !eta_even || !eta_odd || !psi_even || !psi_odd) return fail(LQCD_BAD_ARG, "lqcd_solve_full: null pointer");
     if (psi_even == eta_even || psi_even == eta_odd || psi_odd == eta_even || psi_odd == eta_odd || psi_even == psi_odd)
         return fail(LQCD_BAD_ARG, "lqcd_solve_full: buffers alias");
@@ -612,6 +643,7 @@ int lqcd_solve_full(const void* gauge, const void* eta_even, const void* eta_odd
 
 int lqcd_cg_setup(const void* gauge, const void* b, void* x, double kappa, double mu, double tol) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (ctx.slab) return fail(LQCD_BAD_ARG, "lqcd_cg_setup: not available after lqcd_slab_init (use the lqcd_slab_* calls)");
     if (!gauge || !b || !x) return fail(LQCD_BAD_ARG, "lqcd_cg_setup: null pointer");
     if (b == x) return fail(LQCD_BAD_ARG, "lqcd_cg_setup: b and x alias");
     int rc = check_scalar(kappa, "kappa");
@@ -652,6 +684,7 @@ int lqcd_cg_mdagm(const void* gauge, const void* b, void* x, double kappa, doubl
 int lqcd_bicgstab_mhat(const void* gauge, const void* b, void* x, double kappa, double mu, double tol,
                        int maxit) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (ctx.slab) return fail(LQCD_BAD_ARG, "lqcd_bicgstab_mhat: not available after lqcd_slab_init (use the lqcd_slab_* calls)");
     if (!gauge || !b || !x) return fail(LQCD_BAD_ARG, "lqcd_bicgstab_mhat: null pointer");
     if (b == x) return fail(LQCD_BAD_ARG, "lqcd_bicgstab_mhat: b and x alias");
     if (maxit < 1) return fail(LQCD_BAD_ARG, "maxit must be >= 1");
@@ -694,6 +727,7 @@ int lqcd_unpack_force(const void* force_internal_dev, void* canon_dev) {
 int lqcd_fermion_force(const void* gauge, const void* x_even, const void* x_odd, const void* y_even,
                        const void* y_odd, void* force, double kappa) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (ctx.slab) return fail(LQCD_BAD_ARG, "lqcd_fermion_force: not available after lqcd_slab_init (use the lqcd_slab_* calls)");
     if (!gauge || !x_even || !x_odd || !y_even || !y_odd || !force) return fail(LQCD_BAD_ARG, "lqcd_fermion_force: null pointer");
     int rc = check_scalar(kappa, "kappa");
     if (rc) return rc;
@@ -709,6 +743,7 @@ int lqcd_fermion_force(const void* gauge, const void* x_even, const void* x_odd,
 int lqcd_force_tm(const void* gauge, const void* phi, void* force, double kappa, double mu, double tol,
                   int maxit) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (ctx.slab) return fail(LQCD_BAD_ARG, "lqcd_force_tm: not available after lqcd_slab_init (use the lqcd_slab_* calls)");
     if (!gauge || !phi || !force) return fail(LQCD_BAD_ARG, "lqcd_force_tm: null pointer");
     if (maxit < 1) return fail(LQCD_BAD_ARG, "maxit must be >= 1");
     int rc = check_scalar(kappa, "kappa");
@@ -739,6 +774,7 @@ int lqcd_cg_mdagm_mixed(const void* gauge_double, int recon_double, const void* 
                         int recon_single, const void* b, void* x, double kappa, double mu, double tol,
                         int maxit, double inner_tol) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (ctx.slab) return fail(LQCD_BAD_ARG, "lqcd_cg_mdagm_mixed: not available after lqcd_slab_init (use the lqcd_slab_* calls)");
     if (!gauge_double || !gauge_single || !b || !x) return fail(LQCD_BAD_ARG, "lqcd_cg_mdagm_mixed: null pointer");
     if (b == x) return fail(LQCD_BAD_ARG, "lqcd_cg_mdagm_mixed: b and x alias");
     if ((recon_double != 18 && recon_double != 12) || (recon_single != 18 && recon_single != 12))
@@ -842,6 +878,7 @@ static int fetch_output(void* out_host) {
 int lqcd_mtm_host(const void* gauge_canon_host, const void* in_canon_host, void* out_canon_host,
                   double kappa, double mu, int dagger) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (ctx.slab) return fail(LQCD_BAD_ARG, "lqcd_mtm_host: not available after lqcd_slab_init (use the lqcd_slab_* calls)");
     if (!gauge_canon_host || !in_canon_host || !out_canon_host) return fail(LQCD_BAD_ARG, "lqcd_mtm_host: null pointer");
     int rc = stage_inputs(gauge_canon_host, in_canon_host);
     if (rc) return rc;
@@ -852,6 +889,7 @@ int lqcd_mtm_host(const void* gauge_canon_host, const void* in_canon_host, void*
 int lqcd_cg_mdagm_host(const void* gauge_canon_host, const void* b_canon_host, void* x_canon_host,
                        double kappa, double mu, double tol, int maxit) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (ctx.slab) return fail(LQCD_BAD_ARG, "lqcd_cg_mdagm_host: not available after lqcd_slab_init (use the lqcd_slab_* calls)");
     if (!gauge_canon_host || !b_canon_host || !x_canon_host) return fail(LQCD_BAD_ARG, "lqcd_cg_mdagm_host: null pointer");
     int rc = stage_inputs(gauge_canon_host, b_canon_host);
     if (rc) return rc;
@@ -860,5 +898,215 @@ int lqcd_cg_mdagm_host(const void* gauge_canon_host, const void* b_canon_host, v
     rc = fetch_output(x_canon_host);
     return rc ? rc : status;
 }
+
+// ------------------------------------------------------------------------------------------------
+// Slab decomposition of the time direction over several ranks, one GPU each (
+// DESIGN.md section 7).  The library computes; the caller moves the halos and sums the scalars.
+// ------------------------------------------------------------------------------------------------
+int lqcd_select_context(int id) {
+    if (id < 0 || id >= MAX_CONTEXTS) return fail(LQCD_BAD_ARG, "context id must be in [0, %d)", MAX_CONTEXTS);
+    g_cur = id;
+    return LQCD_OK;
+}
+
+int lqcd_slab_init(const int dims_global[4], const double bc_phase[8], int rank, int nranks) {
+    if (!dims_global || !bc_phase) return fail(LQCD_BAD_ARG, "lqcd_slab_init: null argument");
+    if (nranks < 1 || rank < 0 || rank >= nranks) return fail(LQCD_BAD_ARG, "rank %d of %d", rank, nranks);
+    if (dims_global[3] % nranks) return fail(LQCD_BAD_DIMS, "N_t = %d is not a multiple of %d ranks", dims_global[3], nranks);
+    int loc[4] = {dims_global[0], dims_global[1], dims_global[2], dims_global[3] / nranks};
+    // the local extent must be even so that a site's parity in the slab equals its global parity
+    int rc = lqcd_init(loc, bc_phase);
+    if (rc) return rc;
+    if (ctx.s3 % 32) {
+        free_all();
+        return fail(LQCD_BAD_DIMS, "slab mode needs N_x N_y N_z / 2 = %d sites per time slice and parity to be a multiple of 32",
+                    (loc[0] / 2) * loc[1] * loc[2]);
+    }
+    ctx.slab = true; ctx.rank = rank; ctx.nranks = nranks;
+    ctx.geo.slab = 1;
+    const int Vh = ctx.geo.Vh;                        // = 32 G: no pad sites in slab mode
+    ctx.geo.goff_f = Vh - (ctx.geo.N3 - 1) * ctx.s3;  // x3 = N3 - 1, spatial index s  ->  Vh + s
+    ctx.geo.goff_b = Vh + ctx.s3;                     // x3 = 0,      spatial index s  ->  Vh + s3 + s
+    ctx.geo.tph_f = (rank == nranks - 1);
+    ctx.geo.tph_b = (rank == 0);
+    ctx.geo.Gg = ctx.geo.G + 2 * (ctx.s3 / 32);
+    return LQCD_OK;
+}
+
+static size_t site_bytes() { return spinor_bytes_of(ctx.precision, 1) / 32; }
+
+int lqcd_slab_spinor_halo(size_t* send_lo, size_t* send_hi, size_t* ghost_fwd, size_t* ghost_bwd, size_t* bytes) {
+    if (!ctx.init || !ctx.slab) return fail(LQCD_NOT_INITIALISED, "lqcd_slab_spinor_halo: no slab set up");
+    const size_t sb = site_bytes(), Vh = ctx.geo.Vh, s3 = ctx.s3;
+    if (send_lo) *send_lo = 0;
+    if (send_hi) *send_hi = (Vh - s3) * sb;
+    if (ghost_fwd) *ghost_fwd = Vh * sb;
+    if (ghost_bwd) *ghost_bwd = (Vh + s3) * sb;
+    if (bytes) *bytes = s3 * sb;
+    return LQCD_OK;
+}
+
+int lqcd_slab_gauge_halo(int parity, size_t* send_hi, size_t* ghost_bwd, size_t* bytes) {
+    if (!ctx.init || !ctx.slab) return fail(LQCD_NOT_INITIALISED, "lqcd_slab_gauge_halo: no slab set up");
+    if (parity != 0 && parity != 1) return fail(LQCD_BAD_ARG, "parity must be 0 or 1");
+    const size_t gb = (size_t)ctx.recon * 32 * (ctx.precision == 0 ? 8 : 4);   // bytes of one group of one (parity, mu) array
+    const size_t base = ((size_t)(parity * 4 + 3) * ctx.geo.Gg) * gb;          // mu = 3
+    if (send_hi) *send_hi = base + (size_t)((ctx.geo.Vh - ctx.s3) / 32) * gb;
+    if (ghost_bwd) *ghost_bwd = base + (size_t)((ctx.geo.Vh + ctx.s3) / 32) * gb;
+    if (bytes) *bytes = (size_t)(ctx.s3 / 32) * gb;
+    return LQCD_OK;
+}
+
+// part: 0 every site, 1 interior time slices (no ghost needed), 2 the two boundary time slices
+static int slab_range(int part, SiteRange* r) {
+    const int Vh = ctx.geo.Vh, s3 = ctx.s3;
+    const int inner = Vh - 2 * s3 > 0 ? Vh - 2 * s3 : 0;   // N3 = 2: every slice is a boundary slice
+    if (part == 0) { r->base = 0; r->count = Vh; r->n1 = Vh; r->skip = 0; }
+    else if (part == 1) { r->base = s3; r->count = inner; r->n1 = inner; r->skip = 0; }
+    else if (part == 2) { r->base = 0; r->count = Vh - inner; r->n1 = s3; r->skip = inner; }
+    else return fail(LQCD_BAD_ARG, "part must be 0 (all), 1 (interior) or 2 (boundary)");
+    return LQCD_OK;
+}
+
+int lqcd_slab_dslash(const void* gauge, const void* in, void* out, int parity, double kappa, int part) {
+    if (!ctx.init || !ctx.slab) return fail(LQCD_NOT_INITIALISED, "lqcd_slab_dslash: no slab set up");
+    if (!gauge || !in || !out || in == out) return fail(LQCD_BAD_ARG, "lqcd_slab_dslash: null or aliased pointer");
+    if (parity != 0 && parity != 1) return fail(LQCD_BAD_ARG, "parity must be 0 or 1");
+    int rc = check_scalar(kappa, "kappa");
+    if (rc) return rc;
+    SiteRange rg;
+    if ((rc = slab_range(part, &rg))) return rc;
+    Epilogue ep = {};
+    ep.cu_re = -kappa; ep.cd_re = -kappa;
+    Reduction none = {nullptr};
+    CU(launch_hopping(ctx.precision, ctx.recon, 0, 0, ctx.geo, ep, gauge, in, out, nullptr, parity, 0, none, nullptr,
+                      ctx.block, ctx.stream, &rg));
+    return LQCD_OK;
+}
+
+// One of the two hopping launches of Mhat / Mhat^dag (api.cu header), on the sites of `part`:
+//   stage 1: tmp_odd = M_oo^-1 D_oe in          (needs the ghosts of `in`)
+//   stage 2: out     = M_ee in - D_eo tmp_odd   (needs the ghosts of `tmp_odd`)
+// fuse, scal as in apply_mhat (the sums stay partial: see slab_local_sum).
+static int slab_mhat_stage(const void* gauge, const void* in, void* tmp_odd, void* out, double kappa, double mu,
+                           int dagger, int stage, int part, int fuse, CgScalars* scal) {
+    SiteRange rg;
+    int rc = slab_range(part, &rg);
+    if (rc) return rc;
+    const double c = (dagger ? -1.0 : 1.0) * 2.0 * kappa * mu;
+    if (stage == 1) {
+        const double d = 1.0 + c * c;
+        Epilogue e1 = {};
+        e1.cu_re = -kappa / d; e1.cu_im = +kappa * c / d;
+        e1.cd_re = -kappa / d; e1.cd_im = -kappa * c / d;
+        CU(launch_hopping(ctx.precision, ctx.recon, dagger, 0, ctx.geo, e1, gauge, in, tmp_odd, nullptr, 1, 0, red(), scal,
+                          ctx.block, ctx.stream, &rg));
+    } else {
+        const double k2 = (kappa != 0.0) ? kappa : 1.0;
+        Epilogue e2 = {};
+        e2.cu_re = k2; e2.cd_re = k2;
+        e2.du_re = 1.0 / k2; e2.du_im = c / k2;
+        e2.dd_re = 1.0 / k2; e2.dd_im = -c / k2;
+        e2.su_re = 1.0 / k2; e2.sd_re = 1.0 / k2;
+        const int mode = (fuse == FUSE_PAP) ? 2 : (fuse == FUSE_R) ? 3 : 1;
+        CU(launch_hopping(ctx.precision, ctx.recon, dagger, mode, ctx.geo, e2, gauge, tmp_odd, out, in, 0, 0, red(), scal,
+                          ctx.block, ctx.stream, &rg));
+    }
+    return LQCD_OK;
+}
+
+int lqcd_slab_mhat_stage(const void* gauge, const void* in, void* tmp_odd, void* out, double kappa, double mu,
+                         int dagger, int stage, int part) {
+    if (!ctx.init || !ctx.slab) return fail(LQCD_NOT_INITIALISED, "lqcd_slab_mhat_stage: no slab set up");
+    if (!gauge || !in || !tmp_odd || !out || in == out || in == tmp_odd || tmp_odd == out)
+        return fail(LQCD_BAD_ARG, "lqcd_slab_mhat_stage: null or aliased pointer");
+    if ((dagger != 0 && dagger != 1) || (stage != 1 && stage != 2)) return fail(LQCD_BAD_ARG, "dagger must be 0 or 1, stage 1 or 2");
+    int rc = check_scalar(kappa, "kappa");
+    if (rc) return rc;
+    if ((rc = check_scalar(mu, "mu"))) return rc;
+    if ((rc = ensure_scalars())) return rc;
+    return slab_mhat_stage(gauge, in, tmp_odd, out, kappa, mu, dagger, stage, part, FUSE_NONE, nullptr);
+}
+
+int lqcd_slab_cg_begin(const void* gauge, const void* b, void* x, double kappa, double mu, double tol) {
+    if (!ctx.init || !ctx.slab) return fail(LQCD_NOT_INITIALISED, "lqcd_slab_cg_begin: no slab set up");
+    if (!gauge || !b || !x || b == x) return fail(LQCD_BAD_ARG, "lqcd_slab_cg_begin: null or aliased pointer");
+    int rc = check_scalar(kappa, "kappa");
+    if (rc) return rc;
+    if ((rc = check_scalar(mu, "mu"))) return rc;
+    if (!std::isfinite(tol) || tol < 0.0) return fail(LQCD_BAD_ARG, "tol must be finite and >= 0");
+    if ((rc = ensure_workspace(ctx.precision, 5))) return rc;
+    if (!ctx.slab_sum) CU(cudaMalloc(&ctx.slab_sum, 2 * sizeof(double)));
+    ctx.cg_prec = ctx.precision; ctx.cg_recon = ctx.recon;
+    ctx.cg_gauge = gauge; ctx.cg_b = b; ctx.cg_x = x;
+    ctx.cg_kappa = kappa; ctx.cg_mu = mu; ctx.cg_tol = tol;
+    ctx.cg_active = true;
+    return LQCD_OK;
+}
+
+void* lqcd_slab_sum_ptr(void) { return (ctx.init && ctx.slab) ? (void*)ctx.slab_sum : nullptr; }
+
+// The field whose ghost slices stage `stage` reads (NULL: none).
+void* lqcd_slab_cg_halo_field(int stage) {
+    if (!ctx.init || !ctx.slab || !ctx.cg_active) return nullptr;
+    void** v = ctx.vec[ctx.cg_prec];
+    switch (stage) {
+        case 2: return v[1];            // p
+        case 3: case 7: case 12: case 14: return v[3];   // t1
+        case 6: case 13: return v[4];   // t2
+        case 11: return ctx.cg_x;
+        default: return nullptr;
+    }
+}
+
+int lqcd_slab_cg_stage(int stage, int part) {
+    if (!ctx.init || !ctx.slab) return fail(LQCD_NOT_INITIALISED, "lqcd_slab_cg_stage: no slab set up");
+    if (!ctx.cg_active) return fail(LQCD_BAD_ARG, "lqcd_slab_cg_stage: no solve set up (lqcd_slab_cg_begin)");
+    void** v = ctx.vec[ctx.cg_prec];
+    void *r = v[0], *p = v[1], *q = v[2], *t1 = v[3], *t2 = v[4];
+    const size_t n = n_reals();
+    const int np = hopping_partials(ctx.geo.Vh, ctx.block);
+    const void* U = ctx.cg_gauge;
+    const double ka = ctx.cg_kappa, mu = ctx.cg_mu;
+    switch (stage) {
+        case 0:   // r = p = b, x = 0, the rank's |b|^2
+            CU(launch_cg_init(ctx.cg_prec, n, ctx.cg_b, ctx.cg_x, r, p, ctx.cg_tol, red(), ctx.scal, ctx.stream, ctx.slab_sum));
+            return LQCD_OK;
+        case 1: CU(launch_finalize(FIN_BB, red(), 0, ctx.cg_tol, ctx.scal, ctx.stream, ctx.slab_sum, 1)); return LQCD_OK;
+        case 2: return slab_mhat_stage(U, p, t1, t2, ka, mu, 0, 1, part, FUSE_NONE, ctx.scal);
+        case 3: return slab_mhat_stage(U, p, t1, t2, ka, mu, 0, 2, part, FUSE_PAP, ctx.scal);
+        case 4: CU(launch_finalize(FIN_PAP, red(), np, 0.0, ctx.scal, ctx.stream, ctx.slab_sum, 0)); return LQCD_OK;
+        case 5: CU(launch_finalize(FIN_PAP, red(), 0, 0.0, ctx.scal, ctx.stream, ctx.slab_sum, 1)); return LQCD_OK;
+        case 6: return slab_mhat_stage(U, t2, t1, r, ka, mu, 1, 1, part, FUSE_NONE, ctx.scal);
+        case 7: return slab_mhat_stage(U, t2, t1, r, ka, mu, 1, 2, part, FUSE_R, ctx.scal);
+        case 8: CU(launch_finalize(FIN_RHO, red(), np, 0.0, ctx.scal, ctx.stream, ctx.slab_sum, 0)); return LQCD_OK;
+        case 9:
+            CU(launch_finalize(FIN_RHO, red(), 0, 0.0, ctx.scal, ctx.stream, ctx.slab_sum, 1));
+            CU(launch_cg_update_xp(ctx.cg_prec, n, ctx.cg_x, p, r, 0, ctx.scal, ctx.stream));
+            return LQCD_OK;
+        // true residual |b - Mhat^dag Mhat x| (the `done` gate off)
+        case 11: return slab_mhat_stage(U, ctx.cg_x, t1, t2, ka, mu, 0, 1, part, FUSE_NONE, nullptr);
+        case 12: return slab_mhat_stage(U, ctx.cg_x, t1, t2, ka, mu, 0, 2, part, FUSE_NONE, nullptr);
+        case 13: return slab_mhat_stage(U, t2, t1, q, ka, mu, 1, 1, part, FUSE_NONE, nullptr);
+        case 14: return slab_mhat_stage(U, t2, t1, q, ka, mu, 1, 2, part, FUSE_NONE, nullptr);
+        case 15: CU(launch_true_resid(ctx.cg_prec, n, ctx.cg_b, q, red(), ctx.scal, ctx.stream, ctx.slab_sum)); return LQCD_OK;
+        case 16: CU(launch_finalize(FIN_TRUE, red(), 0, 0.0, ctx.scal, ctx.stream, ctx.slab_sum, 1)); return LQCD_OK;
+        default: return fail(LQCD_BAD_ARG, "lqcd_slab_cg_stage: unknown stage %d", stage);
+    }
+}
+
+// Synchronise and read the solver's scalars: *done = 1 once converged or broken down.
+int lqcd_slab_cg_poll(int* done, int* iters) {
+    if (!ctx.init || !ctx.slab || !ctx.cg_active) return fail(LQCD_BAD_ARG, "lqcd_slab_cg_poll: no solve set up");
+    CgScalars s;
+    CU(cudaMemcpyAsync(&ctx.scal_host[2], ctx.scal, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx.stream));
+    CU(cudaStreamSynchronize(ctx.stream));
+    s = ctx.scal_host[2];
+    if (done) *done = s.done;
+    if (iters) *iters = s.iters;
+    return LQCD_OK;
+}
+
+int lqcd_slab_cg_end(int with_true_resid) { return (ctx.init && ctx.slab && ctx.cg_active) ? cg_finish_stats(with_true_resid != 0) : fail(LQCD_BAD_ARG, "lqcd_slab_cg_end: no solve set up"); }
 
 }  // extern "C"

@@ -60,14 +60,15 @@ struct HopArgs {
     int reverse;   // traverse the sites in descending order (see lqcd_internal.h "snake order")
     Reduction red;
     CgScalars* scal;
+    SiteRange rg;
 };
 
-template <typename T, int RECON, int MU, int FWD, int DAG>
+template <typename T, int RECON, int MU, int FWD, int DAG, bool SLAB>
 __device__ __forceinline__ void hop(T (&acc)[24], const HopArgs& a, int e, int e_nb, bool wrap) {
     constexpr int S = (FWD ? -1 : +1) * (DAG ? -1 : +1);
     T psi[24], u[18], h[12], chi[12];
     load_spinor(a.in, e_nb, psi);
-    load_link<RECON>(a.gauge, a.g.G, FWD ? a.out_parity : 1 - a.out_parity, MU, FWD ? e : e_nb, u);
+    load_link<RECON>(a.gauge, SLAB ? a.g.Gg : a.g.G, FWD ? a.out_parity : 1 - a.out_parity, MU, FWD ? e : e_nb, u);
     project<MU, S>(psi, h);
     if (FWD) su3_mul(u, h, chi);
     else     su3_dag_mul(u, h, chi);
@@ -83,19 +84,22 @@ __device__ __forceinline__ void hop(T (&acc)[24], const HopArgs& a, int e, int e
     accumulate<MU, S>(acc, chi);
 }
 
-template <typename T, int RECON, int DAG, int MODE>
+template <typename T, int RECON, int DAG, int MODE, bool SLAB>
 __global__ void __launch_bounds__(LQCD_HOP_MAX_THREADS, (RECON == 12) ? (sizeof(T) == 4 ? LQCD_HOP_MIN_BLOCKS_F12 : LQCD_HOP_MIN_BLOCKS_D12)
                                                                       : LQCD_HOP_MIN_BLOCKS)
 hopping_kernel(const HopArgs a) {
     if (a.scal != nullptr && a.scal->done) return;
     const int Vh = a.g.Vh;
     const int blk = a.reverse ? (int)(gridDim.x - 1 - blockIdx.x) : (int)blockIdx.x;
-    const int e = blk * blockDim.x + threadIdx.x;
+    // single lattice: site e of all Vh; slab mode: site i of the launch's SiteRange
+    const int i = blk * blockDim.x + threadIdx.x;
+    const bool live = SLAB ? (i < a.rg.count) : (i < Vh);
+    const int e = SLAB ? a.rg.base + i + (i >= a.rg.n1 ? a.rg.skip : 0) : i;
     double nrm = 0.0;
     // MODE 3: alpha = rho / <p, A p> and its inverse were left in the device scalars by
     // finalize(FIN_PAP), which also ends the solve (done = 1, caught above) on a breakdown.
     const double alpha = (MODE == 3) ? a.scal->alpha : 1.0;
-    if (e < Vh) {
+    if (live) {
         // a1: e -> (x0h, x1, x2, x3); r = x0 mod 2 follows from the parity
         const int N0h = a.g.N0h, N1 = a.g.N1, N2 = a.g.N2, N3 = a.g.N3;
         int x0h, x1, x2, x3;
@@ -140,23 +144,28 @@ hopping_kernel(const HopArgs a) {
         {   // mu = 0: neighbour x0h' = x0h + r (forward), x0h + r - 1 (backward)
             const bool wf = (r == 1) && (x0h == N0h - 1);
             const bool wb = (r == 0) && (x0h == 0);
-            hop<T, RECON, 0, 1, DAG>(acc, a, e, wf ? e - (N0h - 1) : e + r, wf);
-            hop<T, RECON, 0, 0, DAG>(acc, a, e, wb ? e + (N0h - 1) : e + r - 1, wb);
+            hop<T, RECON, 0, 1, DAG, SLAB>(acc, a, e, wf ? e - (N0h - 1) : e + r, wf);
+            hop<T, RECON, 0, 0, DAG, SLAB>(acc, a, e, wb ? e + (N0h - 1) : e + r - 1, wb);
         }
         {
             const bool wf = (x1 == N1 - 1), wb = (x1 == 0);
-            hop<T, RECON, 1, 1, DAG>(acc, a, e, wf ? e - (N1 - 1) * s1 : e + s1, wf);
-            hop<T, RECON, 1, 0, DAG>(acc, a, e, wb ? e + (N1 - 1) * s1 : e - s1, wb);
+            hop<T, RECON, 1, 1, DAG, SLAB>(acc, a, e, wf ? e - (N1 - 1) * s1 : e + s1, wf);
+            hop<T, RECON, 1, 0, DAG, SLAB>(acc, a, e, wb ? e + (N1 - 1) * s1 : e - s1, wb);
         }
         {
             const bool wf = (x2 == N2 - 1), wb = (x2 == 0);
-            hop<T, RECON, 2, 1, DAG>(acc, a, e, wf ? e - (N2 - 1) * s2 : e + s2, wf);
-            hop<T, RECON, 2, 0, DAG>(acc, a, e, wb ? e + (N2 - 1) * s2 : e - s2, wb);
+            hop<T, RECON, 2, 1, DAG, SLAB>(acc, a, e, wf ? e - (N2 - 1) * s2 : e + s2, wf);
+            hop<T, RECON, 2, 0, DAG, SLAB>(acc, a, e, wb ? e + (N2 - 1) * s2 : e - s2, wb);
         }
         {
             const bool wf = (x3 == N3 - 1), wb = (x3 == 0);
-            hop<T, RECON, 3, 1, DAG>(acc, a, e, wf ? e - (N3 - 1) * s3 : e + s3, wf);
-            hop<T, RECON, 3, 0, DAG>(acc, a, e, wb ? e + (N3 - 1) * s3 : e - s3, wb);
+            if (SLAB) {   // across the rank's t boundary: the ghost slices (Geometry::goff_*)
+                hop<T, RECON, 3, 1, DAG, SLAB>(acc, a, e, wf ? e + a.g.goff_f : e + s3, wf && a.g.tph_f);
+                hop<T, RECON, 3, 0, DAG, SLAB>(acc, a, e, wb ? e + a.g.goff_b : e - s3, wb && a.g.tph_b);
+            } else {      // the periodic wrap (kept in this form: the goff form costs 70 B of spills)
+                hop<T, RECON, 3, 1, DAG, SLAB>(acc, a, e, wf ? e - (N3 - 1) * s3 : e + s3, wf);
+                hop<T, RECON, 3, 0, DAG, SLAB>(acc, a, e, wb ? e + (N3 - 1) * s3 : e - s3, wb);
+            }
         }
 
         // a6/a7: epilogue, complex coefficient per chirality
@@ -182,7 +191,7 @@ hopping_kernel(const HopArgs a) {
                                  (a.ep.cd_re * a.ep.cd_re + a.ep.cd_im * a.ep.cd_im) * nd);
         }
     }
-    if (e >= Vh && e < a.g.G * 32) {  // pad sites of the last group hold zeros
+    if (!SLAB && !live && e < a.g.G * 32) {  // pad sites of the last group hold zeros
         T z[24];
 #pragma unroll
         for (int i = 0; i < 24; ++i) z[i] = 0;
@@ -190,16 +199,17 @@ hopping_kernel(const HopArgs a) {
     }
     if (MODE >= 2) {  // one partial per warp, plain store; summed by launch_finalize(FIN_PAP / FIN_RHO)
         nrm = warp_sum(nrm);
-        if ((threadIdx.x & 31) == 0) a.red.partials[(blk * blockDim.x + threadIdx.x) >> 5] = nrm;
+        if ((threadIdx.x & 31) == 0 && (!SLAB || live)) a.red.partials[e >> 5] = nrm;
     }
 }
 
 template <typename T, int RECON>
 cudaError_t launch_tr(int dagger, int mode, const HopArgs& a, int block, cudaStream_t st) {
-    const int grid = (a.g.Vh + block - 1) / block;
+    const int grid = (a.rg.count + block - 1) / block;
 #define LQCD_HOP_CASE(D, M)                                                        \
     if (dagger == D && mode == M) {                                                \
-        hopping_kernel<T, RECON, D, M><<<grid, block, 0, st>>>(a);                  \
+        if (a.g.slab) hopping_kernel<T, RECON, D, M, true><<<grid, block, 0, st>>>(a);  \
+        else          hopping_kernel<T, RECON, D, M, false><<<grid, block, 0, st>>>(a); \
         return cudaGetLastError();                                                 \
     }
     LQCD_HOP_CASE(0, 0) LQCD_HOP_CASE(0, 1) LQCD_HOP_CASE(0, 2)
@@ -210,16 +220,20 @@ cudaError_t launch_tr(int dagger, int mode, const HopArgs& a, int block, cudaStr
 
 }  // namespace
 
+// one partial per warp of live sites, indexed by e >> 5 whatever the launch's SiteRange and block size
 int hopping_partials(int Vh, int block) {
-    if (block <= 0 || block > LQCD_HOP_MAX_THREADS || (block % 32) != 0) block = LQCD_HOP_MAX_THREADS;
-    return ((Vh + block - 1) / block) * (block / 32);
+    (void)block;
+    return (Vh + 31) / 32;
 }
 
 cudaError_t launch_hopping(int precision, int recon, int dagger, int mode, const Geometry& g,
                            const Epilogue& ep, const void* gauge, const void* in, void* out,
                            const void* aux, int out_parity, int reverse, Reduction red,
-                           CgScalars* scal, int block, cudaStream_t st) {
+                           CgScalars* scal, int block, cudaStream_t st, const SiteRange* range) {
     HopArgs a;
+    if (range) a.rg = *range;
+    else { a.rg.base = 0; a.rg.count = g.Vh; a.rg.n1 = g.Vh; a.rg.skip = 0; }
+    if (a.rg.count <= 0) return cudaSuccess;
     a.reverse = reverse;
     a.gauge = gauge; a.in = in; a.out = out; a.aux = aux;
     a.g = g; a.ep = ep; a.out_parity = out_parity; a.red = red; a.scal = scal;

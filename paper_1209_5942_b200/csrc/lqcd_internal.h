@@ -54,6 +54,23 @@ struct Geometry {
     int G;                // groups of 32 sites per parity = ceil(Vh / 32)
     FastDiv d0h, d1, d2;  // division by N0h, N1, N2
     double ph_re[4], ph_im[4];
+    // Time-direction neighbours across the lattice's (or, in slab mode, the rank's) t boundary.
+    // Single GPU: the wrap, goff_f = -(N3 - 1) s3, goff_b = +(N3 - 1) s3 (s3 = sites per time slice
+    // and parity).  Slab mode (lqcd_slab_init): ghost time slices appended behind the G groups of a
+    // field, forward ghost (slice t = N3 of the next rank) at site index 32 G + s, backward ghost
+    // (slice t = -1 of the previous rank) at 32 G + s3 + s; the boundary phase applies only on the
+    // rank that owns the global boundary (tph_f on the last rank, tph_b on the first).
+    int slab;             // 1 after lqcd_slab_init
+    int goff_f, goff_b;
+    int tph_f, tph_b;
+    int Gg;               // groups per (parity, mu) array of the gauge field: G, or G + ghost groups
+};
+
+// Which output sites a hopping launch covers: site i of the launch is e = base + i (+ skip if
+// i >= n1).  All sites: base 0, n1 = count = Vh.  Slab mode splits a launch into the interior
+// (no ghost needed: overlaps the halo exchange) and the two boundary time slices.
+struct SiteRange {
+    int base, count, n1, skip;
 };
 
 #ifdef __CUDACC__
@@ -130,15 +147,15 @@ enum { FIN_BI_INIT = 0, FIN_BI_SIGMA = 1, FIN_BI_OMEGA = 2, FIN_BI_R = 3 };
 cudaError_t launch_hopping(int precision, int recon, int dagger, int mode, const Geometry& g,
                            const Epilogue& ep, const void* gauge, const void* in, void* out,
                            const void* aux, int out_parity, int reverse, Reduction red,
-                           CgScalars* scal, int block, cudaStream_t st);
+                           CgScalars* scal, int block, cudaStream_t st, const SiteRange* range = nullptr);
 
 // vector_ops.cu  (n = number of reals in a half-spinor field incl. padding = 24 * 32 * G)
 cudaError_t launch_cg_init(int precision, size_t n, const void* b, void* x, void* r, void* p,
-                           double tol, Reduction red, CgScalars* scal, cudaStream_t st);
+                           double tol, Reduction red, CgScalars* scal, cudaStream_t st, double* sum_io = nullptr);
 cudaError_t launch_cg_update_xp(int precision, size_t n, void* x, void* p, const void* r, int reverse,
                                 CgScalars* scal, cudaStream_t st);
 cudaError_t launch_true_resid(int precision, size_t n, const void* b, const void* ax, Reduction red,
-                              CgScalars* scal, cudaStream_t st);
+                              CgScalars* scal, cudaStream_t st, double* sum_io = nullptr);
 // out = a_chi * in, a_chi = (ur, ui) on the upper and (dr, di) on the lower chirality
 cudaError_t launch_diag_scale(int precision, size_t n, const void* in, void* out, double ur, double ui,
                               double dr, double di, cudaStream_t st);
@@ -149,7 +166,7 @@ cudaError_t launch_residual(size_t n, const void* b, const void* ax, void* r, Re
                             CgScalars* scal, cudaStream_t st);  // r = b - ax (double), |r|^2 -> resid_true
 // sums red.partials[0..n_partials) in a fixed order and applies the FIN_* action to *scal
 cudaError_t launch_finalize(int fin, Reduction red, int n_partials, double tol, CgScalars* scal,
-                            cudaStream_t st);
+                            cudaStream_t st, double* sum_io = nullptr, int apply = 0);
 // BiCGStab vector kernels (vector_ops.cu); partial sums use up to 3 * vector_grid(n) doubles
 cudaError_t launch_bicg_init(int precision, size_t n, const void* b, void* x, void* r, void* p, double tol,
                              Reduction red, BiScalars* bs, cudaStream_t st);

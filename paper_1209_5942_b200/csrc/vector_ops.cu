@@ -59,22 +59,33 @@ __device__ __forceinline__ void block_partial(double v, Reduction red) {
 
 // One block: adds the partials in index order (thread-strided, then a fixed tree) and applies
 // the scalar step of the recurrence on the device.
+//
+// Slab mode (several ranks, lqcd_slab_*) splits it around the all-reduce of the caller:
+//   sum_io != null, apply = 0: only the rank's own sum is formed and stored to *sum_io;
+//   sum_io != null, apply = 1: no summation, the (all-reduced) value of *sum_io is applied.
 __global__ void __launch_bounds__(1024) finalize_kernel(int fin, Reduction red, int n, double tol,
-                                                        CgScalars* scal) {
+                                                        CgScalars* scal, double* sum_io, int apply) {
     __shared__ double sm[32];
     if (fin != FIN_BB && fin != FIN_TRUE && scal->done) {
-        if (fin == FIN_RHO && threadIdx.x == 0) scal->upd = 0;  // nothing for cg_update_xp to apply
+        if (fin == FIN_RHO && threadIdx.x == 0 && (sum_io == nullptr || apply)) scal->upd = 0;  // nothing for cg_update_xp to apply
+        if (sum_io != nullptr && !apply && threadIdx.x == 0) *sum_io = 0.0;
         return;
     }
     double s = 0.0;
-    for (int i = threadIdx.x; i < n; i += 1024) s += red.partials[i];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    s = warp_sum(s);
-    if (lane == 0) sm[warp] = s;
-    __syncthreads();
-    if (warp != 0) return;
-    s = warp_sum(sm[lane]);
-    if (lane != 0) return;
+    if (sum_io != nullptr && apply) {
+        if (threadIdx.x != 0) return;
+        s = *sum_io;
+    } else {
+        for (int i = threadIdx.x; i < n; i += 1024) s += red.partials[i];
+        s = warp_sum(s);
+        if (lane == 0) sm[warp] = s;
+        __syncthreads();
+        if (warp != 0) return;
+        s = warp_sum(sm[lane]);
+        if (lane != 0) return;
+        if (sum_io != nullptr) { *sum_io = s; return; }
+    }
     if (fin == FIN_PAP) {
         const double rho = scal->rho;
         scal->pAp = s;
@@ -454,10 +465,10 @@ inline int grid_for(size_t nvec) { return (int)((nvec + VBLOCK * VUNROLL - 1) / 
 int vector_grid(size_t n) { return grid_for(n / 2); }  // upper bound over both precisions
 
 cudaError_t launch_finalize(int fin, Reduction red, int n_partials, double tol, CgScalars* scal,
-                            cudaStream_t st) {
+                            cudaStream_t st, double* sum_io, int apply) {
     count_launch();
     ProfScope prof(3, st);
-    finalize_kernel<<<1, 1024, 0, st>>>(fin, red, n_partials, tol, scal);
+    finalize_kernel<<<1, 1024, 0, st>>>(fin, red, n_partials, tol, scal, sum_io, apply);
     return cudaGetLastError();
 }
 
@@ -501,22 +512,22 @@ cudaError_t launch_residual(size_t n, const void* b, const void* ax, void* r, Re
     count_launch(2);
     ProfScope prof(3, st);
     residual_kernel<<<grid_for(nv), VBLOCK, 0, st>>>(nv, (const double2*)b, (const double2*)ax, (double2*)r, red);
-    finalize_kernel<<<1, 1024, 0, st>>>(FIN_TRUE, red, grid_for(nv), 0.0, scal);
+    finalize_kernel<<<1, 1024, 0, st>>>(FIN_TRUE, red, grid_for(nv), 0.0, scal, nullptr, 0);
     return cudaGetLastError();
 }
 
 cudaError_t launch_cg_init(int precision, size_t n, const void* b, void* x, void* r, void* p,
-                           double tol, Reduction red, CgScalars* scal, cudaStream_t st) {
+                           double tol, Reduction red, CgScalars* scal, cudaStream_t st, double* sum_io) {
     count_launch(2);
     ProfScope prof(3, st);
     if (precision == 0) {
         const size_t nv = n / 2;
         cg_init_kernel<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, b, x, r, p, red);
-        finalize_kernel<<<1, 1024, 0, st>>>(FIN_BB, red, grid_for(nv), tol, scal);
+        finalize_kernel<<<1, 1024, 0, st>>>(FIN_BB, red, grid_for(nv), tol, scal, sum_io, 0);
     } else {
         const size_t nv = n / 4;
         cg_init_kernel<float><<<grid_for(nv), VBLOCK, 0, st>>>(nv, b, x, r, p, red);
-        finalize_kernel<<<1, 1024, 0, st>>>(FIN_BB, red, grid_for(nv), tol, scal);
+        finalize_kernel<<<1, 1024, 0, st>>>(FIN_BB, red, grid_for(nv), tol, scal, sum_io, 0);
     }
     return cudaGetLastError();
 }
@@ -536,17 +547,17 @@ cudaError_t launch_cg_update_xp(int precision, size_t n, void* x, void* p, const
 }
 
 cudaError_t launch_true_resid(int precision, size_t n, const void* b, const void* ax, Reduction red,
-                              CgScalars* scal, cudaStream_t st) {
+                              CgScalars* scal, cudaStream_t st, double* sum_io) {
     count_launch(2);
     ProfScope prof(3, st);
     if (precision == 0) {
         const size_t nv = n / 2;
         true_resid_kernel<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, b, ax, red);
-        finalize_kernel<<<1, 1024, 0, st>>>(FIN_TRUE, red, grid_for(nv), 0.0, scal);
+        finalize_kernel<<<1, 1024, 0, st>>>(FIN_TRUE, red, grid_for(nv), 0.0, scal, sum_io, 0);
     } else {
         const size_t nv = n / 4;
         true_resid_kernel<float><<<grid_for(nv), VBLOCK, 0, st>>>(nv, b, ax, red);
-        finalize_kernel<<<1, 1024, 0, st>>>(FIN_TRUE, red, grid_for(nv), 0.0, scal);
+        finalize_kernel<<<1, 1024, 0, st>>>(FIN_TRUE, red, grid_for(nv), 0.0, scal, sum_io, 0);
     }
     return cudaGetLastError();
 }

@@ -2,7 +2,7 @@
 """sweep.py -- timings of the BASELINE.json configurations 3, 4, 5 and of the paper's thermal
 lattice shapes (Fig. 7), one JSON line each.  A user-facing companion of bench.py:
 
-    python -m paper_1209_5942_b200.sweep [--configs 3,4,5,thermal,force,gauge] [--out FILE]
+    python -m paper_1209_5942_b200.sweep [--configs 3,4,5,thermal,force,gauge,slab] [--out FILE]
 
 config 3: 16^3x32, near-identity links, kappa=.16 mu=.05: 10 warm-up + 100 timed D_eo/D_oe
           applications, 5 repeats, median (working set fits L2: not a HBM roofline figure)
@@ -271,6 +271,72 @@ def gauge(stream):
     return out
 
 
+def slab(stream):
+    """One rank's share of a 32^3 x 64 lattice cut into R slabs of the time direction (SURVEY.md section
+    8(e)), timed on ONE GPU: the hopping launch over the rank's 32^3 x (64/R) sites
+    in one piece and split into interior + boundary launches (what overlaps the halo exchange), the
+    halo copy itself as two device-to-device block copies, and the bytes a rank sends per application.
+    Per-rank figures only: nothing here measures NVLink."""
+    gdims = (32, 32, 32, 64)
+    kappa = 0.15
+    out = []
+    for R in (1, 2, 4, 8):
+        dims = gdims[:3] + (gdims[3] // R,)
+        Vh = int(np.prod(dims)) // 2
+        U = gen.gauge_haar(dims)
+        B.lqcd_slab_init(gdims, gen.antiperiodic_t(), 0, R)
+        B.lqcd_set_stream(stream)
+        with torch.cuda.stream(stream):
+            g = B.upload_gauge(U)
+            a = B.upload_spinor(gen.spinor_gaussian(Vh), 1)
+            b = B.alloc_spinor()
+            h = B.lqcd_slab_spinor_halo()
+            n = h["bytes"]
+
+            def exchange(f):   # the rank as its own neighbour: same bytes moved as between ranks
+                f[h["ghost_fwd"]:h["ghost_fwd"] + n].copy_(f[h["send_lo"]:h["send_lo"] + n])
+                f[h["ghost_bwd"]:h["ghost_bwd"] + n].copy_(f[h["send_hi"]:h["send_hi"] + n])
+
+            def timed(body, reps=50):
+                for _ in range(5):
+                    body()
+                ts = []
+                for _ in range(3):
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    stream.synchronize()
+                    e0.record(stream)
+                    for _ in range(reps):
+                        body()
+                    e1.record(stream)
+                    stream.synchronize()
+                    ts.append(e0.elapsed_time(e1) / reps)
+                return float(np.median(ts)) * 1e3
+
+            def whole():
+                B.lqcd_slab_dslash(g, a, b, 0, kappa, 0)
+                B.lqcd_slab_dslash(g, b, a, 1, kappa, 0)
+
+            def split():
+                B.lqcd_slab_dslash(g, a, b, 0, kappa, 1)
+                B.lqcd_slab_dslash(g, a, b, 0, kappa, 2)
+                B.lqcd_slab_dslash(g, b, a, 1, kappa, 1)
+                B.lqcd_slab_dslash(g, b, a, 1, kappa, 2)
+
+            exchange(a); exchange(b)
+            us_whole = timed(whole) / 2
+            us_split = timed(split) / 2
+            us_copy = timed(lambda: exchange(a))
+        B.lqcd_finalize()
+        out.append({"config": "slab", "global_lattice": list(gdims), "ranks": R, "local_lattice": list(dims),
+                    "precision": "double", "recon": 18, "us_per_application_whole": us_whole,
+                    "us_per_application_interior_plus_boundary": us_split, "us_halo_copies_on_device": us_copy,
+                    "halo_bytes_sent_per_application": 2 * n,
+                    "us_halo_at_900_GBs_per_direction": n / 900e9 * 1e6,
+                    "gflops_per_rank_whole": Vh * FLOP / us_whole / 1e3,
+                    "gbs_effective_per_rank_whole": Vh * 1536 / us_whole / 1e3})
+    return out
+
+
 def thermal(stream):
     out = []
     for ns in (16, 24, 32, 48):
@@ -291,7 +357,7 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("sweep.py needs a CUDA device: there is no CPU fallback")
     stream = torch.cuda.Stream()
-    table = {"3": config3, "4": config4, "5": config5, "thermal": thermal, "force": force, "gauge": gauge}
+    table = {"3": config3, "4": config4, "5": config5, "thermal": thermal, "force": force, "gauge": gauge, "slab": slab}
     lines = []
     for key in args.configs.split(","):
         for r in table[key.strip()](stream):
