@@ -393,8 +393,6 @@ int lqcd_init(const int dims[4], const double bc_phase[8]) {
     ctx.geo.G = (ctx.geo.Vh + 31) / 32;
     ctx.geo.Gg = ctx.geo.G;
     ctx.s3 = ctx.geo.N0h * ctx.geo.N1 * ctx.geo.N2;
-    ctx.geo.goff_f = -(ctx.geo.N3 - 1) * ctx.s3;   // periodic wrap of the time direction
-    ctx.geo.goff_b = +(ctx.geo.N3 - 1) * ctx.s3;
     ctx.geo.tph_f = ctx.geo.tph_b = 1;
     ctx.geo.slab = 0;
     ctx.slab = false; ctx.rank = 0; ctx.nranks = 1;
@@ -924,9 +922,6 @@ int lqcd_slab_init(const int dims_global[4], const double bc_phase[8], int rank,
     }
     ctx.slab = true; ctx.rank = rank; ctx.nranks = nranks;
     ctx.geo.slab = 1;
-    const int Vh = ctx.geo.Vh;                        // = 32 G: no pad sites in slab mode
-    ctx.geo.goff_f = Vh - (ctx.geo.N3 - 1) * ctx.s3;  // x3 = N3 - 1, spatial index s  ->  Vh + s
-    ctx.geo.goff_b = Vh + ctx.s3;                     // x3 = 0,      spatial index s  ->  Vh + s3 + s
     ctx.geo.tph_f = (rank == nranks - 1);
     ctx.geo.tph_b = (rank == 0);
     ctx.geo.Gg = ctx.geo.G + 2 * (ctx.s3 / 32);

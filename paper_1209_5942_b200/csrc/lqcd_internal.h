@@ -54,14 +54,12 @@ struct Geometry {
     int G;                // groups of 32 sites per parity = ceil(Vh / 32)
     FastDiv d0h, d1, d2;  // division by N0h, N1, N2
     double ph_re[4], ph_im[4];
-    // Time-direction neighbours across the lattice's (or, in slab mode, the rank's) t boundary.
-    // Single GPU: the wrap, goff_f = -(N3 - 1) s3, goff_b = +(N3 - 1) s3 (s3 = sites per time slice
-    // and parity).  Slab mode (lqcd_slab_init): ghost time slices appended behind the G groups of a
-    // field, forward ghost (slice t = N3 of the next rank) at site index 32 G + s, backward ghost
-    // (slice t = -1 of the previous rank) at 32 G + s3 + s; the boundary phase applies only on the
+    // Slab mode (lqcd_slab_init): two ghost time slices sit behind the G groups of a field, the
+    // forward ghost (slice t = N3 of the next rank) at site index Vh + s = e + s3 for a site of the
+    // last slice, the backward ghost (slice t = -1 of the previous rank) at Vh + s3 + s (s = index
+    // inside a slice, s3 = sites per slice and parity); the time boundary phase applies only on the
     // rank that owns the global boundary (tph_f on the last rank, tph_b on the first).
     int slab;             // 1 after lqcd_slab_init
-    int goff_f, goff_b;
     int tph_f, tph_b;
     int Gg;               // groups per (parity, mu) array of the gauge field: G, or G + ghost groups
 };
