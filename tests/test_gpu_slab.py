@@ -231,3 +231,29 @@ def test_slab_argument_checks(B):
     B.lqcd_select_context(0)
     with pytest.raises(B.LqcdError):
         B.lqcd_select_context(8)
+
+
+@pytest.mark.parametrize("overlap", [False, True])
+def test_binding_slab_cg_driver_single_rank(B, oracle_mod, overlap):
+    """binding.slab_cg, the torch.distributed driver, with world = 1: the rank is its own neighbour
+    (block copies instead of send/recv, no all-reduce), every stage, poll and the true residual run
+    through the same code a multi-process job uses."""
+    kappa, mu, tol = 0.15, 0.1, 1e-10
+    U = gen.gauge_haar(DIMS, SEED)
+    b = gen.spinor_gaussian(lu.volume(DIMS) // 2, SEED, gen.STREAM_SOURCE)
+    B.lqcd_select_context(0)
+    B.lqcd_slab_init(DIMS, AP, 0, 1)
+    B.lqcd_set_stream()
+    g = B.upload_gauge(U)
+    B.slab_exchange_gauge(g, 0, 1)
+    s, x = B.upload_spinor(b, 0), B.alloc_spinor()
+    st = B.slab_cg(g, s, x, kappa, mu, tol, 500, 0, 1, overlap=overlap, check_every=3)
+    iters, rr, rt = B.lqcd_cg_stats()
+    xs = B.download_spinor(x, 0)
+    assert st == 0 and 20 <= iters <= 60
+    true_rel = lu.rel_err(oracle_mod.mdagm(DIMS, AP, U, xs, kappa, mu), b)
+    assert true_rel <= 1.05 * tol and abs(rt - true_rel) <= 1e-12
+    # maxit reached: status 1, x = last iterate
+    x2 = B.alloc_spinor()
+    assert B.slab_cg(g, s, x2, kappa, mu, 1e-30, 3, 0, 1, overlap=overlap) == 1
+    assert B.lqcd_cg_stats()[0] == 3
