@@ -271,6 +271,33 @@ void* lqcd_slab_sum_ptr(void);
 int lqcd_slab_cg_poll(int* done, int* iters);
 int lqcd_slab_cg_end(int with_true_resid);
 
+/* The paper's buffer-copy micro-benchmark (Fig. 5: copy bandwidth by element type,
+ * the experiment that fixed its structure-of-arrays format on a 16-byte element), kept as the
+ * library's own HBM probe; timed by the caller (CUDA events on the library's stream).
+ *   elem: LQCD_ELEM_FLOAT (4 B), LQCD_ELEM_DOUBLE (8 B), LQCD_ELEM_VEC16 (16 B = float4 = complex
+ *         double; the storage element of every internal field): thread <-> array element;
+ *         LQCD_ELEM_SU3_AOS (144 B), LQCD_ELEM_SPINOR_AOS (192 B): thread <-> whole struct, the
+ *         array-of-structures access the paper started from; COPY only.
+ *   mode: LQCD_STREAM_COPY   dst[i] = src[i]; reads `bytes`, writes `bytes`;
+ *         LQCD_STREAM_READ   reads `bytes`; dst receives LQCD_STREAM_PROBE_BLOCKS 8-byte words whose
+ *                            XOR is the XOR of all 8-byte words of src;
+ *         LQCD_STREAM_MIX71  src = 7 planes of bytes/7 each, dst[i] = XOR over the planes of element i:
+ *                            reads `bytes`, writes bytes/7 -- the read : write ratio of the hopping
+ *                            term (1344 : 192 B per site).
+ * src, dst: DEVICE pointers, 16-byte aligned, not overlapping; `bytes` (of src) a multiple of 16, of
+ * the struct size for the AoS elements and of 112 in MIX71, else LQCD_BAD_ARG.  bytes = 0 is a no-op.
+ * All arithmetic is bit-wise, so results are exact for any contents.  Asynchronous. */
+#define LQCD_ELEM_FLOAT      0
+#define LQCD_ELEM_DOUBLE     1
+#define LQCD_ELEM_VEC16      2
+#define LQCD_ELEM_SU3_AOS    3
+#define LQCD_ELEM_SPINOR_AOS 4
+#define LQCD_STREAM_COPY  0
+#define LQCD_STREAM_READ  1
+#define LQCD_STREAM_MIX71 2
+#define LQCD_STREAM_PROBE_BLOCKS 1184
+int lqcd_stream_probe(int elem, int mode, const void* src_dev, void* dst_dev, size_t bytes);
+
 /* Number of kernels this library has launched since lqcd_init (all streams). */
 long long lqcd_launch_count(void);
 

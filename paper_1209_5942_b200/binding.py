@@ -17,6 +17,9 @@ LQCD_OK, LQCD_NOT_CONVERGED = 0, 1
 LQCD_NOT_INITIALISED, LQCD_BAD_DIMS, LQCD_BAD_ARG, LQCD_CUDA_ERROR, LQCD_BREAKDOWN = -1, -2, -3, -4, -5
 LQCD_DOUBLE, LQCD_SINGLE = 0, 1
 LQCD_HEATBATH, LQCD_OVERRELAX = 0, 1
+LQCD_ELEM_FLOAT, LQCD_ELEM_DOUBLE, LQCD_ELEM_VEC16, LQCD_ELEM_SU3_AOS, LQCD_ELEM_SPINOR_AOS = 0, 1, 2, 3, 4
+LQCD_STREAM_COPY, LQCD_STREAM_READ, LQCD_STREAM_MIX71 = 0, 1, 2
+LQCD_STREAM_PROBE_BLOCKS = 1184
 
 SYMBOLS = [
     "lqcd_last_error", "lqcd_init", "lqcd_finalize", "lqcd_set_stream", "lqcd_set_format",
@@ -24,7 +27,7 @@ SYMBOLS = [
     "lqcd_unpack_spinor", "lqcd_dslash_eo", "lqcd_mtm", "lqcd_mtm_full", "lqcd_solve_full", "lqcd_cg_mdagm", "lqcd_cg_setup",
     "lqcd_cg_iterate", "lqcd_cg_finish", "lqcd_cg_stats", "lqcd_cg_mdagm_mixed", "lqcd_cg_outer_iterations", "lqcd_bicgstab_mhat", "lqcd_force_bytes", "lqcd_unpack_force", "lqcd_fermion_force", "lqcd_force_tm", "lqcd_mtm_host", "lqcd_cg_mdagm_host",
     "lqcd_launch_count", "lqcd_set_block_size", "lqcd_profile", "lqcd_profile_read",
-    "lqcd_gauge_update", "lqcd_gauge_sweep", "lqcd_plaquette", "lqcd_unpack_gauge",
+    "lqcd_gauge_update", "lqcd_gauge_sweep", "lqcd_plaquette", "lqcd_unpack_gauge", "lqcd_stream_probe",
     "lqcd_select_context", "lqcd_slab_init", "lqcd_slab_spinor_halo", "lqcd_slab_gauge_halo", "lqcd_slab_dslash",
     "lqcd_slab_mhat_stage", "lqcd_slab_cg_begin", "lqcd_slab_cg_stage", "lqcd_slab_cg_halo_field",
     "lqcd_slab_sum_ptr", "lqcd_slab_cg_poll", "lqcd_slab_cg_end",
@@ -78,6 +81,7 @@ def _load():
         "lqcd_gauge_sweep": [vp, i32, dbl, u64, u64],
         "lqcd_plaquette": [vp, ctypes.POINTER(dbl)],
         "lqcd_unpack_gauge": [vp, vp],
+        "lqcd_stream_probe": [i32, i32, vp, vp, ctypes.c_size_t],
         "lqcd_select_context": [i32],
         "lqcd_slab_init": [ctypes.POINTER(i32), ctypes.POINTER(dbl), i32, i32],
         "lqcd_slab_spinor_halo": [ctypes.POINTER(ctypes.c_size_t)] * 5,
@@ -293,6 +297,10 @@ def lqcd_plaquette(gauge):
 
 def lqcd_unpack_gauge(internal_dev, canon_dev):
     return _check(_lib.lqcd_unpack_gauge(_ptr(internal_dev), _ptr(canon_dev)))
+
+
+def lqcd_stream_probe(elem, mode, src_dev, dst_dev, nbytes):
+    return _check(_lib.lqcd_stream_probe(elem, mode, _ptr(src_dev), _ptr(dst_dev), nbytes))
 
 
 # ---------------------------------------------------------------------------- buffer helpers

@@ -18,6 +18,8 @@
 #include "../../include/lqcd.h"
 #include "lqcd_internal.h"
 
+#include <cstdint>
+
 namespace lqcd {
 
 static std::atomic<long long> g_launches{0};
@@ -468,6 +470,22 @@ int lqcd_unpack_gauge(const void* internal_dev, void* canon_dev) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
     if (!canon_dev || !internal_dev) return fail(LQCD_BAD_ARG, "lqcd_unpack_gauge: null pointer");
     CU(launch_unpack_gauge(ctx.precision, ctx.recon, ctx.geo, internal_dev, canon_dev, ctx.stream));
+    return LQCD_OK;
+}
+
+// ---- the paper's copy micro-benchmark (stream_probe.cu; Fig. 5)
+int lqcd_stream_probe(int elem, int mode, const void* src_dev, void* dst_dev, size_t bytes) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    static_assert(LQCD_STREAM_PROBE_BLOCKS == kStreamProbeBlocks, "header and kernel disagree on the READ grid");
+    if (elem < LQCD_ELEM_FLOAT || elem > LQCD_ELEM_SPINOR_AOS) return fail(LQCD_BAD_ARG, "lqcd_stream_probe: elem must be 0..4");
+    if (mode < LQCD_STREAM_COPY || mode > LQCD_STREAM_MIX71) return fail(LQCD_BAD_ARG, "lqcd_stream_probe: mode must be 0..2");
+    if (elem >= LQCD_ELEM_SU3_AOS && mode != LQCD_STREAM_COPY) return fail(LQCD_BAD_ARG, "lqcd_stream_probe: the AoS elements support COPY only");
+    if (bytes == 0) return LQCD_OK;
+    if (!src_dev || !dst_dev) return fail(LQCD_BAD_ARG, "lqcd_stream_probe: null pointer");
+    if (((uintptr_t)src_dev | (uintptr_t)dst_dev) & 15) return fail(LQCD_BAD_ARG, "lqcd_stream_probe: pointers must be 16-byte aligned");
+    const size_t unit = (elem == LQCD_ELEM_SU3_AOS) ? 144 : (elem == LQCD_ELEM_SPINOR_AOS) ? 192 : (mode == LQCD_STREAM_MIX71) ? 112 : 16;
+    if (bytes % unit) return fail(LQCD_BAD_ARG, "lqcd_stream_probe: bytes must be a multiple of 16 (144 / 192 for the AoS elements, 112 in MIX71)");
+    CU(launch_stream_probe(elem, mode, src_dev, dst_dev, bytes, ctx.stream));
     return LQCD_OK;
 }
 

@@ -2,7 +2,7 @@
 """sweep.py -- timings of the BASELINE.json configurations 3, 4, 5 and of the paper's thermal
 lattice shapes (Fig. 7), one JSON line each.  A user-facing companion of bench.py:
 
-    python -m paper_1209_5942_b200.sweep [--configs 3,4,5,thermal,force,gauge,slab] [--out FILE]
+    python -m paper_1209_5942_b200.sweep [--configs 3,4,5,thermal,force,gauge,slab,copy] [--out FILE]
 
 config 3: 16^3x32, near-identity links, kappa=.16 mu=.05: 10 warm-up + 100 timed D_eo/D_oe
           applications, 5 repeats, median (working set fits L2: not a HBM roofline figure)
@@ -271,6 +271,54 @@ def gauge(stream):
     return out
 
 
+def copy(stream):
+    """The paper's buffer-copy micro-benchmark by element type (Fig. 5) through
+    lqcd_stream_probe, plus the READ and 7:1 mixes that bracket the hopping kernel.  Two buffer sizes: 2.1 GB
+    (HBM; every figure that is compared with a kernel) and the paper's 100 MiB, which fits B200's 126 MB L2
+    and is reported only to show that.  GB/s counts bytes read + bytes written."""
+    names = {0: "float (4 B)", 1: "double (8 B)", 2: "16-byte vector", 3: "su3 AoS (144 B)", 4: "spinor AoS (192 B)"}
+    modes = {0: "copy", 1: "read", 2: "mix 7:1"}
+    B.lqcd_init((4, 4, 4, 4), gen.antiperiodic_t())
+    B.lqcd_set_stream(stream)
+    out = []
+    peak = measured_peak()
+    with torch.cuda.stream(stream):
+        for nbytes, where in ((12096 * 175000, "HBM"), (12096 * 8668, "paper's 100 MiB: fits L2")):
+            src = torch.randint(0, 256, (nbytes,), dtype=torch.uint8, device="cuda")
+            dst = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+
+            def timed(body, moved):
+                for _ in range(5):
+                    body()
+                ts = []
+                for _ in range(3):
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    stream.synchronize()
+                    e0.record(stream)
+                    for _ in range(20):
+                        body()
+                    e1.record(stream)
+                    stream.synchronize()
+                    ts.append(e0.elapsed_time(e1) / 20)
+                ms = float(np.median(ts))
+                return ms * 1e3, moved / ms / 1e6
+
+            for elem in range(5):
+                for mode in ((0, 1, 2) if elem < 3 else (0,)):
+                    moved = {0: 2 * nbytes, 1: nbytes, 2: nbytes + nbytes // 7}[mode]
+                    us, gbs = timed(lambda: B.lqcd_stream_probe(elem, mode, src, dst, nbytes), moved)
+                    out.append({"config": "copy", "element": names[elem], "mode": modes[mode], "buffer_bytes": nbytes,
+                                "buffer": where, "us": us, "gbs": gbs, "frac_of_measured_peak": gbs / peak,
+                                "measured_peak_gbs": peak})
+            us, gbs = timed(lambda: dst.copy_(src), 2 * nbytes)
+            out.append({"config": "copy", "element": "torch.Tensor.copy_ (what MEASURED_PEAKS.json times)", "mode": "copy",
+                        "buffer_bytes": nbytes, "buffer": where, "us": us, "gbs": gbs,
+                        "frac_of_measured_peak": gbs / peak, "measured_peak_gbs": peak})
+            del src, dst
+    B.lqcd_finalize()
+    return out
+
+
 def slab(stream):
     """One rank's share of a 32^3 x 64 lattice cut into R slabs of the time direction (SURVEY.md section
     8(e)), timed on ONE GPU: the hopping launch over the rank's 32^3 x (64/R) sites
@@ -357,7 +405,7 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("sweep.py needs a CUDA device: there is no CPU fallback")
     stream = torch.cuda.Stream()
-    table = {"3": config3, "4": config4, "5": config5, "thermal": thermal, "force": force, "gauge": gauge, "slab": slab}
+    table = {"3": config3, "4": config4, "5": config5, "thermal": thermal, "force": force, "gauge": gauge, "slab": slab, "copy": copy}
     lines = []
     for key in args.configs.split(","):
         for r in table[key.strip()](stream):
