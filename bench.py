@@ -22,6 +22,8 @@ roofline= the hopping kernel: algorithmic bytes (1536 B/site, +192 B/site for th
 e2e     = the same per-step work through lqcd_cg_mdagm_host with pinned HOST
           buffers: every step uploads gauge + source, runs one CG iteration (plus
           the solve's true-residual check, not counted as flops) and downloads x.
+roofline.stream_probe_gbs = what lqcd_stream_probe (the paper's copy micro-benchmark, Fig. 5) moves on this
+          box in the same run: copy, read-only and 7 reads : 1 write on 16-byte elements (context for frac).
 --impl reference times the CPU oracle (oracle/, test infrastructure) on the host cores.
 """
 import argparse
@@ -327,6 +329,28 @@ def run_ours(args, rank, world, local_rank):
                   "gflops": world * it_solve * 4 * Vh * FLOP_PER_SITE / dt_solve / 1e9},
     }
     del U_pin
+
+    # ---- what the memory system of THIS box does on a pure stream (lqcd_stream_probe, 16-byte elements,
+    # 1.06 GB read per launch): context for roofline.frac, whose peak stays the driver's measured memcpy figure
+    nb = 12096 * 87500
+    with torch.cuda.stream(stream):
+        ps = torch.randint(0, 256, (nb,), dtype=torch.uint8, device="cuda")
+        pd = torch.empty(nb, dtype=torch.uint8, device="cuda")
+        ceil = {}
+        for name, mode, moved in (("copy", B.LQCD_STREAM_COPY, 2 * nb), ("read", B.LQCD_STREAM_READ, nb),
+                                  ("mix_7_reads_1_write", B.LQCD_STREAM_MIX71, nb + nb // 7)):
+            for _ in range(3):
+                B.lqcd_stream_probe(B.LQCD_ELEM_VEC16, mode, ps, pd, nb)
+            p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            p0.record(stream)
+            for _ in range(10):
+                B.lqcd_stream_probe(B.LQCD_ELEM_VEC16, mode, ps, pd, nb)
+            p1.record(stream)
+            stream.synchronize()
+            ceil[name] = moved * 10 / (p0.elapsed_time(p1) * 1e-3) / 1e9
+        del ps, pd
+    roofline["stream_probe_gbs"] = ceil
+    roofline["frac_of_stream_mix"] = achieved / ceil["mix_7_reads_1_write"]
 
     # ---- oracle on the host cores beside it (rank 0, N = 1 only) ------------------------------
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
