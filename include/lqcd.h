@@ -298,6 +298,13 @@ int lqcd_slab_cg_end(int with_true_resid);
 #define LQCD_STREAM_PROBE_BLOCKS 1184
 int lqcd_stream_probe(int elem, int mode, const void* src_dev, void* dst_dev, size_t bytes);
 
+/* FP64 pipe probe, the secondary bound of the hopping term: LQCD_STREAM_PROBE_BLOCKS
+ * CTAs of 256 threads; thread t runs 8 independent chains x <- fma(x, a, b) of `iters` links, chain c
+ * starting at t + c, and stores the sum of its 8 results to out_dev[t] (LQCD_STREAM_PROBE_BLOCKS * 256
+ * doubles, DEVICE).  16 * iters flop per thread; timed by the caller.  iters < 0, a or b not finite, null
+ * pointer: LQCD_BAD_ARG.  Asynchronous. */
+int lqcd_fp64_probe(double a, double b, int iters, double* out_dev);
+
 /* Number of kernels this library has launched since lqcd_init (all streams). */
 long long lqcd_launch_count(void);
 

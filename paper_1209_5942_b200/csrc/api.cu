@@ -489,6 +489,18 @@ int lqcd_stream_probe(int elem, int mode, const void* src_dev, void* dst_dev, si
     return LQCD_OK;
 }
 
+int lqcd_fp64_probe(double a, double b, int iters, double* out_dev) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (!out_dev) return fail(LQCD_BAD_ARG, "lqcd_fp64_probe: null pointer");
+    if (iters < 0) return fail(LQCD_BAD_ARG, "lqcd_fp64_probe: iters must be >= 0");
+    int rc = check_scalar(a, "a");
+    if (rc) return rc;
+    rc = check_scalar(b, "b");
+    if (rc) return rc;
+    CU(launch_dfma_probe(a, b, iters, out_dev, ctx.stream));
+    return LQCD_OK;
+}
+
 // ---- pure-gauge sector (gauge_update.cu): one launch per sub-sweep, 8 sub-sweeps per sweep
 int lqcd_gauge_update(void* gauge, int mu, int parity, int mode, double beta, unsigned long long seed,
                       unsigned long long tag) {

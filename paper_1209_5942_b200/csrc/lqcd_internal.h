@@ -216,6 +216,7 @@ void count_launch(int n = 1);
 // stream_probe.cu: the paper's buffer-copy micro-benchmark (Fig. 5) as the library's HBM probe
 constexpr int kStreamProbeBlocks = 148 * 8;   // 8 CTAs of 256 threads per SM of a B200: every thread slot taken
 cudaError_t launch_stream_probe(int elem, int mode, const void* src, void* dst, size_t bytes, cudaStream_t st);
+cudaError_t launch_dfma_probe(double a, double b, int iters, double* out, cudaStream_t st);
 
 // api.cu: optional per-launch event timing (lqcd_profile)
 void prof_begin(int category, cudaStream_t st);

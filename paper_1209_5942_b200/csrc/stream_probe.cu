@@ -102,6 +102,22 @@ __global__ void __launch_bounds__(kThreads) aos_copy_kernel(const uint4* __restr
     }
 }
 
+// FP64 pipe probe ("measure with a DFMA micro-benchmark"): every thread runs
+// 8 independent chains x <- fma(x, a, b), `iters` links each; out[t] = sum of its 8 chains, chain c
+// starting at t + c.  2 x 8 x iters flop per thread.
+__global__ void __launch_bounds__(kThreads) dfma_kernel(double a, double b, int iters, double* __restrict__ out) {
+    const int t = blockIdx.x * kThreads + threadIdx.x;
+    double x[8];
+#pragma unroll
+    for (int c = 0; c < 8; ++c) x[c] = (double)(t + c);
+#pragma unroll 4
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int c = 0; c < 8; ++c) x[c] = fma(x[c], a, b);
+    }
+    out[t] = ((x[0] + x[1]) + (x[2] + x[3])) + ((x[4] + x[5]) + (x[6] + x[7]));
+}
+
 template <typename E>
 cudaError_t launch_typed(int mode, const void* src, void* dst, size_t n, int grid, cudaStream_t st) {
     const E* s = reinterpret_cast<const E*>(src);
@@ -137,6 +153,13 @@ cudaError_t launch_stream_probe(int elem, int mode, const void* src, void* dst, 
         case 3: aos_copy_kernel<9><<<grid, kThreads, 0, st>>>((const uint4*)src, (uint4*)dst, n); break;
         default: aos_copy_kernel<12><<<grid, kThreads, 0, st>>>((const uint4*)src, (uint4*)dst, n); break;
     }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_dfma_probe(double a, double b, int iters, double* out, cudaStream_t st) {
+    count_launch();
+    ProfScope prof(4, st);
+    dfma_kernel<<<kStreamProbeBlocks, kThreads, 0, st>>>(a, b, iters, out);
     return cudaGetLastError();
 }
 

@@ -315,6 +315,23 @@ def copy(stream):
                         "buffer_bytes": nbytes, "buffer": where, "us": us, "gbs": gbs,
                         "frac_of_measured_peak": gbs / peak, "measured_peak_gbs": peak})
             del src, dst
+        # FP64 pipe (the hopping term's secondary bound): 8 independent DFMA chains per thread
+        n = B.LQCD_STREAM_PROBE_BLOCKS * 256
+        o = torch.empty(n, dtype=torch.float64, device="cuda")
+        iters = 20000
+        B.lqcd_fp64_probe(0.999999, 1e-3, iters, o)
+        ts = []
+        for _ in range(5):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            stream.synchronize()
+            e0.record(stream)
+            B.lqcd_fp64_probe(0.999999, 1e-3, iters, o)
+            e1.record(stream)
+            stream.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        ms = float(np.median(ts))
+        out.append({"config": "copy", "element": "fp64 pipe: 8 DFMA chains per thread, 1184 CTAs x 256 threads", "mode": "dfma",
+                    "iters": iters, "us": ms * 1e3, "tflops_fp64": 16.0 * iters * n / ms / 1e9})
     B.lqcd_finalize()
     return out
 

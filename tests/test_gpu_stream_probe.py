@@ -96,3 +96,27 @@ def test_bad_arguments(B):
         with pytest.raises(B.LqcdError) as err:
             B.lqcd_stream_probe(*args)
         assert err.value.status == B.LQCD_BAD_ARG
+
+
+def test_fp64_probe_counts_its_chains(B):
+    """a = b = 1: every link adds 1, so thread t ends with sum_c (t + c + iters) = 8 t + 28 + 8 iters, exactly."""
+    import torch
+    n = B.LQCD_STREAM_PROBE_BLOCKS * 256
+    for iters in (0, 1, 5, 1000):
+        out = torch.full((n + 16,), -1.0, dtype=torch.float64, device="cuda")
+        B.lqcd_fp64_probe(1.0, 1.0, iters, out)
+        torch.cuda.synchronize()
+        t = np.arange(n, dtype=np.float64)
+        assert np.array_equal(out[:n].cpu().numpy(), 8 * t + 28 + 8 * iters)
+        assert bool((out[n:] == -1.0).all())
+    # a general (a, b): the chain against the same recurrence in numpy (fma vs a*x+b: one rounding apart per link)
+    out = torch.empty(n, dtype=torch.float64, device="cuda")
+    B.lqcd_fp64_probe(0.5, 0.25, 40, out)
+    x = np.arange(n, dtype=np.float64)[:, None] + np.arange(8, dtype=np.float64)[None, :]
+    for _ in range(40):
+        x = x * 0.5 + 0.25
+    assert np.allclose(out.cpu().numpy(), x.sum(axis=1), rtol=1e-14, atol=0)
+    for bad in [(float("nan"), 1.0, 1, out), (1.0, float("inf"), 1, out), (1.0, 1.0, -1, out), (1.0, 1.0, 1, 0)]:
+        with pytest.raises(B.LqcdError) as err:
+            B.lqcd_fp64_probe(*bad)
+        assert err.value.status == B.LQCD_BAD_ARG
