@@ -36,6 +36,8 @@
 // double/18 252 / 288 / 287, double/12 213.5 / 207.5 / 208, single/18 123.7 / 122.2 / 120.5; at
 // 16^3 x 32 (1.15 waves at 3 CTAs) the 128-register builds are 6% faster (17.5 vs 18.6 us), not
 // enough to carry a second set of instantiations.  Only double/12 moves to 4 CTAs.
+// single/12 re-measured at 5 / 6 / 7 / 8 CTAs (96 / 80 / 72 / 64 registers): 102.9 / 102.3 / 102.4 / 108.1 us per launch,
+// CG iteration 574 / 562 / 561 / 602 us: flat between 6 and 7, 7 stays.
 #ifndef LQCD_HOP_MIN_BLOCKS
 #define LQCD_HOP_MIN_BLOCKS 3
 #endif
