@@ -54,8 +54,8 @@ SOLVE_LEN = 40
 METRIC = "D_tm GFLOPS (1320 flop/site) & achieved HBM GB/s vs B200 peak, double"
 # dram__bytes_read.sum + dram__bytes_write.sum per hopping launch at this workload (mean of the
 # four launches of one step; algorithmic mean 1.7616 GB), from the committed ncu --set full
-# capture profiles/r01b_hopping_full.md.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 1742430000
+# capture of the committed build, profiles/r01g_final.md (r01b_hopping_full.md gave 1.74243 GB).
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 1742503000
 
 
 def measured_peak():
