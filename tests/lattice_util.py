@@ -168,3 +168,12 @@ def exp_i_w_T(a, w):
 def algebra_matrix(F8):
     """sum_a F^a T^a for F8[..., 8] -> [..., 3, 3] (Hermitian, traceless)."""
     return 0.5 * np.einsum("...a,aij->...ij", F8, GELL_MANN)
+
+
+def big_gauge(dims, small_links):
+    """A gauge field for a lattice too large to generate link by link in a test: any arrangement of SU(3)
+    matrices is a valid field, so link i of the big lattice is link (7919 i + 13) mod n of the seeded small
+    field `small_links` (n, 3, 3).  Holds no method arithmetic; oracle and GPU are handed the same array."""
+    V = volume(dims)
+    idx = (np.arange(4 * V, dtype=np.int64) * 7919 + 13) % small_links.shape[0]
+    return small_links[idx].reshape(V, 4, 3, 3)

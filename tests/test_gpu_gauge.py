@@ -231,6 +231,34 @@ def test_full_size_subsweep_sampled_links(B, oracle_mod):
         del g, got
 
 
+def test_subsweep_beyond_4_gib_sampled_links(B, oracle_mod):
+    """48^3 x 96: the gauge field is 6.1 GB, byte offsets pass 2^32 inside it.  One overrelaxation sub-sweep on
+    links stored beyond 4 GiB (odd sites, mu = 1) and one heatbath sub-sweep (even sites, mu = 3): 300 sampled
+    updated links each against the oracle's link-wise evaluator, sampled untouched links bit-identical, and the
+    average plaquette of the whole field against the oracle's."""
+    dims, beta = (48, 48, 48, 96), 5.7
+    V = lu.volume(dims)
+    U = lu.big_gauge(dims, gen.gauge_near_identity((16, 16, 16, 32), SEED, 0.3).reshape(-1, 3, 3))
+    assert U.nbytes > 2 ** 32
+    rng = np.random.default_rng(5)
+    coords_sum = lambda s: (s % 48) + (s // 48) % 48 + (s // 2304) % 48 + (s // 110592)
+    g = _setup(B, dims, U)
+    assert abs(B.lqcd_plaquette(g) - oracle_mod.plaquette(dims, U)) <= 1e-13
+    del g
+    for mode, mu, parity in ((1, 1, 1), (0, 3, 0)):
+        g = _setup(B, dims, U)
+        B.lqcd_gauge_update(g, mu, parity, mode, beta, SEED, 77)
+        got = B.download_gauge(g)
+        cand = np.concatenate([rng.integers(0, V, 2000), [0, 1, V - 1, V - 2, 47, 48 * 48 * 48 - 1]])
+        sites = cand[coords_sum(cand) % 2 == parity][:300]
+        want = oracle_mod.update_links(dims, U, sites, np.full(len(sites), mu), mode, beta, SEED, 77)
+        assert lu.rel_err(got[sites, mu], want) <= TOL_D
+        assert np.max(np.abs(got[sites, mu] - want)) <= TOL_D
+        other = cand[coords_sum(cand) % 2 != parity]
+        assert np.array_equal(got[other], U[other])
+        del g, got
+
+
 def test_recon12_rows_stay_orthonormal_over_many_sweeps(B):
     """12-real storage: without the re-orthonormalisation before the store the unitarity defect grows
     x1.35 per overrelaxation sweep in single precision (1e-5 -> 0.1 in 30 sweeps, measured)."""

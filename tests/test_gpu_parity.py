@@ -407,6 +407,38 @@ def test_full_size_sampled_sites(B, oracle_mod, dims, near_id, kappa, mu):
     assert abs(np.vdot(x, MdMx) - np.vdot(Mx, Mx)) <= 1e-12 * np.vdot(Mx, Mx).real
 
 
+def test_fields_beyond_4_gib_sampled_sites(B, oracle_mod):
+    """Maximum sizes: at 48^3 x 96 the gauge field is 6.1 GB in both the canonical and the internal layout, so
+    byte offsets pass 2^32 inside it (from the mu = 1 links of odd sites on).  Any arrangement of SU(3)
+    matrices is a valid gauge field, so the big field is a fixed pseudo-random gather of the links of a
+    seeded 16^3 x 32 Haar field (lattice_util.big_gauge; generating 42 M fresh links would take minutes); oracle and GPU get the same
+    array.  Checked on sampled sites of both parities, in 18- and 12-real storage, plus the field-wide identity."""
+    dims = (48, 48, 48, 96)
+    V = lu.volume(dims)
+    U = lu.big_gauge(dims, gen.gauge_haar((16, 16, 16, 32), SEED).reshape(-1, 3, 3))
+    assert U.nbytes > 2 ** 32
+    h = V // 2
+    x = gen.spinor_gaussian(h, SEED)
+    sites = _sample_sites(h, 300, 23)
+    kappa, mu = 0.15, 0.1
+    for recon in (18, 12):
+        L = Lat(B, dims, AP, U, 0, recon)
+        assert B.lqcd_gauge_bytes() > (2 ** 32 if recon == 18 else 2 ** 31)
+        for parity in (0, 1):
+            got = L.dslash(x, parity, kappa)[sites]
+            want = oracle_mod.dslash_eo_sites(dims, AP, U, x, sites, parity, kappa)
+            assert lu.rel_err(got, want) <= TOL_D
+        for dagger in (0, 1):
+            got = L.mtm(x, kappa, mu, dagger)
+            want = oracle_mod.mhat_sites(dims, AP, U, x, sites, kappa, mu, dagger)
+            assert lu.rel_err(got[sites], want) <= TOL_D
+            assert np.all(np.isfinite(got))
+        Mx = L.mtm(x, kappa, mu, 0)
+        MdMx = L.mtm(Mx, kappa, mu, 1)
+        assert abs(np.vdot(x, MdMx) - np.vdot(Mx, Mx)) <= 1e-12 * np.vdot(Mx, Mx).real
+        del L
+
+
 def test_config4_cg_24c48(B, oracle_mod):
     dims = (24, 24, 24, 48)
     kappa, mu, tol = 0.15, 0.1, 1e-10
@@ -679,6 +711,22 @@ def test_fermion_force_full_size_sampled_links(B, oracle_mod):
     rng = np.random.default_rng(11)
     sites = np.concatenate([rng.integers(0, V, 290), [0, 1, V - 1, V - 2, V // 2, 31, 32, 1023, 32767, V - 32 * 32 * 32]])
     mus = np.concatenate([rng.integers(0, 4, 290), [0, 1, 2, 3, 0, 0, 1, 2, 3, 3]])
+    want = oracle_mod.fermion_force_links(dims, AP, U, X, Y, sites, mus, kappa)
+    assert lu.rel_err(got[sites, mus], want) <= TOL_D
+    assert np.all(np.isfinite(got))
+
+
+def test_fermion_force_beyond_4_gib_sampled_links(B, oracle_mod):
+    """48^3 x 96: gauge field 6.1 GB, force field 2.7 GB; 300 sampled links against the oracle's link-wise evaluator."""
+    dims = (48, 48, 48, 96)
+    kappa = 0.15
+    V = lu.volume(dims)
+    U = lu.big_gauge(dims, gen.gauge_haar((16, 16, 16, 32), SEED).reshape(-1, 3, 3))
+    X, Y = gen.spinor_gaussian(V, SEED, 7), gen.spinor_gaussian(V, SEED, 8)
+    got = _gpu_force(B, dims, AP, U, X, Y, kappa)
+    rng = np.random.default_rng(12)
+    sites = np.concatenate([rng.integers(0, V, 294), [0, 1, V - 1, V - 2, V // 2, V - 48 * 48 * 48]])
+    mus = np.concatenate([rng.integers(0, 4, 294), [0, 1, 2, 3, 0, 3]])
     want = oracle_mod.fermion_force_links(dims, AP, U, X, Y, sites, mus, kappa)
     assert lu.rel_err(got[sites, mus], want) <= TOL_D
     assert np.all(np.isfinite(got))
