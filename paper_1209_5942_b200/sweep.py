@@ -2,7 +2,7 @@
 """sweep.py -- timings of the BASELINE.json configurations 3, 4, 5 and of the paper's thermal
 lattice shapes (Fig. 7), one JSON line each.  A user-facing companion of bench.py:
 
-    python -m paper_1209_5942_b200.sweep [--configs 3,4,5,thermal,force,gauge,slab,copy] [--out FILE]
+    python -m paper_1209_5942_b200.sweep [--configs 3,4,5,thermal,force,gauge,slab,copy,large] [--out FILE]
 
 config 3: 16^3x32, near-identity links, kappa=.16 mu=.05: 10 warm-up + 100 timed D_eo/D_oe
           applications, 5 repeats, median (working set fits L2: not a HBM roofline figure)
@@ -336,6 +336,44 @@ def copy(stream):
     return out
 
 
+def large(stream):
+    """A production-size lattice, 48^3 x 96 (gauge field 6.1 GB, beyond the paper's 32^3 x 64 sizes): D-slash in
+    the four storage variants and the CG iteration in double.  The links are a fixed gather of a seeded
+    16^3 x 32 Haar field (any arrangement of SU(3) matrices is a valid field; 42 M fresh links take minutes)."""
+    dims = (48, 48, 48, 96)
+    V = int(np.prod(dims))
+    small = gen.gauge_haar((16, 16, 16, 32)).reshape(-1, 3, 3)
+    U = small[(np.arange(4 * V, dtype=np.int64) * 7919 + 13) % small.shape[0]].reshape(V, 4, 3, 3)
+    out = []
+    for precision, recon in ((0, 18), (0, 12), (1, 18), (1, 12)):
+        r = time_dslash(dims, U, precision, recon, 0.15, 10, 50, 3, stream)
+        r.update({"config": "large", "lattice": list(dims), "precision": "double" if precision == 0 else "single",
+                  "recon": recon})
+        out.append(r)
+    Vh = V // 2
+    B.lqcd_init(dims, gen.antiperiodic_t())
+    B.lqcd_set_stream(stream)
+    with torch.cuda.stream(stream):
+        g = B.upload_gauge(U)
+        b = B.upload_spinor(gen.spinor_gaussian(Vh, stream=gen.STREAM_SOURCE), 0)
+        x = B.alloc_spinor()
+        B.lqcd_cg_setup(g, b, x, 0.15, 0.1, 0.0)
+        B.lqcd_cg_iterate(10)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        stream.synchronize()
+        e0.record(stream)
+        B.lqcd_cg_setup(g, b, x, 0.15, 0.1, 0.0)
+        B.lqcd_cg_iterate(40)
+        e1.record(stream)
+        stream.synchronize()
+        B.lqcd_cg_finish()
+        ms = e0.elapsed_time(e1) / 40
+    B.lqcd_finalize()
+    out.append({"config": "large", "lattice": list(dims), "precision": "double", "recon": 18, "what": "CG iteration",
+                "ms_per_iteration": ms, "gflops": 4 * Vh * FLOP / ms / 1e6, "gbs_effective_step": Vh * 7680 / ms / 1e6})
+    return out
+
+
 def slab(stream):
     """One rank's share of a 32^3 x 64 lattice cut into R slabs of the time direction (SURVEY.md section
     8(e)), timed on ONE GPU: the hopping launch over the rank's 32^3 x (64/R) sites
@@ -422,7 +460,7 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("sweep.py needs a CUDA device: there is no CPU fallback")
     stream = torch.cuda.Stream()
-    table = {"3": config3, "4": config4, "5": config5, "thermal": thermal, "force": force, "gauge": gauge, "slab": slab, "copy": copy}
+    table = {"3": config3, "4": config4, "5": config5, "thermal": thermal, "force": force, "gauge": gauge, "slab": slab, "copy": copy, "large": large}
     lines = []
     for key in args.configs.split(","):
         for r in table[key.strip()](stream):
