@@ -439,7 +439,7 @@ long long lqcd_launch_count(void) { return g_launches.load(); }
 
 int lqcd_profile(int enable) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
-    if (enable) { CU(cudaStreamSynchronize(ctx.stream)); prof_clear(); }
+    if (enable == 1) { CU(cudaStreamSynchronize(ctx.stream)); prof_clear(); }   // 2 = resume: keep the records, no sync
     g_prof_on = enable != 0;
     return LQCD_OK;
 }
