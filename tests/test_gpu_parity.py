@@ -730,3 +730,42 @@ def test_fermion_force_beyond_4_gib_sampled_links(B, oracle_mod):
     want = oracle_mod.fermion_force_links(dims, AP, U, X, Y, sites, mus, kappa)
     assert lu.rel_err(got[sites, mus], want) <= TOL_D
     assert np.all(np.isfinite(got))
+
+
+def test_cg_on_a_side_stream_graph_replay_matches_direct_launches(B, oracle_mod):
+    """On a non-default stream the solver replays four iterations at a time as a cached CUDA graph (api.cu
+    cg_graph_ready); the legacy default stream cannot be captured, so the tests above run direct launches.  Same
+    kernels, same arguments, same order: x, the iteration count and the residuals must be bit-identical, a second
+    solve (graph reused) and a solve with other parameters (graph rebuilt) included; and the oracle's operator
+    confirms the residual."""
+    import torch
+    dims = (8, 8, 8, 16)
+    U = gen.gauge_haar(dims, SEED)
+    h = lu.volume(dims) // 2
+    b = gen.spinor_gaussian(h, SEED, gen.STREAM_SOURCE)
+    L = Lat(B, dims, AP, U)
+    ref = {}
+    for kappa, mu in ((0.15, 0.1), (0.14, 0.2)):
+        st, x, stats = L.cg(b, kappa, mu, 1e-10, 500)
+        assert st == 0
+        ref[(kappa, mu)] = (x, stats)
+    side = torch.cuda.Stream()
+    B.lqcd_set_stream(side)
+    with torch.cuda.stream(side):
+        for kappa, mu in ((0.15, 0.1), (0.15, 0.1), (0.14, 0.2)):
+            st, x, stats = L.cg(b, kappa, mu, 1e-10, 500)
+            assert st == 0
+            assert stats == ref[(kappa, mu)][1]
+            assert np.array_equal(x, ref[(kappa, mu)][0])
+        res = b - oracle_mod.mdagm(dims, AP, U, x, 0.14, 0.2)
+        assert np.linalg.norm(res) <= 1.05e-10 * np.linalg.norm(b)
+        # the three-step solver: lqcd_cg_iterate goes through the same graph
+        s_ = B.upload_spinor(b, 0)
+        xd = B.alloc_spinor()
+        B.lqcd_cg_setup(L.g, s_, xd, 0.15, 0.1, 1e-10)
+        B.lqcd_cg_iterate(200)
+        assert B.lqcd_cg_finish() == 0
+        assert B.lqcd_cg_stats() == ref[(0.15, 0.1)][1]
+        assert np.array_equal(B.download_spinor(xd, 0), ref[(0.15, 0.1)][0])
+    torch.cuda.synchronize()
+    B.lqcd_set_stream()
