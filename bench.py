@@ -309,7 +309,8 @@ def run_ours(args, rank, world, local_rank):
         "share_of_step": hop_ms / ms_sampled,
         "vector_kernels_share_of_step": prof[3][0] / ms_sampled,
         "sampled": f"event pairs around every launch of {len(marks)} of the {-(-args.steps // SOLVE_LEN)} solves of the timed "
-                   f"region ({steps_sampled} of {args.steps} steps, {ms_sampled / steps_sampled:.4f} ms per step there)",
+                   f"region ({steps_sampled} of {args.steps} steps, {ms_sampled / steps_sampled:.4f} ms per step there, direct launches; "
+                   f"the other solves replay four iterations at a time as the library's cached CUDA graph)",
     }
 
     line = {

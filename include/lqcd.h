@@ -125,7 +125,11 @@ int lqcd_cg_mdagm(const void* gauge, const void* b, void* x, double kappa, doubl
  *   lqcd_cg_iterate  enqueue up to n iterations; iterations after convergence
  *                    are no-ops on the device                            (async)
  *   lqcd_cg_finish   synchronise, compute the true residual |b - A x|/|b|;
- *                    returns the solve status. */
+ *                    returns the solve status.
+ * On a stream that can be captured (any but the legacy default stream) the solvers enqueue four
+ * iterations at a time as a CUDA graph captured on first use and kept while gauge, x, format, block
+ * size, kappa and mu stay the same (bit-identical to direct launches, ~13 us less device time per
+ * iteration between the kernels); LQCD_CG_GRAPH=0 in the environment turns it off. */
 int lqcd_cg_setup(const void* gauge, const void* b, void* x, double kappa, double mu, double tol);
 int lqcd_cg_iterate(int n);
 int lqcd_cg_finish(void);
