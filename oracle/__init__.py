@@ -24,6 +24,7 @@ from .oracle import (  # noqa: F401
     force_fields,
     force_tm,
     num_threads,
+    set_num_threads,
     plaquette,
     staple,
     update_links,

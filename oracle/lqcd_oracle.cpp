@@ -625,4 +625,18 @@ int orc_num_threads(void) {
 #endif
 }
 
+// Thread count of the OpenMP loops over independent output sites (no arithmetic changes with it): the
+// timed baseline is reported once single-threaded and once on all cores.
+// n <= 0 restores the default; returns the count now in force.
+int orc_set_num_threads(int n) {
+#ifdef _OPENMP
+    static const int dflt = omp_get_max_threads();
+    omp_set_num_threads(n > 0 ? n : dflt);
+    return omp_get_max_threads();
+#else
+    (void)n;
+    return 1;
+#endif
+}
+
 }  // extern "C"

@@ -294,3 +294,10 @@ def kp_samples(lam, seed, tag, n):
 
 def num_threads():
     return int(_load().orc_num_threads())
+
+
+def set_num_threads(n):
+    """Threads of the oracle's OpenMP loops over independent sites (n <= 0: the default); returns the count in force."""
+    lib = _load()
+    lib.orc_set_num_threads.restype = ctypes.c_int
+    return int(lib.orc_set_num_threads(ctypes.c_int(int(n))))

@@ -111,6 +111,7 @@ _lib = _load()
 # mirrors format and sites per parity of each context (lqcd_select_context), for buffer helpers only
 _fmts = [{"precision": LQCD_DOUBLE, "vh": 0} for _ in range(8)]
 _fmt = _fmts[0]
+_cur_ctx = [0]        # the selected context (lqcd_select_context)
 
 
 def _check(status):
@@ -139,6 +140,7 @@ def lqcd_init(dims, bc_phase):
     ph = np.asarray(bc_phase, dtype=np.complex128)
     p = (ctypes.c_double * 8)(*[float(v) for z in ph for v in (z.real, z.imag)])
     rc = _check(_lib.lqcd_init(d, p))
+    _lib_streams.pop(_cur_ctx[0], None)      # lqcd_init resets the library's stream to the legacy default
     _fmt["precision"] = LQCD_DOUBLE
     _fmt["vh"] = int(np.prod([int(v) for v in dims])) // 2
     return rc
@@ -148,9 +150,54 @@ def lqcd_finalize():
     return _check(_lib.lqcd_finalize())
 
 
+_lib_streams = {}     # context id -> the torch stream handed to lqcd_set_stream (None: never set = legacy default)
+
+
 def lqcd_set_stream(stream=None):
     s = torch.cuda.current_stream() if stream is None else stream
-    return _check(_lib.lqcd_set_stream(ctypes.c_void_p(s.cuda_stream)))
+    rc = _check(_lib.lqcd_set_stream(ctypes.c_void_p(s.cuda_stream)))
+    _lib_streams[_cur_ctx[0]] = s
+    return rc
+
+
+def library_stream():
+    """The torch stream the library launches on in the selected context (None before lqcd_set_stream)."""
+    return _lib_streams.get(_cur_ctx[0])
+
+
+def check_same_stream(library_handle, current_handle):
+    """The slab driver's ordering rule: torch.distributed orders its NCCL point-to-point operations and
+    all-reduces against torch's CURRENT stream, the library's kernels run on the stream of
+    lqcd_set_stream.  With two different streams a send could read a boundary slice before the hopping
+    kernel that produces it has finished, and a boundary launch could read ghosts before the receive has
+    landed -- so the two must be one stream (raw cudaStream_t handles compared)."""
+    if int(library_handle or 0) != int(current_handle or 0):
+        raise RuntimeError(f"slab exchange: torch's current stream ({int(current_handle or 0):#x}) is not the library's "
+                           f"stream ({int(library_handle or 0):#x}); run under torch.cuda.stream(<the stream given to "
+                           f"lqcd_set_stream>) or call lqcd_set_stream() for the current stream")
+
+
+class _OnLibraryStream:
+    """Makes the library's stream torch's current stream for the communication calls inside, then checks it."""
+
+    def __init__(self, tensor=None):
+        self.cuda = torch.cuda.is_available() and (tensor is None or (torch.is_tensor(tensor) and tensor.is_cuda))
+        self.cm = None
+
+    def __enter__(self):
+        if not self.cuda:
+            return self
+        s = library_stream()
+        if s is not None:
+            self.cm = torch.cuda.stream(s)
+            self.cm.__enter__()
+        check_same_stream(s.cuda_stream if s is not None else 0, torch.cuda.current_stream().cuda_stream)
+        return self
+
+    def __exit__(self, *a):
+        if self.cm is not None:
+            self.cm.__exit__(*a)
+        return False
 
 
 def lqcd_set_format(precision, recon):
@@ -369,6 +416,7 @@ def lqcd_select_context(ctx_id):
     global _fmt
     rc = _check(_lib.lqcd_select_context(int(ctx_id)))
     _fmt = _fmts[int(ctx_id)]
+    _cur_ctx[0] = int(ctx_id)
     return rc
 
 
@@ -377,6 +425,7 @@ def lqcd_slab_init(dims_global, bc_phase, rank, nranks):
     ph = np.asarray(bc_phase, dtype=np.complex128)
     p = (ctypes.c_double * 8)(*[float(v) for z in ph for v in (z.real, z.imag)])
     rc = _check(_lib.lqcd_slab_init(d, p, int(rank), int(nranks)))
+    _lib_streams.pop(_cur_ctx[0], None)
     _fmt["precision"] = LQCD_DOUBLE
     _fmt["vh"] = int(np.prod([int(v) for v in dims_global])) // (2 * int(nranks))
     return rc
@@ -464,68 +513,76 @@ def slab_exchange_blocks(buf, sends, recvs, rank, world, group=None):
 
 
 def slab_exchange_spinor(field, rank, world, group=None, wait=True):
-    """Fill the two ghost time slices of an internal half-spinor field (tensor or raw pointer)."""
+    """Fill the two ghost time slices of an internal half-spinor field (tensor or raw pointer).  Device
+    fields: issued on the library's stream (check_same_stream), so the sends are ordered after the kernel
+    that wrote the boundary slices and later launches after the receives."""
     h = lqcd_slab_spinor_halo()
     if not torch.is_tensor(field):
         field = device_bytes(field, lqcd_spinor_bytes())
     n = h["bytes"]
-    # first slice -> forward ghost of the previous rank; last slice -> backward ghost of the next
-    reqs = slab_exchange_blocks(field, [(h["send_lo"], n, "prev"), (h["send_hi"], n, "next")],
-                                [(h["ghost_fwd"], n, "next"), (h["ghost_bwd"], n, "prev")], rank, world, group)
-    if wait:
-        for r in reqs:
-            r.wait()
-        return []
+    with _OnLibraryStream(field):
+        # first slice -> forward ghost of the previous rank; last slice -> backward ghost of the next
+        reqs = slab_exchange_blocks(field, [(h["send_lo"], n, "prev"), (h["send_hi"], n, "next")],
+                                    [(h["ghost_fwd"], n, "next"), (h["ghost_bwd"], n, "prev")], rank, world, group)
+        if wait:
+            for r in reqs:
+                r.wait()
+            return []
     return reqs
 
 
 def slab_exchange_gauge(gauge, rank, world, group=None):
     """Once, after lqcd_pack_gauge: receive the time-like links of the previous rank's last slice."""
-    for parity in (0, 1):
-        h = lqcd_slab_gauge_halo(parity)
-        for r in slab_exchange_blocks(gauge, [(h["send_hi"], h["bytes"], "next")],
-                                      [(h["ghost_bwd"], h["bytes"], "prev")], rank, world, group):
-            r.wait()
+    with _OnLibraryStream(gauge):
+        for parity in (0, 1):
+            h = lqcd_slab_gauge_halo(parity)
+            for r in slab_exchange_blocks(gauge, [(h["send_hi"], h["bytes"], "next")],
+                                          [(h["ghost_bwd"], h["bytes"], "prev")], rank, world, group):
+                r.wait()
 
 
-def slab_cg(gauge, b, x, kappa, mu, tol, maxit, rank, world, group=None, overlap=True, check_every=4):
+def slab_cg(gauge, b, x, kappa, mu, tol, maxit, rank, world, group=None, overlap=False, check_every=4):
     """CG on Mhat^dag Mhat across `world` ranks (one process per GPU, torch.distributed initialised):
     the stages of lqcd_slab_cg_stage with the halo exchanges and the three all-reduces between
-    them.  overlap: a hopping stage runs its interior sites while its halos are in flight.  Returns
-    the solve status; lqcd_cg_stats() gives iterations and residuals."""
+    them.  Everything -- kernels, NCCL point-to-point operations, all-reduces -- is issued on ONE
+    stream, the library's (check_same_stream).  overlap: a hopping stage runs its interior sites while
+    its halos are in flight; off by default, because on one GPU the split launch costs 4-16% of the
+    kernel time against a wire time of ~3.5 us (profiles/r01f_slab.md) and no two-GPU measurement says
+    otherwise yet.  Returns the solve status; lqcd_cg_stats() gives iterations and residuals."""
     import torch.distributed as dist
-    lqcd_slab_cg_begin(gauge, b, x, kappa, mu, tol)
-    total = device_bytes(lqcd_slab_sum_ptr(), 8).view(torch.float64)
+    with _OnLibraryStream():
+        lqcd_slab_cg_begin(gauge, b, x, kappa, mu, tol)
+        total = device_bytes(lqcd_slab_sum_ptr(), 8).view(torch.float64)
 
-    def allreduce():
-        if world > 1:
-            dist.all_reduce(total, group=group)
+        def allreduce():
+            if world > 1:
+                dist.all_reduce(total, group=group)
 
-    def hop(stage):
-        f = lqcd_slab_cg_halo_field(stage)
-        if overlap:
-            reqs = slab_exchange_spinor(f, rank, world, group, wait=False)
-            lqcd_slab_cg_stage(stage, 1)
-            for r in reqs:
-                r.wait()
-            lqcd_slab_cg_stage(stage, 2)
-        else:
-            slab_exchange_spinor(f, rank, world, group)
-            lqcd_slab_cg_stage(stage, 0)
+        def hop(stage):
+            f = lqcd_slab_cg_halo_field(stage)
+            if overlap:
+                reqs = slab_exchange_spinor(f, rank, world, group, wait=False)
+                lqcd_slab_cg_stage(stage, 1)
+                for r in reqs:
+                    r.wait()
+                lqcd_slab_cg_stage(stage, 2)
+            else:
+                slab_exchange_spinor(f, rank, world, group)
+                lqcd_slab_cg_stage(stage, 0)
 
-    lqcd_slab_cg_stage(0); allreduce(); lqcd_slab_cg_stage(1)
-    it = 0
-    while it < maxit:
-        hop(2); hop(3)
-        lqcd_slab_cg_stage(4); allreduce(); lqcd_slab_cg_stage(5)
-        hop(6); hop(7)
-        lqcd_slab_cg_stage(8); allreduce(); lqcd_slab_cg_stage(9)
-        it += 1
-        if it % check_every == 0 or it == maxit:
-            done, _ = lqcd_slab_cg_poll()
-            if done:
-                break
-    for stage in (11, 12, 13, 14):
-        hop(stage)
-    lqcd_slab_cg_stage(15); allreduce(); lqcd_slab_cg_stage(16)
-    return lqcd_slab_cg_end(True)
+        lqcd_slab_cg_stage(0); allreduce(); lqcd_slab_cg_stage(1)
+        it = 0
+        while it < maxit:
+            hop(2); hop(3)
+            lqcd_slab_cg_stage(4); allreduce(); lqcd_slab_cg_stage(5)
+            hop(6); hop(7)
+            lqcd_slab_cg_stage(8); allreduce(); lqcd_slab_cg_stage(9)
+            it += 1
+            if it % check_every == 0 or it == maxit:
+                done, _ = lqcd_slab_cg_poll()
+                if done:
+                    break
+        for stage in (11, 12, 13, 14):
+            hop(stage)
+        lqcd_slab_cg_stage(15); allreduce(); lqcd_slab_cg_stage(16)
+        return lqcd_slab_cg_end(True)

@@ -74,7 +74,12 @@ struct Context {
     // four CG iterations as one instantiated CUDA graph, kept while the arguments it was captured with stay the same
     struct CgGraph {
         cudaGraphExec_t exec = nullptr;
-        const void* gauge = nullptr; void* x = nullptr; void* vec0 = nullptr;
+        // the key: every argument of the 28 captured launches, and the stream the capture was tried on
+        bool keyed = false;          // the fields below describe a capture attempt (exec != null: it worked)
+        cudaStream_t stream = nullptr;
+        const void* gauge = nullptr; void* x = nullptr;
+        void* vec[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+        double* partials = nullptr; CgScalars* scal = nullptr;
         int prec = -1, recon = 0, block = 0, launches = 0;
         double kappa = 0.0, mu = 0.0;
     } cgg;
@@ -142,7 +147,13 @@ size_t gauge_bytes_of(int precision, int recon, int G) {
 }
 size_t n_reals() { return (size_t)24 * 32 * ctx.geo.G; }  // reals in one half-spinor field
 
+void drop_cg_graph() {
+    if (ctx.cgg.exec) cudaGraphExecDestroy(ctx.cgg.exec);
+    ctx.cgg = Context::CgGraph();
+}
+
 void free_workspace() {
+    drop_cg_graph();     // its launches hold the workspace pointers
     for (int pr = 0; pr < 2; ++pr)
         for (int i = 0; i < 6; ++i) { if (ctx.vec[pr][i]) cudaFree(ctx.vec[pr][i]); ctx.vec[pr][i] = nullptr; }
     for (int pr = 0; pr < 2; ++pr) { if (ctx.full_b[pr]) cudaFree(ctx.full_b[pr]); ctx.full_b[pr] = nullptr; }
@@ -152,7 +163,6 @@ void free_workspace() {
 }
 
 void free_all() {
-    if (ctx.cgg.exec) cudaGraphExecDestroy(ctx.cgg.exec);
     free_workspace();
     if (ctx.scal) cudaFree(ctx.scal);
     if (ctx.scal_outer) cudaFree(ctx.scal_outer);
@@ -181,6 +191,7 @@ int ensure_scalars() {
     size_t need = (size_t)hopping_partials(ctx.geo.Vh, 32) + 3 * (size_t)vector_grid(n_reals()) + 64;
     if (need < (size_t)plaquette_partials(ctx.geo.Vh)) need = (size_t)plaquette_partials(ctx.geo.Vh);
     if (need > ctx.n_partials) {
+        drop_cg_graph();
         if (ctx.partials) CU(cudaFree(ctx.partials));
         ctx.partials = nullptr;
         CU(cudaMalloc(&ctx.partials, need * sizeof(double)));
@@ -322,15 +333,23 @@ bool cg_graph_ready() {
     static const bool enabled = !(getenv("LQCD_CG_GRAPH") && atoi(getenv("LQCD_CG_GRAPH")) == 0);
     if (!enabled || g_prof_on || ctx.slab) return false;
     Context::CgGraph& c = ctx.cgg;
-    void* vec0 = ctx.vec[ctx.cg_prec][0];
-    if (c.exec && c.gauge == ctx.cg_gauge && c.x == ctx.cg_x && c.vec0 == vec0 && c.prec == ctx.cg_prec &&
-        c.recon == ctx.cg_recon && c.block == ctx.block && c.kappa == ctx.cg_kappa && c.mu == ctx.cg_mu)
-        return true;
+    void** v = ctx.vec[ctx.cg_prec];
+    bool same = c.keyed && c.stream == ctx.stream && c.gauge == ctx.cg_gauge && c.x == ctx.cg_x && c.prec == ctx.cg_prec &&
+                c.recon == ctx.cg_recon && c.block == ctx.block && c.kappa == ctx.cg_kappa && c.mu == ctx.cg_mu &&
+                c.partials == ctx.partials && c.scal == ctx.scal;
+    for (int i = 0; same && i < 5; ++i) same = (c.vec[i] == v[i]);
+    // same arguments as the last attempt: replay its graph, or -- if the capture or the instantiation did not
+    // work there (the legacy default stream cannot be captured) -- keep to direct launches without trying again
+    if (same) return c.exec != nullptr;
     cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
-    if (cudaStreamIsCapturing(ctx.stream, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) return false;
+    if (cudaStreamIsCapturing(ctx.stream, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) { cudaGetLastError(); return false; }
     if (c.exec) { cudaGraphExecDestroy(c.exec); c.exec = nullptr; }
+    c.keyed = true; c.stream = ctx.stream;
+    c.gauge = ctx.cg_gauge; c.x = ctx.cg_x; c.prec = ctx.cg_prec; c.recon = ctx.cg_recon;
+    c.block = ctx.block; c.kappa = ctx.cg_kappa; c.mu = ctx.cg_mu; c.partials = ctx.partials; c.scal = ctx.scal;
+    for (int i = 0; i < 5; ++i) c.vec[i] = v[i];
+    if (ctx.stream == 0 || ctx.stream == cudaStreamLegacy) return false;   // not capturable
     const long long l0 = g_launches.load();
-    // (the legacy default stream cannot be captured: direct launches there)
     if (cudaStreamBeginCapture(ctx.stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return false; }
     int rc = 0;
     for (int i = 0; i < 4 && !rc; ++i) rc = enqueue_iteration();
@@ -342,8 +361,6 @@ bool cg_graph_ready() {
     const cudaError_t ei = cudaGraphInstantiate(&c.exec, graph, 0);
     cudaGraphDestroy(graph);
     if (ei != cudaSuccess) { c.exec = nullptr; cudaGetLastError(); return false; }
-    c.gauge = ctx.cg_gauge; c.x = ctx.cg_x; c.vec0 = vec0; c.prec = ctx.cg_prec; c.recon = ctx.cg_recon;
-    c.block = ctx.block; c.kappa = ctx.cg_kappa; c.mu = ctx.cg_mu;
     return true;
 }
 
@@ -563,6 +580,11 @@ int lqcd_gauge_update(void* gauge, int mu, int parity, int mode, double beta, un
     if (rc) return rc;
     if (mode == LQCD_HEATBATH && !(beta > 0.0)) return fail(LQCD_BAD_ARG, "heatbath needs beta > 0");
     if (tag >= (1ull << 24)) return fail(LQCD_BAD_ARG, "tag must be below 2^24");
+    // the heatbath's random-number counter reaches 1584 V (4 V links x 3 subgroups x 33 attempts x 4 draws) and
+    // shares its 64-bit word with tag << 40 (reading G21): beyond 2^40 two tags would share numbers
+    if (mode == LQCD_HEATBATH && 1584ull * 2ull * (unsigned long long)ctx.geo.Vh >= (1ull << 40))
+        return fail(LQCD_BAD_DIMS, "heatbath: 1584 V = %llu random-number counters per sweep do not fit below 2^40",
+                    1584ull * 2ull * (unsigned long long)ctx.geo.Vh);
     CU(launch_gauge_update(ctx.precision, ctx.recon, mode, ctx.geo, gauge, mu, parity, beta, seed, tag, ctx.stream));
     return LQCD_OK;
 }
@@ -579,7 +601,6 @@ int lqcd_gauge_sweep(void* gauge, int mode, double beta, unsigned long long seed
 int lqcd_plaquette(const void* gauge, double* plaquette_host) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
     if (ctx.slab) return fail(LQCD_BAD_ARG, "lqcd_plaquette: not available after lqcd_slab_init (use the lqcd_slab_* calls)");
-    if (ctx.slab) return fail(LQCD_BAD_ARG, "lqcd_gauge_sweep: not available after lqcd_slab_init (use the lqcd_slab_* calls)");
     if (!gauge || !plaquette_host) return fail(LQCD_BAD_ARG, "lqcd_plaquette: null pointer");
     int rc = ensure_scalars();
     if (rc) return rc;
@@ -733,6 +754,7 @@ int lqcd_cg_setup(const void* gauge, const void* b, void* x, double kappa, doubl
 
 int lqcd_cg_iterate(int n) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (ctx.slab) return fail(LQCD_BAD_ARG, "lqcd_cg_iterate: not available after lqcd_slab_init (use the lqcd_slab_* calls)");
     if (!ctx.cg_active) return fail(LQCD_BAD_ARG, "lqcd_cg_iterate: no solve set up");
     if (n < 0) return fail(LQCD_BAD_ARG, "n must be >= 0");
     int i = 0;
@@ -750,6 +772,7 @@ int lqcd_cg_iterate(int n) {
 
 int lqcd_cg_finish(void) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (ctx.slab) return fail(LQCD_BAD_ARG, "lqcd_cg_finish: not available after lqcd_slab_init (use the lqcd_slab_* calls)");
     if (!ctx.cg_active) return fail(LQCD_BAD_ARG, "lqcd_cg_finish: no solve set up");
     return cg_finish_impl(true);
 }
@@ -888,8 +911,10 @@ int lqcd_cg_mdagm_mixed(const void* gauge_double, int recon_double, const void* 
         CU(cudaStreamSynchronize(ctx.stream));
         bb = sh->bb;
         rho = (outer == 0) ? sh->rho : sh->resid_true;
-        if (!(rho > tol * tol * bb) ) { status = LQCD_OK; break; }     // also catches b = 0
-        if (!std::isfinite(rho)) { status = LQCD_BREAKDOWN; break; }
+        // NaN / inf first (a NaN in b or in the links, an overflow in the double residual): a NaN rho would
+        // otherwise pass the negated convergence test below and be reported as converged
+        if (!std::isfinite(rho) || !std::isfinite(bb)) { status = LQCD_BREAKDOWN; break; }
+        if (!(rho > tol * tol * bb)) { status = LQCD_OK; break; }      // also catches b = 0
         if (total >= maxit) break;
         const double scale = std::sqrt(rho);
         CU(launch_convert_d2f(n, r, ctx.mx_b, 1.0 / scale, ctx.stream));
@@ -917,9 +942,9 @@ int lqcd_cg_mdagm_mixed(const void* gauge_double, int recon_double, const void* 
     }
     ctx.st_iters = total;
     ctx.st_outer = outer;
-    ctx.st_rr = ctx.st_rt = bb > 0 ? std::sqrt(rho / bb) : 0.0;   // the outer residual IS a true residual
+    ctx.st_rr = ctx.st_rt = bb > 0 ? std::sqrt(rho / bb) : (std::isfinite(bb) ? 0.0 : bb);   // the outer residual IS a true residual
     ctx.cg_active = false;
-    if (status == LQCD_BREAKDOWN) return fail(LQCD_BREAKDOWN, "mixed CG: no progress (|r|^2 = %g)", rho);
+    if (status == LQCD_BREAKDOWN) return fail(LQCD_BREAKDOWN, "mixed CG: no progress or not finite (|r|^2 = %g, |b|^2 = %g)", rho, bb);
     return status;
 }
 

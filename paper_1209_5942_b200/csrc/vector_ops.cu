@@ -1,8 +1,9 @@
 // vector_ops.cu -- fused CG vector kernels (the paper's
 // "saxpy" and "LAPACK operations", written there
 // "in a straightforward manner").  Here: two passes per iteration instead of five,
-// 128-bit loads, warp-shuffle block sums, last-block finalisation in a fixed
-// order so that alpha, beta and the convergence decision never leave the device.
+// 128-bit loads, warp-shuffle block sums written as one partial per block, and a separate
+// one-block finalize_kernel that adds the partials in a fixed order and applies the scalar
+// recurrence, so that alpha, beta and the convergence decision never leave the device.
 //
 //   cg_init      x = 0, r = p = b; finalize(FIN_BB): rho = bb = |b|^2
 //   (r -= alpha q and |r|^2 live in the epilogue of the iteration's last hopping launch,

@@ -387,9 +387,11 @@ def _sample_sites(n, count, seed):
     ((32, 32, 32, 64), False, 0.15, 0.1),     # config 5 (bench workload), bench launch configuration
 ])
 def test_full_size_sampled_sites(B, oracle_mod, dims, near_id, kappa, mu):
-    U = gen.gauge_near_identity(dims, SEED, 0.3) if near_id else gen.gauge_haar(dims, SEED)
     h = lu.volume(dims) // 2
-    x = gen.spinor_gaussian(h, SEED)
+    if near_id:
+        U, x = gen.gauge_near_identity(dims, SEED, 0.3), gen.spinor_gaussian(h, SEED)
+    else:
+        U, x, _ = _cached_fields(dims)
     sites = _sample_sites(h, 300, 17)
     L = Lat(B, dims, AP, U)
     for parity in (0, 1):
@@ -405,6 +407,84 @@ def test_full_size_sampled_sites(B, oracle_mod, dims, near_id, kappa, mu):
     Mx = L.mtm(x, kappa, mu, 0)
     MdMx = L.mtm(Mx, kappa, mu, 1)
     assert abs(np.vdot(x, MdMx) - np.vdot(Mx, Mx)) <= 1e-12 * np.vdot(Mx, Mx).real
+
+
+_FIELD_CACHE = {}
+
+
+def _cached_fields(dims):
+    """Seeded Haar links, input spinor and source of a full-size lattice, generated once per test session
+    (32^3 x 64 links take ~20 s to draw); read-only for every test that uses them."""
+    if dims not in _FIELD_CACHE:
+        h = lu.volume(dims) // 2
+        _FIELD_CACHE[dims] = (gen.gauge_haar(dims, SEED), gen.spinor_gaussian(h, SEED),
+                              gen.spinor_gaussian(h, SEED, gen.STREAM_SOURCE))
+    return _FIELD_CACHE[dims]
+
+
+# BASELINE.json configs[4]: "32^3 x 64 in both double and single precision (single also with 12-real gauge
+# reconstruction)"; PAPER.md:267 (single precision), :205, :305 (REC12).  Same launch configuration as the
+# timings of sweep.py / bench.py (default block size, whole-lattice launches).
+@pytest.mark.parametrize("precision,recon,tol", [(0, 12, TOL_D), (1, 18, TOL_S), (1, 12, TOL_S)])
+def test_config5_storage_variants_sampled_sites(B, oracle_mod, precision, recon, tol):
+    dims = (32, 32, 32, 64)
+    kappa, mu = 0.15, 0.1
+    U, x, _ = _cached_fields(dims)
+    h = lu.volume(dims) // 2
+    sites = _sample_sites(h, 300, 29 + recon + precision)
+    # the oracle is fed what the kernel is fed: inputs rounded to the storage precision
+    Ur, xr = _round_inputs(U, x, precision)
+    L = Lat(B, dims, AP, U, precision, recon)
+    for parity in (0, 1):
+        got = L.dslash(x, parity, kappa)
+        want = oracle_mod.dslash_eo_sites(dims, AP, Ur, xr, sites, parity, kappa)
+        assert lu.rel_err(got[sites], want) <= tol
+        assert np.max(np.abs(got[sites] - want)) <= tol * np.max(np.abs(want))     # no single element off
+        assert np.all(np.isfinite(got))
+    for dagger in (0, 1):
+        got = L.mtm(x, kappa, mu, dagger)
+        want = oracle_mod.mhat_sites(dims, AP, Ur, xr, sites, kappa, mu, dagger)
+        assert lu.rel_err(got[sites], want) <= tol
+        assert np.max(np.abs(got[sites] - want)) <= tol * np.max(np.abs(want))
+        assert np.all(np.isfinite(got))
+    # holds at any size: <x, Mhat^dag Mhat x> = |Mhat x|^2 (to the storage precision)
+    Mx = L.mtm(x, kappa, mu, 0)
+    MdMx = L.mtm(Mx, kappa, mu, 1)
+    assert abs(np.vdot(xr, MdMx) - np.vdot(Mx, Mx)) <= (1e-12 if precision == 0 else 1e-5) * np.vdot(Mx, Mx).real
+    del L
+
+
+@pytest.mark.parametrize("precision,recon,tol,slack", [(0, 12, 1e-10, 1.05), (1, 18, 1e-5, 20.0), (1, 12, 1e-5, 20.0)])
+def test_config4_cg_24c48_storage_variants(B, oracle_mod, precision, recon, tol, slack):
+    """CG on the config 4 lattice in the other three storage formats, the residual taken by the ORACLE's
+    (double) operator: double/12 to the double bar; single to what the recursive residual in float delivers."""
+    dims = (24, 24, 24, 48)
+    kappa, mu = 0.15, 0.1
+    U, _, b = _cached_fields(dims)
+    L = Lat(B, dims, AP, U, precision, recon)
+    st, x, (iters, rr, rt) = L.cg(b, kappa, mu, tol, 2000)
+    assert st == 0 and 5 <= iters <= 80 and rr <= tol
+    r = b - oracle_mod.mdagm(dims, AP, U, x, kappa, mu)
+    assert np.linalg.norm(r) / np.linalg.norm(b) <= slack * tol
+    del L
+
+
+def test_config5_mixed_and_bicgstab_solves_32c64(B, oracle_mod):
+    """One mixed-precision solve (single/12 inner, double/18 outer) and one BiCGStab solve at the bench
+    workload's size, each checked by ONE application of the oracle's operator to the GPU's solution."""
+    dims = (32, 32, 32, 64)
+    kappa, mu, tol = 0.15, 0.1, 1e-10
+    U, _, b = _cached_fields(dims)
+    nb = np.linalg.norm(b)
+    st, x, (iters, rr, rt), outer = _mixed_solve(B, dims, U, b, kappa, mu, tol, 2000)
+    assert st == 0 and rr <= tol and outer >= 2 and 20 <= iters <= 120
+    assert np.linalg.norm(b - oracle_mod.mdagm(dims, AP, U, x, kappa, mu)) / nb <= 1.05 * tol
+    L = Lat(B, dims, AP, U)
+    st, x, (iters, rr, rt) = L.bicgstab(b, kappa, mu, tol, 2000)
+    assert st == 0 and rr <= tol and 5 <= iters <= 60
+    true_rel = np.linalg.norm(b - oracle_mod.mhat(dims, AP, U, x, kappa, mu, 0)) / nb
+    assert true_rel <= 1.05 * tol and abs(rt - true_rel) <= 0.05 * tol
+    del L
 
 
 def test_fields_beyond_4_gib_sampled_sites(B, oracle_mod):
@@ -442,8 +522,7 @@ def test_fields_beyond_4_gib_sampled_sites(B, oracle_mod):
 def test_config4_cg_24c48(B, oracle_mod):
     dims = (24, 24, 24, 48)
     kappa, mu, tol = 0.15, 0.1, 1e-10
-    U = gen.gauge_haar(dims, SEED)
-    b = gen.spinor_gaussian(lu.volume(dims) // 2, SEED, gen.STREAM_SOURCE)
+    U, _, b = _cached_fields(dims)
     L = Lat(B, dims, AP, U)
     st, x, (iters, rr, rt) = L.cg(b, kappa, mu, tol, 2000)
     assert st == 0 and 20 <= iters <= 80 and rr <= tol
@@ -502,11 +581,31 @@ def test_mixed_precision_cg_edge_cases(B):
         assert e.value.status == B.LQCD_BAD_ARG
 
 
+def test_a_nan_source_is_a_breakdown_in_every_solver(B):
+    """A NaN in b must never come back as 'converged': all three solvers return LQCD_BREAKDOWN (include/lqcd.h)."""
+    dims = (4, 4, 4, 4)
+    U = gen.gauge_haar(dims, SEED)
+    b = gen.spinor_gaussian(lu.volume(dims) // 2, SEED, gen.STREAM_SOURCE)
+    b[5, 2, 1] = np.nan
+    L = Lat(B, dims, AP, U)
+    for solve in (lambda: L.cg(b, 0.15, 0.1, 1e-10, 50), lambda: L.bicgstab(b, 0.15, 0.1, 1e-10, 50),
+                  lambda: _mixed_solve(B, dims, U, b, 0.15, 0.1, 1e-10, 50)):
+        with pytest.raises(B.LqcdError) as e:
+            solve()
+        assert e.value.status == B.LQCD_BREAKDOWN
+    # ... and a NaN in the links
+    Un = U.copy()
+    Un[7, 1, 0, 0] = np.nan
+    b = gen.spinor_gaussian(lu.volume(dims) // 2, SEED, gen.STREAM_SOURCE)
+    with pytest.raises(B.LqcdError) as e:
+        _mixed_solve(B, dims, Un, b, 0.15, 0.1, 1e-10, 50)
+    assert e.value.status == B.LQCD_BREAKDOWN
+
+
 def test_mixed_precision_cg_24c48(B, oracle_mod):
     dims = (24, 24, 24, 48)
     kappa, mu, tol = 0.15, 0.1, 1e-10
-    U = gen.gauge_haar(dims, SEED)
-    b = gen.spinor_gaussian(lu.volume(dims) // 2, SEED, gen.STREAM_SOURCE)
+    U, _, b = _cached_fields(dims)
     st, x, (iters, rr, rt), outer = _mixed_solve(B, dims, U, b, kappa, mu, tol, 2000)
     assert st == 0 and rr <= tol and 20 <= iters <= 120
     r = b - oracle_mod.mdagm(dims, AP, U, x, kappa, mu)

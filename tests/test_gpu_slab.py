@@ -257,3 +257,51 @@ def test_binding_slab_cg_driver_single_rank(B, oracle_mod, overlap):
     x2 = B.alloc_spinor()
     assert B.slab_cg(g, s, x2, kappa, mu, 1e-30, 3, 0, 1, overlap=overlap) == 1
     assert B.lqcd_cg_stats()[0] == 3
+
+
+def test_binding_slab_cg_driver_on_a_side_stream(B, oracle_mod):
+    """The library on a side stream while torch's current stream is another one: the driver issues its copies /
+    point-to-point operations and all-reduces on the LIBRARY's stream (binding._OnLibraryStream), so halos are
+    ordered against the kernels; the result equals the run on the default stream bit for bit."""
+    import torch
+    kappa, mu, tol = 0.15, 0.1, 1e-10
+    U = gen.gauge_haar(DIMS, SEED)
+    b = gen.spinor_gaussian(lu.volume(DIMS) // 2, SEED, gen.STREAM_SOURCE)
+    B.lqcd_select_context(0)
+    out = []
+    for side in (None, torch.cuda.Stream()):
+        B.lqcd_slab_init(DIMS, AP, 0, 1)
+        assert B.library_stream() is None
+        if side is not None:
+            B.lqcd_set_stream(side)
+            assert B.library_stream() is side
+            with torch.cuda.stream(side):
+                g = B.upload_gauge(U)
+                s, x = B.upload_spinor(b, 0), B.alloc_spinor()
+            side.synchronize()
+        else:
+            B.lqcd_set_stream()
+            g = B.upload_gauge(U)
+            s, x = B.upload_spinor(b, 0), B.alloc_spinor()
+        # called from the default stream either way
+        assert torch.cuda.current_stream().cuda_stream != getattr(side, "cuda_stream", -1)
+        B.slab_exchange_gauge(g, 0, 1)
+        assert B.slab_cg(g, s, x, kappa, mu, tol, 500, 0, 1, overlap=True) == 0
+        torch.cuda.synchronize()
+        import contextlib
+        with (torch.cuda.stream(side) if side is not None else contextlib.nullcontext()):
+            out.append((B.download_spinor(x, 0), B.lqcd_cg_stats()))
+    assert out[0][1] == out[1][1] and np.array_equal(out[0][0], out[1][0])
+    assert lu.rel_err(oracle_mod.mdagm(DIMS, AP, U, out[1][0], kappa, mu), b) <= 1.05 * tol
+    with pytest.raises(RuntimeError):
+        B.check_same_stream(side.cuda_stream, torch.cuda.current_stream().cuda_stream)
+    B.lqcd_slab_init(DIMS, AP, 0, 1)
+    # after lqcd_slab_cg_begin the single-lattice three-step solver stays closed (include/lqcd.h)
+    g, s, x = B.alloc_gauge(), B.alloc_spinor(), B.alloc_spinor()
+    B.lqcd_slab_cg_begin(g, s, x, kappa, mu, tol)
+    for call in (lambda: B.lqcd_cg_iterate(1), B.lqcd_cg_finish):
+        with pytest.raises(B.LqcdError) as e:
+            call()
+        assert e.value.status == B.LQCD_BAD_ARG
+    B.lqcd_select_context(0)
+    B.lqcd_init((4, 4, 4, 4), AP)

@@ -94,3 +94,22 @@ def test_slab_host_logic_without_gpu():
                 pass
     finally:
         B.lqcd_select_context(0)
+
+
+def test_slab_driver_refuses_two_different_streams():
+    """binding.slab_cg / slab_exchange_* issue torch.distributed's operations on the library's stream and check
+    it (binding.check_same_stream): NCCL orders against torch's CURRENT stream, the kernels run on the stream of
+    lqcd_set_stream, and nothing else ties the two.  The rule itself needs no device."""
+    sys.path.insert(0, ROOT)
+    import pytest
+    import paper_1209_5942_b200.binding as B
+    B.check_same_stream(0, 0)                      # legacy default stream on both sides
+    B.check_same_stream(0x7F00DEAD, 0x7F00DEAD)
+    B.check_same_stream(None, 0)
+    for lib, cur in ((0x7F00DEAD, 0), (0, 0x7F00DEAD), (0x7F00DEAD, 0x7F00BEEF)):
+        with pytest.raises(RuntimeError, match="not the library's stream"):
+            B.check_same_stream(lib, cur)
+    # CPU tensors (the gloo tests above) are outside the rule: the guard is a no-op for them
+    with B._OnLibraryStream(torch.zeros(4, dtype=torch.uint8)) as g:
+        assert g.cm is None
+    assert B.library_stream() is None or not torch.cuda.is_available()
