@@ -26,7 +26,7 @@ SYMBOLS = [
     "lqcd_gauge_bytes", "lqcd_spinor_bytes", "lqcd_pack_gauge", "lqcd_pack_spinor",
     "lqcd_unpack_spinor", "lqcd_dslash_eo", "lqcd_mtm", "lqcd_mtm_full", "lqcd_solve_full", "lqcd_cg_mdagm", "lqcd_cg_setup",
     "lqcd_cg_iterate", "lqcd_cg_finish", "lqcd_cg_stats", "lqcd_cg_mdagm_mixed", "lqcd_cg_outer_iterations", "lqcd_bicgstab_mhat", "lqcd_force_bytes", "lqcd_unpack_force", "lqcd_fermion_force", "lqcd_force_tm", "lqcd_mtm_host", "lqcd_cg_mdagm_host",
-    "lqcd_launch_count", "lqcd_set_block_size", "lqcd_profile", "lqcd_profile_read",
+    "lqcd_launch_count", "lqcd_set_block_size", "lqcd_set_hop_variant", "lqcd_profile", "lqcd_profile_read",
     "lqcd_gauge_update", "lqcd_gauge_sweep", "lqcd_plaquette", "lqcd_unpack_gauge", "lqcd_stream_probe", "lqcd_fp64_probe",
     "lqcd_select_context", "lqcd_slab_init", "lqcd_slab_spinor_halo", "lqcd_slab_gauge_halo", "lqcd_slab_dslash",
     "lqcd_slab_mhat_stage", "lqcd_slab_cg_begin", "lqcd_slab_cg_stage", "lqcd_slab_cg_halo_field",
@@ -77,6 +77,7 @@ def _load():
         "lqcd_mtm_host": [vp, vp, vp, dbl, dbl, i32],
         "lqcd_cg_mdagm_host": [vp, vp, vp, dbl, dbl, dbl, i32],
         "lqcd_set_block_size": [i32],
+        "lqcd_set_hop_variant": [i32],
         "lqcd_gauge_update": [vp, i32, i32, i32, dbl, u64, u64],
         "lqcd_gauge_sweep": [vp, i32, dbl, u64, u64],
         "lqcd_plaquette": [vp, ctypes.POINTER(dbl)],
@@ -208,6 +209,10 @@ def lqcd_set_format(precision, recon):
 
 def lqcd_set_block_size(threads):
     return _check(_lib.lqcd_set_block_size(threads))
+
+
+def lqcd_set_hop_variant(variant):
+    return _check(_lib.lqcd_set_hop_variant(variant))
 
 
 def lqcd_gauge_bytes():

@@ -77,9 +77,10 @@ struct Context {
         // the key: every argument of the 28 captured launches, and the stream the capture was tried on
         bool keyed = false;          // the fields below describe a capture attempt (exec != null: it worked)
         cudaStream_t stream = nullptr;
-        const void* gauge = nullptr; void* x = nullptr;
-        void* vec[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
-        double* partials = nullptr; CgScalars* scal = nullptr;
+        int kind = 0;                // 0: CG on Mhat^dag Mhat (enqueue_iteration), 1: BiCGStab on Mhat (enqueue_bicg_iteration)
+        const void* gauge = nullptr; void* x = nullptr; const void* b = nullptr;   // b: BiCGStab's rhat
+        void* vec[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+        double* partials = nullptr; const void* scal = nullptr;
         int prec = -1, recon = 0, block = 0, launches = 0;
         double kappa = 0.0, mu = 0.0;
     } cgg;
@@ -188,7 +189,8 @@ int ensure_scalars() {
         for (int i = 0; i < 2; ++i) CU(cudaEventCreateWithFlags(&ctx.ev[i], cudaEventDisableTiming));
     }
     // one partial per warp of a hopping launch, or up to three per block of a vector kernel (BiCGStab)
-    size_t need = (size_t)hopping_partials(ctx.geo.Vh, 32) + 3 * (size_t)vector_grid(n_reals()) + 64;
+    // (a BiCGStab hopping launch leaves up to five sets of per-warp partials)
+    size_t need = 5 * (size_t)hopping_partials(ctx.geo.Vh, 32) + 3 * (size_t)vector_grid(n_reals()) + 64;
     if (need < (size_t)plaquette_partials(ctx.geo.Vh)) need = (size_t)plaquette_partials(ctx.geo.Vh);
     if (need > ctx.n_partials) {
         drop_cg_graph();
@@ -253,9 +255,11 @@ int hop_minv(int precision, int recon, const void* gauge, const void* in, void* 
 // fuse = FUSE_R:   `out` is CG's residual r; instead of storing Mhat^(dag) in, the second launch
 //                  applies r -= alpha * (Mhat^(dag) in) in place and reduces |r|^2 (FIN_RHO).
 // scal: device scalars whose `done` flag turns the launches into no-ops (CG), or null.
-enum { FUSE_NONE = 0, FUSE_PAP = 1, FUSE_R = 2 };
+// fuse = FUSE_DOT:  also leave the partial sums of |out|^2 and <dotw, out> (hopping.cu MODE 4; BiCGStab sums them).
+enum { FUSE_NONE = 0, FUSE_PAP = 1, FUSE_R = 2, FUSE_DOT = 3 };
 int apply_mhat(int precision, int recon, const void* gauge, const void* in, void* tmp_odd, void* out,
-               double kappa, double mu, int dagger, int fuse, CgScalars* scal) {
+               double kappa, double mu, int dagger, int fuse, CgScalars* scal, const void* dotw = nullptr,
+               const void* dotw2 = nullptr) {
     const double c = (dagger ? -1.0 : 1.0) * 2.0 * kappa * mu;
     int rc = hop_minv(precision, recon, gauge, in, tmp_odd, kappa, mu, dagger, scal);
     if (rc) return rc;
@@ -267,10 +271,10 @@ int apply_mhat(int precision, int recon, const void* gauge, const void* in, void
     e2.du_re = 1.0 / k2; e2.du_im = c / k2;
     e2.dd_re = 1.0 / k2; e2.dd_im = -c / k2;
     e2.su_re = 1.0 / k2; e2.sd_re = 1.0 / k2;
-    const int mode = (fuse == FUSE_PAP) ? 2 : (fuse == FUSE_R) ? 3 : 1;
+    const int mode = (fuse == FUSE_PAP) ? 2 : (fuse == FUSE_R) ? 3 : (fuse == FUSE_DOT) ? (dotw2 ? 5 : 4) : 1;
     CU(launch_hopping(precision, recon, dagger, mode, ctx.geo, e2, gauge, tmp_odd,
-                      out, in, 0, next_reverse(), red(), scal, ctx.block, ctx.stream));
-    if (fuse != FUSE_NONE)
+                      out, in, 0, next_reverse(), red(), scal, ctx.block, ctx.stream, nullptr, dotw, dotw2));
+    if (fuse == FUSE_PAP || fuse == FUSE_R)
         CU(launch_finalize(fuse == FUSE_PAP ? FIN_PAP : FIN_RHO, red(), hopping_partials(ctx.geo.Vh, ctx.block),
                            0.0, scal, ctx.stream));
     return LQCD_OK;
@@ -309,50 +313,54 @@ int enqueue_bicg_iteration() {
     const size_t n = n_reals();
     const int pr = ctx.cg_prec;
     CgScalars* gate = &ctx.bscal->cg;
-    int rc = apply_mhat(pr, ctx.cg_recon, ctx.cg_gauge, p, t1, v, ctx.cg_kappa, ctx.cg_mu, 0, FUSE_NONE, gate);
+    // sigma = <rhat, v> and <s, t>, |t|^2 come out of the hopping launches that produce v and t (MODE 4)
+    const int G = ctx.geo.G;
+    int rc = apply_mhat(pr, ctx.cg_recon, ctx.cg_gauge, p, t1, v, ctx.cg_kappa, ctx.cg_mu, 0, FUSE_DOT, gate, ctx.cg_b);
     if (rc) return rc;
-    CU(launch_bicg_sigma(pr, n, ctx.cg_b, v, next_reverse(), red(), ctx.bscal, ctx.stream));
+    CU(launch_bicg_finalize(FIN_BI_SIGMA_HOP, red(), G, ctx.bscal, ctx.stream));
     CU(launch_bicg_s(pr, n, r, v, s, next_reverse(), ctx.bscal, ctx.stream));
-    if ((rc = apply_mhat(pr, ctx.cg_recon, ctx.cg_gauge, s, t1, t, ctx.cg_kappa, ctx.cg_mu, 0, FUSE_NONE, gate))) return rc;
-    CU(launch_bicg_omega(pr, n, t, s, next_reverse(), red(), ctx.bscal, ctx.stream));
-    CU(launch_bicg_xr(pr, n, ctx.cg_x, p, s, t, ctx.cg_b, r, next_reverse(), red(), ctx.bscal, ctx.stream));
-    CU(launch_bicg_p(pr, n, p, r, v, next_reverse(), ctx.bscal, ctx.stream));
+    if ((rc = apply_mhat(pr, ctx.cg_recon, ctx.cg_gauge, s, t1, t, ctx.cg_kappa, ctx.cg_mu, 0, FUSE_DOT, gate, s, ctx.cg_b))) return rc;
+    CU(launch_bicg_finalize(FIN_BI_OMEGA_BETA, red(), G, ctx.bscal, ctx.stream));
+    CU(launch_bicg_xrp(pr, n, ctx.cg_x, p, s, t, v, r, next_reverse(), red(), ctx.bscal, ctx.stream));
     return LQCD_OK;
 }
 
 // Enqueue up to maxit iterations in chunks; the convergence flag of chunk k is read back while
 // chunk k+1 is already queued, so the device never idles on the host.  `scal` is the solver's
 // device scalar block (a CgScalars, or the CgScalars at the head of a BiScalars).
-// The chunk of four CG iterations (28 launches) as one CUDA graph: between the kernels of a replayed graph
+// The chunk of four CG iterations (28 launches; BiCGStab: 36) as one CUDA graph: between the kernels of a replayed graph
 // the device loses ~1 us instead of the ~3 us of a stream launch, which is 18-27 us of the 63 / 113 us a CG
 // iteration takes on 16^4 / 16^3 x 32 lattices.  Every argument of those launches is
 // fixed during a solve (the scalars live on the device), so the graph is captured once and kept until one of
 // the arguments changes.  Not used while per-launch events are recorded (lqcd_profile), in slab mode, when the
 // caller is itself capturing the stream, or with LQCD_CG_GRAPH=0.
-bool cg_graph_ready() {
+int enqueue_bicg_iteration();
+bool cg_graph_ready(int kind = 0) {
     static const bool enabled = !(getenv("LQCD_CG_GRAPH") && atoi(getenv("LQCD_CG_GRAPH")) == 0);
     if (!enabled || g_prof_on || ctx.slab) return false;
     Context::CgGraph& c = ctx.cgg;
     void** v = ctx.vec[ctx.cg_prec];
-    bool same = c.keyed && c.stream == ctx.stream && c.gauge == ctx.cg_gauge && c.x == ctx.cg_x && c.prec == ctx.cg_prec &&
-                c.recon == ctx.cg_recon && c.block == ctx.block && c.kappa == ctx.cg_kappa && c.mu == ctx.cg_mu &&
-                c.partials == ctx.partials && c.scal == ctx.scal;
-    for (int i = 0; same && i < 5; ++i) same = (c.vec[i] == v[i]);
+    const void* scal = kind ? (const void*)ctx.bscal : (const void*)ctx.scal;
+    const void* bkey = kind ? ctx.cg_b : nullptr;
+    bool same = c.keyed && c.kind == kind && c.stream == ctx.stream && c.gauge == ctx.cg_gauge && c.x == ctx.cg_x && c.b == bkey &&
+                c.prec == ctx.cg_prec && c.recon == ctx.cg_recon && c.block == ctx.block && c.kappa == ctx.cg_kappa &&
+                c.mu == ctx.cg_mu && c.partials == ctx.partials && c.scal == scal;
+    for (int i = 0; same && i < 6; ++i) same = (c.vec[i] == v[i]);
     // same arguments as the last attempt: replay its graph, or -- if the capture or the instantiation did not
     // work there (the legacy default stream cannot be captured) -- keep to direct launches without trying again
     if (same) return c.exec != nullptr;
     cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
     if (cudaStreamIsCapturing(ctx.stream, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) { cudaGetLastError(); return false; }
     if (c.exec) { cudaGraphExecDestroy(c.exec); c.exec = nullptr; }
-    c.keyed = true; c.stream = ctx.stream;
-    c.gauge = ctx.cg_gauge; c.x = ctx.cg_x; c.prec = ctx.cg_prec; c.recon = ctx.cg_recon;
-    c.block = ctx.block; c.kappa = ctx.cg_kappa; c.mu = ctx.cg_mu; c.partials = ctx.partials; c.scal = ctx.scal;
-    for (int i = 0; i < 5; ++i) c.vec[i] = v[i];
+    c.keyed = true; c.kind = kind; c.stream = ctx.stream;
+    c.gauge = ctx.cg_gauge; c.x = ctx.cg_x; c.b = bkey; c.prec = ctx.cg_prec; c.recon = ctx.cg_recon;
+    c.block = ctx.block; c.kappa = ctx.cg_kappa; c.mu = ctx.cg_mu; c.partials = ctx.partials; c.scal = scal;
+    for (int i = 0; i < 6; ++i) c.vec[i] = v[i];
     if (ctx.stream == 0 || ctx.stream == cudaStreamLegacy) return false;   // not capturable
     const long long l0 = g_launches.load();
     if (cudaStreamBeginCapture(ctx.stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return false; }
     int rc = 0;
-    for (int i = 0; i < 4 && !rc; ++i) rc = enqueue_iteration();
+    for (int i = 0; i < 4 && !rc; ++i) rc = kind ? enqueue_bicg_iteration() : enqueue_iteration();
     cudaGraph_t graph = nullptr;
     const cudaError_t e = cudaStreamEndCapture(ctx.stream, &graph);
     c.launches = (int)(g_launches.load() - l0);
@@ -372,7 +380,7 @@ int cg_run_impl(int maxit, int (*enqueue)() = enqueue_iteration, const CgScalars
     bool stop = false;
     while (launched < maxit && !stop) {
         const int n = (maxit - launched < chunk) ? (maxit - launched) : chunk;
-        if (n == chunk && enqueue == enqueue_iteration && cg_graph_ready()) {
+        if (n == chunk && cg_graph_ready(enqueue == enqueue_iteration ? 0 : 1)) {
             CU(cudaGraphLaunch(ctx.cgg.exec, ctx.stream));
             count_launch(ctx.cgg.launches);
         } else {
@@ -496,6 +504,16 @@ int lqcd_set_block_size(int threads) {
     if (threads == 0) threads = LQCD_DEFAULT_BLOCK;
     if (threads < 32 || threads > LQCD_HOP_MAX_THREADS || (threads % 32)) return fail(LQCD_BAD_ARG, "block size must be 32, 64, 96 or 128");
     ctx.block = threads;
+    return LQCD_OK;
+}
+
+int lqcd_set_hop_variant(int variant) {
+    if (variant < 0 || variant > LQCD_HOP_VARIANT_MAX) return fail(LQCD_BAD_ARG, "hopping-kernel variant must be 0..%d", LQCD_HOP_VARIANT_MAX);
+    for (int i = 0; i < MAX_CONTEXTS; ++i) {   // a captured CG chunk holds the kernels of the variant it was captured with
+        if (g_ctx[i].cgg.exec) cudaGraphExecDestroy(g_ctx[i].cgg.exec);
+        g_ctx[i].cgg = Context::CgGraph();
+    }
+    set_hopping_variant(variant);
     return LQCD_OK;
 }
 

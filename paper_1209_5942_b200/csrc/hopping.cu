@@ -17,6 +17,11 @@
 //   a9 (MODE 3) the last hopping launch of a CG iteration never stores q = A p: it
 //      applies r -= alpha q in place and reduces |r|^2 (alpha = rho / pAp read from the
 //      device scalars), which saves one field store, one field load and a launch.
+//   BiCGStab (MODE 4, 5): a MODE 1 launch that also reduces |out|^2 and <w, out> (complex) for one or
+//      two more fields w (rhat for sigma = <rhat, v>; s and rhat for <s, t>, |t|^2, <rhat, t>).  w(x) is brought
+//      into shared memory by cp.async at the start of the thread (LDGSTS: no registers, in flight
+//      with the first hop's loads) and read back in the epilogue, so the inner products cost one
+//      field read instead of a vector kernel of their own (two field reads and a launch).
 //
 // Spin projection table (gamma basis of include/lqcd.h; reading G4),
 // (1 + S gamma_mu) psi = (h0, h1, conj(c0) h0 or h1 ...):
@@ -51,19 +56,6 @@
 namespace lqcd {
 namespace {
 
-struct HopArgs {
-    const void* gauge;
-    const void* in;
-    void* out;
-    const void* aux;
-    Geometry g;
-    Epilogue ep;
-    int out_parity;
-    int reverse;   // traverse the sites in descending order (see lqcd_internal.h "snake order")
-    Reduction red;
-    CgScalars* scal;
-    SiteRange rg;
-};
 
 template <typename T, int RECON, int MU, int FWD, int DAG, bool SLAB>
 __device__ __forceinline__ void hop(T (&acc)[24], const HopArgs& a, int e, int e_nb, bool wrap) {
@@ -101,7 +93,24 @@ hopping_kernel(const HopArgs a) {
     // MODE 3: alpha = rho / <p, A p> and its inverse were left in the device scalars by
     // finalize(FIN_PAP), which also ends the solve (done = 1, caught above) on a breakdown.
     const double alpha = (MODE == 3) ? a.scal->alpha : 1.0;
+    // MODE 4, 5: w(x) (and w2(x)) parked in shared memory, [field][component][thread], 16-byte elements
+    constexpr int WCOMP = (sizeof(T) == 8) ? 12 : 6;
+    constexpr int NW = (MODE == 5) ? 2 : (MODE == 4) ? 1 : 0;
+    __shared__ __align__(16) unsigned char wsm_raw[NW > 0 ? NW * WCOMP * LQCD_HOP_MAX_THREADS * 16 : 16];
+    double dre[NW > 0 ? NW : 1] = {}, dim_[NW > 0 ? NW : 1] = {};
     if (live) {
+        if (NW > 0) {
+#pragma unroll
+            for (int f = 0; f < NW; ++f) {
+                const char* src = reinterpret_cast<const char*>(f ? a.dotw2 : a.dotw) + ((size_t)(e >> 5) * (WCOMP * 32) + (e & 31)) * 16;
+                const unsigned dst = (unsigned)__cvta_generic_to_shared(wsm_raw) + (f * WCOMP * LQCD_HOP_MAX_THREADS + threadIdx.x) * 16;
+#pragma unroll
+                for (int c = 0; c < WCOMP; ++c)
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;\n" ::"r"(dst + c * (LQCD_HOP_MAX_THREADS * 16)),
+                                 "l"(src + c * 512) : "memory");
+            }
+            asm volatile("cp.async.commit_group;\n" ::: "memory");
+        }
         // a1: e -> (x0h, x1, x2, x3); r = x0 mod 2 follows from the parity
         const int N0h = a.g.N0h, N1 = a.g.N1, N2 = a.g.N2, N3 = a.g.N3;
         int x0h, x1, x2, x3;
@@ -183,6 +192,31 @@ hopping_kernel(const HopArgs a) {
             o[2 * c + 1] = fma_(ci, acc[2 * c], cr * acc[2 * c + 1]);
         }
         store_spinor(a.out, e, o);
+        if (NW > 0) {  // <w, out> = sum conj(w) out, in double whatever T is
+            asm volatile("cp.async.wait_all;\n" ::: "memory");
+#pragma unroll
+            for (int f = 0; f < NW; ++f) {
+                if (sizeof(T) == 8) {
+                    const double2* w = reinterpret_cast<const double2*>(wsm_raw) + f * WCOMP * LQCD_HOP_MAX_THREADS + threadIdx.x;
+#pragma unroll
+                    for (int c = 0; c < 12; ++c) {
+                        const double2 v = w[c * LQCD_HOP_MAX_THREADS];
+                        dre[f] = fma(v.x, (double)o[2 * c], fma(v.y, (double)o[2 * c + 1], dre[f]));
+                        dim_[f] = fma(v.x, (double)o[2 * c + 1], fma(-v.y, (double)o[2 * c], dim_[f]));
+                    }
+                } else {
+                    const float4* w = reinterpret_cast<const float4*>(wsm_raw) + f * WCOMP * LQCD_HOP_MAX_THREADS + threadIdx.x;
+#pragma unroll
+                    for (int k = 0; k < 6; ++k) {
+                        const float4 v = w[k * LQCD_HOP_MAX_THREADS];
+                        dre[f] += (double)v.x * (double)o[4 * k] + (double)v.y * (double)o[4 * k + 1] +
+                                  (double)v.z * (double)o[4 * k + 2] + (double)v.w * (double)o[4 * k + 3];
+                        dim_[f] += (double)v.x * (double)o[4 * k + 1] - (double)v.y * (double)o[4 * k] +
+                                   (double)v.z * (double)o[4 * k + 3] - (double)v.w * (double)o[4 * k + 2];
+                    }
+                }
+            }
+        }
         if (MODE >= 2) {  // |out|^2 = |c_u|^2 |acc_upper|^2 + |c_d|^2 |acc_lower|^2
             double nu = 0.0, nd = 0.0;
 #pragma unroll
@@ -206,7 +240,17 @@ hopping_kernel(const HopArgs a) {
     }
     if (MODE >= 2) {  // one partial per warp, plain store; summed by launch_finalize(FIN_PAP / FIN_RHO)
         nrm = warp_sum(nrm);
-        if ((threadIdx.x & 31) == 0 && (!SLAB || live)) a.red.partials[e >> 5] = nrm;
+        if ((threadIdx.x & 31) == 0 && (!SLAB || live) && (NW == 0 || (e >> 5) < a.g.G)) a.red.partials[e >> 5] = nrm;
+    }
+    if (NW > 0) {  // partial set k of warp g at partials[k G + g]: k = 0 (above) |out|^2, then Re, Im <w, out> (, Re, Im <w2, out>)
+#pragma unroll
+        for (int f = 0; f < NW; ++f) {
+            const double sr = warp_sum(dre[f]), si = warp_sum(dim_[f]);
+            if ((threadIdx.x & 31) == 0 && (e >> 5) < a.g.G) {   // warps past the last group hold no partial
+                a.red.partials[(size_t)(2 * f + 1) * a.g.G + (e >> 5)] = sr;
+                a.red.partials[(size_t)(2 * f + 2) * a.g.G + (e >> 5)] = si;
+            }
+        }
     }
 }
 
@@ -222,10 +266,20 @@ cudaError_t launch_tr(int dagger, int mode, const HopArgs& a, int block, cudaStr
     LQCD_HOP_CASE(0, 0) LQCD_HOP_CASE(0, 1) LQCD_HOP_CASE(0, 2)
     LQCD_HOP_CASE(1, 0) LQCD_HOP_CASE(1, 1) LQCD_HOP_CASE(1, 2) LQCD_HOP_CASE(1, 3)
 #undef LQCD_HOP_CASE
+    if (dagger == 0 && (mode == 4 || mode == 5) && !a.g.slab) {   // BiCGStab's fused inner products (single lattice only)
+        if (mode == 4) hopping_kernel<T, RECON, 0, 4, false><<<grid, block, 0, st>>>(a);
+        else           hopping_kernel<T, RECON, 0, 5, false><<<grid, block, 0, st>>>(a);
+        return cudaGetLastError();
+    }
     return cudaErrorInvalidValue;
 }
 
 }  // namespace
+
+// which kernel launch_hopping uses where a staged variant covers the launch (hopping_staged.cu); 0 = the plain kernel
+static int g_hop_variant = 0;
+void set_hopping_variant(int variant) { g_hop_variant = variant; }
+int hopping_variant() { return g_hop_variant; }
 
 // one partial per warp of live sites, indexed by e >> 5 whatever the launch's SiteRange and block size
 int hopping_partials(int Vh, int block) {
@@ -236,8 +290,13 @@ int hopping_partials(int Vh, int block) {
 cudaError_t launch_hopping(int precision, int recon, int dagger, int mode, const Geometry& g,
                            const Epilogue& ep, const void* gauge, const void* in, void* out,
                            const void* aux, int out_parity, int reverse, Reduction red,
-                           CgScalars* scal, int block, cudaStream_t st, const SiteRange* range) {
+                           CgScalars* scal, int block, cudaStream_t st, const SiteRange* range,
+                           const void* dotw, const void* dotw2) {
+    if (g_hop_variant != 0 && hopping_variant_covers(g_hop_variant, mode, g, range))
+        return launch_hopping_variant(g_hop_variant, precision, recon, dagger, mode, g, ep, gauge, in, out, aux, out_parity,
+                                      reverse, scal, block, st);
     HopArgs a;
+    a.dotw = dotw; a.dotw2 = dotw2;
     if (range) a.rg = *range;
     else { a.rg.base = 0; a.rg.count = g.Vh; a.rg.n1 = g.Vh; a.rg.skip = 0; }
     if (a.rg.count <= 0) return cudaSuccess;
@@ -246,7 +305,7 @@ cudaError_t launch_hopping(int precision, int recon, int dagger, int mode, const
     a.g = g; a.ep = ep; a.out_parity = out_parity; a.red = red; a.scal = scal;
     if (block <= 0 || block > LQCD_HOP_MAX_THREADS || (block % 32) != 0) block = LQCD_HOP_MAX_THREADS;
     count_launch();
-    ProfScope prof(mode == 3 ? 5 : mode, st);
+    ProfScope prof(mode == 3 ? 5 : (mode >= 4 ? 1 : mode), st);
     if (precision == 0) {
         return recon == 12 ? launch_tr<double, 12>(dagger, mode, a, block, st)
                            : launch_tr<double, 18>(dagger, mode, a, block, st);

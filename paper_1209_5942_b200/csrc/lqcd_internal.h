@@ -118,6 +118,8 @@ struct BiScalars {
     double alpha_re, alpha_im;
     double omega_re, omega_im;
     double beta_re, beta_im;
+    double sigma_re, sigma_im;  // <rhat, v> of the current iteration (kept for rho' = (rho - alpha sigma) - omega <rhat, t>)
+    int pend;                   // rho' or omega unusable: a breakdown unless this iteration's |r| already meets the tolerance
 };
 
 struct Reduction {
@@ -125,7 +127,14 @@ struct Reduction {
 };
 
 enum { FIN_NONE = 0, FIN_PAP = 1, FIN_BB = 2, FIN_RHO = 3, FIN_TRUE = 4 };
-enum { FIN_BI_INIT = 0, FIN_BI_SIGMA = 1, FIN_BI_OMEGA = 2, FIN_BI_R = 3 };
+enum { FIN_BI_INIT = 0, FIN_BI_SIGMA = 1, FIN_BI_OMEGA = 2, FIN_BI_R = 3,
+       // the same two steps fed by the partial sets of a hopping MODE 4 launch: (|out|^2, Re <w,out>, Im <w,out>)
+       FIN_BI_SIGMA_HOP = 4,    // w = rhat, out = v: sigma = <rhat, v>
+       FIN_BI_OMEGA_HOP = 5,    // w = s, out = t: <t, s> = conj <s, t>, |t|^2
+       // the merged form (one pass for x, r and p): hopping MODE 5 partials (|t|^2, <s,t>, <rhat,t>) give omega AND
+       // rho' = <rhat, r'> = <rhat, s> - omega <rhat, t>, <rhat, s> = rho - alpha sigma, hence beta before r' exists;
+       FIN_BI_OMEGA_BETA = 6,
+       FIN_BI_R2 = 7 };         // |r'|^2 of the merged pass: iteration count, convergence, deferred breakdown
 
 // Thread-block size of the hopping kernel: LQCD_HOP_MAX_THREADS is its __launch_bounds__ limit,
 // LQCD_DEFAULT_BLOCK what lqcd_init selects (lqcd_set_block_size overrides, up to the limit).
@@ -142,10 +151,22 @@ enum { FIN_BI_INIT = 0, FIN_BI_SIGMA = 1, FIN_BI_OMEGA = 2, FIN_BI_R = 3 };
 // hopping.cu
 // mode 0: out = c * bracket;  mode 1: out = c * (bracket + d * aux);  mode 2: mode 1 + |out|^2 partials;
 // mode 3 (dagger = 1 only): out -= alpha * c * (bracket + d * aux) in place, alpha = scal->rho / scal->pAp, + |out|^2 partials
+// mode 4 (dagger = 0, single lattice only): mode 2 + the partials of <dotw, out>; partial set k of warp w at
+//         partials[k G + w]: k = 0 |out|^2, k = 1 Re <dotw, out>, k = 2 Im <dotw, out>
+// mode 5: mode 4 + k = 3, 4: Re, Im <dotw2, out>
 cudaError_t launch_hopping(int precision, int recon, int dagger, int mode, const Geometry& g,
                            const Epilogue& ep, const void* gauge, const void* in, void* out,
                            const void* aux, int out_parity, int reverse, Reduction red,
-                           CgScalars* scal, int block, cudaStream_t st, const SiteRange* range = nullptr);
+                           CgScalars* scal, int block, cudaStream_t st, const SiteRange* range = nullptr,
+                           const void* dotw = nullptr, const void* dotw2 = nullptr);
+
+// hopping_staged.cu: staged variants of the kernel (lqcd_set_hop_variant); they cover modes 0 and 1 on a single lattice
+void set_hopping_variant(int variant);
+int hopping_variant();
+bool hopping_variant_covers(int variant, int mode, const Geometry& g, const SiteRange* range);
+cudaError_t launch_hopping_variant(int variant, int precision, int recon, int dagger, int mode, const Geometry& g,
+                                   const Epilogue& ep, const void* gauge, const void* in, void* out, const void* aux,
+                                   int out_parity, int reverse, CgScalars* scal, int block, cudaStream_t st);
 
 // vector_ops.cu  (n = number of reals in a half-spinor field incl. padding = 24 * 32 * G)
 cudaError_t launch_cg_init(int precision, size_t n, const void* b, void* x, void* r, void* p,
@@ -177,6 +198,9 @@ cudaError_t launch_bicg_omega(int precision, size_t n, const void* t, const void
 cudaError_t launch_bicg_xr(int precision, size_t n, void* x, const void* p, const void* s, const void* t,
                            const void* rhat, void* r, int reverse, Reduction red, BiScalars* bs,
                            cudaStream_t st);
+cudaError_t launch_bicg_xrp(int precision, size_t n, void* x, void* p, const void* s, const void* t, const void* v,
+                            void* r, int reverse, Reduction red, BiScalars* bs, cudaStream_t st);
+cudaError_t launch_bicg_finalize(int fin, Reduction red, int n_partials, BiScalars* bs, cudaStream_t st);
 cudaError_t launch_bicg_p(int precision, size_t n, void* p, const void* r, const void* v, int reverse,
                           BiScalars* bs, cudaStream_t st);
 int vector_grid(size_t n);

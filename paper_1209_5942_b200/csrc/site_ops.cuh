@@ -18,6 +18,23 @@ namespace {
 __device__ __forceinline__ double fma_(double a, double b, double c) { return fma(a, b, c); }
 __device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
 
+// arguments of a hopping launch (hopping.cu, hopping_staged.cu)
+struct HopArgs {
+    const void* gauge;
+    const void* in;
+    void* out;
+    const void* aux;
+    const void* dotw;   // MODE 4, 5: the field w of <w, out>
+    const void* dotw2;  // MODE 5: a second such field
+    Geometry g;
+    Epilogue ep;
+    int out_parity;
+    int reverse;   // traverse the sites in descending order (see lqcd_internal.h "snake order")
+    Reduction red;
+    CgScalars* scal;
+    SiteRange rg;
+};
+
 // ----------------------------------------------------------------------------- field access
 // Grouped layout (lqcd_internal.h): one address per site, compile-time offsets per component.
 __device__ __forceinline__ void load_spinor(const void* base, int idx, double (&psi)[24]) {

@@ -260,10 +260,14 @@ __global__ void __launch_bounds__(VBLOCK) diag_scale_kernel_f(size_t nvec, const
 // ----------------------------------------------------------------------------- BiCGStab on Mhat
 // (PAPER.md:94 names CG and BiCGStab; reading G15 for the recurrence).  Complex
 // scalars live in BiScalars on the device; one iteration is
-//   v = Mhat p | bicg_sigma: <rhat,v> -> alpha | bicg_s: s = r - alpha v | t = Mhat s |
-//   bicg_omega: <t,s>, |t|^2 -> omega | bicg_xr: x += alpha p + omega s, r = s - omega t,
-//   |r|^2, <rhat,r> -> beta, convergence | bicg_p: p = r + beta (p - omega v)
-// = 18 field transfers besides the four hopping launches.
+//   v = Mhat p, <rhat,v> from the hopping launch (MODE 4) -> alpha | bicg_s: s = r - alpha v |
+//   t = Mhat s, <s,t>, |t|^2 from the hopping launch -> omega | bicg_xr: x += alpha p + omega s,
+//   r = s - omega t, |r|^2, <rhat,r> -> beta, convergence | bicg_p: p = r + beta (p - omega v)
+//   bicg_xrp: the last two in one pass, possible because rho' = <rhat, r'> = (rho - alpha sigma) - omega <rhat, t>
+//   is known before r' exists (<rhat, t> comes out of the hopping launch as well, MODE 5), so beta is too
+// = 3 + 8 field transfers in vector kernels + two (rhat, twice) read by hopping launches, besides the
+// four hopping launches (18 + 4 when every step is a kernel of its own: bicg_sigma, bicg_omega, bicg_xr,
+// bicg_p, which remain as the plain form of the recurrence).
 struct cd { double re, im; };
 __device__ __forceinline__ cd cmul(cd a, cd b) { return {a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re}; }
 __device__ __forceinline__ cd cdiv(cd a, cd b) {
@@ -314,10 +318,11 @@ __device__ __forceinline__ void block_partials(double (&v)[K], Reduction red) {
 
 __global__ void __launch_bounds__(1024) bicg_finalize_kernel(int fin, Reduction red, int n, double tol,
                                                              BiScalars* bs) {
-    __shared__ double sm[3][32];
+    __shared__ double sm[5][32];
     if (fin != FIN_BI_INIT && bs->cg.done) return;
-    double s[3] = {0.0, 0.0, 0.0};
-    const int K = (fin == FIN_BI_INIT) ? 1 : (fin == FIN_BI_SIGMA) ? 2 : 3;
+    double s[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    const int K = (fin == FIN_BI_INIT || fin == FIN_BI_R2) ? 1 : (fin == FIN_BI_SIGMA) ? 2 : (fin == FIN_BI_OMEGA_BETA) ? 5 : 3;
+    const int fin_in = fin;
     for (int k = 0; k < K; ++k)
         for (int i = threadIdx.x; i < n; i += 1024) s[k] += red.partials[(size_t)k * n + i];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -329,6 +334,14 @@ __global__ void __launch_bounds__(1024) bicg_finalize_kernel(int fin, Reduction 
     if (warp != 0) return;
     for (int k = 0; k < K; ++k) s[k] = warp_sum(sm[k][lane]);
     if (lane != 0) return;
+    if (fin_in == FIN_BI_SIGMA_HOP) {        // (|v|^2, <rhat, v>) -> (<rhat, v>)
+        s[0] = s[1]; s[1] = s[2];
+        fin = FIN_BI_SIGMA;
+    } else if (fin_in == FIN_BI_OMEGA_HOP) { // (|t|^2, <s, t>) -> (<t, s> = conj <s, t>, |t|^2)
+        const double tt = s[0];
+        s[0] = s[1]; s[1] = -s[2]; s[2] = tt;
+        fin = FIN_BI_OMEGA;
+    }
     if (fin == FIN_BI_INIT) {           // s0 = |b|^2; rhat = r = b so rho = <rhat, r> = |b|^2
         CgScalars& c = bs->cg;
         c.bb = s[0]; c.rho = s[0]; c.pAp = 0.0; c.beta = 0.0; c.alpha = 0.0; c.inv_alpha = 0.0;
@@ -338,15 +351,40 @@ __global__ void __launch_bounds__(1024) bicg_finalize_kernel(int fin, Reduction 
         c.upd = 0;
         bs->rho_re = s[0]; bs->rho_im = 0.0;
         bs->alpha_re = bs->alpha_im = bs->omega_re = bs->omega_im = bs->beta_re = bs->beta_im = 0.0;
+        bs->sigma_re = bs->sigma_im = 0.0;
+        bs->pend = 0;
     } else if (fin == FIN_BI_SIGMA) {   // sigma = <rhat, v>; alpha = rho / sigma
         const cd sigma = {s[0], s[1]};
         if (cbad(sigma)) { bs->cg.status = -5; bs->cg.done = 1; return; }
         const cd a = cdiv({bs->rho_re, bs->rho_im}, sigma);
         bs->alpha_re = a.re; bs->alpha_im = a.im;
+        bs->sigma_re = sigma.re; bs->sigma_im = sigma.im;
     } else if (fin == FIN_BI_OMEGA) {   // omega = <t, s> / |t|^2 (0 if t = 0)
         const double tt = s[2];
         bs->omega_re = tt > 0.0 ? s[0] / tt : 0.0;
         bs->omega_im = tt > 0.0 ? s[1] / tt : 0.0;
+    } else if (fin == FIN_BI_OMEGA_BETA) {   // s = (|t|^2, <s,t>, <rhat,t>)
+        const double tt = s[0];
+        const cd omega = {tt > 0.0 ? s[1] / tt : 0.0, tt > 0.0 ? -s[2] / tt : 0.0};   // <t,s> / |t|^2, <t,s> = conj <s,t>
+        bs->omega_re = omega.re; bs->omega_im = omega.im;
+        const cd rho = {bs->rho_re, bs->rho_im}, alpha = {bs->alpha_re, bs->alpha_im};
+        const cd as = cmul(alpha, {bs->sigma_re, bs->sigma_im});
+        const cd ot = cmul(omega, {s[3], s[4]});
+        const cd rho1 = {(rho.re - as.re) - ot.re, (rho.im - as.im) - ot.im};
+        if (cbad(rho1) || cbad(omega)) {   // decided by FIN_BI_R2, once |r'| is known
+            bs->pend = 1;
+            bs->beta_re = bs->beta_im = 0.0;
+        } else {
+            const cd beta = cmul(cdiv(rho1, rho), cdiv(alpha, omega));
+            bs->beta_re = beta.re; bs->beta_im = beta.im;
+            bs->rho_re = rho1.re; bs->rho_im = rho1.im;
+        }
+    } else if (fin == FIN_BI_R2) {      // s0 = |r'|^2
+        CgScalars& c = bs->cg;
+        c.iters += 1;
+        c.rho = s[0];
+        if (s[0] <= c.tol2bb) { c.done = 1; c.status = 0; return; }
+        if (bs->pend || !isfinite(s[0])) { c.status = -5; c.done = 1; }
     } else if (fin == FIN_BI_R) {       // s0 = |r|^2, (s1, s2) = rho' = <rhat, r>
         CgScalars& c = bs->cg;
         c.iters += 1;
@@ -441,6 +479,34 @@ __global__ void __launch_bounds__(VBLOCK) bicg_xr_kernel(size_t nvec, void* x_, 
         }
     }
     block_partials<3>(a, red);
+}
+
+// the merged pass: x += alpha p + omega s;  r' = s - omega t;  p' = r' + beta (p - omega v);  |r'|^2
+template <typename T>
+__global__ void __launch_bounds__(VBLOCK) bicg_xrp_kernel(size_t nvec, void* x_, void* p_, const void* s_, const void* t_,
+                                                          const void* v_, void* r_, int reverse, Reduction red,
+                                                          const BiScalars* bs) {
+    typedef typename VecOf<T>::type V;
+    if (bs->cg.done) return;
+    const cd alpha = {bs->alpha_re, bs->alpha_im}, omega = {bs->omega_re, bs->omega_im}, beta = {bs->beta_re, bs->beta_im};
+    const cd momega = {-omega.re, -omega.im};
+    V *x = (V*)x_, *r = (V*)r_, *p = (V*)p_;
+    const V *s = (const V*)s_, *t = (const V*)t_, *v = (const V*)v_;
+    LQCD_VEC_INDEX;
+    double a[1] = {0.0};
+#pragma unroll
+    for (int k = 0; k < VUNROLL; ++k) {
+        const size_t i = base + (size_t)k * VBLOCK;
+        if (i < nvec) {
+            const V sv = __ldcs(s + i), pv = p[i];
+            x[i] = caxpy(omega, sv, caxpy(alpha, pv, x[i]));
+            const V rn = caxpy(momega, __ldcs(t + i), sv);
+            r[i] = rn;
+            a[0] += norm2(rn);
+            p[i] = caxpy(beta, caxpy(momega, __ldcs(v + i), pv), rn);
+        }
+    }
+    block_partials<1>(a, red);
 }
 
 template <typename T>
@@ -614,6 +680,22 @@ cudaError_t launch_bicg_xr(int precision, size_t n, void* x, const void* p, cons
     ProfScope prof(3, st);
     LQCD_BICG_DISPATCH(bicg_xr_kernel, x, p, s, t, rhat, r, reverse, red, bs);
     bicg_finalize_kernel<<<1, 1024, 0, st>>>(FIN_BI_R, red, bicg_grid(precision, n), 0.0, bs);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_bicg_xrp(int precision, size_t n, void* x, void* p, const void* s, const void* t, const void* v,
+                            void* r, int reverse, Reduction red, BiScalars* bs, cudaStream_t st) {
+    count_launch(2);
+    ProfScope prof(3, st);
+    LQCD_BICG_DISPATCH(bicg_xrp_kernel, x, p, s, t, v, r, reverse, red, bs);
+    bicg_finalize_kernel<<<1, 1024, 0, st>>>(FIN_BI_R2, red, bicg_grid(precision, n), 0.0, bs);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_bicg_finalize(int fin, Reduction red, int n_partials, BiScalars* bs, cudaStream_t st) {
+    count_launch();
+    ProfScope prof(3, st);
+    bicg_finalize_kernel<<<1, 1024, 0, st>>>(fin, red, n_partials, 0.0, bs);
     return cudaGetLastError();
 }
 

@@ -2,7 +2,7 @@
 """sweep.py -- timings of the BASELINE.json configurations 3, 4, 5 and of the paper's thermal
 lattice shapes (Fig. 7), one JSON line each.  A user-facing companion of bench.py:
 
-    python -m paper_1209_5942_b200.sweep [--configs 3,4,5,thermal,force,gauge,slab,copy,large] [--out FILE]
+    python -m paper_1209_5942_b200.sweep [--configs 3,4,5,thermal,force,gauge,slab,copy,large] [--out FILE] [--hop-variant N]
 
 config 3: 16^3x32, near-identity links, kappa=.16 mu=.05: 10 warm-up + 100 timed D_eo/D_oe
           applications, 5 repeats, median (working set fits L2: not a HBM roofline figure)
@@ -456,14 +456,19 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--configs", default="3,4,5,thermal")
     ap.add_argument("--out", default=None)
+    ap.add_argument("--hop-variant", type=int, default=0,
+                    help="hopping kernel variant (lqcd_set_hop_variant): 0 plain (default), 1..3 link ring of that depth")
     args = ap.parse_args()
     if not torch.cuda.is_available():
         raise SystemExit("sweep.py needs a CUDA device: there is no CPU fallback")
     stream = torch.cuda.Stream()
     table = {"3": config3, "4": config4, "5": config5, "thermal": thermal, "force": force, "gauge": gauge, "slab": slab, "copy": copy, "large": large}
     lines = []
+    B.lqcd_set_hop_variant(args.hop_variant)
     for key in args.configs.split(","):
         for r in table[key.strip()](stream):
+            if args.hop_variant:
+                r["hop_variant"] = args.hop_variant
             line = json.dumps(r)
             print(line, flush=True)
             lines.append(line)

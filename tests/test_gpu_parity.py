@@ -868,3 +868,63 @@ def test_cg_on_a_side_stream_graph_replay_matches_direct_launches(B, oracle_mod)
         assert np.array_equal(B.download_spinor(xd, 0), ref[(0.15, 0.1)][0])
     torch.cuda.synchronize()
     B.lqcd_set_stream()
+
+
+def test_bicgstab_on_a_side_stream_graph_replay_matches_direct_launches(B, oracle_mod):
+    """BiCGStab replays its four-iteration chunk (36 launches) through the same graph cache: bit-identical to direct
+    launches, also when a CG solve (other graph kind, same cache slot) runs in between, in double and in single/12."""
+    import torch
+    dims = (8, 8, 8, 16)
+    U = gen.gauge_haar(dims, SEED)
+    h = lu.volume(dims) // 2
+    b = gen.spinor_gaussian(h, SEED, gen.STREAM_SOURCE)
+    for precision, recon, tol in ((0, 18, 1e-10), (1, 12, 1e-5)):
+        L = Lat(B, dims, AP, U, precision, recon)
+        B.lqcd_set_stream()
+        st, x0, stats0 = L.bicgstab(b, 0.15, 0.1, tol, 500)
+        assert st == 0
+        side = torch.cuda.Stream()
+        B.lqcd_set_stream(side)
+        with torch.cuda.stream(side):
+            for rep in range(3):
+                st, x, stats = L.bicgstab(b, 0.15, 0.1, tol, 500)
+                assert st == 0 and stats == stats0
+                assert np.array_equal(x, x0)
+                if rep == 0:
+                    assert L.cg(b, 0.15, 0.1, tol, 500)[0] == 0
+            if precision == 0:
+                res = b - oracle_mod.mhat(dims, AP, U, x, 0.15, 0.1, 0)
+                assert np.linalg.norm(res) <= 1.05 * tol * np.linalg.norm(b)
+        torch.cuda.synchronize()
+        B.lqcd_set_stream()
+
+
+# --------------------------------------------------------------------------- staged variants of the hopping kernel
+@pytest.mark.parametrize("variant", [1, 2, 3])
+@pytest.mark.parametrize("precision,recon,tol", [(0, 18, TOL_D), (0, 12, TOL_D), (1, 18, TOL_S), (1, 12, TOL_S)])
+def test_hopping_variants_match_oracle(B, oracle_mod, variant, precision, recon, tol):
+    """lqcd_set_hop_variant: every staged variant of the hopping kernel (hopping_staged.cu) against the oracle, in every
+    storage format, on a ragged lattice with complex phases on every wrap (Vh = 192: one and a half thread blocks) and on
+    8^3 x 16; D_eo, D_oe, Mhat and Mhat^dag (plain and M_ee*aux epilogues).  The variant must also be bit-identical to
+    the default kernel: same operations in the same order per site."""
+    kappa, mu = 0.15, 0.1
+    try:
+        for dims, phases in (((4, 6, 2, 8), GENERIC_PH), ((8, 8, 8, 16), AP)):
+            U = gen.gauge_haar(dims, SEED)
+            x = gen.spinor_gaussian(lu.volume(dims) // 2, SEED)
+            Ur, xr = _round_inputs(U, x, precision)
+            B.lqcd_set_hop_variant(0)
+            L = Lat(B, dims, phases, U, precision, recon)
+            ref = [L.dslash(x, 0, kappa), L.dslash(x, 1, kappa), L.mtm(x, kappa, mu, 0), L.mtm(x, kappa, mu, 1)]
+            B.lqcd_set_hop_variant(variant)
+            got = [L.dslash(x, 0, kappa), L.dslash(x, 1, kappa), L.mtm(x, kappa, mu, 0), L.mtm(x, kappa, mu, 1)]
+            want = [oracle_mod.dslash_eo(dims, phases, Ur, xr, 0, kappa), oracle_mod.dslash_eo(dims, phases, Ur, xr, 1, kappa),
+                    oracle_mod.mhat(dims, phases, Ur, xr, kappa, mu, 0), oracle_mod.mhat(dims, phases, Ur, xr, kappa, mu, 1)]
+            for g_, w_, r_ in zip(got, want, ref):
+                assert lu.rel_err(g_, w_) <= tol
+                assert np.array_equal(g_, r_)
+    finally:
+        B.lqcd_set_hop_variant(0)
+    with pytest.raises(B.LqcdError) as e:
+        B.lqcd_set_hop_variant(99)
+    assert e.value.status == B.LQCD_BAD_ARG
