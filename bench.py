@@ -32,6 +32,8 @@ e2e     = the same per-step work through lqcd_cg_mdagm_host with pinned HOST
 roofline.stream_probe_gbs = what lqcd_stream_probe (the paper's copy micro-benchmark, Fig. 5) moves on this
           box in the same run: copy, read-only and 7 reads : 1 write on 16-byte elements (context for frac).
 --impl reference times the CPU oracle (oracle/, test infrastructure) on the host cores.
+--scaling strong (not the contract's arm, which is N independent replicas): the ONE lattice split over the N ranks
+          along t (lqcd_slab_*), a step = one CG iteration of binding.slab_cg with its halo exchanges and all-reduces.
 """
 import argparse
 import json
@@ -491,6 +493,97 @@ def run_ours(args, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+def run_strong(args, rank, world, local_rank):
+    """--scaling strong: ONE 32^3 x 64 lattice, its time direction split over the N ranks (lqcd_slab_*, DESIGN.md
+    section 7); a step is one CG iteration of binding.slab_cg: four hopping stages, each behind the halo exchange of
+    its input field (two blocks per direction, NCCL point-to-point on the library's stream), and two all-reduces of one
+    double.  The default arm (replicas) is what BASELINE.json's north_star fixes; this arm exists so that a multi-GPU run
+    measures the decomposition.  N = 1 runs the same stages with the rank as its own neighbour."""
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    if DIMS[3] % world or (DIMS[3] // world) % 2:
+        raise SystemExit(f"--scaling strong: {world} ranks do not divide N_t = {DIMS[3]} into even slabs")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        os.environ.setdefault("NCCL_DEBUG", "INFO")      # which transport carried the halos: say so in the log
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    import lqcd_inputs as gen
+    import paper_1209_5942_b200.binding as B
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    Vh = int(np.prod(DIMS)) // 2
+    ph = gen.antiperiodic_t()
+    U = gen.gauge_haar(DIMS, gen.BASE_SEED)                           # the same global field on every rank ...
+    b = gen.spinor_gaussian(Vh, gen.BASE_SEED, gen.STREAM_SOURCE)
+    s3 = DIMS[0] * DIMS[1] * DIMS[2]
+    nt = DIMS[3] // world
+    lo, hi = rank * nt * s3, (rank + 1) * nt * s3                      # ... of which this rank keeps its time slab
+    B.lqcd_slab_init(DIMS, ph, rank, world)
+    stream = torch.cuda.Stream()
+    B.lqcd_set_stream(stream)
+    with torch.cuda.stream(stream):
+        g = B.upload_gauge(U[lo:hi])
+        B.slab_exchange_gauge(g, rank, world)
+        src = B.upload_spinor(b[lo // 2:hi // 2], 0)
+        x = B.alloc_spinor()
+    stream.synchronize()
+    del U
+
+    def run_steps(n):
+        done = 0
+        with torch.cuda.stream(stream):
+            while done < n:
+                k = min(SOLVE_LEN, n - done)
+                st = B.slab_cg(g, src, x, KAPPA, MU, 0.0, k, rank, world, overlap=args.overlap, check_every=SOLVE_LEN)
+                if st < 0:
+                    raise SystemExit(f"bench: slab_cg status {st}")
+                done += k
+
+    run_steps(args.warmup)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n0 = B.lqcd_launch_count()
+    barrier()
+    with ClockSampler(local_rank) as clk:
+        e0.record(stream)
+        run_steps(args.steps)
+        e1.record(stream)
+        stream.synchronize()
+    barrier()
+    launches = max_over_ranks(B.lqcd_launch_count() - n0, world, "cuda")
+    ms_max = max_over_ranks(e0.elapsed_time(e1), world, "cuda")
+    iters, rr, rt = B.lqcd_cg_stats()
+    h = B.lqcd_slab_spinor_halo()
+    value = args.steps * 4 * Vh * FLOP_PER_SITE / (ms_max * 1e-3) / 1e9        # the whole lattice, all ranks together
+    cfg = workload_config()
+    cfg["workload"] = cfg["workload"].replace("one step = one CG iteration", f"time direction split over {world} rank(s) "
+                                              f"(slabs of {nt} slices); one step = one CG iteration of binding.slab_cg")
+    cfg.update({"ranks": world, "local_lattice": list(DIMS[:3]) + [nt], "overlap_interior_with_halo": bool(args.overlap),
+                "halo_bytes_sent_per_rank_and_hopping_stage": 2 * int(h["bytes"]),
+                "note": "each solve of %d iterations also pays its setup and the true-residual check (one more "
+                        "application of Mhat^dag Mhat) inside the timed region; stages are issued from Python, ~30 calls per "
+                        "iteration, so small slabs are launch bound (a native driver is future work)" % SOLVE_LEN})
+    line = {"metric": METRIC, "value": value, "unit": "GFLOPS", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": cfg, "clocks": clk.summary(), "gpu_launches": int(launches),
+            "last_solve": {"iterations": iters, "rel_resid_recursive": rr, "rel_resid_true": rt},
+            "gbs_effective_step": args.steps * Vh * STEP_BYTES_PER_SITE / (ms_max * 1e-3) / 1e9,
+            "e2e": None, "roofline": None, "cpu_baseline": None,
+            "measured": "kernels and exchange as one region (CUDA events on the library's stream, max over ranks); the "
+                        "roofline / e2e / cpu_baseline legs belong to the default arm (--scaling weak)"}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    B.lqcd_finalize()
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -499,6 +592,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="weak (default): N independent replicas, the contract's arm; strong: one lattice split over N ranks")
+    ap.add_argument("--overlap", action="store_true", help="--scaling strong: interior sites while the halos are in flight")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     rank = int(os.environ.get("RANK", "0"))
@@ -506,6 +602,9 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank)
+        return
+    if args.scaling == "strong":
+        run_strong(args, rank, world, local_rank)
         return
     run_ours(args, rank, world, local_rank)
 

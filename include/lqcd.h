@@ -334,8 +334,11 @@ int lqcd_set_block_size(int threads);
  *   0      the default: one thread per site, every operand through LDG into registers
  *   1..3   "link ring": each thread prefetches the link of hop h + D (D = variant) into its own shared-memory
  *          slot with cp.async while it works on hop h
+ *   4, 5   "bulk": lane 0 of every warp fetches the warp's forward links (one contiguous block per direction in the
+ *          internal layout) with one cp.async.bulk per direction, completion on the warp's mbarrier; 4 = z and t
+ *          links, 5 = all four directions
  * Returns LQCD_BAD_ARG for other values. */
-#define LQCD_HOP_VARIANT_MAX 3
+#define LQCD_HOP_VARIANT_MAX 5
 int lqcd_set_hop_variant(int variant);
 
 #ifdef __cplusplus

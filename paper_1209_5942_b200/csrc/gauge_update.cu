@@ -19,6 +19,7 @@
 // 9 x 144 = 1296 B per updated link in double/18; the 2.1-fold reuse of the 18 loads is left to
 // L1/L2, as for the neighbour spinors of the hopping kernel.
 #include "site_ops.cuh"
+#include <cstdlib>
 
 // Measured at 32^3 x 64 (us per sub-sweep, heatbath / overrelaxation): double with 2 CTAs per SM
 // (246 registers) 460 / 289, with 3 (168 registers, 8 B of spills) 415 / 291, with the staple loop
@@ -406,6 +407,80 @@ gauge_update_kernel(const GaugeArgs a) {
     gstore<RECON>(a.gauge, G, p, mu, e, L);
 }
 
+
+// Heatbath, warp-specialised (LQCD_HEATBATH_WS=1; not the default, see the end of this comment): a CTA of 256 threads is two warpgroups working on the same 128
+// links.  Warpgroup 1 does nothing but the field-independent part of the three Kennedy-Pendleton steps (kp_precompute:
+// 30 uniforms, 12 logarithms, 6 cospi, 3 sincospi and 3 square roots per link, ~2000 instructions, FP64/integer pipes)
+// and parks the 24 doubles per link in shared memory; warpgroup 0 is the update kernel proper (staple loads and
+// products, latency bound) and meets it at a named barrier before the subgroup steps.  The two instruction streams
+// overlap instead of following each other inside one thread, and setmaxnreg moves the registers to where they are
+// needed: the CTA is launched at 80 registers per thread (three CTAs per SM), warpgroup 1 drops to 40, warpgroup 0
+// takes 120.  Same counters, same values, same decisions as the one-thread form (gauge_update_kernel<.., 0>).
+// Measured at 32^3 x 64 (us per sub-sweep, this kernel / one thread per link): double/18 431 / 398, single/18 307 / 279,
+// double/12 435 / 411, single/12 330 / 307.  The Kennedy-Pendleton arithmetic costs the same ~130 us wherever it runs:
+// it is bound by the FP64 pipe (about 1500 FP64 instructions per link on top of the 2250 of the staple products),
+// not by latency another warp could hide.
+template <typename T, int RECON>
+__global__ void __launch_bounds__(256, 3) heatbath_ws_kernel(const GaugeArgs a) {
+    __shared__ double pre_s[3 * KP_SLOTS * 128];
+    const int wg = threadIdx.x >> 7, tl = threadIdx.x & 127;
+    const int e = blockIdx.x * 128 + tl;
+    const int G = a.g.G, mu = a.mu, p = a.parity;
+    const bool live = e < a.g.Vh;
+    if (wg == 1) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;\n" ::);
+        if (live) {
+            int x0h, x1, x2, x3;
+            site_coords(a.g, e, x0h, x1, x2, x3);
+            const int r = (x1 + x2 + x3 + p) & 1;
+            const unsigned long long link_id = 4ull * (2ull * (unsigned long long)e + (unsigned long long)r) + (unsigned long long)mu;
+#pragma unroll 1
+            for (int i = 0; i < 3; ++i)
+                kp_precompute(a.seed, a.tag, ((link_id * 3ull + (unsigned long long)i) * (unsigned long long)(MAXTRY + 1)) * 4ull,
+                              pre_s + tl + (size_t)i * KP_SLOTS * 128, 128);
+        }
+        __threadfence_block();
+        asm volatile("bar.arrive 1, 256;\n" ::);
+        return;
+    }
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 120;\n" ::);
+    T L[18], A[18];
+    unsigned long long link_id = 0;
+    if (live) {
+        const SiteIdx x = site_of(a.g, e, p);
+        const SiteIdx xpm = step(a.g, x, mu, +1);
+        link_id = 4ull * (2ull * (unsigned long long)e + (unsigned long long)x.r) + (unsigned long long)mu;
+#pragma unroll
+        for (int i = 0; i < 18; ++i) A[i] = 0;
+#pragma unroll kStapleUnroll
+        for (int j = 1; j < 4; ++j) {
+            const int nu = (mu + j) & 3;
+            const SiteIdx xpn = step(a.g, x, nu, +1), xmn = step(a.g, x, nu, -1), xpmmn = step(a.g, xpm, nu, -1);
+            T u[18], w[18], t[18];
+            gload<RECON, false>(a.gauge, G, 1 - p, nu, xpm.e, u);     // U_nu(x+mu)
+            gload<RECON, false>(a.gauge, G, 1 - p, mu, xpn.e, w);     // U_mu(x+nu)
+            mm3<false, true, false>(u, w, t);
+            gload<RECON, false>(a.gauge, G, p, nu, x.e, u);           // U_nu(x)
+            mm3<false, true, true>(t, u, A);
+            gload<RECON, false>(a.gauge, G, p, nu, xpmmn.e, u);       // U_nu(x+mu-nu)
+            gload<RECON, false>(a.gauge, G, 1 - p, mu, xmn.e, w);     // U_mu(x-nu)
+            mm3<true, true, false>(u, w, t);
+            gload<RECON, false>(a.gauge, G, 1 - p, nu, xmn.e, u);     // U_nu(x-nu)
+            mm3<false, false, true>(t, u, A);
+        }
+        gload<RECON, true>(a.gauge, G, p, mu, e, L);
+    }
+    asm volatile("bar.sync 1, 256;\n" ::: "memory");
+    if (live) {
+        const double* pre = pre_s + tl;
+        subgroup_step<0, 0, 0, 1>(L, A, a.beta, a.seed, a.tag, link_id, pre, 128);
+        subgroup_step<0, 1, 1, 2>(L, A, a.beta, a.seed, a.tag, link_id, pre, 128);
+        subgroup_step<0, 2, 0, 2>(L, A, a.beta, a.seed, a.tag, link_id, pre, 128);
+        if (RECON == 12) orthonormalise_rows01(L);
+        gstore<RECON>(a.gauge, G, p, mu, e, L);
+    }
+}
+
 // Average plaquette: one thread per site of parity blockIdx.y, 6 plaquettes
 //   P_mu_nu(x) = U_mu(x) U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag,  mu < nu;
 // one partial sum of Re tr per warp (fixed-order two-stage sum, lqcd_internal.h).
@@ -453,10 +528,13 @@ cudaError_t launch_gauge_update(int precision, int recon, int mode, const Geomet
     const int grid = (g.Vh + 127) / 128;
     count_launch();
     ProfScope prof(7, st);
+    // heatbath: LQCD_HEATBATH_WS=1 selects the warp-specialised kernel (measured slower: profiles/r02_heatbath.md)
+    static const bool ws = getenv("LQCD_HEATBATH_WS") && atoi(getenv("LQCD_HEATBATH_WS")) != 0;
 #define LQCD_GU(TT, RR)                                                                   \
     do {                                                                                  \
-        if (mode == 0) gauge_update_kernel<TT, RR, 0><<<grid, 128, 0, st>>>(a);           \
-        else           gauge_update_kernel<TT, RR, 1><<<grid, 128, 0, st>>>(a);           \
+        if (mode == 0 && ws) heatbath_ws_kernel<TT, RR><<<grid, 256, 0, st>>>(a);         \
+        else if (mode == 0)  gauge_update_kernel<TT, RR, 0><<<grid, 128, 0, st>>>(a);     \
+        else                 gauge_update_kernel<TT, RR, 1><<<grid, 128, 0, st>>>(a);     \
     } while (0)
     if (precision == 0) { if (recon == 12) LQCD_GU(double, 12); else LQCD_GU(double, 18); }
     else                { if (recon == 12) LQCD_GU(float, 12);  else LQCD_GU(float, 18); }

@@ -173,11 +173,14 @@ def config4(stream):
     return out
 
 
+FORMATS = ((0, 18), (0, 12), (1, 18), (1, 12))   # --formats narrows config 5 down (d18,d12,s18,s12)
+
+
 def config5(stream):
     dims = (32, 32, 32, 64)
     U = gen.gauge_haar(dims)
     out = []
-    for precision, recon in ((0, 18), (0, 12), (1, 18), (1, 12)):
+    for precision, recon in FORMATS:
         r = time_dslash(dims, U, precision, recon, 0.15, 20, 200, 3, stream)
         r.update({"config": 5, "lattice": list(dims), "precision": "double" if precision == 0 else "single",
                   "recon": recon})
@@ -457,8 +460,11 @@ def main():
     ap.add_argument("--configs", default="3,4,5,thermal")
     ap.add_argument("--out", default=None)
     ap.add_argument("--hop-variant", type=int, default=0,
-                    help="hopping kernel variant (lqcd_set_hop_variant): 0 plain (default), 1..3 link ring of that depth")
+                    help="hopping kernel variant (lqcd_set_hop_variant): 0 plain (default), 1..3 link ring of that depth, 4 / 5 bulk-staged forward links")
+    ap.add_argument("--formats", default="d18,d12,s18,s12", help="storage variants timed by config 5")
     args = ap.parse_args()
+    global FORMATS
+    FORMATS = tuple({"d18": (0, 18), "d12": (0, 12), "s18": (1, 18), "s12": (1, 12)}[f.strip()] for f in args.formats.split(","))
     if not torch.cuda.is_available():
         raise SystemExit("sweep.py needs a CUDA device: there is no CPU fallback")
     stream = torch.cuda.Stream()

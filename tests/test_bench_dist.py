@@ -49,3 +49,22 @@ def test_reference_arm_prints_one_json_line_rank0_only():
     # a non-zero rank does no work and prints nothing
     r = subprocess.run(cmd, capture_output=True, text=True, env=dict(env, RANK="1", WORLD_SIZE="2"), timeout=60)
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+import pytest
+
+
+@pytest.mark.gpu
+def test_strong_scaling_arm_runs_the_slab_cg_on_one_gpu():
+    """bench.py --scaling strong at N = 1: the slab decomposition's stages with the rank as its own neighbour; the
+    line carries the contract's keys, "scaling": "strong", and the last solve made progress."""
+    cmd = [sys.executable, os.path.join(ROOT, "bench.py"), "--scaling", "strong", "--gpus", "1", "--steps", "12", "--warmup", "4"]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    j = json.loads(lines[0])
+    assert j["scaling"] == "strong" and j["n_gpus"] == 1 and j["unit"] == "GFLOPS" and j["value"] > 0
+    assert j["config"]["ranks"] == 1 and j["config"]["local_lattice"] == [32, 32, 32, 64]
+    assert j["gpu_launches"] > 0 and j["last_solve"]["iterations"] == 12
+    assert 0 < j["last_solve"]["rel_resid_true"] < 1.0
