@@ -69,9 +69,9 @@ METRIC = "D_tm GFLOPS (1320 flop/site) & achieved HBM GB/s vs B200 peak, double"
 # dram__bytes_read.sum + dram__bytes_write.sum per PLAIN hopping launch (MODE 0, exactly 1536 B/site algorithmic =
 # 1.610613 GB) at this workload, from the committed `ncu --set full` capture named in NCU_TRAFFIC_SOURCE; a constant
 # typed in from that file, NOT measured in this run -- refreshed whenever the hopping kernel changes.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 1586500000
-NCU_TRAFFIC_SOURCE = ("profiles/r01g_final.md (ncu --set full of hopping_kernel<double,18,0,0> and <double,18,1,0>, build 78152d3; "
-                      "the kernel's SASS is unchanged since): mean of 1.5872 and 1.5858 GB")
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 1589003000
+NCU_TRAFFIC_SOURCE = ("profiles/r02_hopping_staged.md, column 0 (ncu --set full of hopping_kernel<double,18,0,0>, build fef04fc, raw "
+                      "page in profiles/r02g_hop_v0_raw.csv): dram__bytes_read 1.415640 GB + dram__bytes_write 0.173363 GB")
 
 
 def measured_peak():

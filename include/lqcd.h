@@ -337,8 +337,11 @@ int lqcd_set_block_size(int threads);
  *   4, 5   "bulk": lane 0 of every warp fetches the warp's forward links (one contiguous block per direction in the
  *          internal layout) with one cp.async.bulk per direction, completion on the warp's mbarrier; 4 = z and t
  *          links, 5 = all four directions
+ *   6      "tile": the default kernel with another order of the sites: the four warps of a CTA take a 2 x 2 block in
+ *          (z, t) of one 32-site group in (x, y) instead of four consecutive groups (16 instead of 21 groups of
+ *          neighbour spinors per CTA); covers every launch on a single lattice whose z planes hold whole groups
  * Returns LQCD_BAD_ARG for other values. */
-#define LQCD_HOP_VARIANT_MAX 5
+#define LQCD_HOP_VARIANT_MAX 6
 int lqcd_set_hop_variant(int variant);
 
 #ifdef __cplusplus

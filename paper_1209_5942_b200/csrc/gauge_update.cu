@@ -98,7 +98,7 @@ __device__ __forceinline__ SiteIdx step(const Geometry& g, SiteIdx s, int dir, i
 template <int RECON, bool COHERENT>
 __device__ __forceinline__ void gload(const void* gauge, int G, int par, int mu, int idx, double (&u)[18]) {
     const double2* p = reinterpret_cast<const double2*>(gauge) +
-                       ((size_t)(par * 4 + mu) * G + (idx >> 5)) * ((RECON / 2) * 32) + (idx & 31);
+                       gauge_block(par, mu, G, idx >> 5) * ((RECON / 2) * 32) + (idx & 31);
 #pragma unroll
     for (int j = 0; j < RECON / 2; ++j) {
         const double2 v = COHERENT ? p[j * 32] : __ldg(p + j * 32);
@@ -111,7 +111,7 @@ template <int RECON, bool COHERENT>
 __device__ __forceinline__ void gload(const void* gauge, int G, int par, int mu, int idx, float (&u)[18]) {
     if (RECON == 12) {
         const float4* p = reinterpret_cast<const float4*>(gauge) +
-                          ((size_t)(par * 4 + mu) * G + (idx >> 5)) * (3 * 32) + (idx & 31);
+                          gauge_block(par, mu, G, idx >> 5) * (3 * 32) + (idx & 31);
 #pragma unroll
         for (int j = 0; j < 3; ++j) {
             const float4 v = COHERENT ? p[j * 32] : __ldg(p + j * 32);
@@ -119,7 +119,7 @@ __device__ __forceinline__ void gload(const void* gauge, int G, int par, int mu,
         }
         reconstruct_row2(u);
     } else {
-        const float* blk = reinterpret_cast<const float*>(gauge) + ((size_t)(par * 4 + mu) * G + (idx >> 5)) * (18 * 32);
+        const float* blk = reinterpret_cast<const float*>(gauge) + gauge_block(par, mu, G, idx >> 5) * (18 * 32);
         const float4* p = reinterpret_cast<const float4*>(blk) + (idx & 31);
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
@@ -167,18 +167,18 @@ __device__ __forceinline__ void orthonormalise_rows01(T (&u)[18]) {
 
 template <int RECON>
 __device__ __forceinline__ void gstore(void* gauge, int G, int par, int mu, int idx, const double (&u)[18]) {
-    double2* p = reinterpret_cast<double2*>(gauge) + ((size_t)(par * 4 + mu) * G + (idx >> 5)) * ((RECON / 2) * 32) + (idx & 31);
+    double2* p = reinterpret_cast<double2*>(gauge) + gauge_block(par, mu, G, idx >> 5) * ((RECON / 2) * 32) + (idx & 31);
 #pragma unroll
     for (int j = 0; j < RECON / 2; ++j) p[j * 32] = make_double2(u[2 * j], u[2 * j + 1]);
 }
 template <int RECON>
 __device__ __forceinline__ void gstore(void* gauge, int G, int par, int mu, int idx, const float (&u)[18]) {
     if (RECON == 12) {
-        float4* p = reinterpret_cast<float4*>(gauge) + ((size_t)(par * 4 + mu) * G + (idx >> 5)) * (3 * 32) + (idx & 31);
+        float4* p = reinterpret_cast<float4*>(gauge) + gauge_block(par, mu, G, idx >> 5) * (3 * 32) + (idx & 31);
 #pragma unroll
         for (int j = 0; j < 3; ++j) p[j * 32] = make_float4(u[4 * j], u[4 * j + 1], u[4 * j + 2], u[4 * j + 3]);
     } else {
-        float* blk = reinterpret_cast<float*>(gauge) + ((size_t)(par * 4 + mu) * G + (idx >> 5)) * (18 * 32);
+        float* blk = reinterpret_cast<float*>(gauge) + gauge_block(par, mu, G, idx >> 5) * (18 * 32);
         float4* p = reinterpret_cast<float4*>(blk) + (idx & 31);
 #pragma unroll
         for (int j = 0; j < 4; ++j) p[j * 32] = make_float4(u[4 * j], u[4 * j + 1], u[4 * j + 2], u[4 * j + 3]);

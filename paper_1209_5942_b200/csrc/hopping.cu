@@ -78,7 +78,7 @@ __device__ __forceinline__ void hop(T (&acc)[24], const HopArgs& a, int e, int e
     accumulate<MU, S>(acc, chi);
 }
 
-template <typename T, int RECON, int DAG, int MODE, bool SLAB>
+template <typename T, int RECON, int DAG, int MODE, bool SLAB, bool TILE = false>
 __global__ void __launch_bounds__(LQCD_HOP_MAX_THREADS, (RECON == 12) ? (sizeof(T) == 4 ? LQCD_HOP_MIN_BLOCKS_F12 : LQCD_HOP_MIN_BLOCKS_D12)
                                                                       : LQCD_HOP_MIN_BLOCKS)
 hopping_kernel(const HopArgs a) {
@@ -86,7 +86,13 @@ hopping_kernel(const HopArgs a) {
     const int Vh = a.g.Vh;
     const int blk = a.reverse ? (int)(gridDim.x - 1 - blockIdx.x) : (int)blockIdx.x;
     // single lattice: site e of all Vh; slab mode: site i of the launch's SiteRange
-    const int i = blk * blockDim.x + threadIdx.x;
+    int i = blk * blockDim.x + threadIdx.x;
+    if (TILE) {   // blk = tile (gy, z / 2, t / 2); warp w of the CTA: z = 2 (z / 2) + (w & 1), t = 2 (t / 2) + (w >> 1)
+        const int w = threadIdx.x >> 5;
+        const int q = blk / a.tile_gy, gy = blk - q * a.tile_gy;
+        const int tt = q / a.tile_n2h, zt = q - tt * a.tile_n2h;
+        i = 32 * (gy + a.tile_gy * ((2 * zt + (w & 1)) + a.g.N2 * (2 * tt + (w >> 1)))) + (threadIdx.x & 31);
+    }
     const bool live = SLAB ? (i < a.rg.count) : (i < Vh);
     const int e = SLAB ? a.rg.base + i + (i >= a.rg.n1 ? a.rg.skip : 0) : i;
     double nrm = 0.0;
@@ -259,8 +265,9 @@ cudaError_t launch_tr(int dagger, int mode, const HopArgs& a, int block, cudaStr
     const int grid = (a.rg.count + block - 1) / block;
 #define LQCD_HOP_CASE(D, M)                                                        \
     if (dagger == D && mode == M) {                                                \
-        if (a.g.slab) hopping_kernel<T, RECON, D, M, true><<<grid, block, 0, st>>>(a);  \
-        else          hopping_kernel<T, RECON, D, M, false><<<grid, block, 0, st>>>(a); \
+        if (a.g.slab)           hopping_kernel<T, RECON, D, M, true><<<grid, block, 0, st>>>(a);         \
+        else if (a.tile_gy > 0) hopping_kernel<T, RECON, D, M, false, true><<<grid, block, 0, st>>>(a);  \
+        else                    hopping_kernel<T, RECON, D, M, false><<<grid, block, 0, st>>>(a);        \
         return cudaGetLastError();                                                 \
     }
     LQCD_HOP_CASE(0, 0) LQCD_HOP_CASE(0, 1) LQCD_HOP_CASE(0, 2)
@@ -292,7 +299,7 @@ cudaError_t launch_hopping(int precision, int recon, int dagger, int mode, const
                            const void* aux, int out_parity, int reverse, Reduction red,
                            CgScalars* scal, int block, cudaStream_t st, const SiteRange* range,
                            const void* dotw, const void* dotw2) {
-    if (g_hop_variant != 0 && hopping_variant_covers(g_hop_variant, mode, g, range))
+    if (g_hop_variant >= 1 && g_hop_variant <= 5 && hopping_variant_covers(g_hop_variant, mode, g, range))
         return launch_hopping_variant(g_hop_variant, precision, recon, dagger, mode, g, ep, gauge, in, out, aux, out_parity,
                                       reverse, scal, block, st);
     HopArgs a;
@@ -303,7 +310,13 @@ cudaError_t launch_hopping(int precision, int recon, int dagger, int mode, const
     a.reverse = reverse;
     a.gauge = gauge; a.in = in; a.out = out; a.aux = aux;
     a.g = g; a.ep = ep; a.out_parity = out_parity; a.red = red; a.scal = scal;
+    a.tile_gy = a.tile_n2h = 0;
     if (block <= 0 || block > LQCD_HOP_MAX_THREADS || (block % 32) != 0) block = LQCD_HOP_MAX_THREADS;
+    // variant 6: the 2 x 2 (z, t) tile order, where a z plane is a whole number of groups (modes 0-3, single lattice)
+    if (g_hop_variant == 6 && !g.slab && range == nullptr && mode <= 3 && block == 128 && (g.N0h * g.N1) % 32 == 0) {
+        a.tile_gy = (g.N0h * g.N1) / 32;
+        a.tile_n2h = g.N2 / 2;
+    }
     count_launch();
     ProfScope prof(mode == 3 ? 5 : (mode >= 4 ? 1 : mode), st);
     if (precision == 0) {

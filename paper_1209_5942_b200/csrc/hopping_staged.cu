@@ -63,7 +63,7 @@ __device__ __forceinline__ float2 lds64f(unsigned addr) {
 template <typename T, int RECON>
 __device__ __forceinline__ void link_fetch(unsigned dst, const void* gauge, int G, int par, int mu, int idx) {
     typedef LinkBytes<T, RECON> LB;
-    const char* p = reinterpret_cast<const char*>(gauge) + ((size_t)(par * 4 + mu) * G + (idx >> 5)) * LB::group;
+    const char* p = reinterpret_cast<const char*>(gauge) + gauge_block(par, mu, G, idx >> 5) * LB::group;
 #pragma unroll
     for (int j = 0; j < LB::n16; ++j) cp_async16(dst + j * (LQCD_HOP_MAX_THREADS * 16), p + j * 512 + (idx & 31) * 16);
     if (LB::tail8) cp_async8(dst + LB::n16 * (LQCD_HOP_MAX_THREADS * 16), p + LB::n16 * 512 + (idx & 31) * 8);
@@ -297,7 +297,7 @@ __global__ void __launch_bounds__(LQCD_HOP_MAX_THREADS, NB) hopping_bulk_kernel(
 #pragma unroll
             for (int m = 0; m < NMU; ++m) {
                 const char* src = reinterpret_cast<const char*>(a.gauge) +
-                                  ((size_t)(a.out_parity * 4 + MU0 + m) * a.g.G + (e >> 5)) * LB::group;
+                                  gauge_block(a.out_parity, MU0 + m, a.g.G, e >> 5) * LB::group;
                 bulk_g2s(stage0 + m * LB::group, src, LB::group, bar);
             }
         }
@@ -420,6 +420,7 @@ cudaError_t launch_hopping_variant(int variant, int precision, int recon, int da
     a.reverse = reverse;
     a.gauge = gauge; a.in = in; a.out = out; a.aux = aux; a.dotw = nullptr; a.dotw2 = nullptr;
     a.g = g; a.ep = ep; a.out_parity = out_parity; a.red.partials = nullptr; a.scal = scal;
+    a.tile_gy = a.tile_n2h = 0;
     if (block <= 0 || block > LQCD_HOP_MAX_THREADS || (block % 32) != 0) block = LQCD_HOP_MAX_THREADS;
     count_launch();
     ProfScope prof(mode, st);

@@ -33,7 +33,7 @@ __global__ void __launch_bounds__(PBLOCK) pack_gauge_kernel(Geometry g, const do
     double2 u[9];
 #pragma unroll
     for (int j = 0; j < 9; ++j) u[j] = src[j];
-    const size_t grp = (size_t)pm * g.Gg + (e >> 5);
+    const size_t grp = gauge_block(parity, mu, g.Gg, e >> 5);
     const int lane = e & 31;
     if (sizeof(T) == 8) {
         double2* dst = (double2*)internal + grp * ((RECON / 2) * 32) + lane;
@@ -67,7 +67,7 @@ __global__ void __launch_bounds__(PBLOCK) unpack_gauge_kernel(Geometry g, const 
     const int pm = (int)(tid / Vh);
     const int parity = pm >> 2, mu = pm & 3;
     const size_t lex = 2 * (size_t)e + site_r(g, e, parity);
-    const size_t grp = (size_t)pm * g.Gg + (e >> 5);
+    const size_t grp = gauge_block(parity, mu, g.Gg, e >> 5);
     const int lane = e & 31;
     double2 u[9];
     if (sizeof(T) == 8) {

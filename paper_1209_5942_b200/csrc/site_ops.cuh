@@ -33,6 +33,9 @@ struct HopArgs {
     Reduction red;
     CgScalars* scal;
     SiteRange rg;
+    // variant 6 (TILE): a CTA of four warps takes the four groups {g, g + Gy, g + Gy N2, g + Gy (N2 + 1)} -- the
+    // groups of a 2 x 2 block in (z, t) -- instead of four consecutive groups; Gy = groups per z plane
+    int tile_gy, tile_n2h;   // Gy and N2 / 2 (0: linear order)
 };
 
 // ----------------------------------------------------------------------------- field access
@@ -110,7 +113,7 @@ template <int RECON>
 __device__ __forceinline__ void load_link(const void* gauge, int G, int par, int mu, int idx,
                                           double (&u)[18]) {
     const double2* p = reinterpret_cast<const double2*>(gauge) +
-                       ((size_t)(par * 4 + mu) * G + (idx >> 5)) * ((RECON / 2) * 32) + (idx & 31);
+                       gauge_block(par, mu, G, idx >> 5) * ((RECON / 2) * 32) + (idx & 31);
 #pragma unroll
     for (int j = 0; j < RECON / 2; ++j) {
         const double2 v = __ldcs(p + j * 32);
@@ -124,7 +127,7 @@ __device__ __forceinline__ void load_link(const void* gauge, int G, int par, int
                                           float (&u)[18]) {
     if (RECON == 12) {
         const float4* p = reinterpret_cast<const float4*>(gauge) +
-                          ((size_t)(par * 4 + mu) * G + (idx >> 5)) * (3 * 32) + (idx & 31);
+                          gauge_block(par, mu, G, idx >> 5) * (3 * 32) + (idx & 31);
 #pragma unroll
         for (int j = 0; j < 3; ++j) {
             const float4 v = __ldcs(p + j * 32);
@@ -136,7 +139,7 @@ __device__ __forceinline__ void load_link(const void* gauge, int G, int par, int
         reconstruct_row2(u);
     } else {
         const float* blk = reinterpret_cast<const float*>(gauge) +
-                           ((size_t)(par * 4 + mu) * G + (idx >> 5)) * (18 * 32);
+                           gauge_block(par, mu, G, idx >> 5) * (18 * 32);
         const float4* p = reinterpret_cast<const float4*>(blk) + (idx & 31);
 #pragma unroll
         for (int j = 0; j < 4; ++j) {

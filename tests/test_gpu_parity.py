@@ -900,7 +900,7 @@ def test_bicgstab_on_a_side_stream_graph_replay_matches_direct_launches(B, oracl
 
 
 # --------------------------------------------------------------------------- staged variants of the hopping kernel
-@pytest.mark.parametrize("variant", [1, 2, 3, 4, 5])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4, 5, 6])
 @pytest.mark.parametrize("precision,recon,tol", [(0, 18, TOL_D), (0, 12, TOL_D), (1, 18, TOL_S), (1, 12, TOL_S)])
 def test_hopping_variants_match_oracle(B, oracle_mod, variant, precision, recon, tol):
     """lqcd_set_hop_variant: every staged variant of the hopping kernel (hopping_staged.cu) against the oracle, in every
