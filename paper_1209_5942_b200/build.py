@@ -12,7 +12,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "liblqcd.so")
 SOURCES = ["api.cu", "hopping.cu", "hopping_staged.cu", "force.cu", "gauge_update.cu", "vector_ops.cu", "pack.cu", "stream_probe.cu"]
-HEADERS = [os.path.join(CSRC, "lqcd_internal.h"), os.path.join(CSRC, "site_ops.cuh"), os.path.join(HERE, "..", "include", "lqcd.h")]
+HEADERS = [os.path.join(CSRC, "lqcd_internal.h"), os.path.join(CSRC, "site_ops.cuh"), os.path.join(CSRC, "kp_log_table.h"), os.path.join(HERE, "..", "include", "lqcd.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-Xptxas=-v", "-Xcompiler", "-fPIC",

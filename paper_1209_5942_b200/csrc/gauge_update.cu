@@ -27,6 +27,10 @@
 // unrolled at 4 CTAs 310 / 149.  Re-measured: double at 4 CTAs (128 registers, 60-80 B of spills) 406 / 279.
 // Kennedy-Pendleton draws of the first two attempts precomputed ahead of the staple loads
 // (kp_precompute): heatbath 401 -> 395 (double), 310 -> 279 (single/18), 331 -> 308 (single/12).
+// Round 2: CTAs on a 2 x 2 block in (z, t) of one group instead of four consecutive groups (the staple links shared
+// between sites one step apart in z, t then meet in one CTA's L1): overrelaxation 264.4 / 153.0 / 245.7 / 152.3 us
+// (double/18, single/18, double/12, single/12) against 266.4 / 151.0 / 242.5 / 150.2 in linear order, heatbath 401.7
+// against 397.8 -- no gain, not kept (the same order of sites moved nothing in the hopping kernel either).
 #ifndef LQCD_GAUGE_MIN_BLOCKS_D
 #define LQCD_GAUGE_MIN_BLOCKS_D 3
 #endif
@@ -239,12 +243,35 @@ constexpr int kStapleUnroll = LQCD_GAUGE_UNROLL;
 constexpr int KP_PRE = 2;
 constexpr int KP_SLOTS = 2 * KP_PRE + 4;   // X_t, q_t for t < KP_PRE; sin(theta), cos(theta), sin(phi), cos(phi)
 
+// ln x for x in (0, 1], x a multiple of 2^-53 (a uniform01 draw): the exponent, a 128-entry table on the top seven
+// mantissa bits (kp_log_table.h: ln m = log_c + log1p(m inv_c - 1), |m inv_c - 1| <= 2^-8) and the series of log1p to
+// the seventh power, 12 FP64 instructions against ~35 of the library's log with its special cases; the result is within
+// 2.3e-16 max(|ln x|, 1) of the correctly rounded one (checked over 3e5 arguments against glibc when the table was
+// made), which is what the draws need: a flip of an accept/reject decision against the oracle takes a difference of the
+// size of |r4^2 - (1 - delta / 2)|.
+#include "kp_log_table.h"
+__device__ __forceinline__ double kp_log(double x) {
+    const long long b = __double_as_longlong(x);
+    const int e = (int)(b >> 52) - 1023;
+    const double m = __longlong_as_double((b & 0x000fffffffffffffLL) | 0x3ff0000000000000LL);
+    const double2 t = __ldg(&kp_log_tab[(int)(b >> 45) & 127]);
+    const double eps = fma(m, t.x, -1.0);
+    double p = fma(eps, 1.0 / 7.0, -1.0 / 6.0);
+    p = fma(p, eps, 0.2);
+    p = fma(p, eps, -0.25);
+    p = fma(p, eps, 1.0 / 3.0);
+    p = fma(p, eps, -0.5);
+    p = fma(p * eps, eps, eps);
+    const double de = (double)e;
+    return fma(de, KP_LN2_HI, t.y) + fma(de, KP_LN2_LO, p);
+}
+
 __device__ __forceinline__ void kp_attempt(unsigned long long seed, unsigned long long tag, unsigned long long c,
                                            double& X, double& q) {
     const double r1 = uniform01(seed, tag, c), r2 = uniform01(seed, tag, c + 1);
     const double r3 = uniform01(seed, tag, c + 2), r4 = uniform01(seed, tag, c + 3);
     const double cs = cospi(2.0 * r2);
-    X = -(log(r1) + cs * cs * log(r3));
+    X = -(kp_log(r1) + cs * cs * kp_log(r3));
     q = r4 * r4;
 }
 
@@ -274,17 +301,18 @@ __device__ __forceinline__ bool kp_sample(double lambda, unsigned long long seed
                                           unsigned long long base, const double* pre, int stride, double (&g)[4]) {
     bool ok = false;
     double delta = 0.0;
+    const double il = 1.0 / lambda;   // one division per subgroup; X * (1 / lambda) is within an ulp of X / lambda
 #pragma unroll
     for (int t = 0; t < KP_PRE; ++t) {
         if (!ok) {
-            delta = pre[(2 * t) * stride] / lambda;
+            delta = pre[(2 * t) * stride] * il;
             ok = pre[(2 * t + 1) * stride] <= 1.0 - 0.5 * delta;
         }
     }
     for (int t = KP_PRE; t < MAXTRY && !ok; ++t) {
         double X, q;
         kp_attempt(seed, tag, base + 4ull * t, X, q);
-        delta = X / lambda;
+        delta = X * il;
         ok = q <= 1.0 - 0.5 * delta;
     }
     if (!ok) return false;
@@ -331,7 +359,8 @@ __device__ __forceinline__ void subgroup_step(T (&L)[18], const T (&A)[18], doub
     double w3 = 0.5 * ((double)wi[0] - (double)wi[3]);
     const double k = sqrt(w0 * w0 + w1 * w1 + w2 * w2 + w3 * w3);
     if (!(k > 0.0)) return;
-    w0 /= k; w1 /= k; w2 /= k; w3 /= k;
+    const double ik = 1.0 / k;
+    w0 *= ik; w1 *= ik; w2 *= ik; w3 *= ik;
     double v0, v1, v2, v3;
     if (MODE == 0) {   // heatbath: v = g w^dag
         double g[4];
@@ -363,7 +392,7 @@ __device__ __forceinline__ void subgroup_step(T (&L)[18], const T (&A)[18], doub
 template <typename T, int RECON, int MODE>
 __global__ void __launch_bounds__(128, sizeof(T) == 8 ? LQCD_GAUGE_MIN_BLOCKS_D : LQCD_GAUGE_MIN_BLOCKS_F)
 gauge_update_kernel(const GaugeArgs a) {
-    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    const int e = blockIdx.x * 128 + (threadIdx.x & 127);
     if (e >= a.g.Vh) return;
     const int G = a.g.G, mu = a.mu, p = a.parity;
     const SiteIdx x = site_of(a.g, e, p);
@@ -424,7 +453,7 @@ template <typename T, int RECON>
 __global__ void __launch_bounds__(256, 3) heatbath_ws_kernel(const GaugeArgs a) {
     __shared__ double pre_s[3 * KP_SLOTS * 128];
     const int wg = threadIdx.x >> 7, tl = threadIdx.x & 127;
-    const int e = blockIdx.x * 128 + tl;
+    const int e = blockIdx.x * 128 + (threadIdx.x & 127);
     const int G = a.g.G, mu = a.mu, p = a.parity;
     const bool live = e < a.g.Vh;
     if (wg == 1) {
