@@ -139,6 +139,9 @@ int lqcd_cg_finish(void);
  * iteration = two applications of Mhat; stops when |r| <= tol |b| (recursive residual) or after
  * maxit iterations.  Returns LQCD_OK, LQCD_NOT_CONVERGED or LQCD_BREAKDOWN (<rhat,v>, <rhat,r> or
  * omega zero or not finite); lqcd_cg_stats() gives iterations and the residuals of Mhat x = b.
+ * <rhat,v>, <t,s>, |t|^2 and <rhat,t> are reduced inside the hopping launches that produce v and t, and
+ * <rhat,r'> is taken as (rho - alpha <rhat,v>) - omega <rhat,t> (the same number to rounding), so that x, r
+ * and p are updated in one pass; the four-iteration chunk goes through the graph cache described above.
  * b, x in internal layout; b is read throughout the solve.  Synchronous. */
 int lqcd_bicgstab_mhat(const void* gauge, const void* b, void* x, double kappa, double mu, double tol,
                        int maxit);

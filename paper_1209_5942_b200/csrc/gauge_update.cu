@@ -49,6 +49,7 @@ struct GaugeArgs {
     Geometry g;
     int mu, parity;
     double beta;
+    double c_il;            // 3 / (2 beta): 1 / lambda = c_il / k (heatbath)
     unsigned long long seed, tag;
     Reduction red;          // plaquette only
 };
@@ -146,7 +147,7 @@ __device__ __forceinline__ void orthonormalise_rows01(T (&u)[18]) {
     T n0 = 0;
 #pragma unroll
     for (int i = 0; i < 6; ++i) n0 = fma_(u[i], u[i], n0);
-    const T i0 = (T)1 / sqrt(n0);
+    const T i0 = rsqrt(n0);
 #pragma unroll
     for (int i = 0; i < 6; ++i) u[i] *= i0;
     T dr = 0, di = 0;   // <row0, row1> = sum conj(row0_c) row1_c
@@ -164,7 +165,7 @@ __device__ __forceinline__ void orthonormalise_rows01(T (&u)[18]) {
         u[6 + 2 * c + 1] = im;
         n1 = fma_(re, re, fma_(im, im, n1));
     }
-    const T i1 = (T)1 / sqrt(n1);
+    const T i1 = rsqrt(n1);
 #pragma unroll
     for (int i = 6; i < 12; ++i) u[i] *= i1;
 }
@@ -297,11 +298,12 @@ __device__ __forceinline__ void kp_precompute(unsigned long long seed, unsigned 
     pre[(2 * KP_PRE + 3) * stride] = cp;
 }
 
-__device__ __forceinline__ bool kp_sample(double lambda, unsigned long long seed, unsigned long long tag,
+// il = 1 / lambda = (3 / (2 beta)) (1 / k), handed in as a product of the two reciprocals the caller already has: X * il is
+// within two ulp of the X / lambda of the definition, and the subgroup step has no division left.
+__device__ __forceinline__ bool kp_sample(double il, unsigned long long seed, unsigned long long tag,
                                           unsigned long long base, const double* pre, int stride, double (&g)[4]) {
     bool ok = false;
     double delta = 0.0;
-    const double il = 1.0 / lambda;   // one division per subgroup; X * (1 / lambda) is within an ulp of X / lambda
 #pragma unroll
     for (int t = 0; t < KP_PRE; ++t) {
         if (!ok) {
@@ -332,7 +334,7 @@ __device__ __forceinline__ bool kp_sample(double lambda, unsigned long long seed
 //   = [[a0 + i a3, a2 + i a1], [-a2 + i a1, a0 - i a3]]   (reading G19);
 // (a0, a)(b0, b) = (a0 b0 - a.b, a0 b + b0 a - a x b).
 template <int MODE, int I, int P, int Q, typename T>
-__device__ __forceinline__ void subgroup_step(T (&L)[18], const T (&A)[18], double beta, unsigned long long seed,
+__device__ __forceinline__ void subgroup_step(T (&L)[18], const T (&A)[18], double c_il, unsigned long long seed,
                                               unsigned long long tag, unsigned long long link_id, const double* pre,
                                               int stride) {
     // the four entries (P,P), (P,Q), (Q,P), (Q,Q) of W = L A
@@ -357,15 +359,15 @@ __device__ __forceinline__ void subgroup_step(T (&L)[18], const T (&A)[18], doub
     double w1 = 0.5 * ((double)wi[1] + (double)wi[2]);
     double w2 = 0.5 * ((double)wr[1] - (double)wr[2]);
     double w3 = 0.5 * ((double)wi[0] - (double)wi[3]);
-    const double k = sqrt(w0 * w0 + w1 * w1 + w2 * w2 + w3 * w3);
-    if (!(k > 0.0)) return;
-    const double ik = 1.0 / k;
+    const double k2 = w0 * w0 + w1 * w1 + w2 * w2 + w3 * w3;
+    if (!(k2 > 0.0)) return;
+    const double ik = rsqrt(k2);       // 1 / k from one reciprocal square root (no sqrt, no division)
     w0 *= ik; w1 *= ik; w2 *= ik; w3 *= ik;
     double v0, v1, v2, v3;
     if (MODE == 0) {   // heatbath: v = g w^dag
         double g[4];
         const unsigned long long base = ((link_id * 3ull + (unsigned long long)I) * (unsigned long long)(MAXTRY + 1)) * 4ull;
-        if (!kp_sample(2.0 * beta * k / 3.0, seed, tag, base, pre + (size_t)I * KP_SLOTS * stride, stride, g)) return;
+        if (!kp_sample(c_il * ik, seed, tag, base, pre + (size_t)I * KP_SLOTS * stride, stride, g)) return;
         v0 = g[0] * w0 + (g[1] * w1 + g[2] * w2 + g[3] * w3);
         v1 = w0 * g[1] - g[0] * w1 + (g[2] * w3 - g[3] * w2);
         v2 = w0 * g[2] - g[0] * w2 + (g[3] * w1 - g[1] * w3);
@@ -429,9 +431,9 @@ gauge_update_kernel(const GaugeArgs a) {
     }
     T L[18];
     gload<RECON, true>(a.gauge, G, p, mu, e, L);
-    subgroup_step<MODE, 0, 0, 1>(L, A, a.beta, a.seed, a.tag, link_id, pre, 128);
-    subgroup_step<MODE, 1, 1, 2>(L, A, a.beta, a.seed, a.tag, link_id, pre, 128);
-    subgroup_step<MODE, 2, 0, 2>(L, A, a.beta, a.seed, a.tag, link_id, pre, 128);
+    subgroup_step<MODE, 0, 0, 1>(L, A, a.c_il, a.seed, a.tag, link_id, pre, 128);
+    subgroup_step<MODE, 1, 1, 2>(L, A, a.c_il, a.seed, a.tag, link_id, pre, 128);
+    subgroup_step<MODE, 2, 0, 2>(L, A, a.c_il, a.seed, a.tag, link_id, pre, 128);
     if (RECON == 12) orthonormalise_rows01(L);
     gstore<RECON>(a.gauge, G, p, mu, e, L);
 }
@@ -502,9 +504,9 @@ __global__ void __launch_bounds__(256, 3) heatbath_ws_kernel(const GaugeArgs a) 
     asm volatile("bar.sync 1, 256;\n" ::: "memory");
     if (live) {
         const double* pre = pre_s + tl;
-        subgroup_step<0, 0, 0, 1>(L, A, a.beta, a.seed, a.tag, link_id, pre, 128);
-        subgroup_step<0, 1, 1, 2>(L, A, a.beta, a.seed, a.tag, link_id, pre, 128);
-        subgroup_step<0, 2, 0, 2>(L, A, a.beta, a.seed, a.tag, link_id, pre, 128);
+        subgroup_step<0, 0, 0, 1>(L, A, a.c_il, a.seed, a.tag, link_id, pre, 128);
+        subgroup_step<0, 1, 1, 2>(L, A, a.c_il, a.seed, a.tag, link_id, pre, 128);
+        subgroup_step<0, 2, 0, 2>(L, A, a.c_il, a.seed, a.tag, link_id, pre, 128);
         if (RECON == 12) orthonormalise_rows01(L);
         gstore<RECON>(a.gauge, G, p, mu, e, L);
     }
@@ -552,7 +554,7 @@ cudaError_t launch_gauge_update(int precision, int recon, int mode, const Geomet
                                 int parity, double beta, unsigned long long seed, unsigned long long tag,
                                 cudaStream_t st) {
     GaugeArgs a;
-    a.gauge = gauge; a.g = g; a.mu = mu; a.parity = parity; a.beta = beta; a.seed = seed; a.tag = tag;
+    a.gauge = gauge; a.g = g; a.mu = mu; a.parity = parity; a.beta = beta; a.c_il = (beta != 0.0) ? 1.5 / beta : 0.0; a.seed = seed; a.tag = tag;
     a.red.partials = nullptr;
     const int grid = (g.Vh + 127) / 128;
     count_launch();
@@ -576,7 +578,7 @@ int plaquette_partials(int Vh) { return 2 * ((Vh + 127) / 128) * 4; }
 cudaError_t launch_plaquette(int precision, int recon, const Geometry& g, const void* gauge, Reduction red,
                              cudaStream_t st) {
     GaugeArgs a;
-    a.gauge = const_cast<void*>(gauge); a.g = g; a.mu = 0; a.parity = 0; a.beta = 0; a.seed = 0; a.tag = 0;
+    a.gauge = const_cast<void*>(gauge); a.g = g; a.mu = 0; a.parity = 0; a.beta = 0; a.c_il = 0; a.seed = 0; a.tag = 0;
     a.red = red;
     const dim3 grid((g.Vh + 127) / 128, 2);
     count_launch();
