@@ -185,7 +185,10 @@ int lqcd_force_tm(const void* gauge, const void* phi, void* force, double kappa,
  * lqcd_gauge_sweep : the 8 sub-sweeps mu = 0..3, parity 0 then 1.  Asynchronous.
  * lqcd_plaquette   : average of Re tr P / 3 over the 6 V plaquettes, written to a HOST double; synchronous.
  * lqcd_unpack_gauge: internal -> canonical U[lex(x)][mu][a][b] (complex double; 12-real storage
- *   rebuilds the third row).  Asynchronous. */
+ *   rebuilds the third row).  Asynchronous.
+ * LQCD_HEATBATH_WS=1 in the environment (read once) runs the heatbath with a warp-specialised kernel -- a second
+ * warpgroup per CTA computes the field-independent part of the Kennedy-Pendleton draws -- with the same results;
+ * it is slower than the default (profiles/r02_heatbath.md) and kept as the record of that experiment. */
 #define LQCD_HEATBATH  0
 #define LQCD_OVERRELAX 1
 int lqcd_gauge_update(void* gauge, int mu, int parity, int mode, double beta, unsigned long long seed,

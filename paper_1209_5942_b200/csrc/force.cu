@@ -24,9 +24,7 @@
 // once in shared memory instead of read through L1 by each direction-warp: 480 us (no change: the
 // L2 -> L1 traffic it removes is not the limiter).  One thread per site looping over the four directions
 // with the staged X(x), Y(x) (64-thread CTAs, 168 registers): 513 us; at 128 registers 707 us.
-#ifndef LQCD_FORCE_MIN_BLOCKS
-#define LQCD_FORCE_MIN_BLOCKS 4
-#endif
+constexpr int kForceMinBlocks = 4;
 
 namespace lqcd {
 namespace {
@@ -128,7 +126,7 @@ __device__ __forceinline__ void force_link(const ForceArgs& a, int p, int e, int
 // sweeping one parity after the other put a whole field (805 MB of X, Y) between the two reads
 // and cost a second DRAM pass (ncu: 3.35 GB of traffic against 2.55 GB algorithmic).
 template <typename T, int RECON>
-__global__ void __launch_bounds__(128, LQCD_FORCE_MIN_BLOCKS) force_kernel(const ForceArgs a) {
+__global__ void __launch_bounds__(128, kForceMinBlocks) force_kernel(const ForceArgs a) {
     const int G = a.g.G;
     const int p = (int)blockIdx.x & 1;
     const int e = ((int)blockIdx.x >> 1) * 32 + (threadIdx.x & 31);

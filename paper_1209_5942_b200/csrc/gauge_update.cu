@@ -31,15 +31,9 @@
 // between sites one step apart in z, t then meet in one CTA's L1): overrelaxation 264.4 / 153.0 / 245.7 / 152.3 us
 // (double/18, single/18, double/12, single/12) against 266.4 / 151.0 / 242.5 / 150.2 in linear order, heatbath 401.7
 // against 397.8 -- no gain, not kept (the same order of sites moved nothing in the hopping kernel either).
-#ifndef LQCD_GAUGE_MIN_BLOCKS_D
-#define LQCD_GAUGE_MIN_BLOCKS_D 3
-#endif
-#ifndef LQCD_GAUGE_UNROLL
-#define LQCD_GAUGE_UNROLL 3
-#endif
-#ifndef LQCD_GAUGE_MIN_BLOCKS_F
-#define LQCD_GAUGE_MIN_BLOCKS_F 4
-#endif
+constexpr int kGaugeMinBlocksDouble = 3;   // CTAs of 128 threads per SM the register allocation aims at
+constexpr int kGaugeMinBlocksFloat = 4;
+constexpr int kGaugeStapleUnroll = 3;      // the loop over the three nu != mu, fully unrolled
 
 namespace lqcd {
 namespace {
@@ -228,7 +222,7 @@ __device__ __forceinline__ double uniform01(unsigned long long seed, unsigned lo
 }
 
 constexpr int MAXTRY = 32;   // reading G20
-constexpr int kStapleUnroll = LQCD_GAUGE_UNROLL;
+constexpr int kStapleUnroll = kGaugeStapleUnroll;
 
 // Kennedy-Pendleton: g0 with density sqrt(1 - g0^2) exp(lambda g0), direction uniform.
 // Counters: attempt t uses base + 4 t + (0..3), the direction base + 4 MAXTRY + (0, 1).
@@ -392,7 +386,7 @@ __device__ __forceinline__ void subgroup_step(T (&L)[18], const T (&A)[18], doub
 }
 
 template <typename T, int RECON, int MODE>
-__global__ void __launch_bounds__(128, sizeof(T) == 8 ? LQCD_GAUGE_MIN_BLOCKS_D : LQCD_GAUGE_MIN_BLOCKS_F)
+__global__ void __launch_bounds__(128, sizeof(T) == 8 ? kGaugeMinBlocksDouble : kGaugeMinBlocksFloat)
 gauge_update_kernel(const GaugeArgs a) {
     const int e = blockIdx.x * 128 + (threadIdx.x & 127);
     if (e >= a.g.Vh) return;

@@ -43,15 +43,9 @@
 // enough to carry a second set of instantiations.  Only double/12 moves to 4 CTAs.
 // single/12 re-measured at 5 / 6 / 7 / 8 CTAs (96 / 80 / 72 / 64 registers): 102.9 / 102.3 / 102.4 / 108.1 us per launch,
 // CG iteration 574 / 562 / 561 / 602 us: flat between 6 and 7, 7 stays.
-#ifndef LQCD_HOP_MIN_BLOCKS
-#define LQCD_HOP_MIN_BLOCKS 3
-#endif
-#ifndef LQCD_HOP_MIN_BLOCKS_D12
-#define LQCD_HOP_MIN_BLOCKS_D12 4
-#endif
-#ifndef LQCD_HOP_MIN_BLOCKS_F12
-#define LQCD_HOP_MIN_BLOCKS_F12 7
-#endif
+constexpr int kHopMinBlocks = 3;       // double/18, single/18
+constexpr int kHopMinBlocksD12 = 4;    // double/12
+constexpr int kHopMinBlocksF12 = 7;    // single/12
 
 namespace lqcd {
 namespace {
@@ -79,8 +73,8 @@ __device__ __forceinline__ void hop(T (&acc)[24], const HopArgs& a, int e, int e
 }
 
 template <typename T, int RECON, int DAG, int MODE, bool SLAB, bool TILE = false>
-__global__ void __launch_bounds__(LQCD_HOP_MAX_THREADS, (RECON == 12) ? (sizeof(T) == 4 ? LQCD_HOP_MIN_BLOCKS_F12 : LQCD_HOP_MIN_BLOCKS_D12)
-                                                                      : LQCD_HOP_MIN_BLOCKS)
+__global__ void __launch_bounds__(LQCD_HOP_MAX_THREADS, (RECON == 12) ? (sizeof(T) == 4 ? kHopMinBlocksF12 : kHopMinBlocksD12)
+                                                                      : kHopMinBlocks)
 hopping_kernel(const HopArgs a) {
     if (a.scal != nullptr && a.scal->done) return;
     const int Vh = a.g.Vh;
