@@ -928,3 +928,32 @@ def test_hopping_variants_match_oracle(B, oracle_mod, variant, precision, recon,
     with pytest.raises(B.LqcdError) as e:
         B.lqcd_set_hop_variant(99)
     assert e.value.status == B.LQCD_BAD_ARG
+
+
+@pytest.mark.parametrize("precision,recon,tol", [(0, 18, TOL_D), (1, 12, TOL_S)])
+def test_hopping_variants_at_the_bench_size(B, oracle_mod, precision, recon, tol):
+    """The staged variants at 32^3 x 64, in the launch configuration sweep.py --hop-variant times (the tile order is only
+    active where a z plane holds whole groups: 16 groups per plane here): D_eo and Mhat^dag bit-identical to the default
+    kernel on the whole field, and against the oracle on 300 sampled sites; a CG solve with the tile order through the
+    fused launches (modes 2, 3) bit-identical to the default."""
+    dims = (32, 32, 32, 64)
+    kappa, mu = 0.15, 0.1
+    U, x, b = _cached_fields(dims)
+    h = lu.volume(dims) // 2
+    sites = _sample_sites(h, 300, 77 + recon)
+    Ur, xr = _round_inputs(U, x, precision)
+    try:
+        B.lqcd_set_hop_variant(0)
+        L = Lat(B, dims, AP, U, precision, recon)
+        ref_d, ref_m = L.dslash(x, 0, kappa), L.mtm(x, kappa, mu, 1)
+        assert lu.rel_err(ref_d[sites], oracle_mod.dslash_eo_sites(dims, AP, Ur, xr, sites, 0, kappa)) <= tol
+        assert lu.rel_err(ref_m[sites], oracle_mod.mhat_sites(dims, AP, Ur, xr, sites, kappa, mu, 1)) <= tol
+        st0, x0, stats0 = L.cg(b, kappa, mu, 0.0, 6)
+        for variant in (2, 4, 5, 6):
+            B.lqcd_set_hop_variant(variant)
+            assert np.array_equal(L.dslash(x, 0, kappa), ref_d), variant
+            assert np.array_equal(L.mtm(x, kappa, mu, 1), ref_m), variant
+        st6, x6, stats6 = L.cg(b, kappa, mu, 0.0, 6)      # variant 6 still selected
+        assert (st6, stats6) == (st0, stats0) and np.array_equal(x6, x0)
+    finally:
+        B.lqcd_set_hop_variant(0)
