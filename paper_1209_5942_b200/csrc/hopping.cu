@@ -76,6 +76,7 @@ template <typename T, int RECON, int DAG, int MODE, bool SLAB, bool TILE = false
 __global__ void __launch_bounds__(LQCD_HOP_MAX_THREADS, (RECON == 12) ? (sizeof(T) == 4 ? kHopMinBlocksF12 : kHopMinBlocksD12)
                                                                       : kHopMinBlocks)
 hopping_kernel(const HopArgs a) {
+    chain_prologue();
     if (a.scal != nullptr && a.scal->done) return;
     const int Vh = a.g.Vh;
     const int blk = a.reverse ? (int)(gridDim.x - 1 - blockIdx.x) : (int)blockIdx.x;
@@ -259,18 +260,17 @@ cudaError_t launch_tr(int dagger, int mode, const HopArgs& a, int block, cudaStr
     const int grid = (a.rg.count + block - 1) / block;
 #define LQCD_HOP_CASE(D, M)                                                        \
     if (dagger == D && mode == M) {                                                \
-        if (a.g.slab)           hopping_kernel<T, RECON, D, M, true><<<grid, block, 0, st>>>(a);         \
-        else if (a.tile_gy > 0) hopping_kernel<T, RECON, D, M, false, true><<<grid, block, 0, st>>>(a);  \
-        else                    hopping_kernel<T, RECON, D, M, false><<<grid, block, 0, st>>>(a);        \
-        return cudaGetLastError();                                                 \
+        const bool ch = chained_launches(st);                                        \
+        if (a.g.slab)           return launch_chained(ch, hopping_kernel<T, RECON, D, M, true>, grid, block, 0, st, a);         \
+        else if (a.tile_gy > 0) return launch_chained(ch, hopping_kernel<T, RECON, D, M, false, true>, grid, block, 0, st, a);  \
+        else                    return launch_chained(ch, hopping_kernel<T, RECON, D, M, false>, grid, block, 0, st, a);        \
     }
     LQCD_HOP_CASE(0, 0) LQCD_HOP_CASE(0, 1) LQCD_HOP_CASE(0, 2)
     LQCD_HOP_CASE(1, 0) LQCD_HOP_CASE(1, 1) LQCD_HOP_CASE(1, 2) LQCD_HOP_CASE(1, 3)
 #undef LQCD_HOP_CASE
     if (dagger == 0 && (mode == 4 || mode == 5) && !a.g.slab) {   // BiCGStab's fused inner products (single lattice only)
-        if (mode == 4) hopping_kernel<T, RECON, 0, 4, false><<<grid, block, 0, st>>>(a);
-        else           hopping_kernel<T, RECON, 0, 5, false><<<grid, block, 0, st>>>(a);
-        return cudaGetLastError();
+        if (mode == 4) return launch_chained(chained_launches(st), hopping_kernel<T, RECON, 0, 4, false>, grid, block, 0, st, a);
+        return launch_chained(chained_launches(st), hopping_kernel<T, RECON, 0, 5, false>, grid, block, 0, st, a);
     }
     return cudaErrorInvalidValue;
 }

@@ -260,6 +260,33 @@ struct ProfScope {
     ~ProfScope() { prof_end(st); }
 };
 
+// Programmatic dependent launch (sm_90+) for the kernels of the CG iteration: launched with launch_chained, a kernel may
+// be scheduled while the grid before it in the stream drains -- its CTAs take the SM slots the last wave of that grid
+// frees, run up to chain_prologue() and wait there until the whole of that grid has completed and its writes are
+// visible.  What it hides is the launch and ramp-up between two dependent kernels (7 boundaries per CG iteration), which
+// is most of a CG iteration's fixed cost on small lattices.  chain_prologue() is the first
+// statement of every kernel that is ever launched this way: launch_dependents lets the NEXT chained kernel be scheduled
+// once every CTA of this grid has started; wait returns at once when the kernel was launched the ordinary way.
+#ifdef __CUDACC__
+__device__ __forceinline__ void chain_prologue() {
+    asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
+    asm volatile("griddepcontrol.wait;\n" ::: "memory");
+}
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_chained(bool chained, void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                                  Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = chained ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+#endif
+bool chained_launches(cudaStream_t st);    // api.cu: direct launches only; LQCD_PDL=0 in the environment turns them off
+
 // Global sums are two-stage and fixed-order (deterministic for a given launch configuration):
 // the producing kernel writes one partial per warp (hopping) or per block (vector kernels)
 // with plain stores -- no fence, no atomic, no last-block election, which cost the hopping

@@ -66,6 +66,7 @@ __device__ __forceinline__ void block_partial(double v, Reduction red) {
 //   sum_io != null, apply = 1: no summation, the (all-reduced) value of *sum_io is applied.
 __global__ void __launch_bounds__(1024) finalize_kernel(int fin, Reduction red, int n, double tol,
                                                         CgScalars* scal, double* sum_io, int apply) {
+    chain_prologue();
     __shared__ double sm[32];
     if (fin != FIN_BB && fin != FIN_TRUE && scal->done) {
         if (fin == FIN_RHO && threadIdx.x == 0 && (sum_io == nullptr || apply)) scal->upd = 0;  // nothing for cg_update_xp to apply
@@ -127,6 +128,7 @@ __global__ void __launch_bounds__(1024) finalize_kernel(int fin, Reduction red, 
 template <typename T>
 __global__ void __launch_bounds__(VBLOCK) cg_init_kernel(size_t nvec, const void* b_, void* x_, void* r_,
                                                          void* p_, Reduction red) {
+    chain_prologue();
     typedef typename VecOf<T>::type V;
     const V* b = (const V*)b_;
     V *x = (V*)x_, *r = (V*)r_, *p = (V*)p_;
@@ -153,6 +155,7 @@ __global__ void __launch_bounds__(VBLOCK) cg_update_xp_kernel(size_t nvec, void*
                                                               const void* r_, int reverse,
                                                               CgScalars* scal) {
     typedef typename VecOf<T>::type V;
+    chain_prologue();
     if (!scal->upd) return;            // no r-update happened in this iteration
     const bool more = !scal->done;     // converged in this iteration: x gets its last update, p is dead
     const double alpha = scal->alpha, beta = scal->beta;
@@ -179,6 +182,7 @@ __global__ void __launch_bounds__(VBLOCK) cg_update_xp_kernel(size_t nvec, void*
 template <typename T>
 __global__ void __launch_bounds__(VBLOCK) true_resid_kernel(size_t nvec, const void* b_, const void* ax_,
                                                             Reduction red) {
+    chain_prologue();
     typedef typename VecOf<T>::type V;
     const V *b = (const V*)b_, *ax = (const V*)ax_;
     const size_t base = (size_t)blockIdx.x * (VBLOCK * VUNROLL) + threadIdx.x;
@@ -318,6 +322,7 @@ __device__ __forceinline__ void block_partials(double (&v)[K], Reduction red) {
 
 __global__ void __launch_bounds__(1024) bicg_finalize_kernel(int fin, Reduction red, int n, double tol,
                                                              BiScalars* bs) {
+    chain_prologue();
     __shared__ double sm[5][32];
     if (fin != FIN_BI_INIT && bs->cg.done) return;
     double s[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
@@ -421,6 +426,7 @@ __global__ void __launch_bounds__(VBLOCK) bicg_sigma_kernel(size_t nvec, const v
 template <typename T>
 __global__ void __launch_bounds__(VBLOCK) bicg_s_kernel(size_t nvec, const void* r_, const void* v_, void* s_,
                                                         int reverse, const BiScalars* bs) {
+    chain_prologue();
     typedef typename VecOf<T>::type V;
     if (bs->cg.done) return;
     const cd ma = {-bs->alpha_re, -bs->alpha_im};
@@ -486,6 +492,7 @@ template <typename T>
 __global__ void __launch_bounds__(VBLOCK) bicg_xrp_kernel(size_t nvec, void* x_, void* p_, const void* s_, const void* t_,
                                                           const void* v_, void* r_, int reverse, Reduction red,
                                                           const BiScalars* bs) {
+    chain_prologue();
     typedef typename VecOf<T>::type V;
     if (bs->cg.done) return;
     const cd alpha = {bs->alpha_re, bs->alpha_im}, omega = {bs->omega_re, bs->omega_im}, beta = {bs->beta_re, bs->beta_im};
@@ -535,8 +542,7 @@ cudaError_t launch_finalize(int fin, Reduction red, int n_partials, double tol, 
                             cudaStream_t st, double* sum_io, int apply) {
     count_launch();
     ProfScope prof(3, st);
-    finalize_kernel<<<1, 1024, 0, st>>>(fin, red, n_partials, tol, scal, sum_io, apply);
-    return cudaGetLastError();
+    return launch_chained(chained_launches(st), finalize_kernel, 1, 1024, 0, st, fin, red, n_partials, tol, scal, sum_io, apply);
 }
 
 cudaError_t launch_diag_scale(int precision, size_t n, const void* in, void* out, double ur, double ui,
@@ -605,10 +611,10 @@ cudaError_t launch_cg_update_xp(int precision, size_t n, void* x, void* p, const
     ProfScope prof(3, st);
     if (precision == 0) {
         const size_t nv = n / 2;
-        cg_update_xp_kernel<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, x, p, r, reverse, scal);
+        return launch_chained(chained_launches(st), cg_update_xp_kernel<double>, grid_for(nv), VBLOCK, 0, st, nv, x, p, r, reverse, scal);
     } else {
         const size_t nv = n / 4;
-        cg_update_xp_kernel<float><<<grid_for(nv), VBLOCK, 0, st>>>(nv, x, p, r, reverse, scal);
+        return launch_chained(chained_launches(st), cg_update_xp_kernel<float>, grid_for(nv), VBLOCK, 0, st, nv, x, p, r, reverse, scal);
     }
     return cudaGetLastError();
 }
@@ -635,6 +641,13 @@ cudaError_t launch_true_resid(int precision, size_t n, const void* b, const void
         if (precision == 0) { const size_t nv = n / 2; KERNEL<double><<<grid_for(nv), VBLOCK, 0, st>>>(nv, __VA_ARGS__); } \
         else                { const size_t nv = n / 4; KERNEL<float><<<grid_for(nv), VBLOCK, 0, st>>>(nv, __VA_ARGS__); }  \
     } while (0)
+// the same for the kernels of the production iteration, which begin with chain_prologue() (lqcd_internal.h)
+#define LQCD_BICG_DISPATCH_CHAINED(KERNEL, ...)                                                \
+    do {                                                                                       \
+        const bool ch_ = chained_launches(st);                                                 \
+        if (precision == 0) { const size_t nv = n / 2; (void)launch_chained(ch_, KERNEL<double>, grid_for(nv), VBLOCK, 0, st, nv, __VA_ARGS__); } \
+        else                { const size_t nv = n / 4; (void)launch_chained(ch_, KERNEL<float>, grid_for(nv), VBLOCK, 0, st, nv, __VA_ARGS__); }  \
+    } while (0)
 
 static int bicg_grid(int precision, size_t n) { return grid_for(precision == 0 ? n / 2 : n / 4); }
 
@@ -660,7 +673,7 @@ cudaError_t launch_bicg_s(int precision, size_t n, const void* r, const void* v,
                           BiScalars* bs, cudaStream_t st) {
     count_launch();
     ProfScope prof(3, st);
-    LQCD_BICG_DISPATCH(bicg_s_kernel, r, v, s, reverse, bs);
+    LQCD_BICG_DISPATCH_CHAINED(bicg_s_kernel, r, v, s, reverse, bs);
     return cudaGetLastError();
 }
 
@@ -687,15 +700,15 @@ cudaError_t launch_bicg_xrp(int precision, size_t n, void* x, void* p, const voi
                             void* r, int reverse, Reduction red, BiScalars* bs, cudaStream_t st) {
     count_launch(2);
     ProfScope prof(3, st);
-    LQCD_BICG_DISPATCH(bicg_xrp_kernel, x, p, s, t, v, r, reverse, red, bs);
-    bicg_finalize_kernel<<<1, 1024, 0, st>>>(FIN_BI_R2, red, bicg_grid(precision, n), 0.0, bs);
+    LQCD_BICG_DISPATCH_CHAINED(bicg_xrp_kernel, x, p, s, t, v, r, reverse, red, bs);
+    (void)launch_chained(chained_launches(st), bicg_finalize_kernel, 1, 1024, 0, st, (int)FIN_BI_R2, red, bicg_grid(precision, n), 0.0, bs);
     return cudaGetLastError();
 }
 
 cudaError_t launch_bicg_finalize(int fin, Reduction red, int n_partials, BiScalars* bs, cudaStream_t st) {
     count_launch();
     ProfScope prof(3, st);
-    bicg_finalize_kernel<<<1, 1024, 0, st>>>(fin, red, n_partials, 0.0, bs);
+    (void)launch_chained(chained_launches(st), bicg_finalize_kernel, 1, 1024, 0, st, fin, red, n_partials, 0.0, bs);
     return cudaGetLastError();
 }
 
