@@ -130,7 +130,7 @@ int lqcd_cg_mdagm(const void* gauge, const void* b, void* x, double kappa, doubl
  * iterations at a time as a CUDA graph captured on first use and kept while gauge, x, format, block
  * size, kappa and mu stay the same (bit-identical to direct launches, ~13 us less device time per
  * iteration between the kernels); LQCD_CG_GRAPH=0 in the environment turns it off.  Launches that go straight into
- * a stream (the legacy default stream, a solve while lqcd_profile records, the host-buffer calls) chain the
+ * a stream (the legacy default stream, the host-buffer calls; not while lqcd_profile records) chain the
  * hopping, finalisation and x/p kernels by programmatic dependent launch instead (sm_90+: a kernel is scheduled
  * while the grid before it drains and waits for it at its first instruction): 31 against 44 us per CG iteration at
  * 8^3 x 16, 100 against 113 at 16^3 x 32, 1298 against 1307 at 32^3 x 64, results bit-identical; LQCD_PDL=0 turns it

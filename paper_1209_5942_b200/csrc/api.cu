@@ -28,9 +28,12 @@ void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 // Programmatic dependent launches (lqcd_internal.h) for launches that go straight into the stream.  Not while the
 // stream is being captured, by the library's own CG graph or by the caller: inside a graph the kernels already follow
 // each other at ~2 us, and programmatic edges there measured neutral (24^3 x 48 and up) to 8-13% slower (16^4).
+static bool g_prof_on = false;
+// ... and not while lqcd_profile records an event pair around every launch: a chained kernel starts inside the pair of
+// the kernel before it and the per-launch durations stop meaning what bench.py's roofline figure takes them for.
 bool chained_launches(cudaStream_t st) {
     static const bool on = !(getenv("LQCD_PDL") && atoi(getenv("LQCD_PDL")) == 0);
-    if (!on) return false;
+    if (!on || g_prof_on) return false;
     cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
     if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) { cudaGetLastError(); return false; }
     return cs == cudaStreamCaptureStatusNone;
@@ -38,7 +41,6 @@ bool chained_launches(cudaStream_t st) {
 
 // ---- per-launch event timing (off by default; bench.py turns it on for the roofline figure)
 struct ProfRec { int cat; cudaEvent_t a, b; };
-static bool g_prof_on = false;
 static std::vector<ProfRec> g_prof;
 static std::vector<cudaEvent_t> g_prof_pool;
 static cudaEvent_t prof_event() {

@@ -957,3 +957,33 @@ def test_hopping_variants_at_the_bench_size(B, oracle_mod, precision, recon, tol
         assert (st6, stats6) == (st0, stats0) and np.array_equal(x6, x0)
     finally:
         B.lqcd_set_hop_variant(0)
+
+
+def test_programmatic_dependent_launch_changes_nothing_but_the_time():
+    """Launches on the legacy default stream chain the kernels of the CG and BiCGStab iterations by programmatic
+    dependent launch (lqcd_internal.h: chain_prologue / launch_chained); LQCD_PDL=0 (read once per process) launches them
+    the ordinary way.  Same kernels, same order: the solutions, iteration counts and residuals must be bit-identical."""
+    import hashlib
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    code = (
+        "import sys, hashlib, numpy as np; sys.path.insert(0, %r); sys.path.insert(0, %r)\n"
+        "import lqcd_inputs as gen, lattice_util as lu, paper_1209_5942_b200.binding as B\n"
+        "dims = (8, 8, 8, 16); U = gen.gauge_haar(dims); h = lu.volume(dims) // 2\n"
+        "b = gen.spinor_gaussian(h, stream=gen.STREAM_SOURCE)\n"
+        "B.lqcd_init(dims, gen.antiperiodic_t()); B.lqcd_set_stream(); g = B.upload_gauge(U); s = B.upload_spinor(b, 0)\n"
+        "x = B.alloc_spinor(); out = []\n"
+        "st = B.lqcd_cg_mdagm(g, s, x, 0.15, 0.1, 1e-10, 500); out += [st, B.lqcd_cg_stats(), hashlib.sha256(B.download_spinor(x, 0).tobytes()).hexdigest()]\n"
+        "st = B.lqcd_bicgstab_mhat(g, s, x, 0.15, 0.1, 1e-10, 500); out += [st, B.lqcd_cg_stats(), hashlib.sha256(B.download_spinor(x, 0).tobytes()).hexdigest()]\n"
+        "B.lqcd_mtm(g, s, x, 0.15, 0.1, 1); out += [hashlib.sha256(B.download_spinor(x, 0).tobytes()).hexdigest()]\n"
+        "print('RESULT', out)\n" % (root, os.path.join(root, "tests")))
+    res = []
+    for pdl in ("1", "0"):
+        r = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=600,
+                           env=dict(os.environ, LQCD_PDL=pdl))
+        assert r.returncode == 0, r.stderr[-2000:]
+        res.append([l for l in r.stdout.splitlines() if l.startswith("RESULT")][0])
+    assert res[0] == res[1]
+    assert "RESULT [0, " in res[0]
