@@ -465,10 +465,24 @@ def run_ours(args, rank, world, local_rank):
             p1.record(stream)
             stream.synchronize()
             ceil[name] = moved * 10 / (p0.elapsed_time(p1) * 1e-3) / 1e9
+        # the same 7:1 stream kept up for >= 1 s, with its own clock record: what a pure stream holds on this box when
+        # it runs as long as the sustained leg did (it draws less power than the hopping kernel, so its clock stays higher)
+        n_probe = max(10, int(1000.0 / ((nb + nb // 7) / ceil["mix_7_reads_1_write"] / 1e6)))
+        with ClockSampler(local_rank) as pclk:
+            p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            p0.record(stream)
+            for _ in range(n_probe):
+                B.lqcd_stream_probe(B.LQCD_ELEM_VEC16, B.LQCD_STREAM_MIX71, ps, pd, nb)
+            p1.record(stream)
+            stream.synchronize()
+        mix_sustained = (nb + nb // 7) * n_probe / (p0.elapsed_time(p1) * 1e-3) / 1e9
         del ps, pd
     roofline["stream_probe_gbs"] = ceil
     roofline["frac_of_stream_mix"] = achieved / ceil["mix_7_reads_1_write"]
     sustained["frac_of_stream_mix"] = sustained["roofline_achieved"] / ceil["mix_7_reads_1_write"]
+    sustained["stream_mix_sustained"] = {"gbs": mix_sustained, "launches": n_probe, "seconds": p0.elapsed_time(p1) * 1e-3,
+                                         "clocks": pclk.summary(),
+                                         "frac_of_it": sustained["roofline_achieved"] / mix_sustained}
 
     # ---- oracle on the host cores beside it (rank 0, N = 1 only) ------------------------------
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
