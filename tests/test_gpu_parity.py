@@ -987,3 +987,33 @@ def test_programmatic_dependent_launch_changes_nothing_but_the_time():
         res.append([l for l in r.stdout.splitlines() if l.startswith("RESULT")][0])
     assert res[0] == res[1]
     assert "RESULT [0, " in res[0]
+
+
+def test_random_lattice_shapes_all_formats(B, oracle_mod):
+    """Sixteen seeded random even extents between 2 and 12 (ragged warps, N_mu = 2 in some direction, extents that are
+    not powers of two, z planes that do and do not hold whole 32-site groups), complex phases on every boundary, in all
+    four storage formats: D_eo, D_oe and Mhat^dag against the oracle; the tile-order variant on the same shapes must
+    reproduce the default bit for bit (it is active only where a z plane is a whole number of groups)."""
+    rng = np.random.default_rng(1209_5942)
+    shapes = {(2, 2, 2, 2), (12, 2, 2, 2), (2, 12, 2, 4)}
+    while len(shapes) < 16:
+        shapes.add(tuple(int(2 * rng.integers(1, 7)) for _ in range(4)))
+    kappa, mu = 0.137, 0.21
+    try:
+        for dims in sorted(shapes):
+            U = gen.gauge_haar(dims, SEED)
+            x = gen.spinor_gaussian(lu.volume(dims) // 2, SEED)
+            for precision, recon, tol in ((0, 18, TOL_D), (0, 12, TOL_D), (1, 18, TOL_S), (1, 12, TOL_S)):
+                Ur, xr = _round_inputs(U, x, precision)
+                B.lqcd_set_hop_variant(0)
+                L = Lat(B, dims, GENERIC_PH, U, precision, recon)
+                got = [L.dslash(x, 0, kappa), L.dslash(x, 1, kappa), L.mtm(x, kappa, mu, 1)]
+                want = [oracle_mod.dslash_eo(dims, GENERIC_PH, Ur, xr, 0, kappa), oracle_mod.dslash_eo(dims, GENERIC_PH, Ur, xr, 1, kappa),
+                        oracle_mod.mhat(dims, GENERIC_PH, Ur, xr, kappa, mu, 1)]
+                for g_, w_ in zip(got, want):
+                    assert lu.rel_err(g_, w_) <= tol, (dims, precision, recon)
+                B.lqcd_set_hop_variant(6)
+                for g_, t_ in zip(got, [L.dslash(x, 0, kappa), L.dslash(x, 1, kappa), L.mtm(x, kappa, mu, 1)]):
+                    assert np.array_equal(g_, t_), (dims, precision, recon)
+    finally:
+        B.lqcd_set_hop_variant(0)
