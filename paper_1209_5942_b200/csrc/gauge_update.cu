@@ -33,7 +33,6 @@
 // against 397.8 -- no gain, not kept (the same order of sites moved nothing in the hopping kernel either).
 constexpr int kGaugeMinBlocksDouble = 3;   // CTAs of 128 threads per SM the register allocation aims at
 constexpr int kGaugeMinBlocksFloat = 4;
-constexpr int kGaugeStapleUnroll = 3;      // the loop over the three nu != mu, fully unrolled
 
 namespace lqcd {
 namespace {
@@ -61,33 +60,24 @@ __device__ __forceinline__ SiteIdx site_of(const Geometry& g, int e, int parity)
     return s;
 }
 
-// neighbour in direction dir, sgn = +1 / -1 (periodic; the neighbour has the other parity)
+// neighbour in direction dir, sgn = +1 / -1 (periodic; the neighbour has the other parity).  Written with selects only:
+// a branch per step would cut the kernel into basic blocks and keep ptxas from carrying link loads across them.
 __device__ __forceinline__ SiteIdx step(const Geometry& g, SiteIdx s, int dir, int sgn) {
-    if (dir == 0) {
-        if (sgn > 0) {
-            if (s.r) {
-                if (s.x0h == g.N0h - 1) { s.e -= g.N0h - 1; s.x0h = 0; }
-                else { s.e += 1; s.x0h += 1; }
-            }
-        } else {
-            if (!s.r) {
-                if (s.x0h == 0) { s.e += g.N0h - 1; s.x0h = g.N0h - 1; }
-                else { s.e -= 1; s.x0h -= 1; }
-            }
-        }
-        s.r ^= 1;
-        return s;
-    }
-    const int stride = (dir == 1) ? g.N0h : (dir == 2) ? g.N0h * g.N1 : g.N0h * g.N1 * g.N2;
-    const int n = (dir == 1) ? g.N1 : (dir == 2) ? g.N2 : g.N3;
-    int& c = (dir == 1) ? s.x1 : (dir == 2) ? s.x2 : s.x3;
-    if (sgn > 0) {
-        if (c == n - 1) { s.e -= (n - 1) * stride; c = 0; }
-        else { s.e += stride; c += 1; }
-    } else {
-        if (c == 0) { s.e += (n - 1) * stride; c = n - 1; }
-        else { s.e -= stride; c -= 1; }
-    }
+    // direction 0: the even-odd index moves only when the parity bit r allows it (x0 = 2 x0h + r)
+    const bool up = sgn > 0;
+    const bool move0 = up ? (s.r != 0) : (s.r == 0);
+    const int n = (dir == 0) ? g.N0h : (dir == 1) ? g.N1 : (dir == 2) ? g.N2 : g.N3;
+    const int stride = (dir == 0) ? 1 : (dir == 1) ? g.N0h : (dir == 2) ? g.N0h * g.N1 : g.N0h * g.N1 * g.N2;
+    const int c = (dir == 0) ? s.x0h : (dir == 1) ? s.x1 : (dir == 2) ? s.x2 : s.x3;
+    const bool moves = (dir != 0) || move0;
+    const bool wrap = up ? (c == n - 1) : (c == 0);
+    const int dc = !moves ? 0 : up ? (wrap ? -(n - 1) : 1) : (wrap ? (n - 1) : -1);
+    s.e += dc * stride;
+    s.x0h += (dir == 0) ? dc : 0;
+    s.x1 += (dir == 1) ? dc : 0;
+    s.x2 += (dir == 2) ? dc : 0;
+    s.x3 += (dir == 3) ? dc : 0;
+    s.r ^= (dir == 0) ? 1 : 0;
     return s;
 }
 
@@ -222,7 +212,6 @@ __device__ __forceinline__ double uniform01(unsigned long long seed, unsigned lo
 }
 
 constexpr int MAXTRY = 32;   // reading G20
-constexpr int kStapleUnroll = kGaugeStapleUnroll;
 
 // Kennedy-Pendleton: g0 with density sqrt(1 - g0^2) exp(lambda g0), direction uniform.
 // Counters: attempt t uses base + 4 t + (0..3), the direction base + 4 MAXTRY + (0, 1).
@@ -385,6 +374,43 @@ __device__ __forceinline__ void subgroup_step(T (&L)[18], const T (&A)[18], doub
     }
 }
 
+// A += the six staples of U_mu(x) (Fig. 2).  All neighbour indices first, then one straight line of 18 link loads and
+// 12 products, written software-pipelined: the first link of the next direction nu is asked for BEFORE the last product
+// of the current one, so that the three passes do not each begin with nothing in flight (ptxas keeps to the order it
+// is given across these blocks: with the loads of a pass issued only after the pass before had finished, a thread sat
+// through four exposed round trips instead of one).
+// The link itself, L = U_mu(x), is asked for before the very last product for the same reason.
+template <typename T, int RECON>
+__device__ __forceinline__ void staple_sum(const GaugeArgs& a, const SiteIdx& x, const SiteIdx& xpm, T (&A)[18], T (&L)[18]) {
+    const int G = a.g.G, mu = a.mu, p = a.parity;
+    int nu[3], e_pn[3], e_mn[3], e_pmmn[3];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        nu[j] = (mu + j + 1) & 3;   // the three directions nu != mu
+        e_pn[j] = step(a.g, x, nu[j], +1).e;
+        e_mn[j] = step(a.g, x, nu[j], -1).e;
+        e_pmmn[j] = step(a.g, xpm, nu[j], -1).e;
+    }
+    T u[18], w[18], t[18], nx[18];
+    gload<RECON, false>(a.gauge, G, 1 - p, nu[0], xpm.e, nx);            // U_nu(x+mu) of the first direction
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+#pragma unroll
+        for (int i = 0; i < 18; ++i) u[i] = nx[i];
+        gload<RECON, false>(a.gauge, G, 1 - p, mu, e_pn[j], w);          // U_mu(x+nu)
+        mm3<false, true, false>(u, w, t);
+        gload<RECON, false>(a.gauge, G, p, nu[j], x.e, u);               // U_nu(x)
+        mm3<false, true, true>(t, u, A);
+        gload<RECON, false>(a.gauge, G, p, nu[j], e_pmmn[j], u);         // U_nu(x+mu-nu)
+        gload<RECON, false>(a.gauge, G, 1 - p, mu, e_mn[j], w);          // U_mu(x-nu)
+        mm3<true, true, false>(u, w, t);
+        gload<RECON, false>(a.gauge, G, 1 - p, nu[j], e_mn[j], u);       // U_nu(x-nu)
+        if (j < 2) gload<RECON, false>(a.gauge, G, 1 - p, nu[j + 1], xpm.e, nx);   // next pass: U_nu'(x+mu)
+        else       gload<RECON, true>(a.gauge, G, p, mu, x.e, L);                  // after the last pass: the link itself
+        mm3<false, false, true>(t, u, A);
+    }
+}
+
 template <typename T, int RECON, int MODE>
 __global__ void __launch_bounds__(128, sizeof(T) == 8 ? kGaugeMinBlocksDouble : kGaugeMinBlocksFloat)
 gauge_update_kernel(const GaugeArgs a) {
@@ -407,24 +433,8 @@ gauge_update_kernel(const GaugeArgs a) {
     T A[18];
 #pragma unroll
     for (int i = 0; i < 18; ++i) A[i] = 0;
-#pragma unroll kStapleUnroll
-    for (int j = 1; j < 4; ++j) {
-        const int nu = (mu + j) & 3;   // the three directions nu != mu
-        const SiteIdx xpn = step(a.g, x, nu, +1), xmn = step(a.g, x, nu, -1), xpmmn = step(a.g, xpm, nu, -1);
-        T u[18], w[18], t[18];
-        gload<RECON, false>(a.gauge, G, 1 - p, nu, xpm.e, u);     // U_nu(x+mu)
-        gload<RECON, false>(a.gauge, G, 1 - p, mu, xpn.e, w);     // U_mu(x+nu)
-        mm3<false, true, false>(u, w, t);
-        gload<RECON, false>(a.gauge, G, p, nu, x.e, u);           // U_nu(x)
-        mm3<false, true, true>(t, u, A);
-        gload<RECON, false>(a.gauge, G, p, nu, xpmmn.e, u);       // U_nu(x+mu-nu)
-        gload<RECON, false>(a.gauge, G, 1 - p, mu, xmn.e, w);     // U_mu(x-nu)
-        mm3<true, true, false>(u, w, t);
-        gload<RECON, false>(a.gauge, G, 1 - p, nu, xmn.e, u);     // U_nu(x-nu)
-        mm3<false, false, true>(t, u, A);
-    }
     T L[18];
-    gload<RECON, true>(a.gauge, G, p, mu, e, L);
+    staple_sum<T, RECON>(a, x, xpm, A, L);
     subgroup_step<MODE, 0, 0, 1>(L, A, a.c_il, a.seed, a.tag, link_id, pre, 128);
     subgroup_step<MODE, 1, 1, 2>(L, A, a.c_il, a.seed, a.tag, link_id, pre, 128);
     subgroup_step<MODE, 2, 0, 2>(L, A, a.c_il, a.seed, a.tag, link_id, pre, 128);
@@ -477,23 +487,7 @@ __global__ void __launch_bounds__(256, 3) heatbath_ws_kernel(const GaugeArgs a) 
         link_id = 4ull * (2ull * (unsigned long long)e + (unsigned long long)x.r) + (unsigned long long)mu;
 #pragma unroll
         for (int i = 0; i < 18; ++i) A[i] = 0;
-#pragma unroll kStapleUnroll
-        for (int j = 1; j < 4; ++j) {
-            const int nu = (mu + j) & 3;
-            const SiteIdx xpn = step(a.g, x, nu, +1), xmn = step(a.g, x, nu, -1), xpmmn = step(a.g, xpm, nu, -1);
-            T u[18], w[18], t[18];
-            gload<RECON, false>(a.gauge, G, 1 - p, nu, xpm.e, u);     // U_nu(x+mu)
-            gload<RECON, false>(a.gauge, G, 1 - p, mu, xpn.e, w);     // U_mu(x+nu)
-            mm3<false, true, false>(u, w, t);
-            gload<RECON, false>(a.gauge, G, p, nu, x.e, u);           // U_nu(x)
-            mm3<false, true, true>(t, u, A);
-            gload<RECON, false>(a.gauge, G, p, nu, xpmmn.e, u);       // U_nu(x+mu-nu)
-            gload<RECON, false>(a.gauge, G, 1 - p, mu, xmn.e, w);     // U_mu(x-nu)
-            mm3<true, true, false>(u, w, t);
-            gload<RECON, false>(a.gauge, G, 1 - p, nu, xmn.e, u);     // U_nu(x-nu)
-            mm3<false, false, true>(t, u, A);
-        }
-        gload<RECON, true>(a.gauge, G, p, mu, e, L);
+        staple_sum<T, RECON>(a, x, xpm, A, L);
     }
     asm volatile("bar.sync 1, 256;\n" ::: "memory");
     if (live) {
