@@ -351,8 +351,11 @@ int lqcd_set_block_size(int threads);
  *   6      "tile": the default kernel with another order of the sites: the four warps of a CTA take a 2 x 2 block in
  *          (z, t) of one 32-site group in (x, y) instead of four consecutive groups (16 instead of 21 groups of
  *          neighbour spinors per CTA); covers every launch on a single lattice whose z planes hold whole groups
+ *   7      "general phases": where every phase of lqcd_init is exactly +-1 the default kernel applies it as the sign
+ *          of the accumulation (a multiply-add in place of an add, no branch); variant 7 runs the general kernel
+ *          (a complex multiplication behind a branch on every hop that wraps) on such lattices too, for comparison
  * Returns LQCD_BAD_ARG for other values. */
-#define LQCD_HOP_VARIANT_MAX 6
+#define LQCD_HOP_VARIANT_MAX 7
 int lqcd_set_hop_variant(int variant);
 
 #ifdef __cplusplus

@@ -473,6 +473,9 @@ int lqcd_init(const int dims[4], const double bc_phase[8]) {
         ctx.geo.ph_re[m] = bc_phase[2 * m];
         ctx.geo.ph_im[m] = bc_phase[2 * m + 1];
     }
+    ctx.geo.real_ph = 1;
+    for (int m = 0; m < 4; ++m)
+        if (bc_phase[2 * m + 1] != 0.0) ctx.geo.real_ph = 0;
     ctx.geo.N0h = dims[0] / 2; ctx.geo.N1 = dims[1]; ctx.geo.N2 = dims[2]; ctx.geo.N3 = dims[3];
     ctx.geo.d0h = make_fastdiv((unsigned)ctx.geo.N0h);
     ctx.geo.d1 = make_fastdiv((unsigned)ctx.geo.N1);

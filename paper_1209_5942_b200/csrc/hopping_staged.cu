@@ -421,6 +421,7 @@ cudaError_t launch_hopping_variant(int variant, int precision, int recon, int da
     a.gauge = gauge; a.in = in; a.out = out; a.aux = aux; a.dotw = nullptr; a.dotw2 = nullptr;
     a.g = g; a.ep = ep; a.out_parity = out_parity; a.red.partials = nullptr; a.scal = scal;
     a.tile_gy = a.tile_n2h = 0;
+    a.general_phases = 0;
     if (block <= 0 || block > LQCD_HOP_MAX_THREADS || (block % 32) != 0) block = LQCD_HOP_MAX_THREADS;
     count_launch();
     ProfScope prof(mode, st);

@@ -54,6 +54,7 @@ struct Geometry {
     int G;                // groups of 32 sites per parity = ceil(Vh / 32)
     FastDiv d0h, d1, d2;  // division by N0h, N1, N2
     double ph_re[4], ph_im[4];
+    int real_ph;          // every phase is exactly +1 or -1 (periodic / antiperiodic): the hopping kernel's REALPH build
     // Slab mode (lqcd_slab_init): two ghost time slices sit behind the G groups of a field, the
     // forward ghost (slice t = N3 of the next rank) at site index Vh + s = e + s3 for a site of the
     // last slice, the backward ghost (slice t = -1 of the previous rank) at Vh + s3 + s (s = index

@@ -36,6 +36,7 @@ struct HopArgs {
     // variant 6 (TILE): a CTA of four warps takes the four groups {g, g + Gy, g + Gy N2, g + Gy (N2 + 1)} -- the
     // groups of a 2 x 2 block in (z, t) -- instead of four consecutive groups; Gy = groups per z plane
     int tile_gy, tile_n2h;   // Gy and N2 / 2 (0: linear order)
+    int general_phases;      // variant 7: the branch-per-hop kernel even where every phase is +-1 (for A/B timing)
 };
 
 // ----------------------------------------------------------------------------- field access
@@ -205,6 +206,34 @@ __device__ __forceinline__ void accumulate(T (&acc)[24], const T (&chi)[12]) {
         add_c<P::c1conj>(acc[2 * (3 * P::j1 + a)], acc[2 * (3 * P::j1 + a) + 1],
                          acc[2 * (3 * P::j1 + a)], acc[2 * (3 * P::j1 + a) + 1], chi[2 * (3 + a)],
                          chi[2 * (3 + a) + 1]);
+    }
+}
+
+// acc += sg * (the four spin rows of chi), sg real: the same additions as accumulate() written as multiply-adds, so
+// that a boundary phase of +-1 (periodic / antiperiodic directions) needs no branch and no extra instruction;
+// fma(1, b, a) = a + b and fma(-1, b, a) = a - b exactly, i.e. the same bits as the branch would give.
+template <int C, typename T>
+__device__ __forceinline__ void add_c_scaled(T& ore, T& oim, T are, T aim, T bre, T bim, T sg, T msg) {
+    if (C == 0) { ore = fma_(sg, bre, are);  oim = fma_(sg, bim, aim); }
+    if (C == 1) { ore = fma_(msg, bim, are); oim = fma_(sg, bre, aim); }
+    if (C == 2) { ore = fma_(msg, bre, are); oim = fma_(msg, bim, aim); }
+    if (C == 3) { ore = fma_(sg, bim, are);  oim = fma_(msg, bre, aim); }
+}
+template <int MU, int S, typename T>
+__device__ __forceinline__ void accumulate_scaled(T (&acc)[24], const T (&chi)[12], T sg) {
+    typedef Proj<MU, S> P;
+    const T msg = -sg;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        acc[2 * a] = fma_(sg, chi[2 * a], acc[2 * a]);
+        acc[2 * a + 1] = fma_(sg, chi[2 * a + 1], acc[2 * a + 1]);
+        acc[2 * (3 + a)] = fma_(sg, chi[2 * (3 + a)], acc[2 * (3 + a)]);
+        acc[2 * (3 + a) + 1] = fma_(sg, chi[2 * (3 + a) + 1], acc[2 * (3 + a) + 1]);
+        add_c_scaled<P::c0conj>(acc[2 * (3 * P::j0 + a)], acc[2 * (3 * P::j0 + a) + 1],
+                                acc[2 * (3 * P::j0 + a)], acc[2 * (3 * P::j0 + a) + 1], chi[2 * a], chi[2 * a + 1], sg, msg);
+        add_c_scaled<P::c1conj>(acc[2 * (3 * P::j1 + a)], acc[2 * (3 * P::j1 + a) + 1],
+                                acc[2 * (3 * P::j1 + a)], acc[2 * (3 * P::j1 + a) + 1], chi[2 * (3 + a)],
+                                chi[2 * (3 + a) + 1], sg, msg);
     }
 }
 

@@ -460,7 +460,7 @@ def main():
     ap.add_argument("--configs", default="3,4,5,thermal")
     ap.add_argument("--out", default=None)
     ap.add_argument("--hop-variant", type=int, default=0,
-                    help="hopping kernel variant (lqcd_set_hop_variant): 0 plain (default), 1..3 link ring of that depth, 4 / 5 bulk-staged forward links, 6 the 2 x 2 (z, t) tile order")
+                    help="hopping kernel variant (lqcd_set_hop_variant): 0 plain (default), 1..3 link ring of that depth, 4 / 5 bulk-staged forward links, 6 the 2 x 2 (z, t) tile order, 7 the general-phase kernel on real phases")
     ap.add_argument("--formats", default="d18,d12,s18,s12", help="storage variants timed by config 5")
     args = ap.parse_args()
     global FORMATS

@@ -900,7 +900,7 @@ def test_bicgstab_on_a_side_stream_graph_replay_matches_direct_launches(B, oracl
 
 
 # --------------------------------------------------------------------------- staged variants of the hopping kernel
-@pytest.mark.parametrize("variant", [1, 2, 3, 4, 5, 6])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4, 5, 6, 7])
 @pytest.mark.parametrize("precision,recon,tol", [(0, 18, TOL_D), (0, 12, TOL_D), (1, 18, TOL_S), (1, 12, TOL_S)])
 def test_hopping_variants_match_oracle(B, oracle_mod, variant, precision, recon, tol):
     """lqcd_set_hop_variant: every staged variant of the hopping kernel (hopping_staged.cu) against the oracle, in every
@@ -949,7 +949,7 @@ def test_hopping_variants_at_the_bench_size(B, oracle_mod, precision, recon, tol
         assert lu.rel_err(ref_d[sites], oracle_mod.dslash_eo_sites(dims, AP, Ur, xr, sites, 0, kappa)) <= tol
         assert lu.rel_err(ref_m[sites], oracle_mod.mhat_sites(dims, AP, Ur, xr, sites, kappa, mu, 1)) <= tol
         st0, x0, stats0 = L.cg(b, kappa, mu, 0.0, 6)
-        for variant in (2, 4, 5, 6):
+        for variant in (2, 4, 5, 6, 7):
             B.lqcd_set_hop_variant(variant)
             assert np.array_equal(L.dslash(x, 0, kappa), ref_d), variant
             assert np.array_equal(L.mtm(x, kappa, mu, 1), ref_m), variant
