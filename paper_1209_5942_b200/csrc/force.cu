@@ -84,7 +84,9 @@ __device__ __forceinline__ void phase_mul(T (&chi)[12], T pr, T pi) {
 // The second term of W is -h+[X(x)] (x) (eta U h+[Y(x+mu)])^dag; its anti-Hermitian part equals
 // that of +(eta U h+[Y(x+mu)]) (x) h+[X(x)]^dag, so both terms go through the same accumulation
 // with the transported half spinor first.
-template <typename T, int RECON, int MU>
+// REALPH (every boundary phase +-1, Geometry::real_ph): both terms carry the same real eta, so it multiplies the link's
+// whole W and is applied once, with kappa, when the force is stored -- no branch, no phase multiplication.
+template <typename T, int RECON, int MU, bool REALPH>
 __device__ __forceinline__ void force_link(const ForceArgs& a, int p, int e, int e_nb, bool wrap) {
     T u[18], psi[24], h[12], uh[12], v[12];
     AntiHerm<T> w;
@@ -96,7 +98,7 @@ __device__ __forceinline__ void force_link(const ForceArgs& a, int p, int e, int
     load_spinor(a.x[1 - p], e_nb, psi);
     project<MU, -1>(psi, h);
     su3_mul(u, h, uh);
-    if (wrap) phase_mul(uh, er, ei);
+    if (!REALPH && wrap) phase_mul(uh, er, ei);
     load_spinor(a.y[p], e, psi);
     project<MU, -1>(psi, v);
     outer_acc(w, uh, v);
@@ -104,13 +106,13 @@ __device__ __forceinline__ void force_link(const ForceArgs& a, int p, int e, int
     load_spinor(a.y[1 - p], e_nb, psi);
     project<MU, +1>(psi, h);
     su3_mul(u, h, uh);
-    if (wrap) phase_mul(uh, er, ei);
+    if (!REALPH && wrap) phase_mul(uh, er, ei);
     load_spinor(a.x[p], e, psi);
     project<MU, +1>(psi, v);
     outer_acc(w, uh, v);
 
     // F^a = 2 kappa Im tr(T^a W) = kappa Im tr(lambda^a W)
-    const double k = a.kappa;
+    const double k = (REALPH && wrap) ? a.kappa * a.g.ph_re[MU] : a.kappa;
     double2* out = reinterpret_cast<double2*>(a.force) +
                    ((size_t)(p * 4 + MU) * a.g.G + (e >> 5)) * (4 * 32) + (e & 31);
     out[0] = make_double2(k * (double)w.s[0], k * (double)w.r[0]);                          // lambda 1, 2
@@ -125,7 +127,7 @@ __device__ __forceinline__ void force_link(const ForceArgs& a, int p, int e, int
 // site is read twice, as X(x) by its own block and as X(x+mu) by blocks of the other parity:
 // sweeping one parity after the other put a whole field (805 MB of X, Y) between the two reads
 // and cost a second DRAM pass (ncu: 3.35 GB of traffic against 2.55 GB algorithmic).
-template <typename T, int RECON>
+template <typename T, int RECON, bool REALPH>
 __global__ void __launch_bounds__(128, kForceMinBlocks) force_kernel(const ForceArgs a) {
     const int G = a.g.G;
     const int p = (int)blockIdx.x & 1;
@@ -144,16 +146,16 @@ __global__ void __launch_bounds__(128, kForceMinBlocks) force_kernel(const Force
     const int s1 = N0h, s2 = N0h * N1, s3 = N0h * N1 * N2;
     if (mu == 0) {
         const bool wf = (r == 1) && (x0h == N0h - 1);
-        force_link<T, RECON, 0>(a, p, e, wf ? e - (N0h - 1) : e + r, wf);
+        force_link<T, RECON, 0, REALPH>(a, p, e, wf ? e - (N0h - 1) : e + r, wf);
     } else if (mu == 1) {
         const bool wf = (x1 == N1 - 1);
-        force_link<T, RECON, 1>(a, p, e, wf ? e - (N1 - 1) * s1 : e + s1, wf);
+        force_link<T, RECON, 1, REALPH>(a, p, e, wf ? e - (N1 - 1) * s1 : e + s1, wf);
     } else if (mu == 2) {
         const bool wf = (x2 == N2 - 1);
-        force_link<T, RECON, 2>(a, p, e, wf ? e - (N2 - 1) * s2 : e + s2, wf);
+        force_link<T, RECON, 2, REALPH>(a, p, e, wf ? e - (N2 - 1) * s2 : e + s2, wf);
     } else {
         const bool wf = (x3 == N3 - 1);
-        force_link<T, RECON, 3>(a, p, e, wf ? e - (N3 - 1) * s3 : e + s3, wf);
+        force_link<T, RECON, 3, REALPH>(a, p, e, wf ? e - (N3 - 1) * s3 : e + s3, wf);
     }
 }
 
@@ -192,13 +194,17 @@ cudaError_t launch_fermion_force(int precision, int recon, const Geometry& g, co
     count_launch();
     ProfScope prof(6, st);
     const int grid = 2 * g.G;
-    if (precision == 0) {
-        if (recon == 12) force_kernel<double, 12><<<grid, 128, 0, st>>>(a);
-        else             force_kernel<double, 18><<<grid, 128, 0, st>>>(a);
-    } else {
-        if (recon == 12) force_kernel<float, 12><<<grid, 128, 0, st>>>(a);
-        else             force_kernel<float, 18><<<grid, 128, 0, st>>>(a);
-    }
+    // The branch-free form is what ptxas schedules better only in double/12 (us per launch at 32^3 x 64, one box, A B A B:
+    // 438 against 482; double/18 511 against 503, single/18 278 against 275, single/12 268 against 259), so it is used there.
+    const bool rp = g.real_ph && precision == 0 && recon == 12;
+#define LQCD_FORCE(TT, RR)                                                           \
+    do {                                                                             \
+        if (rp) force_kernel<TT, RR, true><<<grid, 128, 0, st>>>(a);                 \
+        else    force_kernel<TT, RR, false><<<grid, 128, 0, st>>>(a);                \
+    } while (0)
+    if (precision == 0) { if (recon == 12) LQCD_FORCE(double, 12); else LQCD_FORCE(double, 18); }
+    else                { if (recon == 12) LQCD_FORCE(float, 12);  else LQCD_FORCE(float, 18); }
+#undef LQCD_FORCE
     return cudaGetLastError();
 }
 
