@@ -69,9 +69,10 @@ METRIC = "D_tm GFLOPS (1320 flop/site) & achieved HBM GB/s vs B200 peak, double"
 # dram__bytes_read.sum + dram__bytes_write.sum per PLAIN hopping launch (MODE 0, exactly 1536 B/site algorithmic =
 # 1.610613 GB) at this workload, from the committed `ncu --set full` capture named in NCU_TRAFFIC_SOURCE; a constant
 # typed in from that file, NOT measured in this run -- refreshed whenever the hopping kernel changes.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 1589003000
-NCU_TRAFFIC_SOURCE = ("profiles/r02_hopping_staged.md, column 0 (ncu --set full of hopping_kernel<double,18,0,0>, build fef04fc, raw "
-                      "page in profiles/r02g_hop_v0_raw.csv): dram__bytes_read 1.415640 GB + dram__bytes_write 0.173363 GB")
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 1586016000
+NCU_TRAFFIC_SOURCE = ("profiles/r02_hopping_staged.md, section 'The branch per hop' (ncu --set full of the default kernel "
+                      "hopping_kernel<double,18,0,0,...,REALPH>, raw page in profiles/r02z_hop_default_raw.csv): "
+                      "dram__bytes_read 1.415661 GB + dram__bytes_write 0.170355 GB")
 
 
 def measured_peak():
