@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "liblqcd.so")
-SOURCES = ["api.cu", "hopping.cu", "hopping_staged.cu", "force.cu", "gauge_update.cu", "vector_ops.cu", "pack.cu", "stream_probe.cu"]
+SOURCES = ["api.cu", "hopping.cu", "hopping_float.cu", "hopping_staged.cu", "force.cu", "gauge_update.cu", "vector_ops.cu", "pack.cu", "stream_probe.cu"]
 HEADERS = [os.path.join(CSRC, "lqcd_internal.h"), os.path.join(CSRC, "site_ops.cuh"), os.path.join(CSRC, "kp_log_table.h"), os.path.join(HERE, "..", "include", "lqcd.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -30,7 +30,7 @@ def needs_build():
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, s) for s in SOURCES] + HEADERS + [os.path.abspath(__file__)]
+    deps = [os.path.join(CSRC, s) for s in SOURCES] + HEADERS + [os.path.abspath(__file__)]   # hopping_float.cu includes hopping.cu
     return any(os.path.getmtime(d) > t for d in deps)
 
 

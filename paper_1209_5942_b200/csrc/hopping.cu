@@ -288,6 +288,19 @@ cudaError_t launch_tr(int dagger, int mode, const HopArgs& a, int block, cudaStr
 
 }  // namespace
 
+// This file is compiled twice so that its two halves build in parallel (the kernel's instantiations are most of the
+// library's compile time): as hopping.cu, with the double-precision kernels and the dispatcher, and through
+// hopping_float.cu (LQCD_HOP_FLOAT_PART), with the single-precision kernels behind launch_hopping_float.  HopArgs lives in
+// an unnamed namespace, so it crosses between the two as an untyped pointer to the same layout.
+cudaError_t launch_hopping_float(int recon, int dagger, int mode, const void* hop_args, int block, cudaStream_t st);
+#ifdef LQCD_HOP_FLOAT_PART
+cudaError_t launch_hopping_float(int recon, int dagger, int mode, const void* hop_args, int block, cudaStream_t st) {
+    const HopArgs& a = *static_cast<const HopArgs*>(hop_args);
+    return recon == 12 ? launch_tr<float, 12>(dagger, mode, a, block, st)
+                       : launch_tr<float, 18>(dagger, mode, a, block, st);
+}
+#else
+
 // which kernel launch_hopping uses where a staged variant covers the launch (hopping_staged.cu); 0 = the plain kernel
 static int g_hop_variant = 0;
 void set_hopping_variant(int variant) { g_hop_variant = variant; }
@@ -329,8 +342,8 @@ cudaError_t launch_hopping(int precision, int recon, int dagger, int mode, const
         return recon == 12 ? launch_tr<double, 12>(dagger, mode, a, block, st)
                            : launch_tr<double, 18>(dagger, mode, a, block, st);
     }
-    return recon == 12 ? launch_tr<float, 12>(dagger, mode, a, block, st)
-                       : launch_tr<float, 18>(dagger, mode, a, block, st);
+    return launch_hopping_float(recon, dagger, mode, &a, block, st);
 }
+#endif  // LQCD_HOP_FLOAT_PART
 
 }  // namespace lqcd
