@@ -11,7 +11,8 @@
 //      neighbour spinors are reused by 8 output sites, so they go through the
 //      read-only path with default caching (L1 for x/y neighbours, L2 for z/t)
 //   a4 SU(3) x half spinor (U h forward, U^dag h backward)
-//   a5 boundary phase on the hop that wraps, reconstruction to 4 spin rows, accumulate
+//   a5 boundary phase on the hop that wraps, reconstruction to 4 spin rows, accumulate; where every phase is +-1
+//      (REALPH) the phase is the sign s of acc = fma(s, chi, acc) and the thread has no branch at all
 //   a6/a7 epilogue: out = c_chi * (acc + d_chi * aux), c, d complex per chirality:
 //      covers -kappa (dslash_eo), M_oo^{-1} D_oe, and M_ee in - D_eo (.) in one store.
 //   a9 (MODE 3) the last hopping launch of a CG iteration never stores q = A p: it
