@@ -105,16 +105,9 @@ __device__ __forceinline__ void hop_from_slot(T (&acc)[24], const HopArgs& a, co
     project<MU, S>(psi, h);
     if (FWD) su3_mul(u, h, chi);
     else     su3_dag_mul(u, h, chi);
-    if (wrap) {
-        const T pr = (T)a.g.ph_re[MU], pi = FWD ? (T)a.g.ph_im[MU] : -(T)a.g.ph_im[MU];
-#pragma unroll
-        for (int i = 0; i < 6; ++i) {
-            const T re = chi[2 * i], im = chi[2 * i + 1];
-            chi[2 * i] = fma_(-pi, im, pr * re);
-            chi[2 * i + 1] = fma_(pi, re, pr * im);
-        }
-    }
-    accumulate<MU, S>(acc, chi);
+    // the staged variants cover lattices with real boundary phases only (hopping_variant_covers): the phase is the sign
+    // of the accumulation, as in the default kernel's REALPH build, and the thread has no branch
+    accumulate_scaled<MU, S>(acc, chi, wrap ? (T)a.g.ph_re[MU] : (T)1);
 }
 
 template <typename T, int RECON, int DAG, int MODE, int D, int NB>
@@ -409,7 +402,7 @@ cudaError_t launch_bulk_fmt(int precision, int recon, int dagger, int mode, cons
 }  // namespace
 
 bool hopping_variant_covers(int variant, int mode, const Geometry& g, const SiteRange* range) {
-    return variant >= 1 && variant <= 5 && mode <= 1 && !g.slab && range == nullptr;
+    return variant >= 1 && variant <= 5 && mode <= 1 && !g.slab && range == nullptr && g.real_ph;
 }
 
 cudaError_t launch_hopping_variant(int variant, int precision, int recon, int dagger, int mode, const Geometry& g,
