@@ -341,7 +341,8 @@ int lqcd_set_block_size(int threads);
 /* Which hopping kernel runs the launches with a plain or M_ee*aux epilogue on a single lattice (BASELINE.json
  * north_star: "neighbour spinors staged through shared memory or TMA ... every choice is evidenced by ncu
  * counters"; the counters are in profiles/r02_hopping_staged.md).  Process-wide, not per context.  Same result
- * to rounding order as the default; launches a variant does not cover (fused reductions, slab mode) use variant 0.
+ * to rounding order as the default; launches a variant does not cover (fused reductions, slab mode, and for variants
+ * 1-5 lattices with a complex boundary phase) use variant 0.
  *   0      the default: one thread per site, every operand through LDG into registers
  *   1..3   "link ring": each thread prefetches the link of hop h + D (D = variant) into its own shared-memory
  *          slot with cp.async while it works on hop h
