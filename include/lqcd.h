@@ -200,6 +200,20 @@ int lqcd_gauge_update(void* gauge, int mu, int parity, int mode, double beta, un
                       unsigned long long tag);
 int lqcd_gauge_sweep(void* gauge, int mode, double beta, unsigned long long seed, unsigned long long tag);
 int lqcd_plaquette(const void* gauge, double* plaquette_host);
+/* lqcd_plaquette_static: the same average plaquette for callers that may not allocate (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc).  The call makes no cudaMalloc, cudaFree or allocating
+ * library call: the per-warp partial sums, which lqcd_plaquette keeps in a buffer of the context, go to a file-scope
+ * device array of LQCD_PLAQUETTE_STATIC_MAX_PARTIALS doubles (512 KiB, held by every GPU that loads the library until
+ * exit), and the result goes to plaquette_dev, ONE double in DEVICE memory the caller owns.  Asynchronous on the
+ * lqcd_set_stream stream; two launches.  Needs 8 * ceil(V/256) <= LQCD_PLAQUETTE_STATIC_MAX_PARTIALS, i.e. lattices
+ * up to V = 2^21 sites (32^3 x 64); larger ones return LQCD_BAD_ARG with a message and launch nothing.  All calls share
+ * the array, which keeps the last call's contents (nothing in it has to start at zero: every partial a call reads it
+ * has written first); calls that overlap on the GPU -- two streams, two host threads -- race on it, so order them.
+ * The first call on a device looks the array's device address up (no allocation); make it outside a capture.
+ * Same gauge formats as lqcd_plaquette; not available after lqcd_slab_init.  The value agrees with lqcd_plaquette to
+ * summation order (a few ulp). */
+#define LQCD_PLAQUETTE_STATIC_MAX_PARTIALS 65536
+int lqcd_plaquette_static(const void* gauge, double* plaquette_dev);
 int lqcd_unpack_gauge(const void* internal_dev, void* canon_dev);
 
 /* Mixed-precision solve of the same system (the paper's planned next step, PAPER.md:352;

@@ -27,7 +27,7 @@ SYMBOLS = [
     "lqcd_unpack_spinor", "lqcd_dslash_eo", "lqcd_mtm", "lqcd_mtm_full", "lqcd_solve_full", "lqcd_cg_mdagm", "lqcd_cg_setup",
     "lqcd_cg_iterate", "lqcd_cg_finish", "lqcd_cg_stats", "lqcd_cg_mdagm_mixed", "lqcd_cg_outer_iterations", "lqcd_bicgstab_mhat", "lqcd_force_bytes", "lqcd_unpack_force", "lqcd_fermion_force", "lqcd_force_tm", "lqcd_mtm_host", "lqcd_cg_mdagm_host",
     "lqcd_launch_count", "lqcd_set_block_size", "lqcd_set_hop_variant", "lqcd_profile", "lqcd_profile_read",
-    "lqcd_gauge_update", "lqcd_gauge_sweep", "lqcd_plaquette", "lqcd_unpack_gauge", "lqcd_stream_probe", "lqcd_fp64_probe",
+    "lqcd_gauge_update", "lqcd_gauge_sweep", "lqcd_plaquette", "lqcd_plaquette_static", "lqcd_unpack_gauge", "lqcd_stream_probe", "lqcd_fp64_probe",
     "lqcd_select_context", "lqcd_slab_init", "lqcd_slab_spinor_halo", "lqcd_slab_gauge_halo", "lqcd_slab_dslash",
     "lqcd_slab_mhat_stage", "lqcd_slab_cg_begin", "lqcd_slab_cg_stage", "lqcd_slab_cg_halo_field",
     "lqcd_slab_sum_ptr", "lqcd_slab_cg_poll", "lqcd_slab_cg_end",
@@ -81,6 +81,7 @@ def _load():
         "lqcd_gauge_update": [vp, i32, i32, i32, dbl, u64, u64],
         "lqcd_gauge_sweep": [vp, i32, dbl, u64, u64],
         "lqcd_plaquette": [vp, ctypes.POINTER(dbl)],
+        "lqcd_plaquette_static": [vp, vp],
         "lqcd_unpack_gauge": [vp, vp],
         "lqcd_stream_probe": [i32, i32, vp, vp, ctypes.c_size_t],
         "lqcd_fp64_probe": [dbl, dbl, i32, vp],
@@ -346,6 +347,11 @@ def lqcd_plaquette(gauge):
     p = ctypes.c_double(0.0)
     _check(_lib.lqcd_plaquette(_ptr(gauge), ctypes.byref(p)))
     return p.value
+
+
+def lqcd_plaquette_static(gauge, plaquette_dev):
+    """No-allocation variant: the result goes to plaquette_dev, one double in device memory (include/lqcd.h)."""
+    return _check(_lib.lqcd_plaquette_static(_ptr(gauge), _ptr(plaquette_dev)))
 
 
 def lqcd_unpack_gauge(internal_dev, canon_dev):

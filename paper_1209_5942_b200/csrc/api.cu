@@ -646,6 +646,18 @@ int lqcd_plaquette(const void* gauge, double* plaquette_host) {
     return LQCD_OK;
 }
 
+int lqcd_plaquette_static(const void* gauge, double* plaquette_dev) {
+    if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
+    if (ctx.slab) return fail(LQCD_BAD_ARG, "lqcd_plaquette_static: not available after lqcd_slab_init");
+    if (!gauge || !plaquette_dev) return fail(LQCD_BAD_ARG, "lqcd_plaquette_static: null pointer");
+    const int np = plaquette_partials(ctx.geo.Vh);
+    if (np > LQCD_PLAQUETTE_STATIC_MAX_PARTIALS)
+        return fail(LQCD_BAD_ARG, "lqcd_plaquette_static: the lattice needs %d partial sums, the static scratch array holds %d "
+                                  "(lattices up to 2^21 sites); use lqcd_plaquette", np, LQCD_PLAQUETTE_STATIC_MAX_PARTIALS);
+    CU(launch_plaquette_static(ctx.precision, ctx.recon, ctx.geo, gauge, plaquette_dev, ctx.stream));
+    return LQCD_OK;
+}
+
 int lqcd_pack_spinor(const void* canon_dev, void* internal_dev, int parity) {
     if (!ctx.init) return fail(LQCD_NOT_INITIALISED, "not initialised");
     if (!canon_dev || !internal_dev) return fail(LQCD_BAD_ARG, "lqcd_pack_spinor: null pointer");

@@ -19,6 +19,7 @@
 // 9 x 144 = 1296 B per updated link in double/18; the 2.1-fold reuse of the 18 loads is left to
 // L1/L2, as for the neighbour spinors of the hopping kernel.
 #include "site_ops.cuh"
+#include "../../include/lqcd.h"
 #include <cstdlib>
 
 // Measured at 32^3 x 64 (us per sub-sweep, heatbath / overrelaxation): double with 2 CTAs per SM
@@ -578,6 +579,82 @@ cudaError_t launch_plaquette(int precision, int recon, const Geometry& g, const 
         if (recon == 12) plaquette_kernel<float, 12><<<grid, 128, 0, st>>>(a);
         else             plaquette_kernel<float, 18><<<grid, 128, 0, st>>>(a);
     }
+    return cudaGetLastError();
+}
+
+
+// ---------------------------------------------------------------------------------------------------------------------
+// The average plaquette with no allocation anywhere on the path (lqcd_plaquette_static, include/lqcd.h): the per-warp
+// partial sums go to a file-scope device array instead of the context's cudaMalloc'ed buffer.  Every GPU that loads the
+// library holds the array (LQCD_PLAQUETTE_STATIC_MAX_PARTIALS doubles = 512 KiB) until exit.  All calls share it: calls
+// that overlap on the GPU (two streams, two host threads) race on it.  Nothing in it has to start at zero -- a call
+// rewrites every partial it later reads -- so it keeps the last call's contents and is never cleared.
+// ---------------------------------------------------------------------------------------------------------------------
+}  // namespace lqcd
+
+static __device__ __align__(256) double g_plaquette_static_partials[LQCD_PLAQUETTE_STATIC_MAX_PARTIALS];
+
+namespace lqcd {
+namespace {
+
+// fixed-order sum of the n partials; device code names the array directly
+__global__ void __launch_bounds__(256) plaquette_static_sum_kernel(int n, double inv_norm, double* out) {
+    __shared__ double sh[256];
+    double s = 0.0;
+    for (int i = threadIdx.x; i < n; i += 256) s += g_plaquette_static_partials[i];
+    sh[threadIdx.x] = s;
+    __syncthreads();
+#pragma unroll
+    for (int w = 128; w > 0; w >>= 1) {
+        if ((int)threadIdx.x < w) sh[threadIdx.x] += sh[threadIdx.x + w];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *out = sh[0] * inv_norm;
+}
+
+// In host code the array's name is a host-side stand-in, not a device address: the kernel gets what
+// cudaGetSymbolAddress returns, looked up once per device with that device current.
+constexpr int kMaxDevices = 64;
+double* g_static_partials_ptr[kMaxDevices] = {};
+
+cudaError_t plaquette_static_ptr(double** ptr) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    if (!g_static_partials_ptr[dev]) {
+        double* p = nullptr;
+        e = cudaGetSymbolAddress((void**)&p, g_plaquette_static_partials);
+        if (e != cudaSuccess) return e;
+        g_static_partials_ptr[dev] = p;
+    }
+    *ptr = g_static_partials_ptr[dev];
+    return cudaSuccess;
+}
+
+}  // namespace
+
+cudaError_t launch_plaquette_static(int precision, int recon, const Geometry& g, const void* gauge, double* out_dev,
+                                    cudaStream_t st) {
+    double* scratch = nullptr;
+    cudaError_t e = plaquette_static_ptr(&scratch);
+    if (e != cudaSuccess) return e;
+    GaugeArgs a;
+    a.gauge = const_cast<void*>(gauge); a.g = g; a.mu = 0; a.parity = 0; a.beta = 0; a.c_il = 0; a.seed = 0; a.tag = 0;
+    a.red.partials = scratch;
+    const dim3 grid((g.Vh + 127) / 128, 2);
+    count_launch(2);
+    if (precision == 0) {
+        if (recon == 12) plaquette_kernel<double, 12><<<grid, 128, 0, st>>>(a);
+        else             plaquette_kernel<double, 18><<<grid, 128, 0, st>>>(a);
+    } else {
+        if (recon == 12) plaquette_kernel<float, 12><<<grid, 128, 0, st>>>(a);
+        else             plaquette_kernel<float, 18><<<grid, 128, 0, st>>>(a);
+    }
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    // sum of Re tr over the 6 V plaquettes -> average of Re tr / 3
+    plaquette_static_sum_kernel<<<1, 256, 0, st>>>(plaquette_partials(g.Vh), 1.0 / (3.0 * 6.0 * 2.0 * (double)g.Vh), out_dev);
     return cudaGetLastError();
 }
 

@@ -236,6 +236,10 @@ cudaError_t launch_gauge_update(int precision, int recon, int mode, const Geomet
 cudaError_t launch_plaquette(int precision, int recon, const Geometry& g, const void* gauge, Reduction red,
                              cudaStream_t st);
 int plaquette_partials(int Vh);
+// the same with the partials in a file-scope device array (at most LQCD_PLAQUETTE_STATIC_MAX_PARTIALS of them: the caller
+// checks) and the average written to out_dev; allocates nothing
+cudaError_t launch_plaquette_static(int precision, int recon, const Geometry& g, const void* gauge, double* out_dev,
+                                    cudaStream_t st);
 
 // force.cu: F^a_mu(x) for every link from full-lattice X, Y given as half fields (the force is
 // linear in kappa, so a common sign of the odd halves is passed as the sign of kappa).
