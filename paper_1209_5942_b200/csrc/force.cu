@@ -15,8 +15,8 @@
 // (X, Y once each) + 256 (force written) = 1216 in double/18.
 #include "site_ops.cuh"
 
-// CTAs of 128 threads per SM.  The kernel is latency bound (ncu: DRAM traffic = algorithmic bytes,
-// DRAM throughput 62%, 12 warps/SM): in double 4 CTAs (128 registers, no spills) run 460 us at
+// CTAs of 128 threads per SM (per format: table below).  Round 1: the kernel is latency bound (ncu: DRAM traffic =
+// algorithmic bytes, DRAM throughput 62%, 12 warps/SM): in double 4 CTAs (128 registers, no spills) run 460 us at
 // 32^3 x 64 against 497 us with 3 (168 registers) and 497 us with 5 (96 registers, 140 B of spills).
 // Tried and dropped: two threads per link (one per term of W, CTAs of 256, partial sums combined through
 // shared memory; 80 registers, 24 warps/SM): 581 us -- the link is fetched twice and the local spinors
@@ -24,7 +24,23 @@
 // once in shared memory instead of read through L1 by each direction-warp: 480 us (no change: the
 // L2 -> L1 traffic it removes is not the limiter).  One thread per site looping over the four directions
 // with the staged X(x), Y(x) (64-thread CTAs, 168 registers): 513 us; at 128 registers 707 us.
-constexpr int kForceMinBlocks = 4;
+//
+// Round 2 (us per launch at 32^3 x 64 in the sweep's power-capped loop, A B A B on one box; d18 / d12 / s18 / s12):
+//   as above, 4 CTAs                                     505-510 / 422-443 / 270-280 / 258-267
+//   loads first (LF below) at 3 / 4 / 6 / 8 CTAs          487-489 / 420     / 263-270 / 235     <- used, except d12
+//   (the build as committed, another box: 472 / 433 / 262 / 237 = 0.83 / 0.76 / 0.90 / 0.87 of the measured copy bandwidth)
+//   loads first at 4 / 3 / 5 / 6 CTAs                     531     / 448-452 / 276     / 242
+// ptxas issues the link and X(x+mu) up front (21 LDG.128) and the second neighbour spinor only when registers free up, so a
+// thread waits on DRAM twice; LF names all three DRAM-latency reads before any arithmetic (33 LDG.128 up front, 168
+// registers in double/18).  Tried on top of both and dropped:
+// * a grid that fills the GPU once, every CTA walking the blocks b, b + gridDim.x, ... with no barrier between its warps
+//   (ncu: 12.8 of 16 resident warps active, the rest is CTA turnover): 576 us at 4 CTAs per SM, 530 at 8, 553 at 16 (d18);
+// * cp.async.bulk.prefetch.L2 of the link group and the two neighbour groups of the block 296 ... 9472 blocks ahead (five
+//   instructions per warp): 549 / 531 / 600 / 774 / 757 us (d18) -- the prefetched lines compete with the demand loads.
+constexpr int kForceMinBlocks = 4;       // double/12
+constexpr int kForceMinBlocksD18 = 3;    // loads first: 168 registers
+constexpr int kForceMinBlocksF18 = 6;    // loads first: 80 registers
+constexpr int kForceMinBlocksF12 = 8;    // loads first: 64 registers
 
 namespace lqcd {
 namespace {
@@ -86,30 +102,53 @@ __device__ __forceinline__ void phase_mul(T (&chi)[12], T pr, T pi) {
 // with the transported half spinor first.
 // REALPH (every boundary phase +-1, Geometry::real_ph): both terms carry the same real eta, so it multiplies the link's
 // whole W and is applied once, with kappa, when the force is stored -- no branch, no phase multiplication.
-template <typename T, int RECON, int MU, bool REALPH>
+// LF ("loads first"): the link and BOTH neighbour spinors -- the three DRAM-latency reads of the thread -- are named before
+// any arithmetic, so they are in flight together; the local spinors, shared through L1 by the four direction-warps, follow.
+template <typename T, int RECON, int MU, bool REALPH, bool LF>
 __device__ __forceinline__ void force_link(const ForceArgs& a, int p, int e, int e_nb, bool wrap) {
-    T u[18], psi[24], h[12], uh[12], v[12];
     AntiHerm<T> w;
 #pragma unroll
     for (int i = 0; i < 3; ++i) w.s[i] = w.r[i] = w.d[i] = 0;
-    load_link<RECON>(a.gauge, a.g.G, p, MU, e, u);
     const T er = (T)a.g.ph_re[MU], ei = (T)a.g.ph_im[MU];   // boundary phase, used on the wrapping hop only
+    if (LF) {
+        T u[18], xn[24], yn[24], h[12], uh1[12], uh2[12], v[12];
+        load_link<RECON>(a.gauge, a.g.G, p, MU, e, u);
+        load_spinor(a.x[1 - p], e_nb, xn);
+        load_spinor(a.y[1 - p], e_nb, yn);
+        project<MU, -1>(xn, h);
+        su3_mul(u, h, uh1);
+        project<MU, +1>(yn, h);
+        su3_mul(u, h, uh2);
+        if (!REALPH && wrap) {
+            phase_mul(uh1, er, ei);
+            phase_mul(uh2, er, ei);
+        }
+        load_spinor(a.y[p], e, xn);
+        project<MU, -1>(xn, v);
+        outer_acc(w, uh1, v);
+        load_spinor(a.x[p], e, yn);
+        project<MU, +1>(yn, v);
+        outer_acc(w, uh2, v);
+    } else {
+        T u[18], psi[24], h[12], uh[12], v[12];
+        load_link<RECON>(a.gauge, a.g.G, p, MU, e, u);
 
-    load_spinor(a.x[1 - p], e_nb, psi);
-    project<MU, -1>(psi, h);
-    su3_mul(u, h, uh);
-    if (!REALPH && wrap) phase_mul(uh, er, ei);
-    load_spinor(a.y[p], e, psi);
-    project<MU, -1>(psi, v);
-    outer_acc(w, uh, v);
+        load_spinor(a.x[1 - p], e_nb, psi);
+        project<MU, -1>(psi, h);
+        su3_mul(u, h, uh);
+        if (!REALPH && wrap) phase_mul(uh, er, ei);
+        load_spinor(a.y[p], e, psi);
+        project<MU, -1>(psi, v);
+        outer_acc(w, uh, v);
 
-    load_spinor(a.y[1 - p], e_nb, psi);
-    project<MU, +1>(psi, h);
-    su3_mul(u, h, uh);
-    if (!REALPH && wrap) phase_mul(uh, er, ei);
-    load_spinor(a.x[p], e, psi);
-    project<MU, +1>(psi, v);
-    outer_acc(w, uh, v);
+        load_spinor(a.y[1 - p], e_nb, psi);
+        project<MU, +1>(psi, h);
+        su3_mul(u, h, uh);
+        if (!REALPH && wrap) phase_mul(uh, er, ei);
+        load_spinor(a.x[p], e, psi);
+        project<MU, +1>(psi, v);
+        outer_acc(w, uh, v);
+    }
 
     // F^a = 2 kappa Im tr(T^a W) = kappa Im tr(lambda^a W)
     const double k = (REALPH && wrap) ? a.kappa * a.g.ph_re[MU] : a.kappa;
@@ -127,8 +166,8 @@ __device__ __forceinline__ void force_link(const ForceArgs& a, int p, int e, int
 // site is read twice, as X(x) by its own block and as X(x+mu) by blocks of the other parity:
 // sweeping one parity after the other put a whole field (805 MB of X, Y) between the two reads
 // and cost a second DRAM pass (ncu: 3.35 GB of traffic against 2.55 GB algorithmic).
-template <typename T, int RECON, bool REALPH>
-__global__ void __launch_bounds__(128, kForceMinBlocks) force_kernel(const ForceArgs a) {
+template <typename T, int RECON, bool REALPH, bool LF, int NB>
+__global__ void __launch_bounds__(128, NB) force_kernel(const ForceArgs a) {
     const int G = a.g.G;
     const int p = (int)blockIdx.x & 1;
     const int e = ((int)blockIdx.x >> 1) * 32 + (threadIdx.x & 31);
@@ -146,16 +185,16 @@ __global__ void __launch_bounds__(128, kForceMinBlocks) force_kernel(const Force
     const int s1 = N0h, s2 = N0h * N1, s3 = N0h * N1 * N2;
     if (mu == 0) {
         const bool wf = (r == 1) && (x0h == N0h - 1);
-        force_link<T, RECON, 0, REALPH>(a, p, e, wf ? e - (N0h - 1) : e + r, wf);
+        force_link<T, RECON, 0, REALPH, LF>(a, p, e, wf ? e - (N0h - 1) : e + r, wf);
     } else if (mu == 1) {
         const bool wf = (x1 == N1 - 1);
-        force_link<T, RECON, 1, REALPH>(a, p, e, wf ? e - (N1 - 1) * s1 : e + s1, wf);
+        force_link<T, RECON, 1, REALPH, LF>(a, p, e, wf ? e - (N1 - 1) * s1 : e + s1, wf);
     } else if (mu == 2) {
         const bool wf = (x2 == N2 - 1);
-        force_link<T, RECON, 2, REALPH>(a, p, e, wf ? e - (N2 - 1) * s2 : e + s2, wf);
+        force_link<T, RECON, 2, REALPH, LF>(a, p, e, wf ? e - (N2 - 1) * s2 : e + s2, wf);
     } else {
         const bool wf = (x3 == N3 - 1);
-        force_link<T, RECON, 3, REALPH>(a, p, e, wf ? e - (N3 - 1) * s3 : e + s3, wf);
+        force_link<T, RECON, 3, REALPH, LF>(a, p, e, wf ? e - (N3 - 1) * s3 : e + s3, wf);
     }
 }
 
@@ -194,16 +233,21 @@ cudaError_t launch_fermion_force(int precision, int recon, const Geometry& g, co
     count_launch();
     ProfScope prof(6, st);
     const int grid = 2 * g.G;
-    // The branch-free form is what ptxas schedules better only in double/12 (us per launch at 32^3 x 64, one box, A B A B:
-    // 438 against 482; double/18 511 against 503, single/18 278 against 275, single/12 268 against 259), so it is used there.
-    const bool rp = g.real_ph && precision == 0 && recon == 12;
-#define LQCD_FORCE(TT, RR)                                                           \
-    do {                                                                             \
-        if (rp) force_kernel<TT, RR, true><<<grid, 128, 0, st>>>(a);                 \
-        else    force_kernel<TT, RR, false><<<grid, 128, 0, st>>>(a);                \
+    // The order of the loads and the CTAs per SM are per format (table at the top of the file).  The branch-free form of the
+    // boundary phase is what ptxas schedules better in double/12 (438 against 482 us) and makes no difference elsewhere.
+    const bool rp = g.real_ph;
+#define LQCD_FORCE(TT, RR, LFV, NBV)                                                   \
+    do {                                                                               \
+        if (rp) force_kernel<TT, RR, true, LFV, NBV><<<grid, 128, 0, st>>>(a);         \
+        else    force_kernel<TT, RR, false, LFV, NBV><<<grid, 128, 0, st>>>(a);        \
     } while (0)
-    if (precision == 0) { if (recon == 12) LQCD_FORCE(double, 12); else LQCD_FORCE(double, 18); }
-    else                { if (recon == 12) LQCD_FORCE(float, 12);  else LQCD_FORCE(float, 18); }
+    if (precision == 0) {
+        if (recon == 12) LQCD_FORCE(double, 12, false, kForceMinBlocks);
+        else             LQCD_FORCE(double, 18, true, kForceMinBlocksD18);
+    } else {
+        if (recon == 12) LQCD_FORCE(float, 12, true, kForceMinBlocksF12);
+        else             LQCD_FORCE(float, 18, true, kForceMinBlocksF18);
+    }
 #undef LQCD_FORCE
     return cudaGetLastError();
 }
