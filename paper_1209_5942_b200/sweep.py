@@ -2,13 +2,14 @@
 """sweep.py -- timings of the BASELINE.json configurations 3, 4, 5 and of the paper's thermal
 lattice shapes (Fig. 7), one JSON line each.  A user-facing companion of bench.py:
 
-    python -m paper_1209_5942_b200.sweep [--configs 3,4,5,thermal,force,gauge,slab,copy,large] [--out FILE] [--hop-variant N]
+    python -m paper_1209_5942_b200.sweep [--configs 3,4,5,solve5,thermal,force,gauge,slab,copy,large] [--out FILE] [--hop-variant N]
 
 config 3: 16^3x32, near-identity links, kappa=.16 mu=.05: 10 warm-up + 100 timed D_eo/D_oe
           applications, 5 repeats, median (working set fits L2: not a HBM roofline figure)
 config 4: 24^3x48 Haar links: CG on Mhat^dag Mhat to 1e-10; iterations, time to solution,
           per-iteration split between hopping launches and vector kernels
 config 5: 32^3x64, double/single x 18/12-real links: 20 warm-up + 200 timed D-slash applications
+solve5  : config 4's three solves (double CG, BiCGStab, mixed-precision CG) on config 5's lattice
 thermal : N_sigma in {16,24,32,48} x N_tau in {4,8,12,16}, double/18 D-slash
 force   : the fermion-force kernel at 32^3x64 in the four storage variants
 gauge   : heatbath and overrelaxation sweeps at 32^3x64 in the four storage variants
@@ -101,8 +102,7 @@ def config3(stream):
     return [r]
 
 
-def config4(stream):
-    dims = (24, 24, 24, 48)
+def config4(stream, dims=(24, 24, 24, 48), label=4):
     kappa, mu, tol = 0.15, 0.1, 1e-10
     Vh = int(np.prod(dims)) // 2
     U = gen.gauge_haar(dims)
@@ -160,7 +160,7 @@ def config4(stream):
                  "time_to_solution_ms": m0.elapsed_time(m1), "rel_resid_true": mrr,
                  "speedup_vs_double": ms / m0.elapsed_time(m1)}
     B.lqcd_finalize()
-    out.append({"config": 4, "lattice": list(dims), "precision": "double", "recon": 18, "status": int(st),
+    out.append({"config": label, "lattice": list(dims), "precision": "double", "recon": 18, "status": int(st),
                 "iterations": iters, "time_to_solution_ms": ms, "rel_resid_recursive": rr, "rel_resid_true": rt,
                 "ms_per_iteration": ms / max(iters, 1),
                 "gflops": 4 * iters * Vh * FLOP / ms / 1e6,
@@ -171,6 +171,12 @@ def config4(stream):
                 "note": "time to solution includes the solve setup and the final true-residual check (one extra "
                         "application of Mhat^dag Mhat)"})
     return out
+
+
+def solve5(stream):
+    """Config 4's three solves (double CG, BiCGStab on Mhat, mixed-precision CG with a single/12 inner solve) on config 5's
+    32^3x64 lattice, device resident, to 1e-10."""
+    return config4(stream, (32, 32, 32, 64), "solve5")
 
 
 FORMATS = ((0, 18), (0, 12), (1, 18), (1, 12))   # --formats narrows config 5 down (d18,d12,s18,s12)
@@ -468,7 +474,7 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("sweep.py needs a CUDA device: there is no CPU fallback")
     stream = torch.cuda.Stream()
-    table = {"3": config3, "4": config4, "5": config5, "thermal": thermal, "force": force, "gauge": gauge, "slab": slab, "copy": copy, "large": large}
+    table = {"3": config3, "4": config4, "5": config5, "solve5": solve5, "thermal": thermal, "force": force, "gauge": gauge, "slab": slab, "copy": copy, "large": large}
     lines = []
     B.lqcd_set_hop_variant(args.hop_variant)
     for key in args.configs.split(","):
