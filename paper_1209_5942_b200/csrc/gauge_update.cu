@@ -32,6 +32,9 @@
 // between sites one step apart in z, t then meet in one CTA's L1): overrelaxation 264.4 / 153.0 / 245.7 / 152.3 us
 // (double/18, single/18, double/12, single/12) against 266.4 / 151.0 / 242.5 / 150.2 in linear order, heatbath 401.7
 // against 397.8 -- no gain, not kept (the same order of sites moved nothing in the hopping kernel either).
+// CTAs per SM re-measured on the final kernels (overrelaxation sub-sweep, us, A B A B on one box): single/18 at 3 / 4 / 5 / 6
+// CTAs 139.8 / 131.6-132.9 / 144.0 / 143.1, single/12 131.7 / 119.9 / 121.0 / 123.3; double/18 at 2 / 3 CTAs 262.9 /
+// 242.8-245.0, double/12 232.6 / 210-219 (4 CTAs: 259.7, profiles/r02_heatbath.md).  The constants below stay.
 constexpr int kGaugeMinBlocksDouble = 3;   // CTAs of 128 threads per SM the register allocation aims at
 constexpr int kGaugeMinBlocksFloat = 4;
 
