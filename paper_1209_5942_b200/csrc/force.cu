@@ -37,6 +37,11 @@
 //   (ncu: 12.8 of 16 resident warps active, the rest is CTA turnover): 576 us at 4 CTAs per SM, 530 at 8, 553 at 16 (d18);
 // * cp.async.bulk.prefetch.L2 of the link group and the two neighbour groups of the block 296 ... 9472 blocks ahead (five
 //   instructions per warp): 549 / 531 / 600 / 774 / 757 us (d18) -- the prefetched lines compete with the demand loads.
+// * the two combined as a software pipeline: persistent CTAs, the next block's link and neighbour spinors fetched with
+//   cp.async into a per-thread slot of shared memory (33 x 16 B per thread, 68 KB per CTA) while the current block is
+//   worked on from registers: 704 us at 3 CTAs per SM, 586 at 2 (d18), 575 / 521 (d12), results identical.  Every form
+//   that runs the memory requests further ahead of the arithmetic is slower: what the short-lived CTAs give the kernel is
+//   a spread over the phases of a link's life, and with it an even load on the memory system.
 constexpr int kForceMinBlocks = 4;       // double/12
 constexpr int kForceMinBlocksD18 = 3;    // loads first: 168 registers
 constexpr int kForceMinBlocksF18 = 6;    // loads first: 80 registers
