@@ -44,6 +44,11 @@
 // enough to carry a second set of instantiations.  Only double/12 moves to 4 CTAs.
 // single/12 re-measured at 5 / 6 / 7 / 8 CTAs (96 / 80 / 72 / 64 registers): 102.9 / 102.3 / 102.4 / 108.1 us per launch,
 // CG iteration 574 / 562 / 561 / 602 us: flat between 6 and 7, 7 stays.
+// double/12 is the one format the register file binds (acc 48 + link 36 + spinor 48 registers leave no room at 128 to
+// fetch the next hop early, and the register file being per sub-partition there is no budget between 128 and 168: 96-,
+// 64- and 160-thread CTAs with 5 / 7 / 3 per SM all compile to 128).  Tried in round 2: the lower half of the accumulator
+// (spin 2, 3: 12 of the 24 reals) kept in shared memory, 6 LDS.128 + 6 STS.128 per hop, to free 24 registers: 226.9-228.4
+// us at 4 CTAs, 222.3 at 3, 248.4 at 5 against 218.2 on the same box (results identical) -- not kept.
 constexpr int kHopMinBlocks = 3;       // double/18, single/18
 constexpr int kHopMinBlocksD12 = 4;    // double/12
 constexpr int kHopMinBlocksF12 = 7;    // single/12
