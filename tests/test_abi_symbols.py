@@ -59,6 +59,20 @@ def test_host_logic_without_gpu(lib_path):
     assert B.lqcd_last_error() != ""
 
 
+def test_plaquette_static_argument_checks_without_gpu(lib_path):
+    """lqcd_plaquette_static (the no-allocation entry point) rejects null pointers and lattices whose partial sums do not
+    fit its static scratch array before it touches the device."""
+    import ctypes
+    import paper_1209_5942_b200.binding as B
+    B.lqcd_init((4, 4, 4, 4), [1, 1, 1, -1])
+    assert B._lib.lqcd_plaquette_static(None, None) == B.LQCD_BAD_ARG
+    B.lqcd_init((64, 32, 32, 34), [1, 1, 1, -1])     # 8 * ceil(V / 256) = 69632 partial sums > 65536
+    dummy = ctypes.c_void_p(256)                     # never dereferenced: the size check comes first
+    assert B._lib.lqcd_plaquette_static(dummy, dummy) == B.LQCD_BAD_ARG
+    assert "static scratch array holds 65536" in B.lqcd_last_error()
+    B.lqcd_init((4, 4, 4, 4), [1, 1, 1, -1])
+
+
 def test_paper_sizes_fixture():
     vals = {}
     for line in open(os.path.join(ROOT, "tests", "golden", "paper_table2_table3_sizes.txt")):
