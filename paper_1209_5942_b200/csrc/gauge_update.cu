@@ -378,6 +378,76 @@ __device__ __forceinline__ void subgroup_step(T (&L)[18], const T (&A)[18], doub
     }
 }
 
+// Rows 0, 1 of op(a) op(b) (a product of SU(3) matrices is in SU(3): its third row follows from these two).
+template <bool DA, bool DB, typename T>
+__device__ __forceinline__ void mm3_rows01(const T (&a)[18], const T (&b)[18], T (&c)[12]) {
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            T re = 0, im = 0;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const T ar = DA ? a[2 * (3 * k + i)] : a[2 * (3 * i + k)];
+                const T ai = DA ? -a[2 * (3 * k + i) + 1] : a[2 * (3 * i + k) + 1];
+                const T br = DB ? b[2 * (3 * j + k)] : b[2 * (3 * k + j)];
+                const T bi = DB ? -b[2 * (3 * j + k) + 1] : b[2 * (3 * k + j) + 1];
+                re = fma_(ar, br, re);
+                re = fma_(-ai, bi, re);
+                im = fma_(ar, bi, im);
+                im = fma_(ai, br, im);
+            }
+            c[2 * (3 * i + j)] = re;
+            c[2 * (3 * i + j) + 1] = im;
+        }
+}
+// A += S, S the SU(3) matrix whose rows 0, 1 are t01 op(b): rows 0, 1 as computed, row 2 = conj(row0 x row1) accumulated
+// straight into A (8 multiply-adds per entry, the same count as the direct product of a third row would need for ONE of
+// the two products it saves).
+template <bool DB, typename T>
+__device__ __forceinline__ void add_staple_rows01(const T (&t)[12], const T (&b)[18], T (&A)[18]) {
+    T s[12];
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            T re = 0, im = 0;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const T ar = t[2 * (3 * i + k)], ai = t[2 * (3 * i + k) + 1];
+                const T br = DB ? b[2 * (3 * j + k)] : b[2 * (3 * k + j)];
+                const T bi = DB ? -b[2 * (3 * j + k) + 1] : b[2 * (3 * k + j) + 1];
+                re = fma_(ar, br, re);
+                re = fma_(-ai, bi, re);
+                im = fma_(ar, bi, im);
+                im = fma_(ai, br, im);
+            }
+            s[2 * (3 * i + j)] = re;
+            s[2 * (3 * i + j) + 1] = im;
+        }
+#pragma unroll
+    for (int i = 0; i < 12; ++i) A[i] += s[i];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
+        const T ar = s[2 * c1], ai = s[2 * c1 + 1], br = s[6 + 2 * c2], bi = s[6 + 2 * c2 + 1];
+        const T cr = s[2 * c2], ci = s[2 * c2 + 1], dr = s[6 + 2 * c1], di = s[6 + 2 * c1 + 1];
+        // A2_c += conj(s0[c1] s1[c2] - s0[c2] s1[c1])
+        A[12 + 2 * c] = fma_(ci, di, fma_(-cr, dr, fma_(-ai, bi, fma_(ar, br, A[12 + 2 * c]))));
+        A[12 + 2 * c + 1] = fma_(ci, dr, fma_(cr, di, fma_(-ai, br, fma_(-ar, bi, A[12 + 2 * c + 1]))));
+    }
+}
+
+// the two products of a staple, full (t of 18 reals) or two-row (t of 12)
+template <bool DA, bool DB, typename T>
+__device__ __forceinline__ void staple_first(const T (&a)[18], const T (&b)[18], T (&t)[18]) { mm3<DA, DB, false>(a, b, t); }
+template <bool DA, bool DB, typename T>
+__device__ __forceinline__ void staple_first(const T (&a)[18], const T (&b)[18], T (&t)[12]) { mm3_rows01<DA, DB>(a, b, t); }
+template <bool DB, typename T>
+__device__ __forceinline__ void staple_second(const T (&t)[18], const T (&b)[18], T (&A)[18]) { mm3<false, DB, true>(t, b, A); }
+template <bool DB, typename T>
+__device__ __forceinline__ void staple_second(const T (&t)[12], const T (&b)[18], T (&A)[18]) { add_staple_rows01<DB>(t, b, A); }
+
 // A += the six staples of U_mu(x) (Fig. 2).  All neighbour indices first, then one straight line of 18 link loads and
 // 12 products, written software-pipelined: the first link of the next direction nu is asked for BEFORE the last product
 // of the current one, so that the three passes do not each begin with nothing in flight (ptxas keeps to the order it
@@ -395,23 +465,30 @@ __device__ __forceinline__ void staple_sum(const GaugeArgs& a, const SiteIdx& x,
         e_mn[j] = step(a.g, x, nu[j], -1).e;
         e_pmmn[j] = step(a.g, xpm, nu[j], -1).e;
     }
-    T u[18], w[18], t[18], nx[18];
+    // Two-row form of the products (mm3_rows01 / add_staple_rows01: a staple is a product of SU(3) matrices, so its
+    // third row is conj(row0 x row1) and a third of the first product need not be computed): 36 of 216 multiply-adds per
+    // staple less.  Measured at 32^3 x 64 (us per sub-sweep, heatbath / overrelaxation, A B A B on one box, full / two-row):
+    // double/12 321-323 / 212 -> 283-284 / 205-213, single/12 216 / 120 -> 199 / 106, single/18 202 / 134-135 -> 198 / 130-133;
+    // double/18 326-329 / 246-253 -> 342-345 / 274-275 (ptxas spills 40 B and loses the order of the loads): the full
+    // products stay there.
+    constexpr bool TWOROW = !(sizeof(T) == 8 && RECON == 18);
+    T u[18], w[18], t[TWOROW ? 12 : 18], nx[18];
     gload<RECON, false>(a.gauge, G, 1 - p, nu[0], xpm.e, nx);            // U_nu(x+mu) of the first direction
 #pragma unroll
     for (int j = 0; j < 3; ++j) {
 #pragma unroll
         for (int i = 0; i < 18; ++i) u[i] = nx[i];
         gload<RECON, false>(a.gauge, G, 1 - p, mu, e_pn[j], w);          // U_mu(x+nu)
-        mm3<false, true, false>(u, w, t);
+        staple_first<false, true>(u, w, t);
         gload<RECON, false>(a.gauge, G, p, nu[j], x.e, u);               // U_nu(x)
-        mm3<false, true, true>(t, u, A);
+        staple_second<true>(t, u, A);
         gload<RECON, false>(a.gauge, G, p, nu[j], e_pmmn[j], u);         // U_nu(x+mu-nu)
         gload<RECON, false>(a.gauge, G, 1 - p, mu, e_mn[j], w);          // U_mu(x-nu)
-        mm3<true, true, false>(u, w, t);
+        staple_first<true, true>(u, w, t);
         gload<RECON, false>(a.gauge, G, 1 - p, nu[j], e_mn[j], u);       // U_nu(x-nu)
         if (j < 2) gload<RECON, false>(a.gauge, G, 1 - p, nu[j + 1], xpm.e, nx);   // next pass: U_nu'(x+mu)
         else       gload<RECON, true>(a.gauge, G, p, mu, x.e, L);                  // after the last pass: the link itself
-        mm3<false, false, true>(t, u, A);
+        staple_second<false>(t, u, A);
     }
 }
 
