@@ -469,8 +469,10 @@ __device__ __forceinline__ void staple_sum(const GaugeArgs& a, const SiteIdx& x,
     // third row is conj(row0 x row1) and a third of the first product need not be computed): 36 of 216 multiply-adds per
     // staple less.  Measured at 32^3 x 64 (us per sub-sweep, heatbath / overrelaxation, A B A B on one box, full / two-row):
     // double/12 321-323 / 212 -> 283-284 / 205-213, single/12 216 / 120 -> 199 / 106, single/18 202 / 134-135 -> 198 / 130-133;
-    // double/18 326-329 / 246-253 -> 342-345 / 274-275 (ptxas spills 40 B and loses the order of the loads): the full
-    // products stay there.
+    // double/18 326-329 / 246-253 -> 342-345 / 274-275: the full products stay there.  (Not the spills and not the shape of
+    // the source: the same products formed one row at a time with all three operands in registers give 343-344 / 273, and
+    // with the loads the two-row form drops kept alive 373-375 / 307-308.  ncu, profiles/r02_heatbath.md: 16% fewer
+    // instructions, 12% fewer bytes from L2, and more exposed load latency.)
     constexpr bool TWOROW = !(sizeof(T) == 8 && RECON == 18);
     T u[18], w[18], t[TWOROW ? 12 : 18], nx[18];
     gload<RECON, false>(a.gauge, G, 1 - p, nu[0], xpm.e, nx);            // U_nu(x+mu) of the first direction
